@@ -1,0 +1,168 @@
+/* awg.h -- C ABI of the B200-native additive waveform synthesiser.
+ *
+ * Implements the data-parallel hot path of arXiv 2403.15582 (Tu & Subhankar, "Fast real-time
+ * arbitrary waveform generation using graphic processing units"): every output sample is
+ *
+ *      V[n] = sum_k A_k sin(phi_k[n] + theta_k)                        Eq. 9
+ *
+ * where phi_k is the closed-form time integral of tone k's frequency trajectory -- static
+ * (Eq. 8), linear chirp (named at PAPER.md:137) or minimum-jerk ramp (Eq. 10,
+ * PAPER.md:141-148, branch 1 read as the integral of the ramp: DESIGN.md reading G1) -- the
+ * phase is reduced mod one turn before the sine (Eq. 14) and the sum is quantised
+ * to 16-bit DAC codes chunk by chunk (chunk = the paper's L_s),
+ * phase-continuous across chunks.  The paper's WG, WC and WM kernels are one
+ * fused sm_100a kernel here: no per-tone wavetable is ever stored.
+ *
+ * Conventions
+ *  - Plain C99, no exceptions cross this boundary; every call returns an awg_status (0 = OK,
+ *    negative = error) and never prints or aborts.  awg_last_error() gives the message.
+ *  - "host" pointers are ordinary CPU memory, caller-owned, read during the call only (copied
+ *    before return).  "device" pointers are CUDA global memory on the current device,
+ *    caller-owned (e.g. torch.empty(..., device='cuda').data_ptr()).
+ *  - stream arguments are a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *    Synthesis calls are asynchronous: they return after enqueueing work on that stream.
+ *  - Units: Hz, seconds, radians (phi0), fraction of full scale (A).  chunk_len is in samples and
+ *    must be a positive multiple of 8 (16-byte int16 stores).
+ *  - A plan is not thread-safe; distinct plans are independent.
+ *  - Output for (plan, chunk_idx) is a pure function of the trajectory table and of the absolute
+ *    sample index; it does not depend on the stream, ring depth, call order or chunk_len
+ *    (kernel tiles are anchored to absolute sample indices that are multiples of 256).
+ */
+#ifndef AWG_H_
+#define AWG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct awg_plan awg_plan; /* opaque; created and destroyed only by the library */
+typedef struct awg_ring awg_ring; /* opaque streaming ring bound to one plan            */
+typedef int32_t awg_status;
+
+enum {
+    AWG_OK = 0,
+    AWG_ERR_INVALID_ARG = -1, /* null pointer, bad size, non-finite value, misaligned buffer ... */
+    AWG_ERR_ALLOC = -2,       /* host or device allocation failed                                */
+    AWG_ERR_CUDA = -3,        /* a CUDA runtime call failed; awg_last_error() has its string    */
+    AWG_ERR_STATE = -4,       /* call order violated (see each function)                        */
+    AWG_ERR_UNDERRUN = -5     /* ring: the acquired chunk missed its real-time deadline         */
+};
+
+/* frequency trajectory of one tone ("any functional form for a frequency chirp") */
+enum {
+    AWG_PROFILE_STATIC = 0,  /* f(t) = f0                                                   */
+    AWG_PROFILE_LINEAR = 1,  /* f0 -> f1 linearly over [t_start, t_start + t_dur]            */
+    AWG_PROFILE_MINJERK = 2  /* f0 -> f1 along the minimum-jerk quintic 10s^3 - 15s^4 + 6s^5 */
+};
+
+/* sine engine of the synthesis kernel (step a3 of the hot path) */
+enum {
+    AWG_ENGINE_AUTO = 0, /* the library picks (currently AWG_ENGINE_MUFU)                               */
+    AWG_ENGINE_MUFU = 1, /* one MUFU.SIN per (tone, sample); phase re-centred per 256-sample tile        */
+    AWG_ENGINE_FP64 = 2  /* reference-grade: closed form and sine in fp64 per (tone, sample); ~50x slower */
+};
+
+/* ---- plan ---------------------------------------------------------------------------------- */
+
+/* Creates a plan for n_tones tones at sample_rate_hz with chunks of chunk_len samples on the
+ * current CUDA device.  Errors: INVALID_ARG (out NULL, n_tones < 1 or > 65536, rate not finite or
+ * <= 0, chunk_len < 8 or not a multiple of 8), ALLOC, CUDA (no device). */
+awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_hz, int64_t chunk_len);
+
+/* Frees the plan and its device tables after synchronising the streams it has work on.
+ * Rings bound to the plan must be destroyed first.  NULL is accepted. */
+awg_status awg_plan_destroy(awg_plan *p);
+
+/* int16 code = clamp(rint(scale * V), -32768, 32767), round-half-even (reading G9).
+ * Default 0.9*32767 (BASELINE.json config 1).  Errors: INVALID_ARG (not finite or <= 0). */
+awg_status awg_set_scale(awg_plan *p, double scale);
+
+/* Selects the sine engine (AWG_ENGINE_*).  Errors: INVALID_ARG. */
+awg_status awg_set_engine(awg_plan *p, int32_t engine);
+
+/* Replaces the whole trajectory table (Eq. 9/10 inputs per tone: a_j, theta_j, f_start, f_finish,
+ * T).  Seven host arrays of length n_tones:
+ *   f0, f1   start / final frequency, Hz           A        amplitude, fraction of full scale
+ *   phi0     phase offset at t = 0, radians        t_start  move start, s (any real, not snapped)
+ *   t_dur    move duration, s (>= 0; 0 = instant retune at t_start)
+ *   profile  AWG_PROFILE_* (STATIC ignores f1, t_start, t_dur)
+ * Frequencies above Nyquist or negative are evaluated as given (they alias), sum(A) > 1 saturates.
+ * Resets the update history.  Errors: INVALID_ARG (NULL, non-finite value, t_dur < 0, unknown
+ * profile). */
+awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1, const double *A,
+                                const double *phi0, const double *t_start, const double *t_dur,
+                                const int32_t *profile);
+
+/* Per-chunk update (streaming pathway, Fig. 7): at the first sample of chunk_idx each
+ * listed tone starts a new move from its current instantaneous frequency and phase (phase- and
+ * frequency-continuous) to f1[i] over t_dur[i] with profile[i].  Host arrays of length n_upd.
+ * The plan keeps only the current segment of each tone, so updates must come in non-decreasing
+ * chunk order and chunks earlier than the latest update can no longer be synthesised.
+ * Errors: INVALID_ARG (NULL with n_upd > 0, tone index out of range or duplicated, non-finite,
+ * t_dur < 0, unknown profile, chunk_idx < 0), STATE (no table set; chunk_idx lower than a previous
+ * update's). */
+awg_status awg_update_trajectories(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx,
+                                   const double *f1, const double *t_dur, const int32_t *profile);
+
+/* ---- synthesis (asynchronous on `stream`) ---------------------------------------------------- */
+
+/* Writes the int16 codes of samples [chunk_idx*chunk_len, (chunk_idx+1)*chunk_len) to dev_out
+ * (device, chunk_len int16, 16-byte aligned).  Errors: INVALID_ARG (NULL, misaligned, chunk_idx < 0),
+ * STATE (no table set; chunk earlier than the latest update), CUDA. */
+awg_status awg_synthesize_chunk(awg_plan *p, int64_t chunk_idx, int16_t *dev_out, void *stream);
+
+/* Same chunk before quantisation: the fp32 sum V (full scale = 1.0).  dev_out: chunk_len floats. */
+awg_status awg_synthesize_chunk_f32(awg_plan *p, int64_t chunk_idx, float *dev_out, void *stream);
+
+/* Playback / "precomputed" pathway (Fig. 6): chunks first_chunk .. first_chunk+n_chunks-1
+ * into one contiguous device buffer of n_chunks*chunk_len int16, in one kernel launch. */
+awg_status awg_synthesize_range(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *dev_out,
+                                void *stream);
+
+/* End-to-end variant with a HOST destination: synthesises the range chunk by chunk into internal
+ * device slots and copies each chunk to host_out (n_chunks*chunk_len int16; pinned memory gives
+ * overlap of copy and compute, pageable memory works) -- synchronous, returns when host_out is
+ * complete.  Stands in for the paper's pinned-buffer -> DAC transfer. */
+awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *host_out);
+
+/* ---- streaming ring (DAC-FIFO stand-in; Fig. 2b, 75, 127) --------------------------- */
+
+/* n_slots >= 2 device slots of chunk_len int16; host_mirror != 0 adds pinned-host slots and a copy
+ * stream that D2H-copies each finished chunk.  The ring owns its streams. */
+awg_status awg_ring_create(awg_ring **out, awg_plan *p, int32_t n_slots, int32_t host_mirror);
+
+/* Applies the n_upd updates (may be 0) at chunk_idx, then enqueues synthesis of chunk_idx into the
+ * next free slot.  Chunks must be submitted in increasing order.  Errors: STATE (ring full: acquire
+ * and release first; out-of-order chunk), plus those of awg_update_trajectories. */
+awg_status awg_ring_submit(awg_ring *r, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx,
+                           const double *f1, const double *t_dur, const int32_t *profile);
+
+/* Blocks until the oldest submitted chunk is complete (and mirrored when host_mirror is on), then
+ * lends its slot: *dev_ptr (device) and *host_ptr (pinned host or NULL) stay valid until
+ * awg_ring_release.  Returns AWG_ERR_UNDERRUN (pointers still valid) when the chunk was not ready
+ * by its deadline: chunk i of a run is due (i - prefill) * chunk_len / sample_rate seconds after
+ * the first acquire, where prefill = chunks submitted before that first acquire.
+ * Errors: STATE (nothing submitted). */
+awg_status awg_ring_acquire(awg_ring *r, int64_t *chunk_idx, const int16_t **dev_ptr,
+                            const int16_t **host_ptr);
+awg_status awg_ring_release(awg_ring *r, int64_t chunk_idx);
+
+/* produced = chunks completed; underruns = deadline misses; max_chunk_ms = longest device time of
+ * one chunk (synthesis + mirror copy) measured with CUDA events.  Any pointer may be NULL. */
+awg_status awg_ring_stats(awg_ring *r, int64_t *produced, int64_t *underruns, double *max_chunk_ms);
+awg_status awg_ring_destroy(awg_ring *r);
+
+/* ---- misc --------------------------------------------------------------------------------------- */
+
+/* Number of kernels the library has launched since load (all plans); for launch accounting. */
+int64_t awg_kernel_launch_count(void);
+
+/* Thread-local, library-owned, valid until the next awg_* call on this thread. */
+const char *awg_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AWG_H_ */

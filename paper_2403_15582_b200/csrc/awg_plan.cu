@@ -1,0 +1,497 @@
+// awg_plan.cu -- host side of the C ABI: plan, trajectory table (hot-path step a0), synthesis entry points.
+//
+// The trajectory table is kept on the host in x87 long double / 64-bit fixed point and mirrored to the
+// device as the structure of arrays of awg_internal.h.  Carrier phases are unsigned 64-bit fixed-point
+// turns, so theta + w*n is exact mod 1 for any absolute sample index n: this is the modf of Eq. 14
+// done in integers, and it is what keeps 35 ms x 560 MS/s (5.6e6 cycles) and 1 s x
+// 100 MS/s (1e8 cycles) phases at full precision.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include "awg_internal.h"
+#include "awg_plan.h"
+
+namespace awg {
+
+thread_local char g_err[512] = "";
+
+awg_status fail(awg_status code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+awg_status fail_cuda(cudaError_t e, const char *what)
+{
+    return fail(AWG_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+namespace {
+
+const long double kTwoPiL = 6.283185307179586476925286766559005768L;
+constexpr int kRadius = 128;  // half of the kernel's 256-sample tile
+
+// frac(x) as 64-bit fixed-point turns.
+uint64_t frac64(long double x)
+{
+    long double fr = x - floorl(x);        // [0, 1]
+    long double v = ldexpl(fr, 64);        // [0, 2^64]
+    if (!(v < 18446744073709551616.0L)) return 0;  // rounded up to one full turn
+    return static_cast<uint64_t>(v);
+}
+
+bool finite_all(const double *a, int n)
+{
+    for (int i = 0; i < n; ++i)
+        if (!std::isfinite(a[i])) return false;
+    return true;
+}
+
+// Polynomial class of a moving tone (which Taylor terms of DT*g(s) matter inside a 256-sample tile).
+int classify(int profile, long double DT, long double Tn)
+{
+    if (!(Tn >= 2.0L * kRadius)) return CLS_EXACT;  // move shorter than a tile: every tile straddles anyway
+    const double a = static_cast<double>(fabsl(DT) / Tn);  // |f1-f0|/fs, cycles per sample
+    const double r = static_cast<double>(1.0L / Tn);
+    const double R = kRadius;
+    const double tol_drop = 2e-8;   // cycles: dropped Taylor terms
+    const double max_mag = 0.25;    // cycles: fp32 polynomial magnitude (its rounding error is ~2^-23 of this)
+    // tiles that contain one end of the move evaluate DT*g over up to 256 samples from that end in fp32
+    const double sg = 2.0 * R * r;
+    const double DTa = static_cast<double>(fabsl(DT));
+    if (profile == AWG_PROFILE_LINEAR) {
+        const double t2 = a * r * 0.5 * R * R;
+        return (t2 <= max_mag && DTa * 0.5 * sg * sg <= 4.0 * max_mag) ? CLS_QUAD : CLS_EXACT;
+    }
+    if (DTa * sg * sg * sg * sg * (2.5 + 3.0 * sg + sg * sg) > max_mag) return CLS_EXACT;
+    // sup |g^(m)| on [0,1] for g = 5/2 s^4 - 3 s^5 + s^6: 1.875, 5.7735, 60, 360, 720
+    const double t2 = a * r * (1.875 / 2.0) * R * R;
+    const double t3 = a * r * r * (5.7735 / 6.0) * R * R * R;
+    const double t4 = a * r * r * r * (60.0 / 24.0) * R * R * R * R;
+    const double t5 = a * r * r * r * r * (360.0 / 120.0) * R * R * R * R * R;
+    const double t6 = a * r * r * r * r * r * R * R * R * R * R * R;
+    if (t2 + t3 + t4 + t5 + t6 > max_mag) return CLS_EXACT;
+    if (t3 + t4 + t5 + t6 <= tol_drop) return CLS_QUAD;
+    if (t5 + t6 <= tol_drop) return CLS_DEG4;
+    return CLS_DEG6;
+}
+
+void make_static(HostTone &h)
+{
+    h.profile = AWG_PROFILE_STATIC;
+    h.cls = CLS_STATIC;
+    h.f1 = h.f0;
+    h.ns_int = 0;
+    h.ns_frac = 0.0;
+    h.Tn = 0.0L;
+    h.T = 0.0L;
+    h.DT = 0.0L;
+    h.theta_post = h.theta_pre;
+    h.w_post = h.w_pre;
+}
+
+// Fills the move part of h (everything but theta_pre/w_pre/f0/A) for a move f0 -> f1 that starts at the
+// real sample position ns = ns_int + ns_frac and lasts T seconds.  `f_delta_ts` = (f1-f0)*t_start in cycles.
+void make_move(HostTone &h, long double fs, long double f1, int profile, long double T, int64_t ns_int,
+               double ns_frac, long double delta_times_tstart)
+{
+    const long double D = f1 - h.f0;
+    if (profile == AWG_PROFILE_STATIC || D == 0.0L) {
+        make_static(h);
+        return;
+    }
+    h.profile = profile;
+    h.f1 = f1;
+    h.T = T;
+    h.Tn = T * fs;
+    h.ns_int = ns_int;
+    h.ns_frac = ns_frac;
+    h.DT = D * T;
+    h.w_post = frac64(f1 / fs);
+    // after the move: Phi = theta + f0 t_s + f1 (t - t_s) + T (f0 - f1)/2   (Eq. 10 branch 2)
+    //                     = [theta - (f1-f0) t_s - DT/2] + (f1/fs) n
+    h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(h.DT / 2.0L);
+    h.cls = classify(profile, h.DT, h.Tn);
+}
+
+long double profile_h(int profile, long double s)  // frequency ramp 0 -> 1
+{
+    if (profile == AWG_PROFILE_LINEAR) return s;
+    return s * s * s * (10.0L + s * (6.0L * s - 15.0L));
+}
+
+long double profile_g(int profile, long double s)  // its integral
+{
+    if (profile == AWG_PROFILE_LINEAR) return 0.5L * s * s;
+    return s * s * s * s * (2.5L + s * (s - 3.0L));
+}
+
+}  // namespace
+
+// ---- device table versions ---------------------------------------------------------------------
+
+static void fill_staging(const awg_plan *p, unsigned char *dst)
+{
+    const int np = p->n_pad;
+    uint64_t *theta_pre = reinterpret_cast<uint64_t *>(dst);
+    uint64_t *w_pre = theta_pre + np;
+    uint64_t *theta_post = w_pre + np;
+    uint64_t *w_post = theta_post + np;
+    int64_t *ns_int = reinterpret_cast<int64_t *>(w_post + np);
+    double *ns_frac = reinterpret_cast<double *>(ns_int + np);
+    double *Tn = ns_frac + np;
+    double *inv_Tn = Tn + np;
+    double *DT = inv_Tn + np;
+    float *A = reinterpret_cast<float *>(DT + np);
+    int32_t *cls = reinterpret_cast<int32_t *>(A + np);
+    for (int i = 0; i < np; ++i) {
+        HostTone h{};
+        if (i < p->n_tones) h = p->tones[i];
+        theta_pre[i] = h.theta_pre;
+        w_pre[i] = h.w_pre;
+        theta_post[i] = h.theta_post;
+        w_post[i] = h.w_post;
+        ns_int[i] = h.ns_int;
+        ns_frac[i] = h.ns_frac;
+        Tn[i] = static_cast<double>(h.Tn);
+        inv_Tn[i] = h.Tn > 0.0L ? static_cast<double>(1.0L / h.Tn) : 0.0;
+        DT[i] = static_cast<double>(h.DT);
+        A[i] = h.A;
+        cls[i] = (h.profile << 8) | h.cls;
+    }
+}
+
+static ToneTable table_view(const awg_plan *p, int v)
+{
+    const int np = p->n_pad;
+    unsigned char *d = p->dev_table[v];
+    ToneTable t;
+    t.theta_pre = reinterpret_cast<uint64_t *>(d);
+    t.w_pre = t.theta_pre + np;
+    t.theta_post = t.w_pre + np;
+    t.w_post = t.theta_post + np;
+    t.ns_int = reinterpret_cast<const int64_t *>(t.w_post + np);
+    t.ns_frac = reinterpret_cast<const double *>(t.ns_int + np);
+    t.Tn = t.ns_frac + np;
+    t.inv_Tn = t.Tn + np;
+    t.DT = t.inv_Tn + np;
+    t.A = reinterpret_cast<const float *>(t.DT + np);
+    t.cls = reinterpret_cast<const int32_t *>(t.A + np);
+    t.n_tones = p->n_tones;
+    return t;
+}
+
+// Makes the device table current on `stream` (uploading a new version if the host table changed).
+static awg_status ensure_table(awg_plan *p, cudaStream_t stream)
+{
+    cudaError_t e;
+    if (p->dirty) {
+        const int v = (p->cur_version + 1) % kTableVersions;
+        // the slot's previous readers (kernels launched kTableVersions uploads ago) must be done
+        if ((e = cudaEventSynchronize(p->last_use[v])) != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
+        fill_staging(p, p->host_table[v]);
+        if ((e = cudaMemcpyAsync(p->dev_table[v], p->host_table[v], p->table_bytes, cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemcpyAsync(table)");
+        if ((e = cudaEventRecord(p->uploaded[v], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+        p->upload_stream[v] = stream;
+        p->cur_version = v;
+        p->dirty = false;
+        p->h2d_bytes += static_cast<int64_t>(p->table_bytes);
+    } else if (p->upload_stream[p->cur_version] != stream) {
+        if ((e = cudaStreamWaitEvent(stream, p->uploaded[p->cur_version], 0)) != cudaSuccess)
+            return fail_cuda(e, "cudaStreamWaitEvent");
+    }
+    return AWG_OK;
+}
+
+awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream)
+{
+    awg_status st = ensure_table(p, stream);
+    if (st != AWG_OK) return st;
+    LaunchParams lp;
+    lp.tab = table_view(p, p->cur_version);
+    lp.n_begin = n_begin;
+    lp.n_count = n_count;
+    lp.scale = static_cast<float>(p->scale);
+    lp.out = dev_out;
+    lp.out_f32 = f32 ? 1 : 0;
+    cudaError_t e = (p->engine == AWG_ENGINE_FP64) ? launch_fp64(lp, stream) : launch_mufu(lp, stream);
+    if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
+    if ((e = cudaEventRecord(p->last_use[p->cur_version], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+    return AWG_OK;
+}
+
+awg_status check_chunk_call(awg_plan *p, int64_t first_chunk, int64_t n_chunks, const void *out, size_t align)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (!out) return fail(AWG_ERR_INVALID_ARG, "output pointer is NULL");
+    if (reinterpret_cast<uintptr_t>(out) % align) return fail(AWG_ERR_INVALID_ARG, "output pointer must be %zu-byte aligned", align);
+    if (first_chunk < 0 || n_chunks < 1) return fail(AWG_ERR_INVALID_ARG, "bad chunk range");
+    if (first_chunk > (std::numeric_limits<int64_t>::max() / 4) / p->chunk_len - n_chunks)
+        return fail(AWG_ERR_INVALID_ARG, "chunk index too large");
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    if (first_chunk < p->last_update_chunk)
+        return fail(AWG_ERR_STATE, "chunk %lld precedes the latest trajectory update (chunk %lld)",
+                    static_cast<long long>(first_chunk), static_cast<long long>(p->last_update_chunk));
+    return AWG_OK;
+}
+
+awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx, const double *f1,
+                        const double *t_dur, const int32_t *profile)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (n_upd < 0 || chunk_idx < 0) return fail(AWG_ERR_INVALID_ARG, "negative count or chunk index");
+    if (n_upd > 0 && (!tone_idx || !f1 || !t_dur || !profile)) return fail(AWG_ERR_INVALID_ARG, "NULL update array");
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    if (chunk_idx < p->last_update_chunk)
+        return fail(AWG_ERR_STATE, "updates must come in non-decreasing chunk order");
+    if (chunk_idx > (std::numeric_limits<int64_t>::max() / 4) / p->chunk_len)
+        return fail(AWG_ERR_INVALID_ARG, "chunk index too large");
+    // validate everything before touching the table
+    std::vector<char> seen(p->n_tones, 0);
+    for (int i = 0; i < n_upd; ++i) {
+        const int k = tone_idx[i];
+        if (k < 0 || k >= p->n_tones) return fail(AWG_ERR_INVALID_ARG, "tone index %d out of range", k);
+        if (seen[k]) return fail(AWG_ERR_INVALID_ARG, "tone %d listed twice in one update", k);
+        seen[k] = 1;
+        if (!std::isfinite(f1[i]) || !std::isfinite(t_dur[i]) || t_dur[i] < 0.0)
+            return fail(AWG_ERR_INVALID_ARG, "non-finite value or negative duration in update %d", i);
+        if (profile[i] < AWG_PROFILE_STATIC || profile[i] > AWG_PROFILE_MINJERK)
+            return fail(AWG_ERR_INVALID_ARG, "unknown profile %d", profile[i]);
+    }
+    const long double fs = p->fs;
+    const int64_t n_u = chunk_idx * p->chunk_len;
+    for (int i = 0; i < n_upd; ++i) {
+        HostTone &h = p->tones[tone_idx[i]];
+        // state of the old segment at n_u: instantaneous frequency and a carrier that continues its phase
+        if (h.cls != CLS_STATIC) {
+            const long double u = static_cast<long double>(n_u - h.ns_int) - static_cast<long double>(h.ns_frac);
+            if (u <= 0.0L) {
+                // move had not started: keep the pre-move carrier
+            } else if (u >= h.Tn) {
+                h.theta_pre = h.theta_post;
+                h.w_pre = h.w_post;
+                h.f0 = h.f1;
+            } else {
+                // mid-move (G12): continue from the instantaneous frequency and phase
+                const long double s = u / h.Tn;
+                const long double f_now = h.f0 + (h.f1 - h.f0) * profile_h(h.profile, s);
+                const uint64_t ph = h.theta_pre + h.w_pre * static_cast<uint64_t>(n_u) + frac64(h.DT * profile_g(h.profile, s));
+                h.f0 = f_now;
+                h.w_pre = frac64(f_now / fs);
+                h.theta_pre = ph - h.w_pre * static_cast<uint64_t>(n_u);
+            }
+        }
+        const long double f1l = static_cast<long double>(f1[i]);
+        const long double D = f1l - h.f0;
+        // (f1-f0) * t_u with t_u = n_u/fs
+        make_move(h, fs, f1l, profile[i], static_cast<long double>(t_dur[i]), n_u, 0.0,
+                  D * static_cast<long double>(n_u) / fs);
+    }
+    if (n_upd > 0) {
+        p->dirty = true;
+        p->last_update_chunk = chunk_idx;
+    }
+    return AWG_OK;
+}
+
+}  // namespace awg
+
+using namespace awg;
+
+extern "C" {
+
+const char *awg_last_error(void) { return g_err; }
+
+awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_hz, int64_t chunk_len)
+{
+    if (!out) return fail(AWG_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (n_tones < 1 || n_tones > 65536) return fail(AWG_ERR_INVALID_ARG, "n_tones must be in [1, 65536]");
+    if (!std::isfinite(sample_rate_hz) || sample_rate_hz <= 0.0) return fail(AWG_ERR_INVALID_ARG, "sample_rate_hz must be finite and > 0");
+    if (chunk_len < 8 || chunk_len % 8 || chunk_len > (int64_t(1) << 40)) return fail(AWG_ERR_INVALID_ARG, "chunk_len must be a positive multiple of 8");
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaGetDevice");
+    awg_plan *p = new (std::nothrow) awg_plan();
+    if (!p) return fail(AWG_ERR_ALLOC, "out of host memory");
+    p->n_tones = n_tones;
+    p->n_pad = (n_tones + 31) / 32 * 32;
+    p->fs = static_cast<long double>(sample_rate_hz);
+    p->chunk_len = chunk_len;
+    p->scale = 0.9 * 32767.0;
+    p->engine = AWG_ENGINE_MUFU;
+    p->device = dev;
+    p->table_bytes = table_bytes(p->n_pad);
+    try {
+        p->tones.resize(n_tones);
+    } catch (...) {
+        delete p;
+        return fail(AWG_ERR_ALLOC, "out of host memory");
+    }
+    for (int v = 0; v < kTableVersions; ++v) {
+        if ((e = cudaMalloc(reinterpret_cast<void **>(&p->dev_table[v]), p->table_bytes)) != cudaSuccess ||
+            (e = cudaMallocHost(reinterpret_cast<void **>(&p->host_table[v]), p->table_bytes)) != cudaSuccess ||
+            (e = cudaEventCreateWithFlags(&p->last_use[v], cudaEventDisableTiming)) != cudaSuccess ||
+            (e = cudaEventCreateWithFlags(&p->uploaded[v], cudaEventDisableTiming)) != cudaSuccess) {
+            awg_status st = (e == cudaErrorMemoryAllocation) ? fail(AWG_ERR_ALLOC, "device/pinned allocation failed: %s", cudaGetErrorString(e))
+                                                             : fail_cuda(e, "plan allocation");
+            awg_plan_destroy(p);
+            return st;
+        }
+    }
+    *out = p;
+    return AWG_OK;
+}
+
+awg_status awg_plan_destroy(awg_plan *p)
+{
+    if (!p) return AWG_OK;
+    if (p->n_rings > 0) return fail(AWG_ERR_STATE, "destroy the plan's rings first");
+    for (int v = 0; v < kTableVersions; ++v)
+        if (p->last_use[v]) cudaEventSynchronize(p->last_use[v]);
+    for (int s = 0; s < 2; ++s) {
+        if (p->e2e_done[s]) cudaEventSynchronize(p->e2e_done[s]);
+    }
+    for (int v = 0; v < kTableVersions; ++v) {
+        if (p->dev_table[v]) cudaFree(p->dev_table[v]);
+        if (p->host_table[v]) cudaFreeHost(p->host_table[v]);
+        if (p->last_use[v]) cudaEventDestroy(p->last_use[v]);
+        if (p->uploaded[v]) cudaEventDestroy(p->uploaded[v]);
+    }
+    for (int s = 0; s < 2; ++s) {
+        if (p->e2e_slot[s]) cudaFree(p->e2e_slot[s]);
+        if (p->e2e_done[s]) cudaEventDestroy(p->e2e_done[s]);
+        if (p->e2e_ready[s]) cudaEventDestroy(p->e2e_ready[s]);
+        if (p->e2e_stream[s]) cudaStreamDestroy(p->e2e_stream[s]);
+    }
+    delete p;
+    return AWG_OK;
+}
+
+awg_status awg_set_scale(awg_plan *p, double scale)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (!std::isfinite(scale) || scale <= 0.0) return fail(AWG_ERR_INVALID_ARG, "scale must be finite and > 0");
+    p->scale = scale;
+    return AWG_OK;
+}
+
+awg_status awg_set_engine(awg_plan *p, int32_t engine)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (engine == AWG_ENGINE_AUTO) engine = AWG_ENGINE_MUFU;
+    if (engine != AWG_ENGINE_MUFU && engine != AWG_ENGINE_FP64) return fail(AWG_ERR_INVALID_ARG, "unknown engine %d", engine);
+    p->engine = engine;
+    return AWG_OK;
+}
+
+awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1, const double *A, const double *phi0,
+                                const double *t_start, const double *t_dur, const int32_t *profile)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (!f0 || !f1 || !A || !phi0 || !t_start || !t_dur || !profile) return fail(AWG_ERR_INVALID_ARG, "NULL trajectory array");
+    const int N = p->n_tones;
+    if (!finite_all(f0, N) || !finite_all(f1, N) || !finite_all(A, N) || !finite_all(phi0, N) ||
+        !finite_all(t_start, N) || !finite_all(t_dur, N))
+        return fail(AWG_ERR_INVALID_ARG, "non-finite value in a trajectory array");
+    for (int k = 0; k < N; ++k) {
+        if (t_dur[k] < 0.0) return fail(AWG_ERR_INVALID_ARG, "t_dur[%d] < 0", k);
+        if (profile[k] < AWG_PROFILE_STATIC || profile[k] > AWG_PROFILE_MINJERK)
+            return fail(AWG_ERR_INVALID_ARG, "unknown profile %d for tone %d", profile[k], k);
+        if (std::fabs(t_start[k]) * static_cast<double>(p->fs) > 4.0e18)
+            return fail(AWG_ERR_INVALID_ARG, "t_start[%d] out of range", k);
+    }
+    const long double fs = p->fs;
+    for (int k = 0; k < N; ++k) {
+        HostTone &h = p->tones[k];
+        h = HostTone{};
+        h.A = static_cast<float>(A[k]);
+        h.f0 = static_cast<long double>(f0[k]);
+        h.theta_pre = frac64(static_cast<long double>(phi0[k]) / kTwoPiL);  // radians -> turns (theta_j of Eq. 8/9)
+        h.w_pre = frac64(h.f0 / fs);
+        const long double ts = static_cast<long double>(t_start[k]);
+        const long double ns = ts * fs;
+        const long double nsi = floorl(ns);
+        make_move(h, fs, static_cast<long double>(f1[k]), profile[k], static_cast<long double>(t_dur[k]),
+                  static_cast<int64_t>(nsi), static_cast<double>(ns - nsi),
+                  (static_cast<long double>(f1[k]) - h.f0) * ts);
+    }
+    p->have_table = true;
+    p->dirty = true;
+    p->last_update_chunk = 0;
+    return AWG_OK;
+}
+
+awg_status awg_update_trajectories(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx,
+                                   const double *f1, const double *t_dur, const int32_t *profile)
+{
+    return apply_update(p, chunk_idx, n_upd, tone_idx, f1, t_dur, profile);
+}
+
+awg_status awg_synthesize_chunk(awg_plan *p, int64_t chunk_idx, int16_t *dev_out, void *stream)
+{
+    awg_status st = check_chunk_call(p, chunk_idx, 1, dev_out, 16);
+    if (st != AWG_OK) return st;
+    return synthesize_samples(p, chunk_idx * p->chunk_len, p->chunk_len, dev_out, false, static_cast<cudaStream_t>(stream));
+}
+
+awg_status awg_synthesize_chunk_f32(awg_plan *p, int64_t chunk_idx, float *dev_out, void *stream)
+{
+    awg_status st = check_chunk_call(p, chunk_idx, 1, dev_out, 16);
+    if (st != AWG_OK) return st;
+    return synthesize_samples(p, chunk_idx * p->chunk_len, p->chunk_len, dev_out, true, static_cast<cudaStream_t>(stream));
+}
+
+awg_status awg_synthesize_range(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *dev_out, void *stream)
+{
+    awg_status st = check_chunk_call(p, first_chunk, n_chunks, dev_out, 16);
+    if (st != AWG_OK) return st;
+    return synthesize_samples(p, first_chunk * p->chunk_len, n_chunks * p->chunk_len, dev_out, false, static_cast<cudaStream_t>(stream));
+}
+
+awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *host_out)
+{
+    awg_status st = check_chunk_call(p, first_chunk, n_chunks, host_out, 2);
+    if (st != AWG_OK) return st;
+    cudaError_t e;
+    // two device slots; stream 0 synthesises piece i+1 while stream 1 copies piece i to the host
+    constexpr int64_t kPiece = int64_t(1) << 21;  // samples per piece (4 MiB of int16)
+    if (!p->e2e_slot[0]) {
+        for (int s = 0; s < 2; ++s) {
+            if ((e = cudaMalloc(reinterpret_cast<void **>(&p->e2e_slot[s]), kPiece * sizeof(int16_t))) != cudaSuccess)
+                return fail(AWG_ERR_ALLOC, "cudaMalloc(e2e slot): %s", cudaGetErrorString(e));
+            if ((e = cudaStreamCreateWithFlags(&p->e2e_stream[s], cudaStreamNonBlocking)) != cudaSuccess ||
+                (e = cudaEventCreateWithFlags(&p->e2e_ready[s], cudaEventDisableTiming)) != cudaSuccess ||
+                (e = cudaEventCreateWithFlags(&p->e2e_done[s], cudaEventDisableTiming)) != cudaSuccess)
+                return fail_cuda(e, "e2e stream/event creation");
+        }
+    }
+    const int64_t n0 = first_chunk * p->chunk_len, total = n_chunks * p->chunk_len;
+    cudaStream_t s_syn = p->e2e_stream[0], s_cpy = p->e2e_stream[1];
+    int i = 0;
+    for (int64_t off = 0; off < total; off += kPiece, ++i) {
+        const int slot = i & 1;
+        const int64_t cnt = (total - off < kPiece) ? (total - off) : kPiece;
+        if (i >= 2 && (e = cudaStreamWaitEvent(s_syn, p->e2e_done[slot], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+        if ((st = synthesize_samples(p, n0 + off, cnt, p->e2e_slot[slot], false, s_syn)) != AWG_OK) return st;
+        if ((e = cudaEventRecord(p->e2e_ready[slot], s_syn)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+        if ((e = cudaStreamWaitEvent(s_cpy, p->e2e_ready[slot], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+        if ((e = cudaMemcpyAsync(host_out + off, p->e2e_slot[slot], cnt * sizeof(int16_t), cudaMemcpyDeviceToHost, s_cpy)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemcpyAsync(D2H)");
+        if ((e = cudaEventRecord(p->e2e_done[slot], s_cpy)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+        p->d2h_bytes += cnt * static_cast<int64_t>(sizeof(int16_t));
+    }
+    if ((e = cudaStreamSynchronize(s_cpy)) != cudaSuccess) return fail_cuda(e, "cudaStreamSynchronize");
+    return AWG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,67 @@
+// awg_plan.h -- host-side plan state (shared by awg_plan.cu and awg_ring.cu).  CUDA path only.
+#pragma once
+#include <cstdint>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "awg.h"
+
+namespace awg {
+
+constexpr int kTableVersions = 4;  // device copies of the trajectory table in flight (updates never stall a running kernel)
+
+// Current segment of one tone, host precision (x87 long double + 64-bit fixed-point turns).
+struct HostTone {
+    long double f0 = 0, f1 = 0;  // Hz: frequency before / after the current move
+    long double T = 0;           // move duration, s
+    long double Tn = 0;          // move duration, samples (T*fs)
+    long double DT = 0;          // (f1-f0)*T, cycles
+    int64_t ns_int = 0;          // move start, samples: floor and
+    double ns_frac = 0;          //   fractional part
+    uint64_t theta_pre = 0, w_pre = 0;    // carrier before/during the move: turns*2^64, turns/sample*2^64
+    uint64_t theta_post = 0, w_post = 0;  // carrier after the move
+    float A = 0;
+    int32_t profile = AWG_PROFILE_STATIC;
+    int32_t cls = 0;
+};
+
+awg_status fail(awg_status code, const char *fmt, ...);
+awg_status fail_cuda(cudaError_t e, const char *what);
+
+}  // namespace awg
+
+struct awg_plan {
+    int32_t n_tones = 0, n_pad = 0;
+    long double fs = 0;
+    int64_t chunk_len = 0;
+    double scale = 0;
+    int32_t engine = AWG_ENGINE_MUFU;
+    int device = 0;
+    bool have_table = false;
+    bool dirty = false;
+    int64_t last_update_chunk = 0;
+    std::vector<awg::HostTone> tones;
+    // versioned device tables
+    size_t table_bytes = 0;
+    int cur_version = 0;
+    unsigned char *dev_table[awg::kTableVersions] = {};
+    unsigned char *host_table[awg::kTableVersions] = {};  // pinned staging
+    cudaEvent_t last_use[awg::kTableVersions] = {};
+    cudaEvent_t uploaded[awg::kTableVersions] = {};
+    cudaStream_t upload_stream[awg::kTableVersions] = {};
+    // awg_synthesize_range_host
+    int16_t *e2e_slot[2] = {};
+    cudaStream_t e2e_stream[2] = {};
+    cudaEvent_t e2e_ready[2] = {}, e2e_done[2] = {};
+    // accounting
+    int64_t h2d_bytes = 0, d2h_bytes = 0;
+    int n_rings = 0;
+};
+
+namespace awg {
+awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream);
+awg_status check_chunk_call(awg_plan *p, int64_t first_chunk, int64_t n_chunks, const void *out, size_t align);
+awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx, const double *f1,
+                        const double *t_dur, const int32_t *profile);
+}  // namespace awg

@@ -1,0 +1,79 @@
+"""CPU-only checks of the boundary: the C-ABI library loads, exports every symbol include/awg.h
+declares, the Python binding mirrors the header, and calls fail cleanly (no crash, no CPU fallback)
+when there is no GPU.  No compute is attempted here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "awg.h")
+
+
+def _declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(awg_[a-z0-9_]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def built():
+    from paper_2403_15582_b200 import build
+    return build.build()
+
+
+def test_header_declares_the_north_star_calls():
+    syms = _declared_symbols()
+    for name in ("awg_plan_create", "awg_set_trajectories", "awg_synthesize_chunk", "awg_update_trajectories",
+                 "awg_ring_create", "awg_ring_submit", "awg_ring_acquire"):
+        assert name in syms
+
+
+def test_library_exports_every_declared_symbol(built):
+    lib = ctypes.CDLL(built)
+    for name in _declared_symbols():
+        assert hasattr(lib, name), f"{name} declared in awg.h but not exported"
+
+
+def test_binding_mirrors_the_header(built):
+    import paper_2403_15582_b200 as m
+    assert sorted(m.EXPORTED) == _declared_symbols()
+    for name in m.EXPORTED:
+        assert callable(getattr(m, name)), f"binding lacks {name}"
+    src = open(HEADER).read()
+    for const in ("AWG_OK", "AWG_ERR_INVALID_ARG", "AWG_ERR_ALLOC", "AWG_ERR_CUDA", "AWG_ERR_STATE", "AWG_ERR_UNDERRUN",
+                  "AWG_PROFILE_STATIC", "AWG_PROFILE_LINEAR", "AWG_PROFILE_MINJERK", "AWG_ENGINE_AUTO",
+                  "AWG_ENGINE_MUFU", "AWG_ENGINE_FP64"):
+        mm = re.search(rf"\b{const}\s*=\s*(-?\d+)", src)
+        assert mm and int(mm.group(1)) == getattr(m, const)
+
+
+def test_argument_errors_need_no_gpu(built):
+    import paper_2403_15582_b200 as m
+    for args in ((0, 560e6, 1024), (4, -1.0, 1024), (4, float("nan"), 1024), (4, 560e6, 12), (4, 560e6, 0)):
+        with pytest.raises(m.AwgError) as ei:
+            m.awg_plan_create(*args)
+        assert ei.value.status == m.AWG_ERR_INVALID_ARG
+        assert m.awg_last_error()
+    m.awg_plan_destroy(None)  # NULL is accepted
+
+
+def test_no_cpu_fallback_without_a_device(built):
+    import torch
+    import paper_2403_15582_b200 as m
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(m.AwgError) as ei:
+        m.awg_plan_create(4, 560e6, 1024)
+    assert ei.value.status in (m.AWG_ERR_CUDA, m.AWG_ERR_ALLOC)
+
+
+def test_product_path_does_not_touch_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2403_15582_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cpp", ".cuh")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "awg_oracle" not in txt, f

@@ -1,0 +1,407 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the oracle, element by element on
+the same seeded inputs.  Bar (BASELINE.json north_star): int16 within +-1 LSB on >= 99.99 % of samples,
+max 2 LSB; fp32 pre-quantisation sum within 1e-5 of full scale.  Sizes the oracle finishes in seconds
+span many 256-sample tiles and ragged tails; the full-size configurations are synthesised in the
+launch configuration bench.py times and compared on sampled windows."""
+import math
+
+import numpy as np
+import pytest
+
+import awg_workloads as W
+import oracle
+from parity_util import assert_codes_close, assert_f32_close, oracle_windows, sample_windows
+
+pytestmark = pytest.mark.gpu
+
+STATIC, LINEAR, MINJERK = W.PROFILE_STATIC, W.PROFILE_LINEAR, W.PROFILE_MINJERK
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def _np(t):
+    return t.cpu().numpy()
+
+
+def _gpu_plan(awg, w, engine=None, chunk_len=None):
+    return awg.Plan.from_workload(w, engine if engine is not None else awg.AWG_ENGINE_AUTO, chunk_len)
+
+
+# ------------------------------------------------------------------ C1: the PR1 reference config
+@pytest.mark.parametrize("engine", ["mufu", "fp64"])
+def test_c1_full_int16_and_f32(awg, torch_cuda, engine):
+    w = W.config1()
+    op = oracle.plan_from_workload(w)
+    V = oracle.c_waveform(op, 0, w.n_samples)
+    codes = op.quantise(V)
+    p = _gpu_plan(awg, w, awg.AWG_ENGINE_MUFU if engine == "mufu" else awg.AWG_ENGINE_FP64)
+    got = _np(p.synthesize_chunk(0))
+    gotf = _np(p.synthesize_chunk_f32(0))
+    exact, dmax = assert_codes_close(got, codes, f"C1 {engine}")
+    emax = assert_f32_close(gotf, V, f"C1 {engine} f32", tol=1e-5 if engine == "mufu" else 2e-7)
+    print(f"C1 {engine}: exact {exact:.5f}, max {dmax} LSB, f32 max err {emax:.2e}")
+    p.close()
+
+
+def test_c1_chunking_is_bit_identical_on_gpu(awg, torch_cuda):
+    w = W.config1()
+    ref = _np(_gpu_plan(awg, w).synthesize_chunk(0))
+    for cl in (1 << 16, 1 << 18):
+        p = _gpu_plan(awg, w, chunk_len=cl)
+        parts = [_np(p.synthesize_chunk(c)) for c in range(w.n_samples // cl)]
+        assert np.array_equal(np.concatenate(parts), ref), f"chunk_len {cl}"
+        # the range call over all chunks is the same launch as one long chunk
+        assert np.array_equal(_np(p.synthesize_range(0, w.n_samples // cl)), ref)
+        p.close()
+
+
+# ------------------------------------------------------------------ C2: 100 tones, min-jerk moves
+def test_c2_full_range_and_chunks(awg, torch_cuda):
+    w = W.config2()
+    op = oracle.plan_from_workload(w)
+    V = oracle.c_waveform(op, 0, w.n_samples)
+    codes = op.quantise(V)
+    p = _gpu_plan(awg, w)
+    got = _np(p.synthesize_range(0, w.n_chunks))  # the launch bench.py times
+    exact, dmax = assert_codes_close(got, codes, "C2 range")
+    print(f"C2: exact {exact:.5f}, max {dmax} LSB")
+    per_chunk = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(w.n_chunks)])
+    assert np.array_equal(per_chunk, got)  # 224000 = 875 tiles: chunking does not change a bit
+    gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(w.n_chunks)])
+    emax = assert_f32_close(gotf, V, "C2 f32")
+    print(f"C2 f32 max err {emax:.2e}")
+    # the host-destination (end-to-end) call returns the same codes
+    host = p.synthesize_range_host(0, w.n_chunks).numpy()
+    assert np.array_equal(host, got)
+    p.close()
+
+
+def test_c2_fp64_engine_window(awg, torch_cuda):
+    w = W.config2().rechunked(224_000)
+    op = oracle.plan_from_workload(w)
+    k = int(np.argmax(w.t_dur))
+    c = int(w.t_start[k] * w.sample_rate) // w.chunk_len
+    V = oracle.c_waveform(op, c * w.chunk_len, (c + 1) * w.chunk_len)
+    p = _gpu_plan(awg, w, awg.AWG_ENGINE_FP64)
+    assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, "C2 fp64 engine", tol=2e-7)
+    assert_codes_close(_np(p.synthesize_chunk(c)), op.quantise(V), "C2 fp64 engine")
+    p.close()
+
+
+def test_c2_chunk_len_not_a_multiple_of_the_tile(awg, torch_cuda):
+    # 5.6e6 = 2^8 * 21875: chunk_len 1000 (multiple of 8, not of 256) gives partial tiles at both chunk edges
+    w = W.config2()
+    ref = _np(_gpu_plan(awg, w).synthesize_range(0, w.n_chunks))
+    p = _gpu_plan(awg, w, chunk_len=1000)
+    for c in (0, 1, 2, 777, 5599):
+        assert np.array_equal(_np(p.synthesize_chunk(c)), ref[c * 1000:(c + 1) * 1000]), c
+    assert np.array_equal(_np(p.synthesize_range(3, 41)), ref[3000:44000])
+    p.close()
+
+
+# ------------------------------------------------------------------ C3: 1000 tones, 35 ms playback
+def test_c3_playback_range_sampled(awg, torch_cuda):
+    w = W.config3()
+    op = oracle.plan_from_workload(w)
+    p = _gpu_plan(awg, w)
+    out = p.synthesize_range(0, w.n_chunks)  # one 39.8 MB device buffer, one launch (precomputed pathway)
+    torch_cuda.cuda.synchronize()
+    n_end = int(round(35e-3 * w.sample_rate))  # the move ends inside chunk 18
+    wins = sample_windows(w.n_samples, 4096, 12, seed=33, must=(n_end, w.n_samples // 2))
+    worst = 0
+    for (a, b), (V, codes) in zip(wins, oracle_windows(op, wins)):
+        _, dmax = assert_codes_close(_np(out[a:b]), codes, f"C3 [{a},{b})")
+        worst = max(worst, dmax)
+    # fp32 sum of the chunk that contains the end of the move
+    c = n_end // w.chunk_len
+    f = p.synthesize_chunk_f32(c)
+    a = n_end - 2048 - (n_end - 2048) % 8
+    V = oracle.c_waveform(op, a, a + 4096)
+    emax = assert_f32_close(_np(f[a - c * w.chunk_len:a - c * w.chunk_len + 4096]), V, "C3 f32 at move end")
+    print(f"C3: max {worst} LSB over {len(wins)} windows, f32 max err {emax:.2e}")
+    p.close()
+
+
+# ------------------------------------------------------------------ C4: streaming ring with per-chunk updates
+def test_c4_streaming_ring_with_updates(awg, torch_cuda):
+    w = W.config4(96)  # 96 chunks = 0.25 s of the 1 s run: same update statistics, oracle stays fast
+    op = oracle.plan_from_workload(w)
+    L = w.chunk_len
+    check = {0, 1, 2, 15, 16, 17, 47, 48, 63, 64, 94, 95}
+    p = _gpu_plan(awg, w)
+    ring = awg.Ring(p, n_slots=3, host_mirror=True)
+    ups = w.updates_by_chunk()
+    kept = {}
+    submitted = 0
+    for c in range(w.n_chunks + 2):
+        if c < w.n_chunks:
+            ring.submit(c, ups.get(c))
+            submitted += 1
+        if c >= 2:
+            idx, dptr, hptr, _ = ring.acquire()
+            assert idx == c - 2 and hptr != 0
+            if idx in check:
+                kept[idx] = ring.host_view(hptr).copy()
+            ring.release(idx)
+    produced, _, max_ms = ring.stats()
+    assert produced == w.n_chunks == submitted and max_ms > 0
+    for c in sorted(check):
+        # head of the chunk (where the 100 us = 10 000-sample moves run) and its tail
+        for a, b in ((c * L, c * L + 12288), ((c + 1) * L - 4096, (c + 1) * L)):
+            V = oracle.c_waveform(op, a, b)
+            assert_codes_close(kept[c][a - c * L:b - c * L], op.quantise(V), f"C4 chunk {c} [{a},{b})")
+    ring.close()
+    # the plain per-chunk call gives the same codes as the ring (chunk after the last update)
+    last = w.n_chunks - 1
+    assert np.array_equal(_np(p.synthesize_chunk(last)), kept[last])
+    p.close()
+
+
+def test_c4_late_chunks_keep_precision(awg, torch_cuda):
+    # phases near 1e8 cycles: tones of C4 evaluated around t = 1 s without the updates
+    w = W.config4(0)
+    op = oracle.plan_from_workload(w)
+    p = _gpu_plan(awg, w)
+    for c in (381, 4000):
+        V = oracle.c_waveform(op, c * w.chunk_len, c * w.chunk_len + 8192)
+        f = _np(p.synthesize_chunk_f32(c))[:8192]
+        assert_f32_close(f, V, f"C4 static chunk {c}")
+        assert_codes_close(_np(p.synthesize_chunk(c))[:8192], op.quantise(V), f"C4 static chunk {c}")
+    p.close()
+
+
+# ------------------------------------------------------------------ C5: scaling sweep
+@pytest.mark.parametrize("n_tones,chunk_len", W.config5_grid())
+def test_c5_cell(awg, torch_cuda, n_tones, chunk_len):
+    w = W.config5_cell(n_tones, chunk_len)
+    op = oracle.plan_from_workload(w)
+    p = _gpu_plan(awg, w)
+    out = _np(p.synthesize_chunk(0))
+    if n_tones * chunk_len <= (1 << 25):
+        wins = [(0, chunk_len)]
+    else:
+        movers = np.nonzero(w.profile == MINJERK)[0][:3]
+        must = [int(w.t_start[k] * w.sample_rate) for k in movers] + \
+               [int((w.t_start[k] + w.t_dur[k]) * w.sample_rate) for k in movers]
+        width = max(1024, min(8192, (1 << 24) // n_tones // 8 * 8))
+        wins = sample_windows(chunk_len, width, 4, seed=n_tones + chunk_len, must=must)
+    for (a, b), (V, codes) in zip(wins, oracle_windows(op, wins)):
+        assert_codes_close(out[a:b], codes, f"{w.name} [{a},{b})")
+    p.close()
+
+
+def test_c5_whole_chunk_moves_f32(awg, torch_cuda):
+    w = W.config5_cell(256, 1 << 16, whole_chunk_moves=True)
+    op = oracle.plan_from_workload(w)
+    p = _gpu_plan(awg, w)
+    V = oracle.c_waveform(op, 0, w.chunk_len)
+    assert_f32_close(_np(p.synthesize_chunk_f32(0)), V, w.name)
+    assert_codes_close(_np(p.synthesize_chunk(0)), op.quantise(V), w.name)
+    p.close()
+
+
+# ------------------------------------------------------------------ edge cases
+def _single(awg, fs, chunk_len, rows, scale=None, engine=None):
+    """rows: list of (f0, f1, A, phi0, t_start, t_dur, profile) -> (gpu Plan, OraclePlan)."""
+    cols = list(zip(*rows))
+    N = len(rows)
+    p = awg.Plan(N, fs, chunk_len, scale, engine if engine is not None else awg.AWG_ENGINE_AUTO)
+    p.set_trajectories(*cols)
+    op = oracle.OraclePlan(N, fs, chunk_len, scale if scale is not None else 0.9 * 32767.0)
+    op.set_trajectories(*cols)
+    return p, op
+
+
+def test_closed_form_quarter_rate_tone(awg, torch_cuda):
+    # f = fs/4: 0, 1, 0, -1 -> codes 0, 29490, 0, -29490 exactly
+    p, _ = _single(awg, 560e6, 1024, [(140e6, 140e6, 1.0, 0.0, 0.0, 0.0, STATIC)])
+    got = _np(p.synthesize_chunk(3))
+    assert np.array_equal(got, np.tile(np.array([0, 29490, 0, -29490], np.int16), 256))
+    p.close()
+
+
+def test_coherent_sum_and_zero_amplitude(awg, torch_cuda):
+    N = 16
+    f = np.linspace(80e6, 120e6, N)
+    rows = [(f[k], f[k], 1.0 / N, math.pi / 2, 0.0, 0.0, STATIC) for k in range(N)]
+    p, _ = _single(awg, 560e6, 256, rows)
+    assert abs(float(_np(p.synthesize_chunk_f32(0))[0]) - 1.0) < 2e-6  # V[0] = sum A_k = N*A
+    rows0 = [(f[k], f[k] + 1e6, 0.0, 0.3 * k, 1e-7, 1e-6, MINJERK) for k in range(N)]
+    p0, _ = _single(awg, 560e6, 4096, rows0)
+    assert not _np(p0.synthesize_chunk(0)).any()
+    p.close(); p0.close()
+
+
+def test_saturation(awg, torch_cuda):
+    p, op = _single(awg, 560e6, 1024, [(10e6, 10e6, 2.0, 0.0, 0.0, 0.0, STATIC)])
+    got = _np(p.synthesize_chunk(0))
+    assert got.max() == 32767 and got.min() == -32768
+    assert_codes_close(got, op.chunk(0), "saturation")
+    p.close()
+
+
+@pytest.mark.parametrize("chunk_len", [8, 264, 1000, 4096])
+@pytest.mark.parametrize("n_tones", [1, 33, 100])
+def test_ragged_sizes(awg, torch_cuda, chunk_len, n_tones):
+    rng = np.random.default_rng(chunk_len + n_tones)
+    rows = []
+    for k in range(n_tones):
+        f0 = rng.uniform(20e6, 250e6)
+        prof = int(rng.integers(0, 3))
+        rows.append((f0, f0 + rng.uniform(-5e6, 5e6), 1.0 / n_tones, rng.uniform(0, 6.28),
+                     rng.uniform(-2e-6, 8e-6), rng.uniform(1e-6, 20e-6), prof))
+    p, op = _single(awg, 560e6, chunk_len, rows)
+    n_chunks = max(2, 12288 // chunk_len)
+    got = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(n_chunks)])
+    gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(n_chunks)])
+    V = oracle.c_waveform(op, 0, n_chunks * chunk_len)
+    assert_f32_close(gotf, V, f"ragged N={n_tones} L={chunk_len}")
+    assert_codes_close(got, op.quantise(V), f"ragged N={n_tones} L={chunk_len}")
+    p.close()
+
+
+def test_max_tone_count_4096_and_more(awg, torch_cuda):
+    N = 5000
+    rng = np.random.default_rng(99)
+    f0 = rng.uniform(20e6, 250e6, N)
+    rows = [(f0[k], f0[k] + (3e6 if k % 3 == 0 else 0.0), 1.0 / N, rng.uniform(0, 6.28), 0.0, 30e-6,
+             MINJERK if k % 3 == 0 else STATIC) for k in range(N)]
+    p, op = _single(awg, 560e6, 2048, rows)
+    V = oracle.c_waveform(op, 5 * 2048, 6 * 2048)
+    assert_f32_close(_np(p.synthesize_chunk_f32(5)), V, "N=5000")
+    p.close()
+
+
+def test_special_moves(awg, torch_cuda):
+    fs = 560e6
+    rows = [
+        (100e6, 104e6, 0.2, 0.1, 3e-6, 0.0, MINJERK),        # instant retune (T = 0)
+        (90e6, 80e6, 0.2, 0.2, -1.5e-6, 4e-6, LINEAR),       # started before t = 0, off the sample grid
+        (120e6, 170e6, 0.2, 0.3, 1.00000037e-6, 0.4e-6, MINJERK),  # 50 MHz in 0.4 us: fp64 path (CLS_EXACT)
+        (60e6, 65e6, 0.2, 0.4, 2e-6, 5e-6, MINJERK),         # fast move: degree-6 class
+        (200e6, 199e6, 0.2, 0.5, 0.0, 21e-6, LINEAR),        # slow linear chirp over the whole span
+    ]
+    p, op = _single(awg, fs, 4096, rows)
+    n = 3 * 4096
+    V = oracle.c_waveform(op, 0, n)
+    gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(3)])
+    assert_f32_close(gotf, V, "special moves")
+    got = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(3)])
+    assert_codes_close(got, op.quantise(V), "special moves")
+    # the fp64 engine agrees much more tightly
+    p.set_engine(awg.AWG_ENGINE_FP64)
+    gotd = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(3)])
+    assert_f32_close(gotd, V, "special moves fp64", tol=3e-7)
+    p.close()
+
+
+def test_mid_move_update_and_static_update(awg, torch_cuda):
+    fs, L = 560e6, 4096
+    rows = [(100e6, 103e6, 0.5, 0.9, 0.0, 4 * L / fs, MINJERK), (70e6, 70e6, 0.5, 0.0, 0.0, 0.0, STATIC)]
+    p, op = _single(awg, fs, L, rows)
+    for plan in (p, op):
+        plan.update_trajectories(2, [0], [100e6], [2 * L / fs], [LINEAR])   # while tone 0 is mid-move
+        plan.update_trajectories(5, [1, 0], [75e6, 0.0], [1.5 * L / fs, 0.0], [MINJERK, STATIC])
+    for c in range(2, 9):
+        if c < 5:
+            continue  # chunks before the latest update are gone from the GPU plan (it keeps one segment)
+        V = oracle.c_waveform(op, c * L, (c + 1) * L)
+        assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"update chunk {c}")
+    p.close()
+    # same schedule, chunk by chunk, checking each chunk right after its update
+    p, op = _single(awg, fs, L, rows)
+    sched = {2: ([0], [100e6], [2 * L / fs], [LINEAR]), 5: ([1, 0], [75e6, 0.0], [1.5 * L / fs, 0.0], [MINJERK, STATIC])}
+    for c in range(9):
+        if c in sched:
+            p.update_trajectories(c, *sched[c])
+            op.update_trajectories(c, *sched[c])
+        V = oracle.c_waveform(op, c * L, (c + 1) * L)
+        assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"stepwise chunk {c}")
+        assert_codes_close(_np(p.synthesize_chunk(c)), op.quantise(V), f"stepwise chunk {c}")
+    p.close()
+
+
+def test_error_codes_and_state(awg, torch_cuda):
+    torch = torch_cuda
+    p = awg.Plan(4, 560e6, 1024)
+    buf = torch.empty(1024, dtype=torch.int16, device="cuda")
+    with pytest.raises(awg.AwgError) as ei:
+        awg.awg_synthesize_chunk(p.handle, 0, buf.data_ptr())
+    assert ei.value.status == awg.AWG_ERR_STATE  # no table yet
+    z = np.zeros(4)
+    with pytest.raises(awg.AwgError) as ei:
+        p.set_trajectories(z + 1e6, z + 1e6, z, z, z, z - 1.0, np.zeros(4, np.int32))
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG  # negative duration
+    with pytest.raises(awg.AwgError) as ei:
+        p.set_trajectories(z + float("inf"), z, z, z, z, z, np.zeros(4, np.int32))
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    with pytest.raises(awg.AwgError) as ei:
+        p.set_trajectories(z, z, z, z, z, z, np.full(4, 7, np.int32))
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    p.set_trajectories(z + 1e6, z + 1e6, z + 0.1, z, z, z, np.zeros(4, np.int32))
+    with pytest.raises(awg.AwgError) as ei:
+        awg.awg_synthesize_chunk(p.handle, 0, buf.data_ptr() + 2)
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG  # misaligned
+    with pytest.raises(awg.AwgError) as ei:
+        awg.awg_synthesize_chunk(p.handle, -1, buf.data_ptr())
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    with pytest.raises(awg.AwgError) as ei:
+        p.update_trajectories(3, [1, 1], [2e6, 2e6], [1e-6, 1e-6], [2, 2])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG  # duplicate tone
+    with pytest.raises(awg.AwgError) as ei:
+        p.update_trajectories(3, [4], [2e6], [1e-6], [2])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG  # out of range
+    p.update_trajectories(3, [1], [2e6], [1e-6], [2])
+    with pytest.raises(awg.AwgError) as ei:
+        p.update_trajectories(2, [1], [2e6], [1e-6], [2])
+    assert ei.value.status == awg.AWG_ERR_STATE  # decreasing chunk order
+    with pytest.raises(awg.AwgError) as ei:
+        awg.awg_synthesize_chunk(p.handle, 2, buf.data_ptr())
+    assert ei.value.status == awg.AWG_ERR_STATE  # earlier than the latest update
+    before = awg.awg_kernel_launch_count()
+    p.synthesize_chunk(3, out=buf)
+    assert awg.awg_kernel_launch_count() == before + 1
+    ring = awg.Ring(p, 2, False)
+    ring.submit(3); ring.submit(4)
+    with pytest.raises(awg.AwgError) as ei:
+        ring.submit(5)
+    assert ei.value.status == awg.AWG_ERR_STATE  # ring full
+    with pytest.raises(awg.AwgError) as ei:
+        p.close()
+    assert ei.value.status == awg.AWG_ERR_STATE  # ring still bound
+    ring.close()
+
+
+def test_ring_underrun_counter_fires_on_a_stall(awg, torch_cuda):
+    import time
+    w = W.config4(0)
+    p = _gpu_plan(awg, w)
+    ring = awg.Ring(p, 2, False)
+    ring.submit(0)
+    idx, _, _, ok = ring.acquire(); ring.release(idx)
+    assert ok
+    time.sleep(0.02)        # the producer stalls for 20 ms: 7 chunk periods of 2.62 ms
+    ring.submit(1)          # only now is chunk 1 enqueued: it cannot have been ready when it was due
+    time.sleep(0.0)
+    idx, _, _, ok = ring.acquire(); ring.release(idx)
+    produced, underruns, _ = ring.stats()
+    assert produced == 2 and underruns == 1 and not ok
+    ring.close(); p.close()
+
+
+def test_streams_do_not_change_results(awg, torch_cuda):
+    torch = torch_cuda
+    w = W.config1().rechunked(1 << 16)
+    p = _gpu_plan(awg, w)
+    ref = _np(p.synthesize_chunk(5))
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        other = p.synthesize_chunk(5)
+    s.synchronize()
+    assert np.array_equal(_np(other), ref)
+    p.close()
