@@ -1,0 +1,459 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the additive-synthesis hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+One "step" = one pass of the whole hot path (trajectory table resident -> phase re-centring -> sine ->
+accumulate -> quantise -> int16 stores) over BASELINE.json config 2: 100 tones at 560 MS/s for 10 ms
+(5.6 M samples, 25 chunks of 224 000), synthesised by ONE awg_synthesize_range launch into a device
+buffer.  Metric: tone-samples/s (G).  Rank 0 prints ONE JSON line.
+
+  value      device-timed (CUDA events on the launch stream), inputs resident in HBM
+  e2e        the same workload through the C ABI with HOST buffers: awg_set_trajectories from host arrays
+             (H2D table upload) + awg_synthesize_range_host into pinned host memory (D2H of the int16 codes)
+  roofline   the synthesis kernel is bound by the XU (MUFU) pipe, one MUFU.SIN per tone-sample:
+             peak = 16 MUFU/clk/SM x 148 SMs x sm_max_mhz; bound "alu"
+  cpu_baseline  the oracle (oracle/awg_oracle_c.c, as it stands) on this box's host cores, bounded sample
+  extras     the other configs (C1, C3, C4 ring, C5 sweep) and the real-time capacity search
+
+Multi-GPU (--gpus N under torchrun): the path shards by time with no exchange (every chunk is a pure
+function of the absolute sample index), so each rank synthesises its own replica of the workload --
+"replicas only", weak scaling, no data-path collective; NCCL is used for the barrier and the max-over-ranks
+time only.  --impl reference times the oracle on the host cores (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import awg_workloads as W  # noqa: E402
+
+METRIC = "tone-samples/s"
+UNIT = "Gtone-samples/s"
+MUFU_PER_CLK_PER_SM = 16  # sm_100: 4 SFU lanes per SM sub-partition (measured 15.85/clk/SM, profiles/)
+N_SM = 148
+L2_BYTES = 126 * (1 << 20)
+
+
+def read_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples = []  # (t, sm_mhz, reasons_bitmask)
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _reasons(self):
+        nv = self.nv
+        for name in ("nvmlDeviceGetCurrentClocksEventReasons", "nvmlDeviceGetCurrentClocksThrottleReasons"):
+            fn = getattr(nv, name, None)
+            if fn is not None:
+                try:
+                    return int(fn(self.h))
+                except Exception:
+                    pass
+        return 0
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                mhz = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.samples.append((time.perf_counter(), mhz, self._reasons()))
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join(timeout=1.0)
+
+    def summary(self, t0: float, t1: float):
+        if self.nv is None or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml_unavailable"]}
+        inside = [s for s in self.samples if t0 <= s[0] <= t1]
+        if not inside:  # region shorter than the sampling period: take the nearest sample
+            inside = [min(self.samples, key=lambda s: abs(s[0] - 0.5 * (t0 + t1)))]
+        mask = 0
+        for s in inside:
+            mask |= s[2]
+        names = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+                 0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+                 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+        reasons = [n for b, n in names.items() if mask & b and n != "gpu_idle"]
+        return {"sm_mhz": float(np.median([s[1] for s in inside])), "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(inside)}
+
+
+# --------------------------------------------------------------------------------------------------
+def max_over_ranks(x: float, dist, device) -> float:
+    """MAX all-reduce of a scalar over the ranks (identity when dist is None)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank_per_step: int, steps: int, world: int, seconds_max_over_ranks: float) -> float:
+    """Aggregate units/s of N independent replicas: every rank does the same work, the slowest rank sets the time."""
+    return world * units_per_rank_per_step * steps / seconds_max_over_ranks
+
+
+def oracle_rate(w, n_samples: int, repeats: int = 1):
+    """tone-samples/s of the C oracle on the first n_samples of workload w, all host cores."""
+    import oracle
+    op = oracle.plan_from_workload(w)
+    n_samples = min(n_samples, w.n_samples)
+    oracle.c_waveform(op, 0, 4096)  # build + page in
+    best = None
+    for _ in range(repeats):
+        t = time.perf_counter()
+        V = oracle.c_waveform(op, 0, n_samples)
+        op.quantise(V)
+        dt = time.perf_counter() - t
+        best = dt if best is None else min(best, dt)
+    return w.n_tones * n_samples / best, oracle.c_num_threads(), best
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    w = W.config2()
+    op = oracle.plan_from_workload(w)
+    # warm-up doubles as a rate probe: size the per-step sample so that the K steps end within ~2 minutes
+    t0 = time.perf_counter()
+    for _ in range(max(1, args.warmup)):
+        oracle.c_waveform(op, 0, 1 << 16)
+    rate = max(1, args.warmup) * (1 << 16) * w.n_tones / (time.perf_counter() - t0)
+    n = int(min(1 << 20, max(4096, rate * 120.0 / args.steps / w.n_tones)))
+    n -= n % 4096
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        op.quantise(oracle.c_waveform(op, 0, n))
+    dt = time.perf_counter() - t0
+    val = w.n_tones * n * args.steps / dt / 1e9
+    cores = oracle.c_num_threads()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "C2: 100 tones, 560 MS/s, 10 ms (BASELINE.json configs[1])",
+                   "sample": f"first {n} of {w.n_samples} samples per step"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"first {n} samples x {w.n_tones} tones of C2 per step, {args.steps} steps"},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+def device_time_range(torch, plan, n_chunks, bufs, steps, warmup):
+    """ms per step of awg_synthesize_range, CUDA events on the launch stream, rotating output buffers."""
+    stream = torch.cuda.current_stream()
+    for i in range(warmup):
+        plan.synthesize_range(0, n_chunks, out=bufs[i % len(bufs)], stream=stream)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record(stream)
+    for i in range(steps):
+        plan.synthesize_range(0, n_chunks, out=bufs[i % len(bufs)], stream=stream)
+    b.record(stream)
+    b.synchronize()
+    return a.elapsed_time(b) / steps
+
+
+def make_bufs(torch, n_samples):
+    n_buf = max(2, -(-int(1.06 * L2_BYTES) // (2 * n_samples)))
+    return [torch.empty(n_samples, dtype=torch.int16, device="cuda") for _ in range(n_buf)]
+
+
+def stream_through_ring(awg, w, host_mirror, n_chunks=None, n_slots=4):
+    """Runs workload w (with its per-chunk updates) through the ring as fast as it goes.
+    Returns (underruns, max_chunk_ms, wall_s, chunks)."""
+    p = awg.Plan.from_workload(w)
+    ring = awg.Ring(p, n_slots=n_slots, host_mirror=host_mirror)
+    ups = w.updates_by_chunk()
+    n_chunks = n_chunks or w.n_chunks
+    depth = n_slots - 1
+    t0 = time.perf_counter()
+    for c in range(n_chunks + depth):
+        if c < n_chunks:
+            ring.submit(c, ups.get(c))
+        if c >= depth:
+            idx, _, _, _ = ring.acquire()
+            ring.release(idx)
+    wall = time.perf_counter() - t0
+    produced, underruns, max_ms = ring.stats()
+    ring.close()
+    p.close()
+    return underruns, max_ms, wall, produced
+
+
+def realtime_capacity(torch, awg, fs, chunk_len, mix, host_mirror, seconds, lo=16, hi=65536):
+    """Largest tone count whose every chunk completes within chunk_len/fs: bisection on N,
+    each probe streams `seconds` of signal through the ring and reads the longest per-chunk device time."""
+    deadline_ms = chunk_len / fs * 1e3
+    n_chunks = max(8, int(round(seconds * fs / chunk_len)))
+
+    def ok(n):
+        w = W.capacity_toneset(n, fs, chunk_len, mix, n_chunks=n_chunks)
+        _, max_ms, _, _ = stream_through_ring(awg, w, host_mirror, n_chunks=n_chunks, n_slots=3)
+        return max_ms <= deadline_ms, max_ms
+
+    good, bad = None, None
+    n = lo
+    while n <= hi:  # exponential search for the first failing count
+        passed, _ = ok(n)
+        if passed:
+            good = n
+            n *= 2
+        else:
+            bad = n
+            break
+    if good is None:
+        return 0
+    if bad is None:
+        return good
+    while bad - good > max(8, good // 64):
+        mid = (good + bad) // 2
+        passed, _ = ok(mid)
+        if passed:
+            good = mid
+        else:
+            bad = mid
+    return good
+
+
+def run_extras(torch, awg, peak_sin, quick):
+    out = {}
+    # per-config device throughput (range launch for C1/C3, per-cell chunk launch for C5)
+    cfgs = {}
+    for name, w in (("C1", W.config1()), ("C3", W.config3())):
+        p = awg.Plan.from_workload(w)
+        bufs = make_bufs(torch, w.n_samples)
+        ms = device_time_range(torch, p, w.n_chunks, bufs, 5 if name == "C3" else 50, 3)
+        cfgs[name] = {"tones": w.n_tones, "samples": w.n_samples, "ms": ms, "gts_per_s": w.tone_samples / ms / 1e6,
+                      "out_MS_per_s": w.n_samples / ms / 1e3, "frac_xu_peak": w.tone_samples / (ms * 1e-3) / peak_sin}
+        del bufs
+        p.close()
+    w4 = W.config4(96 if quick else 382)
+    for mirror in (False, True):
+        und, max_ms, wall, produced = stream_through_ring(awg, w4, mirror)
+        cfgs["C4_ring" + ("_d2h" if mirror else "")] = {
+            "tones": w4.n_tones, "chunks": produced, "underruns": und, "max_chunk_ms": max_ms,
+            "deadline_ms": w4.chunk_len / w4.sample_rate * 1e3, "wall_s": wall,
+            "gts_per_s": w4.n_tones * w4.chunk_len * produced / wall / 1e9,
+            "realtime_margin": (w4.chunk_len / w4.sample_rate) / (wall / produced)}
+    out["configs"] = cfgs
+    sweep = {}
+    for n_t, cl in W.config5_grid():
+        w = W.config5_cell(n_t, cl)
+        p = awg.Plan.from_workload(w)
+        bufs = make_bufs(torch, cl)
+        ms = device_time_range(torch, p, 1, bufs, 20, 3)
+        sweep[f"N{n_t}_L{cl.bit_length() - 1}"] = round(w.tone_samples / ms / 1e6, 2)
+        del bufs
+        p.close()
+    out["C5_gts_per_s"] = sweep
+    secs = 0.2 if quick else 1.0
+    cap = {}
+    for fs, cl, tag in ((560e6, 1 << 20, "560MS"), (100e6, 1 << 18, "100MS")):
+        for mix in ("static", "half", "moving"):
+            for mirror in (False, True):
+                key = f"{tag}_{mix}" + ("_d2h" if mirror else "")
+                cap[key] = realtime_capacity(torch, awg, fs, cl, mix, mirror, secs)
+    out["max_realtime_tones"] = cap
+    out["max_realtime_tones_note"] = (f"largest N with every chunk's device time <= chunk_len/fs over {secs:g} s of "
+                                      "signal through the ring (3 slots); tone sets drawn like C5; _d2h = pinned-host mirror on")
+    out["paper_context"] = {"hardware": "Quadro RTX 6000 + PCIe 2.0 DAC (PAPER.md:69)", "streaming_tones_560MS": 20,
+                            "streaming_tones_100MS": 194, "playback_tones_35ms_560MS": 1000,
+                            "static_fp32_gts_per_s": 79.4}
+    return out
+
+
+def run_ours(args):
+    import torch
+    import paper_2403_15582_b200 as awg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    peaks, peaks_src = read_peaks()
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_sin = MUFU_PER_CLK_PER_SM * N_SM * sm_max_mhz * 1e6  # MUFU.SIN per second at max clock
+
+    w = W.config2()
+    plan = awg.Plan.from_workload(w)
+    bufs = make_bufs(torch, w.n_samples)
+    stream = torch.cuda.current_stream()
+    host_out = torch.empty(w.n_samples, dtype=torch.int16, pin_memory=True)
+    traj = (w.f0, w.f1, w.A, w.phi0, w.t_start, w.t_dur, w.profile)
+
+    # ---- device-timed value -------------------------------------------------------------------
+    sampler = ClockSampler(local)
+    sampler.start()
+    for i in range(max(3, args.warmup)):
+        plan.synthesize_range(0, w.n_chunks, out=bufs[i % len(bufs)], stream=stream)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    launches0 = awg.awg_kernel_launch_count()
+    t_host0 = time.perf_counter()
+    ev0.record(stream)
+    for i in range(args.steps):
+        plan.synthesize_range(0, w.n_chunks, out=bufs[i % len(bufs)], stream=stream)
+    ev1.record(stream)
+    barrier()
+    t_host1 = time.perf_counter()
+    launches = awg.awg_kernel_launch_count() - launches0
+    ms_total = ev0.elapsed_time(ev1)
+    sampler.stop()
+    clocks = sampler.summary(t_host0, t_host1)
+    ms_total_max = max_over_ranks(ms_total, dist, "cuda")
+    ms_per_step = ms_total_max / args.steps
+    value = whole_job_rate(w.tone_samples, args.steps, world, ms_total_max * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with host buffers -----------------------------------------
+    for _ in range(2):
+        plan.set_trajectories(*traj)
+        plan.synthesize_range_host(0, w.n_chunks, out=host_out)
+    io0 = plan.io_bytes()
+    e2e_steps = max(3, min(args.steps, 50))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        plan.set_trajectories(*traj)                                  # host arrays -> table -> H2D upload
+        plan.synthesize_range_host(0, w.n_chunks, out=host_out)       # synthesis + D2H of every int16 code
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    io1 = plan.io_bytes()
+    dt_max = max_over_ranks(dt, dist, "cuda")
+    e2e_value = whole_job_rate(w.tone_samples, e2e_steps, world, dt_max) / 1e9
+    e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (io1[0] - io0[0]) // e2e_steps,
+           "d2h_bytes_per_step": (io1[1] - io0[1]) // e2e_steps, "steps": e2e_steps,
+           "ms_per_step": dt_max / e2e_steps * 1e3,
+           "what": "awg_set_trajectories(host arrays) + awg_synthesize_range_host(pinned host int16)"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant (only) kernel ---------------------------------------------------
+    ms_local = ms_total / args.steps
+    achieved = w.tone_samples / (ms_local * 1e-3)  # MUFU.SIN per second = tone-samples per second of one launch
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get("awg_mufu_kernel_C2_dram_bytes_per_launch")
+    except Exception:
+        pass
+    roofline = {
+        "bound": "alu", "pipe": "XU (MUFU.SIN), one per tone-sample", "achieved": achieved / 1e9, "peak": peak_sin / 1e9,
+        "unit": "Gsin/s", "frac": achieved / peak_sin, "traffic": traffic,
+        "peak_how": f"16 MUFU/clk/SM x 148 SMs x {sm_max_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peaks_src})",
+        "kernel": "awg_mufu_kernel", "launch_ms": ms_local,
+        "hbm": {"algorithmic_bytes_per_launch": 2 * w.n_samples, "achieved_gbs": 2 * w.n_samples / (ms_local * 1e-3) / 1e9,
+                "peak_gbs": peaks.get("hbm_gbs"), "frac": 2 * w.n_samples / (ms_local * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0))},
+    }
+    if clocks.get("sm_mhz"):
+        roofline["frac_at_achieved_clock"] = achieved / (MUFU_PER_CLK_PER_SM * N_SM * clocks["sm_mhz"] * 1e6)
+
+    # ---- oracle on this box's host cores (bounded sample) ----------------------------------------
+    n_cpu = 1 << 22
+    rate, cores, secs = oracle_rate(w, n_cpu)
+    cpu_baseline = {"value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+                    "sample": f"first {min(n_cpu, w.n_samples)} of {w.n_samples} samples x {w.n_tones} tones of C2, "
+                              f"{secs:.2f} s wall"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "C2: 100 tones at 560 MS/s for 10 ms = 5.6 M samples, 50 min-jerk movers (BASELINE.json configs[1], seed 1)",
+                   "tones": w.n_tones, "samples_per_step": w.n_samples, "launch": "one awg_synthesize_range per step",
+                   "l2": f"output rotates over {len(bufs)} device buffers ({len(bufs) * 2 * w.n_samples / 1e6:.0f} MB > 126 MB L2); "
+                         "the only input is the 9 KB tone table",
+                   "parallelism": "replicas only (no data-path collective)" if world > 1 else "1 GPU"},
+        "out_MS_per_s": world * w.n_samples / ms_per_step / 1e3,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "phase_dtype": "u64 fixed-point turns + fp64 re-centring, u32/fp32 in the inner loop",
+    }
+    if world == 1 and not args.no_extras:
+        line["extras"] = run_extras(torch, awg, peak_sin, not args.full)
+    plan.close()
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-extras", action="store_true", help="skip the other configs and the capacity search")
+    ap.add_argument("--full", action="store_true", help="extras at full length: 382-chunk C4, 1 s per capacity probe")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

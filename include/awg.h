@@ -141,10 +141,10 @@ awg_status awg_ring_submit(awg_ring *r, int64_t chunk_idx, int32_t n_upd, const 
 
 /* Blocks until the oldest submitted chunk is complete (and mirrored when host_mirror is on), then
  * lends its slot: *dev_ptr (device) and *host_ptr (pinned host or NULL) stay valid until
- * awg_ring_release.  Returns AWG_ERR_UNDERRUN (pointers still valid) when the chunk was not ready
- * by its deadline: chunk i of a run is due (i - prefill) * chunk_len / sample_rate seconds after
- * the first acquire, where prefill = chunks submitted before that first acquire.
- * Errors: STATE (nothing submitted). */
+ * awg_ring_release.  A virtual DAC starts when the first acquire returns and consumes one chunk every
+ * chunk_len / sample_rate seconds: the j-th acquired chunk (j = 0, 1, ...) is due j periods after that
+ * instant.  Returns AWG_ERR_UNDERRUN (pointers still valid, chunk still lent) when the chunk was
+ * submitted after it was due or was not complete when due.  Errors: STATE (nothing submitted). */
 awg_status awg_ring_acquire(awg_ring *r, int64_t *chunk_idx, const int16_t **dev_ptr,
                             const int16_t **host_ptr);
 awg_status awg_ring_release(awg_ring *r, int64_t chunk_idx);
@@ -155,6 +155,10 @@ awg_status awg_ring_stats(awg_ring *r, int64_t *produced, int64_t *underruns, do
 awg_status awg_ring_destroy(awg_ring *r);
 
 /* ---- misc --------------------------------------------------------------------------------------- */
+
+/* Bytes this plan has copied host->device (trajectory table uploads) and device->host (host-destination
+ * synthesis and ring mirror) since creation.  Either pointer may be NULL. */
+awg_status awg_plan_io_bytes(awg_plan *p, int64_t *h2d_bytes, int64_t *d2h_bytes);
 
 /* Number of kernels the library has launched since load (all plans); for launch accounting. */
 int64_t awg_kernel_launch_count(void);

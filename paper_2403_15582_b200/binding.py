@@ -2,7 +2,7 @@
 
 Every step of the hot path runs in the CUDA library; nothing here computes.  PyTorch is used for
 device memory and streams only.  There is no CPU fallback: if ``libawg_b200.so`` is missing the
-import fails (build it with ``python -m paper_2403_15582_b200.build``).
+import fails (build it with ``python paper_2403_15582_b200/build.py``).
 """
 from __future__ import annotations
 
@@ -36,7 +36,7 @@ EXPORTED = (
     "awg_plan_create", "awg_plan_destroy", "awg_set_scale", "awg_set_engine", "awg_set_trajectories",
     "awg_update_trajectories", "awg_synthesize_chunk", "awg_synthesize_chunk_f32", "awg_synthesize_range",
     "awg_synthesize_range_host", "awg_ring_create", "awg_ring_submit", "awg_ring_acquire", "awg_ring_release",
-    "awg_ring_stats", "awg_ring_destroy", "awg_kernel_launch_count", "awg_last_error",
+    "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_kernel_launch_count", "awg_last_error",
 )
 
 
@@ -44,7 +44,7 @@ def _load() -> ctypes.CDLL:
     if not os.path.exists(LIB_PATH):
         raise ImportError(
             f"{LIB_PATH} is missing: the CUDA extension has not been built "
-            "(python -m paper_2403_15582_b200.build).  There is no CPU fallback.")
+            "(python paper_2403_15582_b200/build.py).  There is no CPU fallback.")
     lib = ctypes.CDLL(LIB_PATH)
     P, D, I32, I64 = c_void_p, c_double, c_int32, c_int64
     sig = {
@@ -64,11 +64,16 @@ def _load() -> ctypes.CDLL:
         "awg_ring_release": (I32, [P, I64]),
         "awg_ring_stats": (I32, [P, POINTER(I64), POINTER(I64), POINTER(D)]),
         "awg_ring_destroy": (I32, [P]),
+        "awg_plan_io_bytes": (I32, [P, POINTER(I64), POINTER(I64)]),
         "awg_kernel_launch_count": (I64, []),
         "awg_last_error": (c_char_p, []),
     }
     for name, (res, args) in sig.items():
-        fn = getattr(lib, name)
+        try:
+            fn = getattr(lib, name)
+        except AttributeError as e:
+            raise ImportError(f"{LIB_PATH} is stale (no symbol {name}): rebuild it with "
+                              "python paper_2403_15582_b200/build.py") from e
         fn.restype = res
         fn.argtypes = args
     return lib
@@ -199,6 +204,12 @@ def awg_ring_destroy(ring) -> None:
     _check(_lib.awg_ring_destroy(ring))
 
 
+def awg_plan_io_bytes(plan) -> Tuple[int, int]:
+    a, b = c_int64(), c_int64()
+    _check(_lib.awg_plan_io_bytes(plan, byref(a), byref(b)))
+    return a.value, b.value
+
+
 def awg_kernel_launch_count() -> int:
     return int(_lib.awg_kernel_launch_count())
 
@@ -274,6 +285,9 @@ class Plan:
             raise ValueError("host output tensor has the wrong dtype, size or device")
         awg_synthesize_range_host(self._h, first_chunk, n_chunks, out.data_ptr())
         return out
+
+    def io_bytes(self) -> Tuple[int, int]:
+        return awg_plan_io_bytes(self._h)
 
     def close(self) -> None:
         if self._h is not None:

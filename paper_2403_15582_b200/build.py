@@ -1,6 +1,9 @@
 """Builds the C-ABI shared library in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2403_15582_b200.build [--force] [--verbose]
+    python paper_2403_15582_b200/build.py [--force] [--verbose]
+
+Run it by path (or through ``__graft_entry__.build()``): importing the package itself needs the
+library this script produces.
 
 Output: paper_2403_15582_b200/libawg_b200.so (git-ignored; it travels to the GPU box with the tree).
 """

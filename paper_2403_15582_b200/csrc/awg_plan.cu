@@ -377,6 +377,14 @@ awg_status awg_plan_destroy(awg_plan *p)
     return AWG_OK;
 }
 
+awg_status awg_plan_io_bytes(awg_plan *p, int64_t *h2d_bytes, int64_t *d2h_bytes)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (h2d_bytes) *h2d_bytes = p->h2d_bytes;
+    if (d2h_bytes) *d2h_bytes = p->d2h_bytes;
+    return AWG_OK;
+}
+
 awg_status awg_set_scale(awg_plan *p, double scale)
 {
     if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");

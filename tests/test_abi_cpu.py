@@ -19,8 +19,12 @@ def _declared_symbols():
 
 @pytest.fixture(scope="module")
 def built():
-    from paper_2403_15582_b200 import build
-    return build.build()
+    # loaded by path: importing the package needs the library this script builds
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("awg_build", os.path.join(ROOT, "paper_2403_15582_b200", "build.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod.build()
 
 
 def test_header_declares_the_north_star_calls():
