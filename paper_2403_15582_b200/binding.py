@@ -30,6 +30,7 @@ AWG_PROFILE_MINJERK = 2
 AWG_ENGINE_AUTO = 0
 AWG_ENGINE_MUFU = 1
 AWG_ENGINE_FP64 = 2
+AWG_ENGINE_FMA = 3
 
 #: every symbol include/awg.h declares (tests check that the library exports each of them)
 EXPORTED = (

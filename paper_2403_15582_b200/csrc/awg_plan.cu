@@ -84,6 +84,17 @@ int classify(int profile, long double DT, long double Tn)
     return CLS_DEG6;
 }
 
+// Rotation table of a carrier for the angle-addition engine: A cos(2 pi j w), A sin(2 pi j w), j = 0..7,
+// from the 64-bit fixed-point frequency (j*w wraps exactly), evaluated in long double, rounded once to fp32.
+void make_rot(float *rot, uint64_t w, float A)
+{
+    for (int j = 0; j < kSPT; ++j) {
+        const long double turns = ldexpl(static_cast<long double>(static_cast<int64_t>(w * static_cast<uint64_t>(j))), -64);
+        rot[j] = static_cast<float>(static_cast<long double>(A) * cosl(kTwoPiL * turns));
+        rot[kSPT + j] = static_cast<float>(static_cast<long double>(A) * sinl(kTwoPiL * turns));
+    }
+}
+
 void make_static(HostTone &h)
 {
     h.profile = AWG_PROFILE_STATIC;
@@ -96,6 +107,8 @@ void make_static(HostTone &h)
     h.DT = 0.0L;
     h.theta_post = h.theta_pre;
     h.w_post = h.w_pre;
+    make_rot(h.rot_pre, h.w_pre, h.A);
+    std::memcpy(h.rot_post, h.rot_pre, sizeof h.rot_post);
 }
 
 // Fills the move part of h (everything but theta_pre/w_pre/f0/A) for a move f0 -> f1 that starts at the
@@ -120,6 +133,8 @@ void make_move(HostTone &h, long double fs, long double f1, int profile, long do
     //                     = [theta - (f1-f0) t_s - DT/2] + (f1/fs) n
     h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(h.DT / 2.0L);
     h.cls = classify(profile, h.DT, h.Tn);
+    make_rot(h.rot_pre, h.w_pre, h.A);
+    make_rot(h.rot_post, h.w_post, h.A);
 }
 
 long double profile_h(int profile, long double s)  // frequency ramp 0 -> 1
@@ -140,53 +155,38 @@ long double profile_g(int profile, long double s)  // its integral
 
 static void fill_staging(const awg_plan *p, unsigned char *dst)
 {
-    const int np = p->n_pad;
-    uint64_t *theta_pre = reinterpret_cast<uint64_t *>(dst);
-    uint64_t *w_pre = theta_pre + np;
-    uint64_t *theta_post = w_pre + np;
-    uint64_t *w_post = theta_post + np;
-    int64_t *ns_int = reinterpret_cast<int64_t *>(w_post + np);
-    double *ns_frac = reinterpret_cast<double *>(ns_int + np);
-    double *Tn = ns_frac + np;
-    double *inv_Tn = Tn + np;
-    double *DT = inv_Tn + np;
-    float *A = reinterpret_cast<float *>(DT + np);
-    int32_t *cls = reinterpret_cast<int32_t *>(A + np);
-    for (int i = 0; i < np; ++i) {
-        HostTone h{};
-        if (i < p->n_tones) h = p->tones[i];
-        theta_pre[i] = h.theta_pre;
-        w_pre[i] = h.w_pre;
-        theta_post[i] = h.theta_post;
-        w_post[i] = h.w_post;
-        ns_int[i] = h.ns_int;
-        ns_frac[i] = h.ns_frac;
-        Tn[i] = static_cast<double>(h.Tn);
-        inv_Tn[i] = h.Tn > 0.0L ? static_cast<double>(1.0L / h.Tn) : 0.0;
-        DT[i] = static_cast<double>(h.DT);
-        A[i] = h.A;
-        cls[i] = (h.profile << 8) | h.cls;
+    ToneRec *out = reinterpret_cast<ToneRec *>(dst);
+    for (int i = 0; i < p->n_pad; ++i) {
+        ToneRec r;
+        std::memset(&r, 0, sizeof r);
+        if (i < p->n_tones) {
+            const HostTone &h = p->tones[i];
+            r.A = h.A;
+            r.cls = (h.profile << 8) | h.cls;
+            r.theta_pre = h.theta_pre;
+            r.w_pre = h.w_pre;
+            r.theta_post = h.theta_post;
+            r.w_post = h.w_post;
+            r.ns_int = static_cast<double>(h.ns_int);
+            r.ns_frac = h.ns_frac;
+            r.Tn = static_cast<double>(h.Tn);
+            if (h.Tn > 0.0L) {
+                const long double rT = 1.0L / h.Tn;
+                r.inv_Tn = static_cast<double>(rT);
+                r.DT = static_cast<double>(h.DT);
+                r.q1 = static_cast<double>(h.DT * rT);
+                long double q = kTwoPiL * h.DT * rT, fact = 1.0L;  // 2 pi DT / Tn^k / k!
+                for (int k = 2; k <= 6; ++k) {
+                    q *= rT;
+                    fact *= k;
+                    r.q[k - 2] = static_cast<float>(q / fact);
+                }
+            }
+            std::memcpy(r.rot_pre, h.rot_pre, sizeof r.rot_pre);
+            std::memcpy(r.rot_post, h.rot_post, sizeof r.rot_post);
+        }
+        out[i] = r;
     }
-}
-
-static ToneTable table_view(const awg_plan *p, int v)
-{
-    const int np = p->n_pad;
-    unsigned char *d = p->dev_table[v];
-    ToneTable t;
-    t.theta_pre = reinterpret_cast<uint64_t *>(d);
-    t.w_pre = t.theta_pre + np;
-    t.theta_post = t.w_pre + np;
-    t.w_post = t.theta_post + np;
-    t.ns_int = reinterpret_cast<const int64_t *>(t.w_post + np);
-    t.ns_frac = reinterpret_cast<const double *>(t.ns_int + np);
-    t.Tn = t.ns_frac + np;
-    t.inv_Tn = t.Tn + np;
-    t.DT = t.inv_Tn + np;
-    t.A = reinterpret_cast<const float *>(t.DT + np);
-    t.cls = reinterpret_cast<const int32_t *>(t.A + np);
-    t.n_tones = p->n_tones;
-    return t;
 }
 
 // Makes the device table current on `stream` (uploading a new version if the host table changed).
@@ -217,13 +217,14 @@ awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, voi
     awg_status st = ensure_table(p, stream);
     if (st != AWG_OK) return st;
     LaunchParams lp;
-    lp.tab = table_view(p, p->cur_version);
+    lp.tab = reinterpret_cast<const ToneRec *>(p->dev_table[p->cur_version]);
+    lp.n_tones = p->n_tones;
     lp.n_begin = n_begin;
     lp.n_count = n_count;
     lp.scale = static_cast<float>(p->scale);
     lp.out = dev_out;
     lp.out_f32 = f32 ? 1 : 0;
-    cudaError_t e = (p->engine == AWG_ENGINE_FP64) ? launch_fp64(lp, stream) : launch_mufu(lp, stream);
+    cudaError_t e = launch_synth(lp, p->engine, stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
     if ((e = cudaEventRecord(p->last_use[p->cur_version], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
     return AWG_OK;
@@ -328,9 +329,9 @@ awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_h
     p->fs = static_cast<long double>(sample_rate_hz);
     p->chunk_len = chunk_len;
     p->scale = 0.9 * 32767.0;
-    p->engine = AWG_ENGINE_MUFU;
+    p->engine = AWG_ENGINE_FMA;
     p->device = dev;
-    p->table_bytes = table_bytes(p->n_pad);
+    p->table_bytes = static_cast<size_t>(p->n_pad) * sizeof(ToneRec);
     try {
         p->tones.resize(n_tones);
     } catch (...) {
@@ -396,8 +397,9 @@ awg_status awg_set_scale(awg_plan *p, double scale)
 awg_status awg_set_engine(awg_plan *p, int32_t engine)
 {
     if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
-    if (engine == AWG_ENGINE_AUTO) engine = AWG_ENGINE_MUFU;
-    if (engine != AWG_ENGINE_MUFU && engine != AWG_ENGINE_FP64) return fail(AWG_ERR_INVALID_ARG, "unknown engine %d", engine);
+    if (engine == AWG_ENGINE_AUTO) engine = AWG_ENGINE_FMA;
+    if (engine != AWG_ENGINE_MUFU && engine != AWG_ENGINE_FP64 && engine != AWG_ENGINE_FMA)
+        return fail(AWG_ERR_INVALID_ARG, "unknown engine %d", engine);
     p->engine = engine;
     return AWG_OK;
 }

@@ -24,6 +24,12 @@ def torch_cuda():
     return torch
 
 
+@pytest.fixture(params=["fma", "mufu"])
+def eng(request, awg):
+    """Both fast engines: AWG_ENGINE_FMA (angle addition on static tiles; the default) and AWG_ENGINE_MUFU."""
+    return {"fma": awg.AWG_ENGINE_FMA, "mufu": awg.AWG_ENGINE_MUFU}[request.param]
+
+
 def _np(t):
     return t.cpu().numpy()
 
@@ -33,26 +39,26 @@ def _gpu_plan(awg, w, engine=None, chunk_len=None):
 
 
 # ------------------------------------------------------------------ C1: the PR1 reference config
-@pytest.mark.parametrize("engine", ["mufu", "fp64"])
+@pytest.mark.parametrize("engine", ["fma", "mufu", "fp64"])
 def test_c1_full_int16_and_f32(awg, torch_cuda, engine):
     w = W.config1()
     op = oracle.plan_from_workload(w)
     V = oracle.c_waveform(op, 0, w.n_samples)
     codes = op.quantise(V)
-    p = _gpu_plan(awg, w, awg.AWG_ENGINE_MUFU if engine == "mufu" else awg.AWG_ENGINE_FP64)
+    p = _gpu_plan(awg, w, {"fma": awg.AWG_ENGINE_FMA, "mufu": awg.AWG_ENGINE_MUFU, "fp64": awg.AWG_ENGINE_FP64}[engine])
     got = _np(p.synthesize_chunk(0))
     gotf = _np(p.synthesize_chunk_f32(0))
     exact, dmax = assert_codes_close(got, codes, f"C1 {engine}")
-    emax = assert_f32_close(gotf, V, f"C1 {engine} f32", tol=1e-5 if engine == "mufu" else 2e-7)
+    emax = assert_f32_close(gotf, V, f"C1 {engine} f32", tol=2e-7 if engine == "fp64" else 1e-5)
     print(f"C1 {engine}: exact {exact:.5f}, max {dmax} LSB, f32 max err {emax:.2e}")
     p.close()
 
 
-def test_c1_chunking_is_bit_identical_on_gpu(awg, torch_cuda):
+def test_c1_chunking_is_bit_identical_on_gpu(awg, torch_cuda, eng):
     w = W.config1()
-    ref = _np(_gpu_plan(awg, w).synthesize_chunk(0))
+    ref = _np(_gpu_plan(awg, w, eng).synthesize_chunk(0))
     for cl in (1 << 16, 1 << 18):
-        p = _gpu_plan(awg, w, chunk_len=cl)
+        p = _gpu_plan(awg, w, eng, chunk_len=cl)
         parts = [_np(p.synthesize_chunk(c)) for c in range(w.n_samples // cl)]
         assert np.array_equal(np.concatenate(parts), ref), f"chunk_len {cl}"
         # the range call over all chunks is the same launch as one long chunk
@@ -61,12 +67,12 @@ def test_c1_chunking_is_bit_identical_on_gpu(awg, torch_cuda):
 
 
 # ------------------------------------------------------------------ C2: 100 tones, min-jerk moves
-def test_c2_full_range_and_chunks(awg, torch_cuda):
+def test_c2_full_range_and_chunks(awg, torch_cuda, eng):
     w = W.config2()
     op = oracle.plan_from_workload(w)
     V = oracle.c_waveform(op, 0, w.n_samples)
     codes = op.quantise(V)
-    p = _gpu_plan(awg, w)
+    p = _gpu_plan(awg, w, eng)
     got = _np(p.synthesize_range(0, w.n_chunks))  # the launch bench.py times
     exact, dmax = assert_codes_close(got, codes, "C2 range")
     print(f"C2: exact {exact:.5f}, max {dmax} LSB")
@@ -93,11 +99,11 @@ def test_c2_fp64_engine_window(awg, torch_cuda):
     p.close()
 
 
-def test_c2_chunk_len_not_a_multiple_of_the_tile(awg, torch_cuda):
+def test_c2_chunk_len_not_a_multiple_of_the_tile(awg, torch_cuda, eng):
     # 5.6e6 = 2^8 * 21875: chunk_len 1000 (multiple of 8, not of 256) gives partial tiles at both chunk edges
     w = W.config2()
-    ref = _np(_gpu_plan(awg, w).synthesize_range(0, w.n_chunks))
-    p = _gpu_plan(awg, w, chunk_len=1000)
+    ref = _np(_gpu_plan(awg, w, eng).synthesize_range(0, w.n_chunks))
+    p = _gpu_plan(awg, w, eng, chunk_len=1000)
     for c in (0, 1, 2, 777, 5599):
         assert np.array_equal(_np(p.synthesize_chunk(c)), ref[c * 1000:(c + 1) * 1000]), c
     assert np.array_equal(_np(p.synthesize_range(3, 41)), ref[3000:44000])
@@ -105,10 +111,10 @@ def test_c2_chunk_len_not_a_multiple_of_the_tile(awg, torch_cuda):
 
 
 # ------------------------------------------------------------------ C3: 1000 tones, 35 ms playback
-def test_c3_playback_range_sampled(awg, torch_cuda):
+def test_c3_playback_range_sampled(awg, torch_cuda, eng):
     w = W.config3()
     op = oracle.plan_from_workload(w)
-    p = _gpu_plan(awg, w)
+    p = _gpu_plan(awg, w, eng)
     out = p.synthesize_range(0, w.n_chunks)  # one 39.8 MB device buffer, one launch (precomputed pathway)
     torch_cuda.cuda.synchronize()
     n_end = int(round(35e-3 * w.sample_rate))  # the move ends inside chunk 18
@@ -128,12 +134,12 @@ def test_c3_playback_range_sampled(awg, torch_cuda):
 
 
 # ------------------------------------------------------------------ C4: streaming ring with per-chunk updates
-def test_c4_streaming_ring_with_updates(awg, torch_cuda):
+def test_c4_streaming_ring_with_updates(awg, torch_cuda, eng):
     w = W.config4(96)  # 96 chunks = 0.25 s of the 1 s run: same update statistics, oracle stays fast
     op = oracle.plan_from_workload(w)
     L = w.chunk_len
     check = {0, 1, 2, 15, 16, 17, 47, 48, 63, 64, 94, 95}
-    p = _gpu_plan(awg, w)
+    p = _gpu_plan(awg, w, eng)
     ring = awg.Ring(p, n_slots=3, host_mirror=True)
     ups = w.updates_by_chunk()
     kept = {}
@@ -162,11 +168,11 @@ def test_c4_streaming_ring_with_updates(awg, torch_cuda):
     p.close()
 
 
-def test_c4_late_chunks_keep_precision(awg, torch_cuda):
+def test_c4_late_chunks_keep_precision(awg, torch_cuda, eng):
     # phases near 1e8 cycles: tones of C4 evaluated around t = 1 s without the updates
     w = W.config4(0)
     op = oracle.plan_from_workload(w)
-    p = _gpu_plan(awg, w)
+    p = _gpu_plan(awg, w, eng)
     for c in (381, 4000):
         V = oracle.c_waveform(op, c * w.chunk_len, c * w.chunk_len + 8192)
         f = _np(p.synthesize_chunk_f32(c))[:8192]
@@ -177,10 +183,10 @@ def test_c4_late_chunks_keep_precision(awg, torch_cuda):
 
 # ------------------------------------------------------------------ C5: scaling sweep
 @pytest.mark.parametrize("n_tones,chunk_len", W.config5_grid())
-def test_c5_cell(awg, torch_cuda, n_tones, chunk_len):
+def test_c5_cell(awg, torch_cuda, eng, n_tones, chunk_len):
     w = W.config5_cell(n_tones, chunk_len)
     op = oracle.plan_from_workload(w)
-    p = _gpu_plan(awg, w)
+    p = _gpu_plan(awg, w, eng)
     out = _np(p.synthesize_chunk(0))
     if n_tones * chunk_len <= (1 << 25):
         wins = [(0, chunk_len)]
@@ -195,10 +201,10 @@ def test_c5_cell(awg, torch_cuda, n_tones, chunk_len):
     p.close()
 
 
-def test_c5_whole_chunk_moves_f32(awg, torch_cuda):
+def test_c5_whole_chunk_moves_f32(awg, torch_cuda, eng):
     w = W.config5_cell(256, 1 << 16, whole_chunk_moves=True)
     op = oracle.plan_from_workload(w)
-    p = _gpu_plan(awg, w)
+    p = _gpu_plan(awg, w, eng)
     V = oracle.c_waveform(op, 0, w.chunk_len)
     assert_f32_close(_np(p.synthesize_chunk_f32(0)), V, w.name)
     assert_codes_close(_np(p.synthesize_chunk(0)), op.quantise(V), w.name)
@@ -247,7 +253,7 @@ def test_saturation(awg, torch_cuda):
 
 @pytest.mark.parametrize("chunk_len", [8, 264, 1000, 4096])
 @pytest.mark.parametrize("n_tones", [1, 33, 100])
-def test_ragged_sizes(awg, torch_cuda, chunk_len, n_tones):
+def test_ragged_sizes(awg, torch_cuda, eng, chunk_len, n_tones):
     rng = np.random.default_rng(chunk_len + n_tones)
     rows = []
     for k in range(n_tones):
@@ -255,7 +261,7 @@ def test_ragged_sizes(awg, torch_cuda, chunk_len, n_tones):
         prof = int(rng.integers(0, 3))
         rows.append((f0, f0 + rng.uniform(-5e6, 5e6), 1.0 / n_tones, rng.uniform(0, 6.28),
                      rng.uniform(-2e-6, 8e-6), rng.uniform(1e-6, 20e-6), prof))
-    p, op = _single(awg, 560e6, chunk_len, rows)
+    p, op = _single(awg, 560e6, chunk_len, rows, engine=eng)
     n_chunks = max(2, 12288 // chunk_len)
     got = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(n_chunks)])
     gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(n_chunks)])
@@ -265,19 +271,19 @@ def test_ragged_sizes(awg, torch_cuda, chunk_len, n_tones):
     p.close()
 
 
-def test_max_tone_count_4096_and_more(awg, torch_cuda):
+def test_max_tone_count_4096_and_more(awg, torch_cuda, eng):
     N = 5000
     rng = np.random.default_rng(99)
     f0 = rng.uniform(20e6, 250e6, N)
     rows = [(f0[k], f0[k] + (3e6 if k % 3 == 0 else 0.0), 1.0 / N, rng.uniform(0, 6.28), 0.0, 30e-6,
              MINJERK if k % 3 == 0 else STATIC) for k in range(N)]
-    p, op = _single(awg, 560e6, 2048, rows)
+    p, op = _single(awg, 560e6, 2048, rows, engine=eng)
     V = oracle.c_waveform(op, 5 * 2048, 6 * 2048)
     assert_f32_close(_np(p.synthesize_chunk_f32(5)), V, "N=5000")
     p.close()
 
 
-def test_special_moves(awg, torch_cuda):
+def test_special_moves(awg, torch_cuda, eng):
     fs = 560e6
     rows = [
         (100e6, 104e6, 0.2, 0.1, 3e-6, 0.0, MINJERK),        # instant retune (T = 0)
@@ -286,7 +292,7 @@ def test_special_moves(awg, torch_cuda):
         (60e6, 65e6, 0.2, 0.4, 2e-6, 5e-6, MINJERK),         # fast move: degree-6 class
         (200e6, 199e6, 0.2, 0.5, 0.0, 21e-6, LINEAR),        # slow linear chirp over the whole span
     ]
-    p, op = _single(awg, fs, 4096, rows)
+    p, op = _single(awg, fs, 4096, rows, engine=eng)
     n = 3 * 4096
     V = oracle.c_waveform(op, 0, n)
     gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(3)])
@@ -300,10 +306,10 @@ def test_special_moves(awg, torch_cuda):
     p.close()
 
 
-def test_mid_move_update_and_static_update(awg, torch_cuda):
+def test_mid_move_update_and_static_update(awg, torch_cuda, eng):
     fs, L = 560e6, 4096
     rows = [(100e6, 103e6, 0.5, 0.9, 0.0, 4 * L / fs, MINJERK), (70e6, 70e6, 0.5, 0.0, 0.0, 0.0, STATIC)]
-    p, op = _single(awg, fs, L, rows)
+    p, op = _single(awg, fs, L, rows, engine=eng)
     for plan in (p, op):
         plan.update_trajectories(2, [0], [100e6], [2 * L / fs], [LINEAR])   # while tone 0 is mid-move
         plan.update_trajectories(5, [1, 0], [75e6, 0.0], [1.5 * L / fs, 0.0], [MINJERK, STATIC])
@@ -314,7 +320,7 @@ def test_mid_move_update_and_static_update(awg, torch_cuda):
         assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"update chunk {c}")
     p.close()
     # same schedule, chunk by chunk, checking each chunk right after its update
-    p, op = _single(awg, fs, L, rows)
+    p, op = _single(awg, fs, L, rows, engine=eng)
     sched = {2: ([0], [100e6], [2 * L / fs], [LINEAR]), 5: ([1, 0], [75e6, 0.0], [1.5 * L / fs, 0.0], [MINJERK, STATIC])}
     for c in range(9):
         if c in sched:
