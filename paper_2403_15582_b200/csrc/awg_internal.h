@@ -62,6 +62,8 @@ struct LaunchParams {
 };
 
 cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream);
+// table[idx[j]] = src[j] for j < n (partial trajectory-table update)
+cudaError_t launch_scatter(ToneRec *table, const ToneRec *src, const int32_t *idx, int n, cudaStream_t stream);
 void count_launch();
 
 }  // namespace awg

@@ -476,6 +476,16 @@ __global__ void __launch_bounds__(256) awg_fp64_kernel(const LaunchParams lp)
     store_tile(lp, n_thread, out);
 }
 
+// Partial trajectory-table update: one 256-byte record per block of 16 threads x 16 bytes.
+__global__ void awg_scatter_kernel(ToneRec *table, const ToneRec *src, const int32_t *idx, int n)
+{
+    const int j = blockIdx.x;
+    if (j >= n) return;
+    const uint4 *s4 = reinterpret_cast<const uint4 *>(src + j);
+    uint4 *d4 = reinterpret_cast<uint4 *>(table + idx[j]);
+    d4[threadIdx.x] = s4[threadIdx.x];
+}
+
 template <bool ROT>
 void launch_split(const LaunchParams &lp, int split, unsigned tiles, cudaStream_t stream)
 {
@@ -489,6 +499,14 @@ void launch_split(const LaunchParams &lp, int split, unsigned tiles, cudaStream_
 }
 
 }  // namespace
+
+cudaError_t launch_scatter(ToneRec *table, const ToneRec *src, const int32_t *idx, int n, cudaStream_t stream)
+{
+    if (n <= 0) return cudaSuccess;
+    awg_scatter_kernel<<<n, sizeof(ToneRec) / sizeof(uint4), 0, stream>>>(table, src, idx, n);
+    count_launch();
+    return cudaGetLastError();
+}
 
 cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream)
 {

@@ -5,6 +5,7 @@
 // turns, so theta + w*n is exact mod 1 for any absolute sample index n: this is the modf of Eq. 14
 // done in integers, and it is what keeps 35 ms x 560 MS/s (5.6e6 cycles) and 1 s x
 // 100 MS/s (1e8 cycles) phases at full precision.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -85,13 +86,17 @@ int classify(int profile, long double DT, long double Tn)
 }
 
 // Rotation table of a carrier for the angle-addition engine: A cos(2 pi j w), A sin(2 pi j w), j = 0..7,
-// from the 64-bit fixed-point frequency (j*w wraps exactly), evaluated in long double, rounded once to fp32.
+// from the 64-bit fixed-point frequency, evaluated in double, rounded once to fp32.
 void make_rot(float *rot, uint64_t w, float A)
 {
+    const double two_pi = 6.283185307179586476925286766559;
     for (int j = 0; j < kSPT; ++j) {
-        const long double turns = ldexpl(static_cast<long double>(static_cast<int64_t>(w * static_cast<uint64_t>(j))), -64);
-        rot[j] = static_cast<float>(static_cast<long double>(A) * cosl(kTwoPiL * turns));
-        rot[kSPT + j] = static_cast<float>(static_cast<long double>(A) * sinl(kTwoPiL * turns));
+        // j*w wraps exactly in u64; as a signed fraction of a turn it is exact in double to 2^-53
+        const double turns = std::ldexp(static_cast<double>(static_cast<int64_t>(w * static_cast<uint64_t>(j))), -64);
+        double sn, cs;
+        sincos(two_pi * turns, &sn, &cs);
+        rot[j] = static_cast<float>(static_cast<double>(A) * cs);
+        rot[kSPT + j] = static_cast<float>(static_cast<double>(A) * sn);
     }
 }
 
@@ -153,62 +158,88 @@ long double profile_g(int profile, long double s)  // its integral
 
 // ---- device table versions ---------------------------------------------------------------------
 
-static void fill_staging(const awg_plan *p, unsigned char *dst)
+static void fill_record(const HostTone &h, ToneRec &r)
 {
-    ToneRec *out = reinterpret_cast<ToneRec *>(dst);
-    for (int i = 0; i < p->n_pad; ++i) {
-        ToneRec r;
-        std::memset(&r, 0, sizeof r);
-        if (i < p->n_tones) {
-            const HostTone &h = p->tones[i];
-            r.A = h.A;
-            r.cls = (h.profile << 8) | h.cls;
-            r.theta_pre = h.theta_pre;
-            r.w_pre = h.w_pre;
-            r.theta_post = h.theta_post;
-            r.w_post = h.w_post;
-            r.ns_int = static_cast<double>(h.ns_int);
-            r.ns_frac = h.ns_frac;
-            r.Tn = static_cast<double>(h.Tn);
-            if (h.Tn > 0.0L) {
-                const long double rT = 1.0L / h.Tn;
-                r.inv_Tn = static_cast<double>(rT);
-                r.DT = static_cast<double>(h.DT);
-                r.q1 = static_cast<double>(h.DT * rT);
-                long double q = kTwoPiL * h.DT * rT, fact = 1.0L;  // 2 pi DT / Tn^k / k!
-                for (int k = 2; k <= 6; ++k) {
-                    q *= rT;
-                    fact *= k;
-                    r.q[k - 2] = static_cast<float>(q / fact);
-                }
-            }
-            std::memcpy(r.rot_pre, h.rot_pre, sizeof r.rot_pre);
-            std::memcpy(r.rot_post, h.rot_post, sizeof r.rot_post);
+    std::memset(&r, 0, sizeof r);
+    r.A = h.A;
+    r.cls = (h.profile << 8) | h.cls;
+    r.theta_pre = h.theta_pre;
+    r.w_pre = h.w_pre;
+    r.theta_post = h.theta_post;
+    r.w_post = h.w_post;
+    r.ns_int = static_cast<double>(h.ns_int);
+    r.ns_frac = h.ns_frac;
+    r.Tn = static_cast<double>(h.Tn);
+    if (h.Tn > 0.0L) {
+        const long double rT = 1.0L / h.Tn;
+        r.inv_Tn = static_cast<double>(rT);
+        r.DT = static_cast<double>(h.DT);
+        r.q1 = static_cast<double>(h.DT * rT);
+        long double q = kTwoPiL * h.DT * rT, fact = 1.0L;  // 2 pi DT / Tn^k / k!
+        for (int k = 2; k <= 6; ++k) {
+            q *= rT;
+            fact *= k;
+            r.q[k - 2] = static_cast<float>(q / fact);
         }
-        out[i] = r;
     }
+    std::memcpy(r.rot_pre, h.rot_pre, sizeof r.rot_pre);
+    std::memcpy(r.rot_post, h.rot_post, sizeof r.rot_post);
 }
 
-// Makes the device table current on `stream` (uploading a new version if the host table changed).
-static awg_status ensure_table(awg_plan *p, cudaStream_t stream)
+// Makes the device table current on `stream`.  A changed table goes to the next of kTableVersions device
+// copies, so kernels still reading the previous version are never disturbed.  After set_trajectories the
+// whole table is uploaded; after per-chunk updates only the changed records travel: the new version is a
+// device-to-device copy of the current one plus a scatter of the updated records (parameters
+// cross the bus only when they change).
+awg_status ensure_table(awg_plan *p, cudaStream_t stream)
 {
     cudaError_t e;
-    if (p->dirty) {
-        const int v = (p->cur_version + 1) % kTableVersions;
-        // the slot's previous readers (kernels launched kTableVersions uploads ago) must be done
-        if ((e = cudaEventSynchronize(p->last_use[v])) != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
-        fill_staging(p, p->host_table[v]);
-        if ((e = cudaMemcpyAsync(p->dev_table[v], p->host_table[v], p->table_bytes, cudaMemcpyHostToDevice, stream)) != cudaSuccess)
-            return fail_cuda(e, "cudaMemcpyAsync(table)");
-        if ((e = cudaEventRecord(p->uploaded[v], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-        p->upload_stream[v] = stream;
-        p->cur_version = v;
-        p->dirty = false;
-        p->h2d_bytes += static_cast<int64_t>(p->table_bytes);
-    } else if (p->upload_stream[p->cur_version] != stream) {
-        if ((e = cudaStreamWaitEvent(stream, p->uploaded[p->cur_version], 0)) != cudaSuccess)
+    if (!p->dirty_all && p->dirty_tones.empty()) {
+        if (p->upload_stream[p->cur_version] != stream &&
+            (e = cudaStreamWaitEvent(stream, p->uploaded[p->cur_version], 0)) != cudaSuccess)
             return fail_cuda(e, "cudaStreamWaitEvent");
+        return AWG_OK;
     }
+    const int cur = p->cur_version;
+    const int v = (cur + 1) % kTableVersions;
+    // the slot's previous readers (kernels launched kTableVersions uploads ago) must be done
+    if ((e = cudaEventSynchronize(p->last_use[v])) != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
+    std::sort(p->dirty_tones.begin(), p->dirty_tones.end());
+    p->dirty_tones.erase(std::unique(p->dirty_tones.begin(), p->dirty_tones.end()), p->dirty_tones.end());
+    const size_t n_dirty = p->dirty_tones.size();
+    ToneRec *host = reinterpret_cast<ToneRec *>(p->host_table[v]);
+    if (p->dirty_all || n_dirty * 4 > static_cast<size_t>(p->n_tones)) {
+        for (int i = 0; i < p->n_pad; ++i) {
+            if (i < p->n_tones) fill_record(p->tones[i], host[i]);
+            else std::memset(&host[i], 0, sizeof(ToneRec));
+        }
+        if ((e = cudaMemcpyAsync(p->dev_table[v], host, p->table_bytes, cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemcpyAsync(table)");
+        p->h2d_bytes += static_cast<int64_t>(p->table_bytes);
+    } else {
+        int32_t *host_idx = reinterpret_cast<int32_t *>(p->host_table[v] + p->table_bytes);
+        for (size_t j = 0; j < n_dirty; ++j) {
+            fill_record(p->tones[p->dirty_tones[j]], host[j]);
+            host_idx[j] = p->dirty_tones[j];
+        }
+        if (p->upload_stream[cur] != stream && (e = cudaStreamWaitEvent(stream, p->uploaded[cur], 0)) != cudaSuccess)
+            return fail_cuda(e, "cudaStreamWaitEvent");
+        if ((e = cudaMemcpyAsync(p->dev_table[v], p->dev_table[cur], p->table_bytes, cudaMemcpyDeviceToDevice, stream)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemcpyAsync(table d2d)");
+        if ((e = cudaEventRecord(p->last_use[cur], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+        if ((e = cudaMemcpyAsync(p->dev_stage[v], host, n_dirty * sizeof(ToneRec), cudaMemcpyHostToDevice, stream)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(p->dev_stage[v] + p->table_bytes, host_idx, n_dirty * sizeof(int32_t), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemcpyAsync(updated records)");
+        if ((e = launch_scatter(reinterpret_cast<ToneRec *>(p->dev_table[v]), reinterpret_cast<const ToneRec *>(p->dev_stage[v]),
+                                reinterpret_cast<const int32_t *>(p->dev_stage[v] + p->table_bytes), static_cast<int>(n_dirty), stream)) != cudaSuccess)
+            return fail_cuda(e, "scatter launch");
+        p->h2d_bytes += static_cast<int64_t>(n_dirty * (sizeof(ToneRec) + sizeof(int32_t)));
+    }
+    if ((e = cudaEventRecord(p->uploaded[v], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+    p->upload_stream[v] = stream;
+    p->cur_version = v;
+    p->dirty_all = false;
+    p->dirty_tones.clear();
     return AWG_OK;
 }
 
@@ -298,7 +329,7 @@ awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int
                   D * static_cast<long double>(n_u) / fs);
     }
     if (n_upd > 0) {
-        p->dirty = true;
+        p->dirty_tones.insert(p->dirty_tones.end(), tone_idx, tone_idx + n_upd);
         p->last_update_chunk = chunk_idx;
     }
     return AWG_OK;
@@ -339,8 +370,10 @@ awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_h
         return fail(AWG_ERR_ALLOC, "out of host memory");
     }
     for (int v = 0; v < kTableVersions; ++v) {
+        const size_t stage_bytes = p->table_bytes + static_cast<size_t>(p->n_pad) * sizeof(int32_t);
         if ((e = cudaMalloc(reinterpret_cast<void **>(&p->dev_table[v]), p->table_bytes)) != cudaSuccess ||
-            (e = cudaMallocHost(reinterpret_cast<void **>(&p->host_table[v]), p->table_bytes)) != cudaSuccess ||
+            (e = cudaMalloc(reinterpret_cast<void **>(&p->dev_stage[v]), stage_bytes)) != cudaSuccess ||
+            (e = cudaMallocHost(reinterpret_cast<void **>(&p->host_table[v]), stage_bytes)) != cudaSuccess ||
             (e = cudaEventCreateWithFlags(&p->last_use[v], cudaEventDisableTiming)) != cudaSuccess ||
             (e = cudaEventCreateWithFlags(&p->uploaded[v], cudaEventDisableTiming)) != cudaSuccess) {
             awg_status st = (e == cudaErrorMemoryAllocation) ? fail(AWG_ERR_ALLOC, "device/pinned allocation failed: %s", cudaGetErrorString(e))
@@ -364,6 +397,7 @@ awg_status awg_plan_destroy(awg_plan *p)
     }
     for (int v = 0; v < kTableVersions; ++v) {
         if (p->dev_table[v]) cudaFree(p->dev_table[v]);
+        if (p->dev_stage[v]) cudaFree(p->dev_stage[v]);
         if (p->host_table[v]) cudaFreeHost(p->host_table[v]);
         if (p->last_use[v]) cudaEventDestroy(p->last_use[v]);
         if (p->uploaded[v]) cudaEventDestroy(p->uploaded[v]);
@@ -436,7 +470,8 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
                   (static_cast<long double>(f1[k]) - h.f0) * ts);
     }
     p->have_table = true;
-    p->dirty = true;
+    p->dirty_all = true;
+    p->dirty_tones.clear();
     p->last_update_chunk = 0;
     return AWG_OK;
 }

@@ -40,14 +40,16 @@ struct awg_plan {
     int32_t engine = AWG_ENGINE_MUFU;
     int device = 0;
     bool have_table = false;
-    bool dirty = false;
+    bool dirty_all = false;                 // whole table changed (awg_set_trajectories)
+    std::vector<int32_t> dirty_tones;       // tones changed by updates since the last upload
     int64_t last_update_chunk = 0;
     std::vector<awg::HostTone> tones;
     // versioned device tables
     size_t table_bytes = 0;
     int cur_version = 0;
     unsigned char *dev_table[awg::kTableVersions] = {};
-    unsigned char *host_table[awg::kTableVersions] = {};  // pinned staging
+    unsigned char *host_table[awg::kTableVersions] = {};  // pinned staging: records, then int32 indices
+    unsigned char *dev_stage[awg::kTableVersions] = {};   // device staging for partial updates (same layout)
     cudaEvent_t last_use[awg::kTableVersions] = {};
     cudaEvent_t uploaded[awg::kTableVersions] = {};
     cudaStream_t upload_stream[awg::kTableVersions] = {};
@@ -61,6 +63,7 @@ struct awg_plan {
 };
 
 namespace awg {
+awg_status ensure_table(awg_plan *p, cudaStream_t stream);
 awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream);
 awg_status check_chunk_call(awg_plan *p, int64_t first_chunk, int64_t n_chunks, const void *out, size_t align);
 awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx, const double *f1,

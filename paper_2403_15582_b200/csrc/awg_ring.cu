@@ -105,6 +105,8 @@ awg_status awg_ring_submit(awg_ring *r, int64_t chunk_idx, int32_t n_upd, const 
     RingSlot &s = r->slots[r->n_submitted % r->n_slots];
     if ((st = check_chunk_call(p, chunk_idx, 1, s.dev, 16)) != AWG_OK) return st;
     cudaError_t e;
+    // table upload (if an update is pending) goes first so that the chunk's device time measures synthesis + mirror
+    if ((st = ensure_table(p, r->s_syn)) != AWG_OK) return st;
     if ((e = cudaEventRecord(s.start, r->s_syn)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
     if ((st = synthesize_samples(p, chunk_idx * p->chunk_len, p->chunk_len, s.dev, false, r->s_syn)) != AWG_OK) return st;
     if ((e = cudaEventRecord(s.synth_done, r->s_syn)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");

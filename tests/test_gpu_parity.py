@@ -369,9 +369,10 @@ def test_error_codes_and_state(awg, torch_cuda):
     with pytest.raises(awg.AwgError) as ei:
         awg.awg_synthesize_chunk(p.handle, 2, buf.data_ptr())
     assert ei.value.status == awg.AWG_ERR_STATE  # earlier than the latest update
+    p.synthesize_chunk(3, out=buf)          # uploads the pending update first
     before = awg.awg_kernel_launch_count()
     p.synthesize_chunk(3, out=buf)
-    assert awg.awg_kernel_launch_count() == before + 1
+    assert awg.awg_kernel_launch_count() == before + 1  # exactly one kernel per synthesis call
     ring = awg.Ring(p, 2, False)
     ring.submit(3); ring.submit(4)
     with pytest.raises(awg.AwgError) as ei:
