@@ -187,6 +187,31 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+ENGINES = {"auto": lambda awg: awg.AWG_ENGINE_AUTO, "fma": lambda awg: awg.AWG_ENGINE_FMA,
+           "mufu": lambda awg: awg.AWG_ENGINE_MUFU}
+
+
+def pick_workload(name: str):
+    """The timed workload: C2 (the headline, BASELINE.json configs[1]) unless --workload asks for another one
+    (profiling aid: C1, C3, C5:<tones>:<log2 chunk>, CAP:<static|half|moving>:<tones>)."""
+    if name == "C2":
+        return W.config2(), ("C2: 100 tones at 560 MS/s for 10 ms = 5.6 M samples, 50 min-jerk movers "
+                             "(BASELINE.json configs[1], seed 1)")
+    if name == "C1":
+        return W.config1(), "C1: 16 tones, 2^20 samples (BASELINE.json configs[0])"
+    if name == "C3":
+        return W.config3(), "C3: 1000 tones min-jerk for 35 ms at 560 MS/s, 19 x 2^20 samples (BASELINE.json configs[2])"
+    kind, *rest = name.split(":")
+    if kind == "C5":
+        n_t, lg = int(rest[0]), int(rest[1])
+        return W.config5_cell(n_t, 1 << lg), f"C5 cell: {n_t} tones x 2^{lg} samples (BASELINE.json configs[4])"
+    if kind == "CAP":
+        n_t = int(rest[1])
+        return (W.capacity_toneset(n_t, 560e6, 1 << 20, rest[0], n_chunks=4),
+                f"capacity tone set: {n_t} tones ({rest[0]}), 4 x 2^20 samples at 560 MS/s")
+    raise SystemExit(f"unknown --workload {name}")
+
+
 # --------------------------------------------------------------------------------------------------
 def device_time_range(torch, plan, n_chunks, bufs, steps, warmup):
     """ms per step of awg_synthesize_range, CUDA events on the launch stream, rotating output buffers."""
@@ -336,8 +361,8 @@ def run_ours(args):
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     peak_sin = MUFU_PER_CLK_PER_SM * N_SM * sm_max_mhz * 1e6  # MUFU.SIN per second at max clock
 
-    w = W.config2()
-    plan = awg.Plan.from_workload(w)
+    w, w_desc = pick_workload(args.workload)
+    plan = awg.Plan.from_workload(w, engine=ENGINES[args.engine](awg))
     bufs = make_bufs(torch, w.n_samples)
     stream = torch.cuda.current_stream()
     host_out = torch.empty(w.n_samples, dtype=torch.int16, pin_memory=True)
@@ -423,7 +448,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "C2: 100 tones at 560 MS/s for 10 ms = 5.6 M samples, 50 min-jerk movers (BASELINE.json configs[1], seed 1)",
+        "config": {"workload": w_desc, "engine": args.engine,
                    "tones": w.n_tones, "samples_per_step": w.n_samples, "launch": "one awg_synthesize_range per step",
                    "l2": f"output rotates over {len(bufs)} device buffers ({len(bufs) * 2 * w.n_samples / 1e6:.0f} MB > 126 MB L2); "
                          "the only input is the 9 KB tone table",
@@ -446,6 +471,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", default="C2", help="timed workload (default C2 = the headline; others are profiling aids)")
+    ap.add_argument("--engine", choices=sorted(ENGINES), default="auto", help="sine engine of the timed plan")
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs and the capacity search")
     ap.add_argument("--full", action="store_true", help="extras at full length: 382-chunk C4, 1 s per capacity probe")
     args = ap.parse_args()

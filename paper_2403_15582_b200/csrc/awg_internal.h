@@ -18,9 +18,29 @@ enum : int32_t {
     CLS_EXACT = 7    // fp32 in-tile polynomial not accurate enough: moving tiles use the fp64 path
 };
 
-constexpr int kSPT = 8;  // consecutive samples per thread (one 16-byte int16 store); also the rotation-table length
+// Kernel geometry.  A thread owns kSPT consecutive samples of a block; a block is 32 lanes x kSPT = 512 samples
+// (the span of one phase re-centring); a warp tile is kBlocksPerTile consecutive blocks, anchored at absolute
+// sample indices that are multiples of kTile.
+constexpr int kSPT = 16;
+constexpr int kBlock = 32 * kSPT;
+constexpr int kBlocksPerTile = 4;
+constexpr int kTile = kBlocksPerTile * kBlock;
+constexpr int kPairs = kSPT / 2;  // symmetric sample pairs per thread: centre +- (j + 1/2), j = 0..kPairs-1
 
-// Device trajectory table (hot-path step a0): one 256-byte record per tone, read by one lane per
+// Carrier table of the angle-addition engine (hot-path step a3, static tiles): with phi the carrier phase at the
+// half-integer centre of a thread's 16 samples, the samples at centre +- (j + 1/2) are
+//     A sin(phi +- (j+1/2) w) = sin(phi) * [A cos((j+1/2) w)]  +-  cos(phi) * [A sin((j+1/2) w)]
+// so ONE multiply-add per tone-sample accumulates the even part P_j and the odd part Q_j; the next block of the
+// tile is reached by rotating (sin phi, cos phi) by kBlock*w.
+struct __align__(16) RotTable {
+    float C[kPairs];    // A cos(2 pi (j + 1/2) w)
+    float S[kPairs];    // A sin(2 pi (j + 1/2) w)
+    float cr, sr;       // cos, sin of 2 pi kBlock w
+    float pad_[2];
+};
+static_assert(sizeof(RotTable) == 80, "RotTable must be 80 bytes");
+
+// Device trajectory table (hot-path step a0): one 288-byte record per tone, read by one lane per
 // (tone, tile) with 16-byte loads.  Phases are in TURNS as unsigned 64-bit fixed point (1 turn = 2^64), so
 // the carrier phase theta + w*n wraps exactly mod 1 for any n: the range reduction of Eq. 14
 // done in integer arithmetic.  With u = (n - ns_int) - ns_frac the real number of samples since the move began:
@@ -44,12 +64,11 @@ struct __align__(16) ToneRec {
     double q1;             // DT/Tn = (f1-f0)/fs, cycles per sample
     float q[5];            // q[k-2] = 2*pi*DT/Tn^k/k!, k = 2..6: radians per sample^k for unit g^(k)
     float pad_[5];
-    // ---- 2 x 64 bytes: rotation tables of the two carriers for the angle-addition engine,
-    //      {A cos(2 pi j w), j = 0..7} then {A sin(2 pi j w), j = 0..7}
-    float rot_pre[2 * kSPT];
-    float rot_post[2 * kSPT];
+    // ---- 2 x 80 bytes: tables of the two carriers for the angle-addition engine
+    RotTable rot_pre;
+    RotTable rot_post;
 };
-static_assert(sizeof(ToneRec) == 256, "ToneRec must be 256 bytes");
+static_assert(sizeof(ToneRec) == 288, "ToneRec must be 288 bytes");
 
 struct LaunchParams {
     const ToneRec *tab;

@@ -1,16 +1,19 @@
 // awg_kernels.cu -- sm_100a synthesis kernels: the fused WG + WC (+ quantise) of PAPER.md:158-186.
 //
 // Hot-path steps (SURVEY.md section 8(a) / DESIGN.md):
-//   a1  per (tone, 256-sample tile) phase re-centring in 64-bit fixed point + fp64      tile_prologue()
-//   a2  per tone-sample phase  c0 + c1*k (u32 turns, wraps exactly) + fp32 polynomial  mufu_loop<KIND>()
-//   a3  sine: MUFU.SIN per tone-sample (MUFU engine, and every moving tile), or one MUFU.SIN + MUFU.COS per
-//       8 samples rotated by a per-tone table {A cos(j w), A sin(j w)} (angle addition, static tiles of the
-//       FMA engine):  A sin(phi0 + j w) = sin(phi0) * A cos(j w) + cos(phi0) * A sin(j w)        rot_loop()
-//   a4  fp32 register accumulation over tones, 8 samples per thread                    acc[4] (float2)
-//   a5  quantise: cvt.rni.sat.s16.f32(scale * acc)                                     store_tile()
-//   a6  one 16-byte store of 8 consecutive int16 per thread                            store_tile()
+//   a1  per (tone, 512-sample block) phase re-centring in 64-bit fixed point + fp64     block_prologue()
+//   a2  per tone-sample phase  c0 + c1*k (u32 turns, wraps exactly) + fp32 polynomial   mufu_loop<KIND>()
+//   a3  sine.  MUFU engine, and every block in which a tone is moving: one MUFU.SIN per tone-sample.
+//       Angle-addition engine, tiles in which a tone is static: one MUFU.SIN + one MUFU.COS per (thread, tone,
+//       2048-sample tile), then per symmetric sample pair centre +- (j + 1/2)
+//           A sin(phi +- (j+1/2) w) = sin(phi) [A cos((j+1/2) w)]  +-  cos(phi) [A sin((j+1/2) w)]
+//       i.e. ONE fp32 multiply-add per tone-sample into the even/odd accumulators P_j, Q_j      static_pass()
+//   a4  fp32 register accumulation over tones: 4 blocks x 16 samples per thread
+//   a5  quantise: cvt.rni.sat.s16.f32(scale * acc)                                      store_block()
+//   a6  two 16-byte stores of 8 consecutive int16 per thread and block                  store_block()
 // No tensor cores (north_star), no per-tone wavetable in DRAM (the paper's limiter); output
 // traffic is 2 bytes per sample.
+#include <cstddef>
 #include <cstdint>
 #include <atomic>
 
@@ -23,10 +26,10 @@ void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 namespace {
 
-constexpr int kTile = 32 * kSPT;      // samples per warp tile, anchored at absolute multiples of 256
-constexpr int kHalf = kTile / 2;      // Taylor expansions are centred on the tile
+constexpr int kHalf = kBlock / 2;     // Taylor expansions are centred on the block
 constexpr int kWarps = 8;             // warps per CTA
-constexpr int kBatch = 32;            // tones per prologue batch: one tone per lane
+constexpr int kBatch = 32;            // tones (pass 1) or (tone, block) items (pass 2) per batch: one per lane
+constexpr int kMaxBatches = 65536 / kWarps / kBatch;   // per warp, at the largest tone count and widest split
 constexpr float kTurnToRad = 1.4629180792671596e-9f;   // 2*pi / 2^32: int32 phase (turns * 2^32) -> radians
 constexpr double kTwo64 = 18446744073709551616.0;
 
@@ -81,40 +84,37 @@ __device__ __forceinline__ uint64_t exact_phase(const ToneRec &r, int64_t n)
     return r.theta_pre + r.w_pre * static_cast<uint64_t>(n) + frac_to_fix64(x);
 }
 
-// Kinds of (tone, tile) record, in the order the inner loops run them.
+// Kinds of (tone, block) record, in the order the inner loops run them.
 enum : int {
     K_NONE = -1,
     K_STATIC = 0,  // carrier only
     K_QUAD = 1,    // + k^2 term
     K_DEG4 = 2,    // + k^2..k^4
     K_DEG6 = 3,    // + k^2..k^6
-    K_SBEG = 4,    // the move starts inside this tile: pre-move carrier + P(max(k - kb, 0))
-    K_SEND = 5,    // the move ends inside this tile:  post-move carrier + P(max(kb - k, 0))
-    K_EXACT = 6,   // anything else (both ends in one tile, T = 0, CLS_EXACT tones): fp64 per sample
+    K_SBEG = 4,    // the move starts inside this block: pre-move carrier + P(max(k - kb, 0))
+    K_SEND = 5,    // the move ends inside this block:  post-move carrier + P(max(kb - k, 0))
+    K_EXACT = 6,   // anything else (both ends in one block, T = 0, CLS_EXACT tones): fp64 per sample
     K_COUNT = 7
 };
 
-// One re-centred (tone, tile) record:
-//   phase(k) = c0 + c1*k [u32 turns, wrapping] + poly(k) [radians, fp32],  k = n - tile centre
-//   K_QUAD..K_DEG6: poly = k^2 (c2 + k (c3 + k (c4 + k (c5 + k c6))))     (Taylor series about the tile centre)
+// One re-centred (tone, block) record:
+//   phase(k) = c0 + c1*k [u32 turns, wrapping] + poly(k) [radians, fp32],  k = n - block centre
+//   K_QUAD..K_DEG6: poly = k^2 (c2 + k (c3 + k (c4 + k (c5 + k c6))))     (Taylor series about the block centre)
 //   K_SBEG/K_SEND:  poly = w^2 (c2 + w^2 (c3 + w (c4 + w c5))), w = max(+-(k - kb), 0), c6 = +-kb
-//   K_STATIC with the FMA engine: `rot` points at the carrier's rotation table in the tone record
-struct TileRec {
+struct BlockRec {
     uint32_t c0, c1;
     float A;
     float c2, c3, c4, c5, c6;
     int kind;
-    const float *rot;
 };
 
-// Step a1.  Lane-private: tone record `rec` at the tile whose first sample is tile_base (absolute);
-// tb_d = (double)tile_base, nc = tile_base + 128.
-__device__ __forceinline__ TileRec tile_prologue(const ToneRec *rec, int t, uint64_t nc, double tb_d)
+// Step a1.  Lane-private: tone record `rec` (index t) at the block whose first sample is blk_base (absolute);
+// bb_d = (double)blk_base, nc = blk_base + kHalf.
+__device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, uint64_t nc, double bb_d)
 {
-    TileRec r;
+    BlockRec r;
     r.c2 = r.c3 = r.c4 = r.c5 = r.c6 = 0.f;
     r.kind = K_STATIC;
-    r.rot = rec->rot_pre;
     const uint4 v0 = ldg16(rec);  // A, cls, theta_pre
     r.A = __uint_as_float(v0.x);
     const int32_t cls = static_cast<int32_t>(v0.y);
@@ -130,8 +130,8 @@ __device__ __forceinline__ TileRec tile_prologue(const ToneRec *rec, int t, uint
         const uint4 v2 = ldg16(reinterpret_cast<const char *>(rec) + 32);  // w_post, ns_int
         const uint4 v3 = ldg16(reinterpret_cast<const char *>(rec) + 48);  // ns_frac, Tn
         const double Tn = f64_of(v3.z, v3.w);
-        const double ua = (tb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the tile's first sample
-        const double ub = ua + static_cast<double>(kTile - 1);
+        const double ua = (bb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the block's first sample
+        const double ub = ua + static_cast<double>(kBlock - 1);
         const bool linear = (cls >> 8) == AWG_PROFILE_LINEAR;
         if (ub <= 0.0) {
             w = w_pre;
@@ -139,7 +139,6 @@ __device__ __forceinline__ TileRec tile_prologue(const ToneRec *rec, int t, uint
         } else if (ua >= Tn) {
             w = u64_of(v2.x, v2.y);
             ph = u64_of(v1.z, v1.w) + w * nc;
-            r.rot = rec->rot_post;
         } else if (c == CLS_EXACT || (ua < 0.0 && ub > Tn)) {
             r.kind = K_EXACT;
             r.c0 = static_cast<uint32_t>(t);
@@ -154,8 +153,8 @@ __device__ __forceinline__ TileRec tile_prologue(const ToneRec *rec, int t, uint
             const float q2 = __uint_as_float(v5.z), q3 = __uint_as_float(v5.w);
             const float q4 = __uint_as_float(v6.x), q5 = __uint_as_float(v6.y), q6 = __uint_as_float(v6.z);
             if (ua >= 0.0 && ub <= Tn) {
-                // whole tile inside the move (g(0) = 0 and DT g(1) = post - pre, so the closed ends are included):
-                // Taylor-expand DT*g((u_c + k)/Tn) about the tile centre.  Phase and frequency (g, g') in fp64,
+                // whole block inside the move (g(0) = 0 and DT g(1) = post - pre, so the closed ends are included):
+                // Taylor-expand DT*g((u_c + k)/Tn) about the block centre.  Phase and frequency (g, g') in fp64,
                 // the higher derivatives only feed fp32 coefficients and are evaluated in fp32.
                 const double s = (ua + static_cast<double>(kHalf)) * rT;
                 const float sf = static_cast<float>(s);
@@ -169,7 +168,7 @@ __device__ __forceinline__ TileRec tile_prologue(const ToneRec *rec, int t, uint
                     g1 = s2 * s * (10.0 + s * (6.0 * s - 15.0));
                     r.c2 = q2 * (sf * sf * (30.f + sf * (30.f * sf - 60.f)));
                 }
-                w = w_pre + frac_to_fix64(f64_of(v5.x, v5.y) * g1);  // instantaneous frequency at the tile centre
+                w = w_pre + frac_to_fix64(f64_of(v5.x, v5.y) * g1);  // instantaneous frequency at the block centre
                 ph = theta_pre + w_pre * nc + frac_to_fix64(DT * g0);
                 r.kind = K_QUAD;
                 if (c >= CLS_DEG4) {
@@ -183,7 +182,7 @@ __device__ __forceinline__ TileRec tile_prologue(const ToneRec *rec, int t, uint
                     }
                 }
             } else {
-                // exactly one end of the move lies inside the tile.  With w the (clamped) distance into the move
+                // exactly one end of the move lies inside the block.  With w the (clamped) distance into the move
                 // from that end, both ends have the same polynomial: DT (w/Tn)^2/2 (LINEAR) or
                 // DT (5/2 (w/Tn)^4 - 3 (w/Tn)^5 + (w/Tn)^6) (MINJERK) on top of the carrier valid outside the move
                 // [at the end: g(1+x) - (1/2 + x) = 5/2 x^4 + 3 x^5 + x^6, x = -w/Tn].  q[k-2] = 2 pi DT/Tn^k/k!.
@@ -213,22 +212,29 @@ __device__ __forceinline__ TileRec tile_prologue(const ToneRec *rec, int t, uint
     return r;
 }
 
-// Per-warp shared-memory record of one (tone, tile): 80 bytes.
-//   q[0] = {c0 bits, c1 bits, A, c2};  moving kinds: q[1] = {c3, c4, c5, c6}
-//   static tiles of the FMA engine:    q[1..2] = A cos(j w), j = 0..7;  q[3..4] = A sin(j w), j = 0..7
+// Per-warp shared-memory record of one (tone, block) item of pass 2: q[0] = {c0 bits, c1 bits, A, c2};
+// q[1] = {c3, c4, c5, c6}.  K_EXACT: c0 = tone index.
 struct __align__(16) SmemRec {
-    float4 q[5];
+    float4 q[2];
+};
+
+// 16 samples of one block of one thread, as 8 packed pairs: a[j] = samples (2j, 2j+1).
+struct Acc16 {
+    float2 a[kPairs];
+};
+
+struct KindCounts {
+    int n[K_COUNT];
 };
 
 // Steps a2-a4, MUFU path, for `count` records starting at rec[first], all of kind KIND.  Samples go in pairs
 // through the packed fp32x2 instructions of sm_100 (FMUL2 / FFMA2: one issue slot for two samples).
 template <int KIND>
 __device__ __forceinline__ void mufu_loop(const SmemRec *rec, int first, int count, int koff,
-                                          const float2 (&kf)[kSPT / 2], const float2 (&kk)[kSPT / 2],
-                                          float2 (&acc)[kSPT / 2])
+                                          const float2 (&kfs)[kPairs], const float2 (&kks)[kPairs], Acc16 &acc)
 {
     const float2 K2 = dup2(kTurnToRad);
-#pragma unroll 2
+#pragma unroll 1
     for (int i = first; i < first + count; ++i) {
         const float4 a = rec[i].q[0];
         const uint32_t c0 = __float_as_uint(a.x), c1 = __float_as_uint(a.y);
@@ -237,246 +243,411 @@ __device__ __forceinline__ void mufu_loop(const SmemRec *rec, int first, int cou
         float4 b;
         if (KIND >= K_DEG4) b = rec[i].q[1];
 #pragma unroll
-        for (int j = 0; j < kSPT / 2; ++j) {
+        for (int j = 0; j < kPairs; ++j) {
             const uint32_t p0 = base + c1 * static_cast<uint32_t>(2 * j);
             const uint32_t p1 = base + c1 * static_cast<uint32_t>(2 * j + 1);
             const float2 f = make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1)));
+            const float2 kf = kfs[j];
             float2 x;
             if (KIND == K_STATIC) {
                 x = __fmul2_rn(f, K2);
             } else if (KIND == K_SBEG || KIND == K_SEND) {
                 float2 w;
-                w.x = fmaxf((KIND == K_SBEG ? kf[j].x : -kf[j].x) - b.w, 0.f);
-                w.y = fmaxf((KIND == K_SBEG ? kf[j].y : -kf[j].y) - b.w, 0.f);
+                w.x = fmaxf((KIND == K_SBEG ? kf.x : -kf.x) - b.w, 0.f);
+                w.y = fmaxf((KIND == K_SBEG ? kf.y : -kf.y) - b.w, 0.f);
                 const float2 w2 = __fmul2_rn(w, w);
                 float2 poly = __ffma2_rn(dup2(b.z), w, dup2(b.y));
                 poly = __ffma2_rn(poly, w, dup2(b.x));
                 poly = __ffma2_rn(poly, w2, dup2(a.w));
                 x = __ffma2_rn(f, K2, __fmul2_rn(poly, w2));
             } else {
+                const float2 kk = kks[j];
                 float2 poly;
                 if (KIND == K_QUAD) {
                     poly = dup2(a.w);
                 } else if (KIND == K_DEG4) {
-                    poly = __ffma2_rn(dup2(b.y), kf[j], dup2(b.x));
-                    poly = __ffma2_rn(poly, kf[j], dup2(a.w));
+                    poly = __ffma2_rn(dup2(b.y), kf, dup2(b.x));
+                    poly = __ffma2_rn(poly, kf, dup2(a.w));
                 } else {
-                    poly = __ffma2_rn(dup2(b.w), kf[j], dup2(b.z));
-                    poly = __ffma2_rn(poly, kf[j], dup2(b.y));
-                    poly = __ffma2_rn(poly, kf[j], dup2(b.x));
-                    poly = __ffma2_rn(poly, kf[j], dup2(a.w));
+                    poly = __ffma2_rn(dup2(b.w), kf, dup2(b.z));
+                    poly = __ffma2_rn(poly, kf, dup2(b.y));
+                    poly = __ffma2_rn(poly, kf, dup2(b.x));
+                    poly = __ffma2_rn(poly, kf, dup2(a.w));
                 }
-                x = __ffma2_rn(f, K2, __fmul2_rn(poly, kk[j]));
+                x = __ffma2_rn(f, K2, __fmul2_rn(poly, kk));
             }
-            acc[j] = __ffma2_rn(dup2(A), make_float2(mufu_sin(x.x), mufu_sin(x.y)), acc[j]);
+            acc.a[j] = __ffma2_rn(dup2(A), make_float2(mufu_sin(x.x), mufu_sin(x.y)), acc.a[j]);
         }
     }
 }
 
-// Steps a2-a4, angle-addition path, static tiles: per (thread, tone) ONE sine and ONE cosine of the phase at the
-// thread's first sample, then 8 samples by rotation with the tone's table:
-//   A sin(phi0 + j w) = sin(phi0) * [A cos(j w)] + cos(phi0) * [A sin(j w)],  j = 0..7   -> 8 FFMA2 for 8 samples.
-__device__ __forceinline__ void rot_loop(const SmemRec *rec, int first, int count, int koff, float2 (&acc)[kSPT / 2])
-{
-#pragma unroll 2
-    for (int i = first; i < first + count; ++i) {
-        const float4 a = rec[i].q[0];
-        const float4 c03 = rec[i].q[1], c47 = rec[i].q[2], s03 = rec[i].q[3], s47 = rec[i].q[4];
-        const uint32_t p = __float_as_uint(a.x) + __float_as_uint(a.y) * static_cast<uint32_t>(koff);
-        const float x = __int2float_rn(static_cast<int32_t>(p)) * kTurnToRad;
-        const float2 sn = dup2(mufu_sin(x)), cs = dup2(mufu_cos(x));
-        acc[0] = __ffma2_rn(sn, make_float2(c03.x, c03.y), acc[0]);
-        acc[1] = __ffma2_rn(sn, make_float2(c03.z, c03.w), acc[1]);
-        acc[2] = __ffma2_rn(sn, make_float2(c47.x, c47.y), acc[2]);
-        acc[3] = __ffma2_rn(sn, make_float2(c47.z, c47.w), acc[3]);
-        acc[0] = __ffma2_rn(cs, make_float2(s03.x, s03.y), acc[0]);
-        acc[1] = __ffma2_rn(cs, make_float2(s03.z, s03.w), acc[1]);
-        acc[2] = __ffma2_rn(cs, make_float2(s47.x, s47.y), acc[2]);
-        acc[3] = __ffma2_rn(cs, make_float2(s47.z, s47.w), acc[3]);
-    }
-}
-
-struct Acc8 {
-    float v[kSPT];
-};
-
 // fp64 path for the K_EXACT records (tones whose fp32 polynomial would be inaccurate, moves shorter than
-// a tile, instant retunes): exact phase per sample, same sine.
-// Out of line and by value so that the hot loops keep their accumulators in registers.
-__device__ __noinline__ Acc8 exact_loop(const ToneRec *tab, const SmemRec *rec, int first, int count,
-                                        int64_t n_thread, Acc8 acc)
+// a block, instant retunes): exact phase per sample, same sine.
+__device__ __forceinline__ void exact_loop(const ToneRec *tab, const SmemRec *rec, int first, int count,
+                                           int64_t n_thread, Acc16 &acc)
 {
     for (int i = first; i < first + count; ++i) {
         const ToneRec &tr = tab[__float_as_uint(rec[i].q[0].x)];
         const float A = rec[i].q[0].z;
+#pragma unroll 1
+        for (int j = 0; j < kPairs; ++j) {
+            const uint32_t p0 = round32(exact_phase(tr, n_thread + 2 * j));
+            const uint32_t p1 = round32(exact_phase(tr, n_thread + 2 * j + 1));
+            float2 v = acc.a[0];
+            // rotate through the pairs so that the loop body indexes a[] statically
+            v.x = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p0)) * kTurnToRad), v.x);
+            v.y = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p1)) * kTurnToRad), v.y);
 #pragma unroll
-        for (int j = 0; j < kSPT; ++j) {
-            const uint32_t p = round32(exact_phase(tr, n_thread + j));
-            acc.v[j] = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p)) * kTurnToRad), acc.v[j]);
+            for (int m = 0; m < kPairs - 1; ++m) acc.a[m] = acc.a[m + 1];
+            acc.a[kPairs - 1] = v;
         }
     }
+}
+
+// All records of ONE block (sorted by kind, starting at rec[first]) added to that block's 16 samples.
+// Out of line: the kernel calls it once per block with that block's accumulators, so the (large) loop code
+// exists once and the accumulators of the other blocks stay in the caller's registers.
+__device__ __noinline__ Acc16 block_loops(const ToneRec *tab, const SmemRec *rec, int first, KindCounts cnt,
+                                          int64_t n_thread, Acc16 acc)
+{
+    const int lane = threadIdx.x & 31;
+    const int koff = lane * kSPT - kHalf;
+    float2 kf[kPairs], kk[kPairs];  // in-block offsets k of the thread's samples, and k^2
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) {
+        kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
+        kk[j] = __fmul2_rn(kf[j], kf[j]);
+    }
+    mufu_loop<K_STATIC>(rec, first, cnt.n[K_STATIC], koff, kf, kk, acc);
+    first += cnt.n[K_STATIC];
+    if (cnt.n[K_QUAD]) mufu_loop<K_QUAD>(rec, first, cnt.n[K_QUAD], koff, kf, kk, acc);
+    first += cnt.n[K_QUAD];
+    if (cnt.n[K_DEG4]) mufu_loop<K_DEG4>(rec, first, cnt.n[K_DEG4], koff, kf, kk, acc);
+    first += cnt.n[K_DEG4];
+    if (cnt.n[K_DEG6]) mufu_loop<K_DEG6>(rec, first, cnt.n[K_DEG6], koff, kf, kk, acc);
+    first += cnt.n[K_DEG6];
+    if (cnt.n[K_SBEG]) mufu_loop<K_SBEG>(rec, first, cnt.n[K_SBEG], koff, kf, kk, acc);
+    first += cnt.n[K_SBEG];
+    if (cnt.n[K_SEND]) mufu_loop<K_SEND>(rec, first, cnt.n[K_SEND], koff, kf, kk, acc);
+    first += cnt.n[K_SEND];
+    if (cnt.n[K_EXACT]) exact_loop(tab, rec, first, cnt.n[K_EXACT], n_thread, acc);
     return acc;
 }
 
-__device__ __forceinline__ void store_tile(const LaunchParams &lp, int64_t n_thread, const float (&acc)[kSPT])
+// Steps a5-a6 for one block of one thread: 16 consecutive samples starting at absolute index n_thread, as two
+// 8-sample halves (launch ranges are multiples of 8 samples, so each half is inside or outside as a whole).
+__device__ __forceinline__ void store_block(const LaunchParams &lp, int64_t n_thread, const Acc16 &acc)
 {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int64_t off = n_thread + 8 * h - lp.n_begin;
+        if (off < 0 || off >= lp.n_count) continue;
+        const float2 *a = acc.a + 4 * h;
+        if (lp.out_f32) {
+            float4 *o = reinterpret_cast<float4 *>(static_cast<float *>(lp.out) + off);
+            o[0] = make_float4(a[0].x, a[0].y, a[1].x, a[1].y);
+            o[1] = make_float4(a[2].x, a[2].y, a[3].x, a[3].y);
+        } else {
+            uint32_t w[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                int32_t lo, hi;
+                asm("cvt.rni.sat.s16.f32 %0, %1;" : "=r"(lo) : "f"(lp.scale * a[j].x));
+                asm("cvt.rni.sat.s16.f32 %0, %1;" : "=r"(hi) : "f"(lp.scale * a[j].y));
+                w[j] = (static_cast<uint32_t>(lo) & 0xffffu) | (static_cast<uint32_t>(hi) << 16);
+            }
+            *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+    }
+}
+
+// Even/odd accumulators of the angle-addition pass for one block: sample (8 + j) = P_j + Q_j, sample (7 - j) = P_j - Q_j.
+struct PQ {
+    float2 P[kPairs / 2], Q[kPairs / 2];  // pairs (j, j+1), j = 0, 2, 4, 6
+};
+
+__device__ __forceinline__ void pq_add(PQ &pq, float s, float c, const float4 &C03, const float4 &C47, const float4 &S03,
+                                       const float4 &S47)
+{
+    const float2 s2 = dup2(s), c2 = dup2(c);
+    pq.P[0] = __ffma2_rn(s2, make_float2(C03.x, C03.y), pq.P[0]);
+    pq.P[1] = __ffma2_rn(s2, make_float2(C03.z, C03.w), pq.P[1]);
+    pq.P[2] = __ffma2_rn(s2, make_float2(C47.x, C47.y), pq.P[2]);
+    pq.P[3] = __ffma2_rn(s2, make_float2(C47.z, C47.w), pq.P[3]);
+    pq.Q[0] = __ffma2_rn(c2, make_float2(S03.x, S03.y), pq.Q[0]);
+    pq.Q[1] = __ffma2_rn(c2, make_float2(S03.z, S03.w), pq.Q[1]);
+    pq.Q[2] = __ffma2_rn(c2, make_float2(S47.x, S47.y), pq.Q[2]);
+    pq.Q[3] = __ffma2_rn(c2, make_float2(S47.z, S47.w), pq.Q[3]);
+}
+
+// next block of the tile: the phase advances by kBlock*w
+__device__ __forceinline__ void rotate(float &s, float &c, float cr, float sr)
+{
+    const float s1 = fmaf(s, cr, c * sr);
+    const float c1 = fmaf(c, cr, -(s * sr));
+    s = s1;
+    c = c1;
+}
+
+__device__ __forceinline__ Acc16 pq_to_samples(const PQ &pq)
+{
+    Acc16 d;
+#pragma unroll
+    for (int m = 0; m < kPairs / 2; ++m) {
+        const float2 p = pq.P[m], q = pq.Q[m];              // j = 2m, 2m+1
+        d.a[4 + m] = make_float2(p.x + q.x, p.y + q.y);      // samples 8 + 2m, 9 + 2m
+        d.a[3 - m] = make_float2(p.y - q.y, p.x - q.x);      // samples 6 - 2m, 7 - 2m
+    }
+    return d;
+}
+
+// A work unit is RB consecutive blocks of one 2048-sample tile (RB = 4: the whole tile).  SPLIT warps share a
+// unit, each taking 1/SPLIT of the tones; a CTA holds kWarps/SPLIT units.  RB only sets how much work a warp
+// takes (small launches use small units to fill the GPU): every sample goes through the same arithmetic for
+// every RB, because all phases are anchored to the tile (block r is reached by r rotations from block 0).
+// ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine); everything else
+// (and every tone when !ROT) takes the per-block MUFU pass.
+template <int SPLIT, bool ROT, int RB>
+__global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchParams lp)
+{
+    constexpr int kUnitsPerCta = kWarps / SPLIT;
+    constexpr int kUnitsPerTile = kBlocksPerTile / RB;
+    __shared__ SmemRec s_rec[kWarps][kBatch];          // pass 2 records; pass 1 uses the first 16 bytes of each
+    __shared__ uint32_t s_mov[kWarps][kMaxBatches];    // per batch of 32 tones: which ones take pass 2 in this tile
+    __shared__ __align__(16) float s_red[SPLIT > 1 ? kWarps : 1][SPLIT > 1 ? kBlock : 1];
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int unit_in_cta = warp / SPLIT;
+    const int rank = warp % SPLIT;
+    const unsigned lt = (1u << lane) - 1u;
+
+    // tiles are anchored to absolute sample indices (chunk-size invariance, SURVEY.md 8(b) "Determinism")
+    const int64_t first_tile = lp.n_begin / kTile;  // n_begin >= 0
+    const int64_t unit = static_cast<int64_t>(blockIdx.x) * kUnitsPerCta + unit_in_cta;
+    const int64_t tile = first_tile + unit / kUnitsPerTile;
+    const int r0 = static_cast<int>(unit % kUnitsPerTile) * RB;  // first block of the unit within its tile
+    const int64_t tile_base = tile * kTile;
+    const int64_t unit_base = tile_base + static_cast<int64_t>(r0) * kBlock;
+    const int64_t n_end = lp.n_begin + lp.n_count;
+    const bool tile_live = unit_base < n_end && unit_base + RB * kBlock > lp.n_begin;
+
+    const int per = (lp.n_tones + SPLIT - 1) / SPLIT;
+    const int t_begin = rank * per;
+    const int t_end = min(lp.n_tones, t_begin + per);
+    SmemRec *rec = s_rec[warp];
+    uint32_t *mov = s_mov[warp];
+
+    Acc16 acc[RB];
+#pragma unroll
+    for (int r = 0; r < RB; ++r)
+#pragma unroll
+        for (int j = 0; j < kPairs; ++j) acc[r].a[j] = make_float2(0.f, 0.f);
+
+    if (tile_live) {
+        int n_pass2 = 0;
+        // ---- pass 1: tones that are static over the whole tile (angle addition), and the list of the others
+        if (ROT) {
+            PQ pq[RB];
+#pragma unroll
+            for (int r = 0; r < RB; ++r)
+#pragma unroll
+                for (int m = 0; m < kPairs / 2; ++m) pq[r].P[m] = pq[r].Q[m] = make_float2(0.f, 0.f);
+            const double tb_d = static_cast<double>(tile_base);
+            // phase reference of block 0: its centre tile_base + kHalf, minus the half sample of the pair centring
+            const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
+            const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the block centre
+            for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
+                const int t = tb + lane;
+                bool is_static = false, is_mover = false;
+                uint32_t c0 = 0, c1 = 0, tabofs = 0;
+                if (t < t_end) {
+                    const ToneRec *tr = lp.tab + t;
+                    const uint4 v0 = ldg16(tr);                                          // A, cls, theta_pre
+                    const uint4 v1 = ldg16(reinterpret_cast<const char *>(tr) + 16);   // w_pre, theta_post
+                    uint64_t th = u64_of(v0.z, v0.w), w = u64_of(v1.x, v1.y);
+                    tabofs = static_cast<uint32_t>(t) * static_cast<uint32_t>(sizeof(ToneRec)) +
+                             static_cast<uint32_t>(offsetof(ToneRec, rot_pre));
+                    is_static = true;
+                    if ((static_cast<int32_t>(v0.y) & 0xff) != CLS_STATIC) {
+                        const uint4 v2 = ldg16(reinterpret_cast<const char *>(tr) + 32);  // w_post, ns_int
+                        const uint4 v3 = ldg16(reinterpret_cast<const char *>(tr) + 48);  // ns_frac, Tn
+                        const double ua = (tb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the tile's first sample
+                        const double ub = ua + static_cast<double>(kTile - 1);
+                        if (ub <= 0.0) {
+                            // whole tile before the move: pre-move carrier
+                        } else if (ua >= f64_of(v3.z, v3.w)) {
+                            th = u64_of(v1.z, v1.w);
+                            w = u64_of(v2.x, v2.y);
+                            tabofs += static_cast<uint32_t>(offsetof(ToneRec, rot_post) - offsetof(ToneRec, rot_pre));
+                        } else {
+                            is_static = false;
+                            is_mover = true;
+                        }
+                    }
+                    c0 = round32(th + w * a0 - (w >> 1));
+                    c1 = round32(w);
+                }
+                const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
+                const unsigned m_sta = __ballot_sync(0xffffffffu, is_static);
+                if (lane == 0) mov[b] = m_mov;
+                n_pass2 += __popc(m_mov);
+                const int n_sta = __popc(m_sta);
+                __syncwarp();  // previous batch's readers are done
+                if (is_static) *reinterpret_cast<uint4 *>(&rec[__popc(m_sta & lt)]) = make_uint4(c0, c1, tabofs, 0u);
+                __syncwarp();
+#pragma unroll 1
+                for (int i = 0; i < n_sta; ++i) {
+                    const uint4 h = *reinterpret_cast<const uint4 *>(&rec[i]);
+                    const float4 *g = reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(lp.tab) + h.z);
+                    const float4 C03 = __ldg(g), C47 = __ldg(g + 1), S03 = __ldg(g + 2), S47 = __ldg(g + 3);
+                    const float4 rs = __ldg(g + 4);  // cr, sr
+                    const uint32_t p = h.x + h.y * static_cast<uint32_t>(off);
+                    const float x = __int2float_rn(static_cast<int32_t>(p)) * kTurnToRad;
+                    float s = mufu_sin(x), c = mufu_cos(x);  // block 0 of the tile
+#pragma unroll 1
+                    for (int r = 0; r < r0; ++r) rotate(s, c, rs.x, rs.y);
+                    pq_add(pq[0], s, c, C03, C47, S03, S47);
+#pragma unroll
+                    for (int r = 1; r < RB; ++r) {
+                        rotate(s, c, rs.x, rs.y);
+                        pq_add(pq[r], s, c, C03, C47, S03, S47);
+                    }
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < RB; ++r) acc[r] = pq_to_samples(pq[r]);
+        } else {
+            for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
+                const int left = t_end - tb;
+                if (lane == 0) mov[b] = left >= 32 ? 0xffffffffu : ((1u << left) - 1u);
+            }
+            n_pass2 = t_end - t_begin;
+            __syncwarp();
+        }
+
+        // ---- pass 2: per (tone, block) re-centring and one MUFU.SIN per tone-sample
+        if (n_pass2 > 0) {
+            __syncwarp();
+            for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
+                const unsigned m = mov[b];
+                if (m == 0) continue;
+                const int nm = __popc(m);
+                // lane = (tone slot, block of the unit).  Few movers: all their blocks in one sub-batch (32/RB tones
+                // x RB blocks); many: one sub-batch per block with 32 tones, so each block_loops call has more to do.
+                const bool by_block = nm > kBatch / RB;
+                const int n_sub = by_block ? RB : 1;
+                for (int q = 0; q < n_sub; ++q) {
+                    const int slot = by_block ? lane : lane / RB;
+                    const int r_lane = by_block ? q : lane % RB;
+                    const int64_t blk_base = unit_base + static_cast<int64_t>(r_lane) * kBlock;
+                    BlockRec br;
+                    br.kind = K_NONE;
+                    if (slot < nm && blk_base < n_end && blk_base + kBlock > lp.n_begin) {
+                        const int t = tb + static_cast<int>(__fns(m, 0, slot + 1));
+                        br = block_prologue(lp.tab + t, t, static_cast<uint64_t>(blk_base + kHalf), static_cast<double>(blk_base));
+                    }
+                    // sort the records by (block, kind) so each inner loop is warp-uniform (no divergence)
+                    KindCounts cnt[RB];
+                    int first_of[RB];
+                    int pos = -1, before = 0;
+#pragma unroll
+                    for (int r = 0; r < RB; ++r) {
+                        first_of[r] = before;
+#pragma unroll
+                        for (int kd = 0; kd < K_COUNT; ++kd) {
+                            const bool mine = (r_lane == r) && (br.kind == kd);
+                            const unsigned bm = __ballot_sync(0xffffffffu, mine);
+                            cnt[r].n[kd] = __popc(bm);
+                            if (mine) pos = before + __popc(bm & lt);
+                            before += cnt[r].n[kd];
+                        }
+                    }
+                    __syncwarp();  // previous sub-batch's readers are done
+                    if (pos >= 0) {
+                        rec[pos].q[0] = make_float4(__uint_as_float(br.c0), __uint_as_float(br.c1), br.A, br.c2);
+                        rec[pos].q[1] = make_float4(br.c3, br.c4, br.c5, br.c6);
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int r = 0; r < RB; ++r) {
+                        const int n_r = (r + 1 < RB ? first_of[r + 1] : before) - first_of[r];
+                        if (n_r > 0)
+                            acc[r] = block_loops(lp.tab, rec, first_of[r], cnt[r], unit_base + r * kBlock + lane * kSPT, acc[r]);
+                    }
+                }
+            }
+        }
+    }
+
+    // ---- partial sums of the SPLIT warps of a tile meet in shared memory, block by block
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+        if (SPLIT > 1) {
+            if (r > 0) __syncthreads();
+            if (rank != 0) {
+                float4 *mine = reinterpret_cast<float4 *>(&s_red[warp][lane * kSPT]);
+#pragma unroll
+                for (int v = 0; v < kSPT / 4; ++v)
+                    mine[v] = make_float4(acc[r].a[2 * v].x, acc[r].a[2 * v].y, acc[r].a[2 * v + 1].x, acc[r].a[2 * v + 1].y);
+            }
+            __syncthreads();
+            if (rank == 0) {
+                // fixed summation order (rank 0, 1, ...) keeps the result independent of scheduling
+                for (int r2 = 1; r2 < SPLIT; ++r2) {
+                    const float4 *o = reinterpret_cast<const float4 *>(&s_red[warp + r2][lane * kSPT]);
+#pragma unroll
+                    for (int v = 0; v < kSPT / 4; ++v) {
+                        const float4 u = o[v];
+                        acc[r].a[2 * v].x += u.x; acc[r].a[2 * v].y += u.y;
+                        acc[r].a[2 * v + 1].x += u.z; acc[r].a[2 * v + 1].y += u.w;
+                    }
+                }
+            }
+        }
+        if (rank == 0 && tile_live) store_block(lp, unit_base + r * kBlock + lane * kSPT, acc[r]);
+    }
+}
+
+// Reference-grade engine: closed form in fp64 + 64-bit fixed point and fp64 sine for every
+// (tone, sample); one thread per 8 consecutive samples.  ~50x slower than the MUFU engine.
+constexpr int kSPT64 = 8;
+__global__ void __launch_bounds__(256) awg_fp64_kernel(const LaunchParams lp)
+{
+    const int64_t g = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const int64_t n_thread = lp.n_begin + g * kSPT64;
+    if (g * kSPT64 >= lp.n_count) return;
+    double acc[kSPT64];
+#pragma unroll
+    for (int j = 0; j < kSPT64; ++j) acc[j] = 0.0;
+    for (int t = 0; t < lp.n_tones; ++t) {
+        const ToneRec &tr = lp.tab[t];
+        const double A = static_cast<double>(tr.A);
+#pragma unroll
+        for (int j = 0; j < kSPT64; ++j) {
+            const int64_t ph = static_cast<int64_t>(exact_phase(tr, n_thread + j));  // signed: [-0.5, 0.5) turn
+            acc[j] += A * sinpi(static_cast<double>(ph) * (2.0 / kTwo64));
+        }
+    }
     const int64_t off = n_thread - lp.n_begin;
-    if (off < 0 || off >= lp.n_count) return;  // n_begin and n_count are multiples of 8: all or nothing per thread
     if (lp.out_f32) {
         float4 *o = reinterpret_cast<float4 *>(static_cast<float *>(lp.out) + off);
-        o[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-        o[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+        o[0] = make_float4(static_cast<float>(acc[0]), static_cast<float>(acc[1]), static_cast<float>(acc[2]), static_cast<float>(acc[3]));
+        o[1] = make_float4(static_cast<float>(acc[4]), static_cast<float>(acc[5]), static_cast<float>(acc[6]), static_cast<float>(acc[7]));
     } else {
         uint32_t w[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             int32_t lo, hi;
-            asm("cvt.rni.sat.s16.f32 %0, %1;" : "=r"(lo) : "f"(lp.scale * acc[2 * j]));
-            asm("cvt.rni.sat.s16.f32 %0, %1;" : "=r"(hi) : "f"(lp.scale * acc[2 * j + 1]));
+            asm("cvt.rni.sat.s16.f32 %0, %1;" : "=r"(lo) : "f"(lp.scale * static_cast<float>(acc[2 * j])));
+            asm("cvt.rni.sat.s16.f32 %0, %1;" : "=r"(hi) : "f"(lp.scale * static_cast<float>(acc[2 * j + 1])));
             w[j] = (static_cast<uint32_t>(lo) & 0xffffu) | (static_cast<uint32_t>(hi) << 16);
         }
         *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = make_uint4(w[0], w[1], w[2], w[3]);
     }
 }
 
-// SPLIT warps share one 256-sample tile, each taking 1/SPLIT of the tones; a CTA holds kWarps/SPLIT tiles.
-// ROT: static tiles use the angle-addition path (FMA engine) instead of one MUFU.SIN per tone-sample.
-template <int SPLIT, bool ROT>
-__global__ void __launch_bounds__(kWarps * 32, 4) awg_synth_kernel(const LaunchParams lp)
-{
-    constexpr int kTilesPerCta = kWarps / SPLIT;
-    __shared__ SmemRec s_rec[kWarps][kBatch];
-    __shared__ __align__(16) float s_red[SPLIT > 1 ? kWarps : 1][SPLIT > 1 ? kTile : 1];
-
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    const int tile_in_cta = warp / SPLIT;
-    const int rank = warp % SPLIT;
-
-    // tiles are anchored to absolute sample indices (chunk-size invariance, SURVEY.md 8(b) "Determinism")
-    const int64_t first_tile = lp.n_begin / kTile;  // n_begin >= 0
-    const int64_t tile = first_tile + static_cast<int64_t>(blockIdx.x) * kTilesPerCta + tile_in_cta;
-    const int64_t tile_base = tile * kTile;
-    const bool tile_live = tile_base < lp.n_begin + lp.n_count;
-
-    const int koff = lane * kSPT - kHalf;
-    float2 kf[kSPT / 2], kk[kSPT / 2], acc2[kSPT / 2];
-#pragma unroll
-    for (int j = 0; j < kSPT / 2; ++j) {
-        kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
-        kk[j] = make_float2(kf[j].x * kf[j].x, kf[j].y * kf[j].y);
-        acc2[j] = make_float2(0.f, 0.f);
-    }
-
-    const int per = (lp.n_tones + SPLIT - 1) / SPLIT;
-    const int t_begin = rank * per;
-    const int t_end = min(lp.n_tones, t_begin + per);
-    SmemRec *rec = s_rec[warp];
-
-    if (tile_live) {
-        const uint64_t nc = static_cast<uint64_t>(tile_base + kHalf);
-        const double tb_d = static_cast<double>(tile_base);
-        for (int tb = t_begin; tb < t_end; tb += kBatch) {
-            const int t = tb + lane;
-            TileRec r;
-            r.kind = K_NONE;
-            if (t < t_end) r = tile_prologue(lp.tab + t, t, nc, tb_d);
-            // compact the batch by kind so each inner loop is warp-uniform (no divergence)
-            int n_of[K_COUNT];
-            int pos = -1, before = 0;
-            const unsigned lt = (1u << lane) - 1u;
-#pragma unroll
-            for (int kd = 0; kd < K_COUNT; ++kd) {
-                const unsigned m = __ballot_sync(0xffffffffu, r.kind == kd);
-                n_of[kd] = __popc(m);
-                if (r.kind == kd) pos = before + __popc(m & lt);
-                before += n_of[kd];
-            }
-            __syncwarp();  // previous batch's readers are done
-            if (pos >= 0) {
-                rec[pos].q[0] = make_float4(__uint_as_float(r.c0), __uint_as_float(r.c1), r.A, r.c2);
-                if (ROT && r.kind == K_STATIC) {
-                    const float4 *g = reinterpret_cast<const float4 *>(r.rot);
-#pragma unroll
-                    for (int v = 0; v < 4; ++v) rec[pos].q[1 + v] = __ldg(g + v);
-                } else {
-                    rec[pos].q[1] = make_float4(r.c3, r.c4, r.c5, r.c6);
-                }
-            }
-            __syncwarp();
-            int first = 0;
-            if (ROT) rot_loop(rec, first, n_of[K_STATIC], koff, acc2);
-            else mufu_loop<K_STATIC>(rec, first, n_of[K_STATIC], koff, kf, kk, acc2);
-            first += n_of[K_STATIC];
-            if (n_of[K_QUAD]) mufu_loop<K_QUAD>(rec, first, n_of[K_QUAD], koff, kf, kk, acc2);
-            first += n_of[K_QUAD];
-            if (n_of[K_DEG4]) mufu_loop<K_DEG4>(rec, first, n_of[K_DEG4], koff, kf, kk, acc2);
-            first += n_of[K_DEG4];
-            if (n_of[K_DEG6]) mufu_loop<K_DEG6>(rec, first, n_of[K_DEG6], koff, kf, kk, acc2);
-            first += n_of[K_DEG6];
-            if (n_of[K_SBEG]) mufu_loop<K_SBEG>(rec, first, n_of[K_SBEG], koff, kf, kk, acc2);
-            first += n_of[K_SBEG];
-            if (n_of[K_SEND]) mufu_loop<K_SEND>(rec, first, n_of[K_SEND], koff, kf, kk, acc2);
-            first += n_of[K_SEND];
-            if (n_of[K_EXACT]) {
-                Acc8 a8;
-#pragma unroll
-                for (int j = 0; j < kSPT / 2; ++j) { a8.v[2 * j] = acc2[j].x; a8.v[2 * j + 1] = acc2[j].y; }
-                a8 = exact_loop(lp.tab, rec, first, n_of[K_EXACT], tile_base + lane * kSPT, a8);
-#pragma unroll
-                for (int j = 0; j < kSPT / 2; ++j) acc2[j] = make_float2(a8.v[2 * j], a8.v[2 * j + 1]);
-            }
-        }
-    }
-
-    float acc[kSPT];
-#pragma unroll
-    for (int j = 0; j < kSPT / 2; ++j) { acc[2 * j] = acc2[j].x; acc[2 * j + 1] = acc2[j].y; }
-    if (SPLIT > 1) {
-        float4 *mine = reinterpret_cast<float4 *>(&s_red[warp][lane * kSPT]);
-        mine[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-        mine[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
-        __syncthreads();
-        if (rank != 0 || !tile_live) return;
-        // fixed summation order (rank 0, 1, ...) keeps the result independent of scheduling
-        for (int r2 = 1; r2 < SPLIT; ++r2) {
-            const float4 *o = reinterpret_cast<const float4 *>(&s_red[warp + r2][lane * kSPT]);
-            const float4 u = o[0], v = o[1];
-            acc[0] += u.x; acc[1] += u.y; acc[2] += u.z; acc[3] += u.w;
-            acc[4] += v.x; acc[5] += v.y; acc[6] += v.z; acc[7] += v.w;
-        }
-    } else if (!tile_live) {
-        return;
-    }
-    store_tile(lp, tile_base + lane * kSPT, acc);
-}
-
-// Reference-grade engine: closed form in fp64 + 64-bit fixed point and fp64 sine for every
-// (tone, sample); one thread per 8 consecutive samples.  ~50x slower than the MUFU engine.
-__global__ void __launch_bounds__(256) awg_fp64_kernel(const LaunchParams lp)
-{
-    const int64_t g = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    const int64_t n_thread = lp.n_begin + g * kSPT;
-    if (g * kSPT >= lp.n_count) return;
-    double acc[kSPT];
-#pragma unroll
-    for (int j = 0; j < kSPT; ++j) acc[j] = 0.0;
-    for (int t = 0; t < lp.n_tones; ++t) {
-        const ToneRec &tr = lp.tab[t];
-        const double A = static_cast<double>(tr.A);
-#pragma unroll
-        for (int j = 0; j < kSPT; ++j) {
-            const int64_t ph = static_cast<int64_t>(exact_phase(tr, n_thread + j));  // signed: [-0.5, 0.5) turn
-            acc[j] += A * sinpi(static_cast<double>(ph) * (2.0 / kTwo64));
-        }
-    }
-    float out[kSPT];
-#pragma unroll
-    for (int j = 0; j < kSPT; ++j) out[j] = static_cast<float>(acc[j]);
-    store_tile(lp, n_thread, out);
-}
-
-// Partial trajectory-table update: one 256-byte record per block of 16 threads x 16 bytes.
+// Partial trajectory-table update: one tone record per block of sizeof(ToneRec)/16 threads x 16 bytes.
 __global__ void awg_scatter_kernel(ToneRec *table, const ToneRec *src, const int32_t *idx, int n)
 {
     const int j = blockIdx.x;
@@ -486,16 +657,27 @@ __global__ void awg_scatter_kernel(ToneRec *table, const ToneRec *src, const int
     d4[threadIdx.x] = s4[threadIdx.x];
 }
 
-template <bool ROT>
-void launch_split(const LaunchParams &lp, int split, unsigned tiles, cudaStream_t stream)
+template <bool ROT, int RB>
+void launch_split(const LaunchParams &lp, int split, int64_t tiles, cudaStream_t stream)
 {
-    auto grid_for = [&](int s) { return (tiles + (kWarps / s) - 1) / (kWarps / s); };
+    const int64_t units = tiles * (kBlocksPerTile / RB);
+    auto grid_for = [&](int s) { return static_cast<unsigned>((units + (kWarps / s) - 1) / (kWarps / s)); };
     switch (split) {
-        case 1: awg_synth_kernel<1, ROT><<<grid_for(1), kWarps * 32, 0, stream>>>(lp); break;
-        case 2: awg_synth_kernel<2, ROT><<<grid_for(2), kWarps * 32, 0, stream>>>(lp); break;
-        case 4: awg_synth_kernel<4, ROT><<<grid_for(4), kWarps * 32, 0, stream>>>(lp); break;
-        default: awg_synth_kernel<8, ROT><<<grid_for(8), kWarps * 32, 0, stream>>>(lp); break;
+        case 1: awg_synth_kernel<1, ROT, RB><<<grid_for(1), kWarps * 32, 0, stream>>>(lp); break;
+        case 2: awg_synth_kernel<2, ROT, RB><<<grid_for(2), kWarps * 32, 0, stream>>>(lp); break;
+        case 4: awg_synth_kernel<4, ROT, RB><<<grid_for(4), kWarps * 32, 0, stream>>>(lp); break;
+        default: awg_synth_kernel<8, ROT, RB><<<grid_for(8), kWarps * 32, 0, stream>>>(lp); break;
     }
+}
+
+template <bool ROT>
+void launch_rb(const LaunchParams &lp, int split, int64_t tiles, int n_sm, cudaStream_t stream)
+{
+    // the largest unit that still gives every SM its two resident CTAs
+    const int64_t want = 2 * static_cast<int64_t>(n_sm) * (kWarps / split);  // units
+    if (tiles >= want) launch_split<ROT, 4>(lp, split, tiles, stream);
+    else if (tiles * 2 >= want) launch_split<ROT, 2>(lp, split, tiles, stream);
+    else launch_split<ROT, 1>(lp, split, tiles, stream);
 }
 
 }  // namespace
@@ -512,19 +694,27 @@ cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream
 {
     if (lp.n_count <= 0) return cudaSuccess;
     if (engine == AWG_ENGINE_FP64) {
-        const int64_t threads = lp.n_count / kSPT;
+        const int64_t threads = lp.n_count / kSPT64;
         awg_fp64_kernel<<<static_cast<unsigned>((threads + 255) / 256), 256, 0, stream>>>(lp);
     } else {
         const int64_t first_tile = lp.n_begin / kTile;
         const int64_t last_tile = (lp.n_begin + lp.n_count - 1) / kTile;
-        const unsigned tiles = static_cast<unsigned>(last_tile - first_tile + 1);
+        const int64_t tiles = last_tile - first_tile + 1;
+        static int n_sm = 0;
+        if (n_sm == 0) {
+            int dev = 0, v = 0;
+            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+                n_sm = v;
+            else
+                n_sm = 148;
+        }
         // Warps per tile depend on the tone count ONLY (>= 32 tones per warp, at most 8 warps), never on the
         // launch size: the order in which tone partial sums are added is then the same for every chunking,
         // which keeps the output bit-identical across chunk sizes (include/awg.h "pure function").
         int split = 1;
         while (split < kWarps && lp.n_tones / (split * 2) >= 32) split *= 2;
-        if (engine == AWG_ENGINE_FMA) launch_split<true>(lp, split, tiles, stream);
-        else launch_split<false>(lp, split, tiles, stream);
+        if (engine == AWG_ENGINE_FMA) launch_rb<true>(lp, split, tiles, n_sm, stream);
+        else launch_rb<false>(lp, split, tiles, n_sm, stream);
     }
     count_launch();
     return cudaGetLastError();

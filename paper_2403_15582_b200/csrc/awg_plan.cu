@@ -38,7 +38,7 @@ awg_status fail_cuda(cudaError_t e, const char *what)
 namespace {
 
 const long double kTwoPiL = 6.283185307179586476925286766559005768L;
-constexpr int kRadius = 128;  // half of the kernel's 256-sample tile
+constexpr int kRadius = kBlock / 2;  // half of the kernel's 512-sample block (span of one Taylor re-centring)
 
 // frac(x) as 64-bit fixed-point turns.
 uint64_t frac64(long double x)
@@ -56,7 +56,7 @@ bool finite_all(const double *a, int n)
     return true;
 }
 
-// Polynomial class of a moving tone (which Taylor terms of DT*g(s) matter inside a 256-sample tile).
+// Polynomial class of a moving tone (which Taylor terms of DT*g(s) matter inside a 512-sample block).
 int classify(int profile, long double DT, long double Tn)
 {
     if (!(Tn >= 2.0L * kRadius)) return CLS_EXACT;  // move shorter than a tile: every tile straddles anyway
@@ -65,7 +65,7 @@ int classify(int profile, long double DT, long double Tn)
     const double R = kRadius;
     const double tol_drop = 2e-8;   // cycles: dropped Taylor terms
     const double max_mag = 0.25;    // cycles: fp32 polynomial magnitude (its rounding error is ~2^-23 of this)
-    // tiles that contain one end of the move evaluate DT*g over up to 256 samples from that end in fp32
+    // blocks that contain one end of the move evaluate DT*g over up to 2R samples from that end in fp32
     const double sg = 2.0 * R * r;
     const double DTa = static_cast<double>(fabsl(DT));
     if (profile == AWG_PROFILE_LINEAR) {
@@ -85,19 +85,30 @@ int classify(int profile, long double DT, long double Tn)
     return CLS_DEG6;
 }
 
-// Rotation table of a carrier for the angle-addition engine: A cos(2 pi j w), A sin(2 pi j w), j = 0..7,
-// from the 64-bit fixed-point frequency, evaluated in double, rounded once to fp32.
-void make_rot(float *rot, uint64_t w, float A)
+// Table of a carrier for the angle-addition engine (RotTable, awg_internal.h): A cos, A sin of (j + 1/2) w for the
+// symmetric sample pairs, and cos, sin of kBlock*w for the block-to-block rotation.  Angles come from the 64-bit
+// fixed-point frequency in long double (the products stay below 2^10 turns: rounding <= 2^-54 turn), the
+// trigonometric functions are evaluated in double and rounded once to fp32.
+void make_rot(RotTable &rot, uint64_t w, float A)
 {
+    const long double wl = ldexpl(static_cast<long double>(w), -64);  // turns per sample, exact
     const double two_pi = 6.283185307179586476925286766559;
-    for (int j = 0; j < kSPT; ++j) {
-        // j*w wraps exactly in u64; as a signed fraction of a turn it is exact in double to 2^-53
-        const double turns = std::ldexp(static_cast<double>(static_cast<int64_t>(w * static_cast<uint64_t>(j))), -64);
+    auto angle = [&](long double mult) {
+        long double t = mult * wl;
+        t -= floorl(t + 0.5L);  // [-1/2, 1/2) turn
+        return two_pi * static_cast<double>(t);
+    };
+    std::memset(&rot, 0, sizeof rot);
+    for (int j = 0; j < kPairs; ++j) {
         double sn, cs;
-        sincos(two_pi * turns, &sn, &cs);
-        rot[j] = static_cast<float>(static_cast<double>(A) * cs);
-        rot[kSPT + j] = static_cast<float>(static_cast<double>(A) * sn);
+        sincos(angle(static_cast<long double>(j) + 0.5L), &sn, &cs);
+        rot.C[j] = static_cast<float>(static_cast<double>(A) * cs);
+        rot.S[j] = static_cast<float>(static_cast<double>(A) * sn);
     }
+    double sn, cs;
+    sincos(angle(static_cast<long double>(kBlock)), &sn, &cs);
+    rot.cr = static_cast<float>(cs);
+    rot.sr = static_cast<float>(sn);
 }
 
 void make_static(HostTone &h)
@@ -113,7 +124,7 @@ void make_static(HostTone &h)
     h.theta_post = h.theta_pre;
     h.w_post = h.w_pre;
     make_rot(h.rot_pre, h.w_pre, h.A);
-    std::memcpy(h.rot_post, h.rot_pre, sizeof h.rot_post);
+    h.rot_post = h.rot_pre;
 }
 
 // Fills the move part of h (everything but theta_pre/w_pre/f0/A) for a move f0 -> f1 that starts at the
@@ -182,8 +193,8 @@ static void fill_record(const HostTone &h, ToneRec &r)
             r.q[k - 2] = static_cast<float>(q / fact);
         }
     }
-    std::memcpy(r.rot_pre, h.rot_pre, sizeof r.rot_pre);
-    std::memcpy(r.rot_post, h.rot_post, sizeof r.rot_post);
+    r.rot_pre = h.rot_pre;
+    r.rot_post = h.rot_post;
 }
 
 // Makes the device table current on `stream`.  A changed table goes to the next of kTableVersions device

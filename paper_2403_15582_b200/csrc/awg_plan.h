@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include "awg.h"
+#include "awg_internal.h"
 
 namespace awg {
 
@@ -24,7 +25,7 @@ struct HostTone {
     float A = 0;
     int32_t profile = AWG_PROFILE_STATIC;
     int32_t cls = 0;
-    float rot_pre[16] = {}, rot_post[16] = {};  // {A cos(2 pi j w)}, {A sin(2 pi j w)}, j = 0..7, per carrier
+    RotTable rot_pre = {}, rot_post = {};  // angle-addition tables of the two carriers
 };
 
 awg_status fail(awg_status code, const char *fmt, ...);
