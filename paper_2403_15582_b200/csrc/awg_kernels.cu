@@ -212,10 +212,26 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
     return r;
 }
 
-// Per-warp shared-memory record of one (tone, block) item of pass 2: q[0] = {c0 bits, c1 bits, A, c2};
-// q[1] = {c3, c4, c5, c6}.  K_EXACT: c0 = tone index.
-struct __align__(16) SmemRec {
+// ---- shared memory of one warp ------------------------------------------------------------------------------
+// One tile-static tone of the current batch (angle-addition pass): carrier phase (u32 turns) at the half-integer
+// pair centre of lane 0 in block 0 [c0], per sample [c1] and per block [d], and the tone's pair tables.
+struct __align__(16) StageRec {
+    uint32_t c0, c1, d, pad_;
+    float4 C03, C47, S03, S47;
+};
+static_assert(sizeof(StageRec) == 80, "StageRec must be 80 bytes");
+
+// One re-centred (tone, block) record of the MUFU pass: q[0] = {c0 bits, c1 bits, A, c2}; q[1] = {c3, c4, c5, c6}.
+// K_EXACT: c0 = tone index.
+struct __align__(16) MovRec {
     float4 q[2];
+};
+
+struct __align__(16) WarpSmem {
+    StageRec st[kBatch + 1];                // +1: the loop prefetches one carrier record ahead
+    MovRec mrec[kBatch];
+    float4 park[kBlocksPerTile][kSPT / 4][32];   // partial sums of the tile: [block][4 samples][lane]
+    uint32_t mov[kMaxBatches];              // per batch of 32 tones: which ones take the MUFU pass in this tile
 };
 
 // 16 samples of one block of one thread, as 8 packed pairs: a[j] = samples (2j, 2j+1).
@@ -223,114 +239,89 @@ struct Acc16 {
     float2 a[kPairs];
 };
 
-struct KindCounts {
-    int n[K_COUNT];
-};
+__device__ __forceinline__ void park_store(WarpSmem &ws, int r, int lane, const Acc16 &acc)
+{
+#pragma unroll
+    for (int v = 0; v < kSPT / 4; ++v)
+        ws.park[r][v][lane] = make_float4(acc.a[2 * v].x, acc.a[2 * v].y, acc.a[2 * v + 1].x, acc.a[2 * v + 1].y);
+}
 
-// Steps a2-a4, MUFU path, for `count` records starting at rec[first], all of kind KIND.  Samples go in pairs
-// through the packed fp32x2 instructions of sm_100 (FMUL2 / FFMA2: one issue slot for two samples).
+__device__ __forceinline__ void park_add(const WarpSmem &ws, int r, int lane, Acc16 &acc)
+{
+#pragma unroll
+    for (int v = 0; v < kSPT / 4; ++v) {
+        const float4 u = ws.park[r][v][lane];
+        acc.a[2 * v].x += u.x; acc.a[2 * v].y += u.y;
+        acc.a[2 * v + 1].x += u.z; acc.a[2 * v + 1].y += u.w;
+    }
+}
+
+// Steps a2-a4, MUFU path, for ONE record of kind KIND.  Samples go in pairs through the packed fp32x2
+// instructions of sm_100 (FMUL2 / FFMA2: one issue slot for two samples); the 16 sine chains are independent.
 template <int KIND>
-__device__ __forceinline__ void mufu_loop(const SmemRec *rec, int first, int count, int koff,
-                                          const float2 (&kfs)[kPairs], const float2 (&kks)[kPairs], Acc16 &acc)
+__device__ __forceinline__ void mufu_rec(const float4 a, const float4 b, int koff, const float2 (&kfs)[kPairs],
+                                         const float2 (&kks)[kPairs], Acc16 &acc)
 {
     const float2 K2 = dup2(kTurnToRad);
-#pragma unroll 1
-    for (int i = first; i < first + count; ++i) {
-        const float4 a = rec[i].q[0];
-        const uint32_t c0 = __float_as_uint(a.x), c1 = __float_as_uint(a.y);
-        const float A = a.z;
-        const uint32_t base = c0 + c1 * static_cast<uint32_t>(koff);
-        float4 b;
-        if (KIND >= K_DEG4) b = rec[i].q[1];
-#pragma unroll
-        for (int j = 0; j < kPairs; ++j) {
-            const uint32_t p0 = base + c1 * static_cast<uint32_t>(2 * j);
-            const uint32_t p1 = base + c1 * static_cast<uint32_t>(2 * j + 1);
-            const float2 f = make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1)));
-            const float2 kf = kfs[j];
-            float2 x;
-            if (KIND == K_STATIC) {
-                x = __fmul2_rn(f, K2);
-            } else if (KIND == K_SBEG || KIND == K_SEND) {
-                float2 w;
-                w.x = fmaxf((KIND == K_SBEG ? kf.x : -kf.x) - b.w, 0.f);
-                w.y = fmaxf((KIND == K_SBEG ? kf.y : -kf.y) - b.w, 0.f);
-                const float2 w2 = __fmul2_rn(w, w);
-                float2 poly = __ffma2_rn(dup2(b.z), w, dup2(b.y));
-                poly = __ffma2_rn(poly, w, dup2(b.x));
-                poly = __ffma2_rn(poly, w2, dup2(a.w));
-                x = __ffma2_rn(f, K2, __fmul2_rn(poly, w2));
-            } else {
-                const float2 kk = kks[j];
-                float2 poly;
-                if (KIND == K_QUAD) {
-                    poly = dup2(a.w);
-                } else if (KIND == K_DEG4) {
-                    poly = __ffma2_rn(dup2(b.y), kf, dup2(b.x));
-                    poly = __ffma2_rn(poly, kf, dup2(a.w));
-                } else {
-                    poly = __ffma2_rn(dup2(b.w), kf, dup2(b.z));
-                    poly = __ffma2_rn(poly, kf, dup2(b.y));
-                    poly = __ffma2_rn(poly, kf, dup2(b.x));
-                    poly = __ffma2_rn(poly, kf, dup2(a.w));
-                }
-                x = __ffma2_rn(f, K2, __fmul2_rn(poly, kk));
-            }
-            acc.a[j] = __ffma2_rn(dup2(A), make_float2(mufu_sin(x.x), mufu_sin(x.y)), acc.a[j]);
-        }
-    }
-}
-
-// fp64 path for the K_EXACT records (tones whose fp32 polynomial would be inaccurate, moves shorter than
-// a block, instant retunes): exact phase per sample, same sine.
-__device__ __forceinline__ void exact_loop(const ToneRec *tab, const SmemRec *rec, int first, int count,
-                                           int64_t n_thread, Acc16 &acc)
-{
-    for (int i = first; i < first + count; ++i) {
-        const ToneRec &tr = tab[__float_as_uint(rec[i].q[0].x)];
-        const float A = rec[i].q[0].z;
-#pragma unroll 1
-        for (int j = 0; j < kPairs; ++j) {
-            const uint32_t p0 = round32(exact_phase(tr, n_thread + 2 * j));
-            const uint32_t p1 = round32(exact_phase(tr, n_thread + 2 * j + 1));
-            float2 v = acc.a[0];
-            // rotate through the pairs so that the loop body indexes a[] statically
-            v.x = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p0)) * kTurnToRad), v.x);
-            v.y = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p1)) * kTurnToRad), v.y);
-#pragma unroll
-            for (int m = 0; m < kPairs - 1; ++m) acc.a[m] = acc.a[m + 1];
-            acc.a[kPairs - 1] = v;
-        }
-    }
-}
-
-// All records of ONE block (sorted by kind, starting at rec[first]) added to that block's 16 samples.
-// Out of line: the kernel calls it once per block with that block's accumulators, so the (large) loop code
-// exists once and the accumulators of the other blocks stay in the caller's registers.
-__device__ __noinline__ Acc16 block_loops(const ToneRec *tab, const SmemRec *rec, int first, KindCounts cnt,
-                                          int64_t n_thread, Acc16 acc)
-{
-    const int lane = threadIdx.x & 31;
-    const int koff = lane * kSPT - kHalf;
-    float2 kf[kPairs], kk[kPairs];  // in-block offsets k of the thread's samples, and k^2
+    const uint32_t c0 = __float_as_uint(a.x), c1 = __float_as_uint(a.y);
+    const float A = a.z;
+    const uint32_t base = c0 + c1 * static_cast<uint32_t>(koff);
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) {
-        kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
-        kk[j] = __fmul2_rn(kf[j], kf[j]);
+        const uint32_t p0 = base + c1 * static_cast<uint32_t>(2 * j);
+        const uint32_t p1 = base + c1 * static_cast<uint32_t>(2 * j + 1);
+        const float2 f = make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1)));
+        const float2 kf = kfs[j];
+        float2 x;
+        if (KIND == K_STATIC) {
+            x = __fmul2_rn(f, K2);
+        } else if (KIND == K_SBEG || KIND == K_SEND) {
+            float2 w;
+            w.x = fmaxf((KIND == K_SBEG ? kf.x : -kf.x) - b.w, 0.f);
+            w.y = fmaxf((KIND == K_SBEG ? kf.y : -kf.y) - b.w, 0.f);
+            const float2 w2 = __fmul2_rn(w, w);
+            float2 poly = __ffma2_rn(dup2(b.z), w, dup2(b.y));
+            poly = __ffma2_rn(poly, w, dup2(b.x));
+            poly = __ffma2_rn(poly, w2, dup2(a.w));
+            x = __ffma2_rn(f, K2, __fmul2_rn(poly, w2));
+        } else {
+            const float2 kk = kks[j];
+            float2 poly;
+            if (KIND == K_QUAD) {
+                poly = dup2(a.w);
+            } else if (KIND == K_DEG4) {
+                poly = __ffma2_rn(dup2(b.y), kf, dup2(b.x));
+                poly = __ffma2_rn(poly, kf, dup2(a.w));
+            } else {
+                poly = __ffma2_rn(dup2(b.w), kf, dup2(b.z));
+                poly = __ffma2_rn(poly, kf, dup2(b.y));
+                poly = __ffma2_rn(poly, kf, dup2(b.x));
+                poly = __ffma2_rn(poly, kf, dup2(a.w));
+            }
+            x = __ffma2_rn(f, K2, __fmul2_rn(poly, kk));
+        }
+        acc.a[j] = __ffma2_rn(dup2(A), make_float2(mufu_sin(x.x), mufu_sin(x.y)), acc.a[j]);
     }
-    mufu_loop<K_STATIC>(rec, first, cnt.n[K_STATIC], koff, kf, kk, acc);
-    first += cnt.n[K_STATIC];
-    if (cnt.n[K_QUAD]) mufu_loop<K_QUAD>(rec, first, cnt.n[K_QUAD], koff, kf, kk, acc);
-    first += cnt.n[K_QUAD];
-    if (cnt.n[K_DEG4]) mufu_loop<K_DEG4>(rec, first, cnt.n[K_DEG4], koff, kf, kk, acc);
-    first += cnt.n[K_DEG4];
-    if (cnt.n[K_DEG6]) mufu_loop<K_DEG6>(rec, first, cnt.n[K_DEG6], koff, kf, kk, acc);
-    first += cnt.n[K_DEG6];
-    if (cnt.n[K_SBEG]) mufu_loop<K_SBEG>(rec, first, cnt.n[K_SBEG], koff, kf, kk, acc);
-    first += cnt.n[K_SBEG];
-    if (cnt.n[K_SEND]) mufu_loop<K_SEND>(rec, first, cnt.n[K_SEND], koff, kf, kk, acc);
-    first += cnt.n[K_SEND];
-    if (cnt.n[K_EXACT]) exact_loop(tab, rec, first, cnt.n[K_EXACT], n_thread, acc);
+}
+
+// fp64 path for a K_EXACT record (tones whose fp32 polynomial would be inaccurate, moves shorter than a block,
+// instant retunes): exact phase per sample, same sine.
+__device__ __noinline__ Acc16 exact_rec(const ToneRec *tab, const float4 a, int64_t n_thread, Acc16 acc)
+{
+    const ToneRec &tr = tab[__float_as_uint(a.x)];
+    const float A = a.z;
+#pragma unroll 1
+    for (int j = 0; j < kPairs; ++j) {
+        const uint32_t p0 = round32(exact_phase(tr, n_thread + 2 * j));
+        const uint32_t p1 = round32(exact_phase(tr, n_thread + 2 * j + 1));
+        float2 v = acc.a[0];
+        // rotate through the pairs so that the loop body indexes a[] statically
+        v.x = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p0)) * kTurnToRad), v.x);
+        v.y = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p1)) * kTurnToRad), v.y);
+#pragma unroll
+        for (int m = 0; m < kPairs - 1; ++m) acc.a[m] = acc.a[m + 1];
+        acc.a[kPairs - 1] = v;
+    }
     return acc;
 }
 
@@ -380,15 +371,6 @@ __device__ __forceinline__ void pq_add(PQ &pq, float s, float c, const float4 &C
     pq.Q[3] = __ffma2_rn(c2, make_float2(S47.z, S47.w), pq.Q[3]);
 }
 
-// next block of the tile: the phase advances by kBlock*w
-__device__ __forceinline__ void rotate(float &s, float &c, float cr, float sr)
-{
-    const float s1 = fmaf(s, cr, c * sr);
-    const float c1 = fmaf(c, cr, -(s * sr));
-    s = s1;
-    c = c1;
-}
-
 __device__ __forceinline__ Acc16 pq_to_samples(const PQ &pq)
 {
     Acc16 d;
@@ -401,73 +383,154 @@ __device__ __forceinline__ Acc16 pq_to_samples(const PQ &pq)
     return d;
 }
 
-// A work unit is RB consecutive blocks of one 2048-sample tile (RB = 4: the whole tile).  SPLIT warps share a
-// unit, each taking 1/SPLIT of the tones; a CTA holds kWarps/SPLIT units.  RB only sets how much work a warp
-// takes (small launches use small units to fill the GPU): every sample goes through the same arithmetic for
-// every RB, because all phases are anchored to the tile (block r is reached by r rotations from block 0).
-// ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine); everything else
-// (and every tone when !ROT) takes the per-block MUFU pass.
-template <int SPLIT, bool ROT, int RB>
+// sin and cos of a u32-turn phase: one range multiply feeds both MUFU operations
+__device__ __forceinline__ void sincos_turns(uint32_t p, float &s, float &c)
+{
+    const float x = __int2float_rn(static_cast<int32_t>(p)) * kTurnToRad;
+    s = mufu_sin(x);
+    c = mufu_cos(x);
+}
+
+template <int SPLIT>
+__device__ __forceinline__ void team_sync(int team)
+{
+    if (SPLIT == kWarps) __syncthreads();
+    else if (SPLIT > 1) asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(SPLIT * 32) : "memory");
+}
+
+// MUFU pass of one warp over one tile: every (tone, block) pair listed in ws.mov is re-centred (step a1, one lane
+// per pair, up to 32 pairs at a time, block-major so the records of a block are contiguous) and then evaluated
+// with one MUFU.SIN per tone-sample into that block's 16 samples, which live in ws.park between sub-batches.
+// Few registers are live here (one block's accumulators), so the 16 sine chains of a record run in parallel.
+__device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws, int t_begin, int t_end, int64_t tile_base,
+                                           int64_t n_end, int lane, uint32_t &park_valid)
+{
+    const int koff = lane * kSPT - kHalf;
+    float2 kf[kPairs], kk[kPairs];  // in-block offsets k of the thread's samples, and k^2
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) {
+        kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
+        kk[j] = __fmul2_rn(kf[j], kf[j]);
+    }
+    for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
+        const unsigned m = ws.mov[b];
+        if (m == 0) continue;
+        const int nm = __popc(m);
+        const int n_pairs = nm * kBlocksPerTile;
+        for (int q0 = 0; q0 < n_pairs; q0 += kBatch) {
+            const int idx = q0 + lane;
+            BlockRec br;
+            br.kind = K_NONE;
+            if (idx < n_pairs) {
+                const int r_lane = idx / nm;
+                const int slot = idx - r_lane * nm;
+                const int64_t blk_base = tile_base + static_cast<int64_t>(r_lane) * kBlock;
+                if (blk_base < n_end && blk_base + kBlock > lp.n_begin) {
+                    const int t = tb + static_cast<int>(__fns(m, 0, slot + 1));
+                    br = block_prologue(lp.tab + t, t, static_cast<uint64_t>(blk_base + kHalf), static_cast<double>(blk_base));
+                }
+            }
+            const unsigned kv = __ballot_sync(0xffffffffu, br.kind >= 0);
+            const unsigned k0 = __ballot_sync(0xffffffffu, (br.kind & 1) != 0);
+            const unsigned k1 = __ballot_sync(0xffffffffu, (br.kind & 2) != 0);
+            const unsigned k2 = __ballot_sync(0xffffffffu, (br.kind & 4) != 0);
+            __syncwarp();  // the previous sub-batch's readers are done
+            if (br.kind >= 0) {
+                ws.mrec[lane].q[0] = make_float4(__uint_as_float(br.c0), __uint_as_float(br.c1), br.A, br.c2);
+                ws.mrec[lane].q[1] = make_float4(br.c3, br.c4, br.c5, br.c6);
+            }
+            __syncwarp();
+#pragma unroll 1
+            for (int r = 0; r < kBlocksPerTile; ++r) {
+                const int lo = max(r * nm - q0, 0), hi = min((r + 1) * nm - q0, kBatch);
+                if (lo >= hi) continue;
+                const unsigned in_r = kv & (0xffffffffu >> (32 - hi)) & (0xffffffffu << lo);
+                if (in_r == 0) continue;
+                Acc16 acc;
+#pragma unroll
+                for (int j = 0; j < kPairs; ++j) acc.a[j] = make_float2(0.f, 0.f);
+                if (park_valid & (1u << r)) park_add(ws, r, lane, acc);
+#pragma unroll 1
+                for (int i = lo; i < hi; ++i) {
+                    if (!((in_r >> i) & 1u)) continue;
+                    const float4 a = ws.mrec[i].q[0];
+                    const float4 bq = ws.mrec[i].q[1];
+                    const int kind = ((k0 >> i) & 1u) | (((k1 >> i) & 1u) << 1) | (((k2 >> i) & 1u) << 2);
+                    switch (kind) {
+                        case K_STATIC: mufu_rec<K_STATIC>(a, bq, koff, kf, kk, acc); break;
+                        case K_QUAD: mufu_rec<K_QUAD>(a, bq, koff, kf, kk, acc); break;
+                        case K_DEG4: mufu_rec<K_DEG4>(a, bq, koff, kf, kk, acc); break;
+                        case K_DEG6: mufu_rec<K_DEG6>(a, bq, koff, kf, kk, acc); break;
+                        case K_SBEG: mufu_rec<K_SBEG>(a, bq, koff, kf, kk, acc); break;
+                        case K_SEND: mufu_rec<K_SEND>(a, bq, koff, kf, kk, acc); break;
+                        default: acc = exact_rec(lp.tab, a, tile_base + r * kBlock + lane * kSPT, acc); break;
+                    }
+                }
+                park_store(ws, r, lane, acc);
+                park_valid |= 1u << r;
+            }
+        }
+    }
+}
+
+// A work unit is one 2048-sample tile (4 blocks of 512) x the tones of one warp.  SPLIT warps (a team) share a
+// tile, each taking 1/SPLIT of the tones; their partial sums meet in shared memory and are added in rank order.
+// The grid is persistent (two CTAs per SM); teams walk the tiles of the launch with a stride of the team count,
+// team index = team_in_cta * gridDim.x + blockIdx.x, so a final partial round spreads over all SMs.
+// ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine), everything else (and
+// every tone when !ROT) takes the MUFU pass.  Every sample goes through the same arithmetic for every launch
+// geometry because all phases are anchored to absolute tile positions.
+template <int SPLIT, bool ROT>
 __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchParams lp)
 {
-    constexpr int kUnitsPerCta = kWarps / SPLIT;
-    constexpr int kUnitsPerTile = kBlocksPerTile / RB;
-    __shared__ SmemRec s_rec[kWarps][kBatch];          // pass 2 records; pass 1 uses the first 16 bytes of each
-    __shared__ uint32_t s_mov[kWarps][kMaxBatches];    // per batch of 32 tones: which ones take pass 2 in this tile
-    __shared__ __align__(16) float s_red[SPLIT > 1 ? kWarps : 1][SPLIT > 1 ? kBlock : 1];
+    constexpr int kTeams = kWarps / SPLIT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    WarpSmem *ws_all = reinterpret_cast<WarpSmem *>(smem_raw);
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    const int unit_in_cta = warp / SPLIT;
+    const int team = warp / SPLIT;
     const int rank = warp % SPLIT;
     const unsigned lt = (1u << lane) - 1u;
+    WarpSmem &ws = ws_all[warp];
 
     // tiles are anchored to absolute sample indices (chunk-size invariance, SURVEY.md 8(b) "Determinism")
     const int64_t first_tile = lp.n_begin / kTile;  // n_begin >= 0
-    const int64_t unit = static_cast<int64_t>(blockIdx.x) * kUnitsPerCta + unit_in_cta;
-    const int64_t tile = first_tile + unit / kUnitsPerTile;
-    const int r0 = static_cast<int>(unit % kUnitsPerTile) * RB;  // first block of the unit within its tile
-    const int64_t tile_base = tile * kTile;
-    const int64_t unit_base = tile_base + static_cast<int64_t>(r0) * kBlock;
     const int64_t n_end = lp.n_begin + lp.n_count;
-    const bool tile_live = unit_base < n_end && unit_base + RB * kBlock > lp.n_begin;
+    const int64_t n_tiles = (n_end - 1) / kTile - first_tile + 1;
+    const int64_t n_teams = static_cast<int64_t>(gridDim.x) * kTeams;
 
     const int per = (lp.n_tones + SPLIT - 1) / SPLIT;
     const int t_begin = rank * per;
     const int t_end = min(lp.n_tones, t_begin + per);
-    SmemRec *rec = s_rec[warp];
-    uint32_t *mov = s_mov[warp];
+    const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the centre of block 0
 
-    Acc16 acc[RB];
-#pragma unroll
-    for (int r = 0; r < RB; ++r)
-#pragma unroll
-        for (int j = 0; j < kPairs; ++j) acc[r].a[j] = make_float2(0.f, 0.f);
+    for (int64_t unit = static_cast<int64_t>(team) * gridDim.x + blockIdx.x; unit < n_tiles; unit += n_teams) {
+        const int64_t tile_base = (first_tile + unit) * kTile;
+        Acc16 acc[kBlocksPerTile];
+        int n_mov = 0;
 
-    if (tile_live) {
-        int n_pass2 = 0;
-        // ---- pass 1: tones that are static over the whole tile (angle addition), and the list of the others
         if (ROT) {
-            PQ pq[RB];
+            // ---- angle-addition pass: tones that are static over the whole tile; the others are listed in ws.mov
+            PQ pq[kBlocksPerTile];
 #pragma unroll
-            for (int r = 0; r < RB; ++r)
+            for (int r = 0; r < kBlocksPerTile; ++r)
 #pragma unroll
                 for (int m = 0; m < kPairs / 2; ++m) pq[r].P[m] = pq[r].Q[m] = make_float2(0.f, 0.f);
             const double tb_d = static_cast<double>(tile_base);
-            // phase reference of block 0: its centre tile_base + kHalf, minus the half sample of the pair centring
+            // phase reference: the centre of block 0, minus the half sample of the pair centring
             const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
-            const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the block centre
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int t = tb + lane;
                 bool is_static = false, is_mover = false;
-                uint32_t c0 = 0, c1 = 0, tabofs = 0;
+                uint32_t c0 = 0, c1 = 0, d = 0;
+                const float4 *tabp = nullptr;
                 if (t < t_end) {
                     const ToneRec *tr = lp.tab + t;
                     const uint4 v0 = ldg16(tr);                                          // A, cls, theta_pre
                     const uint4 v1 = ldg16(reinterpret_cast<const char *>(tr) + 16);   // w_pre, theta_post
                     uint64_t th = u64_of(v0.z, v0.w), w = u64_of(v1.x, v1.y);
-                    tabofs = static_cast<uint32_t>(t) * static_cast<uint32_t>(sizeof(ToneRec)) +
-                             static_cast<uint32_t>(offsetof(ToneRec, rot_pre));
+                    tabp = reinterpret_cast<const float4 *>(&tr->rot_pre);
                     is_static = true;
                     if ((static_cast<int32_t>(v0.y) & 0xff) != CLS_STATIC) {
                         const uint4 v2 = ldg16(reinterpret_cast<const char *>(tr) + 32);  // w_post, ns_int
@@ -479,7 +542,7 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
                         } else if (ua >= f64_of(v3.z, v3.w)) {
                             th = u64_of(v1.z, v1.w);
                             w = u64_of(v2.x, v2.y);
-                            tabofs += static_cast<uint32_t>(offsetof(ToneRec, rot_post) - offsetof(ToneRec, rot_pre));
+                            tabp = reinterpret_cast<const float4 *>(&tr->rot_post);
                         } else {
                             is_static = false;
                             is_mover = true;
@@ -487,125 +550,82 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
                     }
                     c0 = round32(th + w * a0 - (w >> 1));
                     c1 = round32(w);
+                    d = round32(w * static_cast<uint64_t>(kBlock));
                 }
                 const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
                 const unsigned m_sta = __ballot_sync(0xffffffffu, is_static);
-                if (lane == 0) mov[b] = m_mov;
-                n_pass2 += __popc(m_mov);
+                if (lane == 0) ws.mov[b] = m_mov;
+                n_mov += __popc(m_mov);
                 const int n_sta = __popc(m_sta);
-                __syncwarp();  // previous batch's readers are done
-                if (is_static) *reinterpret_cast<uint4 *>(&rec[__popc(m_sta & lt)]) = make_uint4(c0, c1, tabofs, 0u);
+                __syncwarp();  // the previous batch's readers are done
+                if (is_static) {
+                    StageRec &sr = ws.st[__popc(m_sta & lt)];
+                    const float4 C03 = __ldg(tabp), C47 = __ldg(tabp + 1), S03 = __ldg(tabp + 2), S47 = __ldg(tabp + 3);
+                    *reinterpret_cast<uint4 *>(&sr) = make_uint4(c0, c1, d, 0u);
+                    sr.C03 = C03; sr.C47 = C47; sr.S03 = S03; sr.S47 = S47;
+                }
                 __syncwarp();
+                uint4 cc = *reinterpret_cast<const uint4 *>(&ws.st[0]);
 #pragma unroll 1
                 for (int i = 0; i < n_sta; ++i) {
-                    const uint4 h = *reinterpret_cast<const uint4 *>(&rec[i]);
-                    const float4 *g = reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(lp.tab) + h.z);
-                    const float4 C03 = __ldg(g), C47 = __ldg(g + 1), S03 = __ldg(g + 2), S47 = __ldg(g + 3);
-                    const float4 rs = __ldg(g + 4);  // cr, sr
-                    const uint32_t p = h.x + h.y * static_cast<uint32_t>(off);
-                    const float x = __int2float_rn(static_cast<int32_t>(p)) * kTurnToRad;
-                    float s = mufu_sin(x), c = mufu_cos(x);  // block 0 of the tile
-#pragma unroll 1
-                    for (int r = 0; r < r0; ++r) rotate(s, c, rs.x, rs.y);
-                    pq_add(pq[0], s, c, C03, C47, S03, S47);
+                    const StageRec &sr = ws.st[i];
+                    const float4 C03 = sr.C03, C47 = sr.C47, S03 = sr.S03, S47 = sr.S47;
+                    const uint4 cn = *reinterpret_cast<const uint4 *>(&ws.st[i + 1]);  // next tone's carrier (slot n_sta: unused)
+                    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(off);
+                    float s[kBlocksPerTile], c[kBlocksPerTile];
 #pragma unroll
-                    for (int r = 1; r < RB; ++r) {
-                        rotate(s, c, rs.x, rs.y);
-                        pq_add(pq[r], s, c, C03, C47, S03, S47);
-                    }
+                    for (int r = 0; r < kBlocksPerTile; ++r) sincos_turns(p0 + static_cast<uint32_t>(r) * cc.z, s[r], c[r]);
+#pragma unroll
+                    for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], s[r], c[r], C03, C47, S03, S47);
+                    cc = cn;
                 }
             }
 #pragma unroll
-            for (int r = 0; r < RB; ++r) acc[r] = pq_to_samples(pq[r]);
+            for (int r = 0; r < kBlocksPerTile; ++r) acc[r] = pq_to_samples(pq[r]);
         } else {
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int left = t_end - tb;
-                if (lane == 0) mov[b] = left >= 32 ? 0xffffffffu : ((1u << left) - 1u);
+                if (lane == 0) ws.mov[b] = left >= 32 ? 0xffffffffu : ((1u << left) - 1u);
             }
-            n_pass2 = t_end - t_begin;
-            __syncwarp();
+            n_mov = max(t_end - t_begin, 0);
         }
 
-        // ---- pass 2: per (tone, block) re-centring and one MUFU.SIN per tone-sample
-        if (n_pass2 > 0) {
-            __syncwarp();
-            for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
-                const unsigned m = mov[b];
-                if (m == 0) continue;
-                const int nm = __popc(m);
-                // lane = (tone slot, block of the unit).  Few movers: all their blocks in one sub-batch (32/RB tones
-                // x RB blocks); many: one sub-batch per block with 32 tones, so each block_loops call has more to do.
-                const bool by_block = nm > kBatch / RB;
-                const int n_sub = by_block ? RB : 1;
-                for (int q = 0; q < n_sub; ++q) {
-                    const int slot = by_block ? lane : lane / RB;
-                    const int r_lane = by_block ? q : lane % RB;
-                    const int64_t blk_base = unit_base + static_cast<int64_t>(r_lane) * kBlock;
-                    BlockRec br;
-                    br.kind = K_NONE;
-                    if (slot < nm && blk_base < n_end && blk_base + kBlock > lp.n_begin) {
-                        const int t = tb + static_cast<int>(__fns(m, 0, slot + 1));
-                        br = block_prologue(lp.tab + t, t, static_cast<uint64_t>(blk_base + kHalf), static_cast<double>(blk_base));
-                    }
-                    // sort the records by (block, kind) so each inner loop is warp-uniform (no divergence)
-                    KindCounts cnt[RB];
-                    int first_of[RB];
-                    int pos = -1, before = 0;
+        const int64_t n_thread = tile_base + lane * kSPT;
+        if (SPLIT == 1 && ROT && n_mov == 0) {
 #pragma unroll
-                    for (int r = 0; r < RB; ++r) {
-                        first_of[r] = before;
-#pragma unroll
-                        for (int kd = 0; kd < K_COUNT; ++kd) {
-                            const bool mine = (r_lane == r) && (br.kind == kd);
-                            const unsigned bm = __ballot_sync(0xffffffffu, mine);
-                            cnt[r].n[kd] = __popc(bm);
-                            if (mine) pos = before + __popc(bm & lt);
-                            before += cnt[r].n[kd];
-                        }
-                    }
-                    __syncwarp();  // previous sub-batch's readers are done
-                    if (pos >= 0) {
-                        rec[pos].q[0] = make_float4(__uint_as_float(br.c0), __uint_as_float(br.c1), br.A, br.c2);
-                        rec[pos].q[1] = make_float4(br.c3, br.c4, br.c5, br.c6);
-                    }
-                    __syncwarp();
-#pragma unroll
-                    for (int r = 0; r < RB; ++r) {
-                        const int n_r = (r + 1 < RB ? first_of[r + 1] : before) - first_of[r];
-                        if (n_r > 0)
-                            acc[r] = block_loops(lp.tab, rec, first_of[r], cnt[r], unit_base + r * kBlock + lane * kSPT, acc[r]);
-                    }
-                }
-            }
+            for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, acc[r]);
+            continue;
         }
-    }
 
-    // ---- partial sums of the SPLIT warps of a tile meet in shared memory, block by block
+        // ---- partial sums go to shared memory; the MUFU pass adds the moving tones block by block
+        uint32_t park_valid = 0;
+        if (ROT) {
 #pragma unroll
-    for (int r = 0; r < RB; ++r) {
-        if (SPLIT > 1) {
-            if (r > 0) __syncthreads();
-            if (rank != 0) {
-                float4 *mine = reinterpret_cast<float4 *>(&s_red[warp][lane * kSPT]);
+            for (int r = 0; r < kBlocksPerTile; ++r) park_store(ws, r, lane, acc[r]);
+            park_valid = (1u << kBlocksPerTile) - 1u;
+        }
+        __syncwarp();
+        if (n_mov > 0) mover_pass(lp, ws, t_begin, t_end, tile_base, n_end, lane, park_valid);
+#pragma unroll 1
+        for (int r = 0; r < kBlocksPerTile; ++r) {
+            if (park_valid & (1u << r)) continue;
 #pragma unroll
-                for (int v = 0; v < kSPT / 4; ++v)
-                    mine[v] = make_float4(acc[r].a[2 * v].x, acc[r].a[2 * v].y, acc[r].a[2 * v + 1].x, acc[r].a[2 * v + 1].y);
-            }
-            __syncthreads();
-            if (rank == 0) {
+            for (int v = 0; v < kSPT / 4; ++v) ws.park[r][v][lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        team_sync<SPLIT>(team);
+        if (rank == 0) {
+#pragma unroll 1
+            for (int r = 0; r < kBlocksPerTile; ++r) {
+                Acc16 sum;
+#pragma unroll
+                for (int j = 0; j < kPairs; ++j) sum.a[j] = make_float2(0.f, 0.f);
                 // fixed summation order (rank 0, 1, ...) keeps the result independent of scheduling
-                for (int r2 = 1; r2 < SPLIT; ++r2) {
-                    const float4 *o = reinterpret_cast<const float4 *>(&s_red[warp + r2][lane * kSPT]);
 #pragma unroll
-                    for (int v = 0; v < kSPT / 4; ++v) {
-                        const float4 u = o[v];
-                        acc[r].a[2 * v].x += u.x; acc[r].a[2 * v].y += u.y;
-                        acc[r].a[2 * v + 1].x += u.z; acc[r].a[2 * v + 1].y += u.w;
-                    }
-                }
+                for (int r2 = 0; r2 < SPLIT; ++r2) park_add(ws_all[warp + r2], r, lane, sum);
+                store_block(lp, n_thread + r * kBlock, sum);
             }
         }
-        if (rank == 0 && tile_live) store_block(lp, unit_base + r * kBlock + lane * kSPT, acc[r]);
+        team_sync<SPLIT>(team);  // the next tile's partial sums overwrite the park areas
     }
 }
 
@@ -657,27 +677,34 @@ __global__ void awg_scatter_kernel(ToneRec *table, const ToneRec *src, const int
     d4[threadIdx.x] = s4[threadIdx.x];
 }
 
-template <bool ROT, int RB>
-void launch_split(const LaunchParams &lp, int split, int64_t tiles, cudaStream_t stream)
+template <int SPLIT, bool ROT>
+cudaError_t launch_one(const LaunchParams &lp, int64_t tiles, int n_sm, cudaStream_t stream)
 {
-    const int64_t units = tiles * (kBlocksPerTile / RB);
-    auto grid_for = [&](int s) { return static_cast<unsigned>((units + (kWarps / s) - 1) / (kWarps / s)); };
-    switch (split) {
-        case 1: awg_synth_kernel<1, ROT, RB><<<grid_for(1), kWarps * 32, 0, stream>>>(lp); break;
-        case 2: awg_synth_kernel<2, ROT, RB><<<grid_for(2), kWarps * 32, 0, stream>>>(lp); break;
-        case 4: awg_synth_kernel<4, ROT, RB><<<grid_for(4), kWarps * 32, 0, stream>>>(lp); break;
-        default: awg_synth_kernel<8, ROT, RB><<<grid_for(8), kWarps * 32, 0, stream>>>(lp); break;
+    constexpr int kTeams = kWarps / SPLIT;
+    constexpr size_t kSmem = sizeof(WarpSmem) * kWarps;
+    static bool configured = false;  // per instantiation; benign if two threads race (same value is set twice)
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(awg_synth_kernel<SPLIT, ROT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(kSmem));
+        if (e != cudaSuccess) return e;
+        configured = true;
     }
+    // persistent grid: two CTAs per SM, fewer when the launch has fewer tiles than teams
+    const int64_t want = (tiles + kTeams - 1) / kTeams;
+    const unsigned grid = static_cast<unsigned>(want < 2 * n_sm ? want : 2 * n_sm);
+    awg_synth_kernel<SPLIT, ROT><<<grid, kWarps * 32, kSmem, stream>>>(lp);
+    return cudaGetLastError();
 }
 
 template <bool ROT>
-void launch_rb(const LaunchParams &lp, int split, int64_t tiles, int n_sm, cudaStream_t stream)
+cudaError_t launch_split(const LaunchParams &lp, int split, int64_t tiles, int n_sm, cudaStream_t stream)
 {
-    // the largest unit that still gives every SM its two resident CTAs
-    const int64_t want = 2 * static_cast<int64_t>(n_sm) * (kWarps / split);  // units
-    if (tiles >= want) launch_split<ROT, 4>(lp, split, tiles, stream);
-    else if (tiles * 2 >= want) launch_split<ROT, 2>(lp, split, tiles, stream);
-    else launch_split<ROT, 1>(lp, split, tiles, stream);
+    switch (split) {
+        case 1: return launch_one<1, ROT>(lp, tiles, n_sm, stream);
+        case 2: return launch_one<2, ROT>(lp, tiles, n_sm, stream);
+        case 4: return launch_one<4, ROT>(lp, tiles, n_sm, stream);
+        default: return launch_one<8, ROT>(lp, tiles, n_sm, stream);
+    }
 }
 
 }  // namespace
@@ -693,9 +720,11 @@ cudaError_t launch_scatter(ToneRec *table, const ToneRec *src, const int32_t *id
 cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream)
 {
     if (lp.n_count <= 0) return cudaSuccess;
+    cudaError_t e;
     if (engine == AWG_ENGINE_FP64) {
         const int64_t threads = lp.n_count / kSPT64;
         awg_fp64_kernel<<<static_cast<unsigned>((threads + 255) / 256), 256, 0, stream>>>(lp);
+        e = cudaGetLastError();
     } else {
         const int64_t first_tile = lp.n_begin / kTile;
         const int64_t last_tile = (lp.n_begin + lp.n_count - 1) / kTile;
@@ -713,11 +742,11 @@ cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream
         // which keeps the output bit-identical across chunk sizes (include/awg.h "pure function").
         int split = 1;
         while (split < kWarps && lp.n_tones / (split * 2) >= 32) split *= 2;
-        if (engine == AWG_ENGINE_FMA) launch_rb<true>(lp, split, tiles, n_sm, stream);
-        else launch_rb<false>(lp, split, tiles, n_sm, stream);
+        e = (engine == AWG_ENGINE_FMA) ? launch_split<true>(lp, split, tiles, n_sm, stream)
+                                       : launch_split<false>(lp, split, tiles, n_sm, stream);
     }
     count_launch();
-    return cudaGetLastError();
+    return e;
 }
 
 }  // namespace awg
