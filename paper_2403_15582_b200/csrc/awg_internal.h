@@ -78,6 +78,7 @@ struct LaunchParams {
     int64_t n_count;   // samples to produce (multiple of 8)
     float scale;       // int16 full-scale factor
     void *out;         // int16* or float* (device)
+    uint32_t *sched;   // {next tile, teams finished}: the launch's tile-scheduler slot (filled in by launch_synth)
 };
 
 cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream);

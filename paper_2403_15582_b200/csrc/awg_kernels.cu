@@ -16,6 +16,7 @@
 #include <cstddef>
 #include <cstdint>
 #include <atomic>
+#include <mutex>
 
 #include "awg_internal.h"
 
@@ -27,11 +28,14 @@ void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 namespace {
 
 constexpr int kHalf = kBlock / 2;     // Taylor expansions are centred on the block
-constexpr int kWarps = 8;             // warps per CTA
+constexpr int kWarps = 4;             // warps per CTA
+constexpr int kCtasPerSm = 3;         // 12 warps per SM leave 168 registers per thread: tables and sines double-buffered
 constexpr int kBatch = 32;            // tones (pass 1) or (tone, block) items (pass 2) per batch: one per lane
 constexpr int kMaxBatches = 65536 / kWarps / kBatch;   // per warp, at the largest tone count and widest split
 constexpr float kTurnToRad = 1.4629180792671596e-9f;   // 2*pi / 2^32: int32 phase (turns * 2^32) -> radians
 constexpr double kTwo64 = 18446744073709551616.0;
+constexpr int kListBatches = 8;                        // batches of 32 tones compacted at a time for the MUFU pass
+constexpr int kListCap = kListBatches * kBatch;
 
 __device__ __forceinline__ float mufu_sin(float x_rad)
 {
@@ -121,14 +125,18 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
     const int c = cls & 0xff;
     const uint64_t theta_pre = u64_of(v0.z, v0.w);
     const uint4 v1 = ldg16(reinterpret_cast<const char *>(rec) + 16);  // w_pre, theta_post
+    // all seven loads are issued before the first use: one memory round trip per record instead of three
+    const uint4 v2 = ldg16(reinterpret_cast<const char *>(rec) + 32);  // w_post, ns_int
+    const uint4 v3 = ldg16(reinterpret_cast<const char *>(rec) + 48);  // ns_frac, Tn
+    const uint4 v4 = ldg16(reinterpret_cast<const char *>(rec) + 64);  // inv_Tn, DT
+    const uint4 v5 = ldg16(reinterpret_cast<const char *>(rec) + 80);  // q1, q[0], q[1]
+    const uint4 v6 = ldg16(reinterpret_cast<const char *>(rec) + 96);  // q[2], q[3], q[4]
     const uint64_t w_pre = u64_of(v1.x, v1.y);
     uint64_t ph, w;
     if (c == CLS_STATIC) {
         w = w_pre;
         ph = theta_pre + w * nc;
     } else {
-        const uint4 v2 = ldg16(reinterpret_cast<const char *>(rec) + 32);  // w_post, ns_int
-        const uint4 v3 = ldg16(reinterpret_cast<const char *>(rec) + 48);  // ns_frac, Tn
         const double Tn = f64_of(v3.z, v3.w);
         const double ua = (bb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the block's first sample
         const double ub = ua + static_cast<double>(kBlock - 1);
@@ -145,9 +153,6 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
             r.c1 = 0;
             return r;
         } else {
-            const uint4 v4 = ldg16(reinterpret_cast<const char *>(rec) + 64);  // inv_Tn, DT
-            const uint4 v5 = ldg16(reinterpret_cast<const char *>(rec) + 80);  // q1, q[0], q[1]
-            const uint4 v6 = ldg16(reinterpret_cast<const char *>(rec) + 96);  // q[2], q[3], q[4]
             const double rT = f64_of(v4.x, v4.y);
             const double DT = f64_of(v4.z, v4.w);
             const float q2 = __uint_as_float(v5.z), q3 = __uint_as_float(v5.w);
@@ -232,6 +237,9 @@ struct __align__(16) WarpSmem {
     MovRec mrec[kBatch];
     float4 park[kBlocksPerTile][kSPT / 4][32];   // partial sums of the tile: [block][4 samples][lane]
     uint32_t mov[kMaxBatches];              // per batch of 32 tones: which ones take the MUFU pass in this tile
+    uint32_t next;                          // (rank-0 warp of a team) the team's next tile, drawn by the leader
+    uint32_t pad_[3];
+    uint16_t list[kListCap];                // compacted tone indices (relative to the warp's first tone) of the MUFU pass
 };
 
 // 16 samples of one block of one thread, as 8 packed pairs: a[j] = samples (2j, 2j+1).
@@ -391,6 +399,36 @@ __device__ __forceinline__ void sincos_turns(uint32_t p, float &s, float &c)
     c = mufu_cos(x);
 }
 
+// Requests the carrier part of a tone record (A, cls, theta_pre | w_pre, theta_post | w_post, ns_int | ns_frac, Tn) and
+// pulls its two angle-addition tables (bytes 128..287) towards L1.
+__device__ __forceinline__ void fetch_tone(const ToneRec *tr, uint4 &v0, uint4 &v1, uint4 &v2, uint4 &v3)
+{
+    const char *p = reinterpret_cast<const char *>(tr);
+    v0 = ldg16(p);
+    v1 = ldg16(p + 16);
+    v2 = ldg16(p + 32);
+    v3 = ldg16(p + 48);
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 128));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 208));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 272));
+}
+
+// Sines and cosines of one tile-static tone at the thread's pair centre in each of the tile's four blocks.
+// cc = {phase at lane 0's centre of block 0, phase per sample, phase per block, -} in u32 turns.
+__device__ __forceinline__ void sincos_tile(const uint4 cc, int off, float (&s)[kBlocksPerTile], float (&c)[kBlocksPerTile])
+{
+    static_assert(kBlocksPerTile == 4, "sincos_tile packs the four blocks as two pairs");
+    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(off);
+    const uint32_t p1 = p0 + cc.z, p2 = p1 + cc.z, p3 = p2 + cc.z;
+    const float2 K2 = dup2(kTurnToRad);
+    const float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1))), K2);
+    const float2 x23 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p2)), __int2float_rn(static_cast<int32_t>(p3))), K2);
+    s[0] = mufu_sin(x01.x); c[0] = mufu_cos(x01.x);
+    s[1] = mufu_sin(x01.y); c[1] = mufu_cos(x01.y);
+    s[2] = mufu_sin(x23.x); c[2] = mufu_cos(x23.x);
+    s[3] = mufu_sin(x23.y); c[3] = mufu_cos(x23.y);
+}
+
 template <int SPLIT>
 __device__ __forceinline__ void team_sync(int team)
 {
@@ -398,35 +436,56 @@ __device__ __forceinline__ void team_sync(int team)
     else if (SPLIT > 1) asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(SPLIT * 32) : "memory");
 }
 
-// MUFU pass of one warp over one tile: every (tone, block) pair listed in ws.mov is re-centred (step a1, one lane
-// per pair, up to 32 pairs at a time, block-major so the records of a block are contiguous) and then evaluated
-// with one MUFU.SIN per tone-sample into that block's 16 samples, which live in ws.park between sub-batches.
-// Few registers are live here (one block's accumulators), so the 16 sine chains of a record run in parallel.
+// MUFU pass of one warp over one tile.  The tones flagged in ws.mov are compacted into ws.list (kListCap at a
+// time); every (tone, block) pair of the list is re-centred (step a1, one lane per pair, block-major so the records
+// of a block are contiguous) and the records of each block are then run KIND BY KIND (warp-uniform loops over ballot
+// masks, no per-record switch) with one MUFU.SIN per tone-sample into that block's 16 samples, which live in ws.park
+// between sub-batches.  Few registers are live here (one block's accumulators), so the 16 sine chains of a record
+// run in parallel.  Which records share a sub-batch depends only on the tile and the tone partition, never on the
+// launch range, so the fp32 summation order is the same for every chunking.
+#define AWG_RUN_KIND(K)                                                      \
+    {                                                                        \
+        unsigned m_ = in_r & mk[K];                                          \
+        while (m_) {                                                         \
+            const int i_ = __ffs(m_) - 1;                                    \
+            m_ &= m_ - 1;                                                    \
+            mufu_rec<K>(ws.mrec[i_].q[0], ws.mrec[i_].q[1], koff, kf, kk, acc); \
+        }                                                                    \
+    }
+
 __device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws, int t_begin, int t_end, int64_t tile_base,
                                            int64_t n_end, int lane, uint32_t &park_valid)
 {
     const int koff = lane * kSPT - kHalf;
+    const unsigned lt = (1u << lane) - 1u;
     float2 kf[kPairs], kk[kPairs];  // in-block offsets k of the thread's samples, and k^2
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) {
         kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
         kk[j] = __fmul2_rn(kf[j], kf[j]);
     }
-    for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
-        const unsigned m = ws.mov[b];
-        if (m == 0) continue;
-        const int nm = __popc(m);
-        const int n_pairs = nm * kBlocksPerTile;
+    const int n_batches = (t_end - t_begin + kBatch - 1) / kBatch;
+    for (int b0 = 0; b0 < n_batches; b0 += kListBatches) {
+        const int b1 = min(b0 + kListBatches, n_batches);
+        int n = 0;
+        for (int b = b0; b < b1; ++b) {
+            const unsigned m = ws.mov[b];
+            if ((m >> lane) & 1u) ws.list[n + __popc(m & lt)] = static_cast<uint16_t>(b * kBatch + lane);
+            n += __popc(m);
+        }
+        if (n == 0) continue;
+        __syncwarp();
+        const int n_pairs = n * kBlocksPerTile;
         for (int q0 = 0; q0 < n_pairs; q0 += kBatch) {
             const int idx = q0 + lane;
             BlockRec br;
             br.kind = K_NONE;
             if (idx < n_pairs) {
-                const int r_lane = idx / nm;
-                const int slot = idx - r_lane * nm;
+                const int r_lane = (idx >= n) + (idx >= 2 * n) + (idx >= 3 * n);
+                static_assert(kBlocksPerTile == 4, "r_lane assumes four blocks per tile");
                 const int64_t blk_base = tile_base + static_cast<int64_t>(r_lane) * kBlock;
                 if (blk_base < n_end && blk_base + kBlock > lp.n_begin) {
-                    const int t = tb + static_cast<int>(__fns(m, 0, slot + 1));
+                    const int t = t_begin + ws.list[idx - r_lane * n];
                     br = block_prologue(lp.tab + t, t, static_cast<uint64_t>(blk_base + kHalf), static_cast<double>(blk_base));
                 }
             }
@@ -434,6 +493,14 @@ __device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws,
             const unsigned k0 = __ballot_sync(0xffffffffu, (br.kind & 1) != 0);
             const unsigned k1 = __ballot_sync(0xffffffffu, (br.kind & 2) != 0);
             const unsigned k2 = __ballot_sync(0xffffffffu, (br.kind & 4) != 0);
+            unsigned mk[K_COUNT];
+            mk[K_STATIC] = kv & ~k0 & ~k1 & ~k2;
+            mk[K_QUAD] = kv & k0 & ~k1 & ~k2;
+            mk[K_DEG4] = kv & ~k0 & k1 & ~k2;
+            mk[K_DEG6] = kv & k0 & k1 & ~k2;
+            mk[K_SBEG] = kv & ~k0 & ~k1 & k2;
+            mk[K_SEND] = kv & k0 & ~k1 & k2;
+            mk[K_EXACT] = kv & ~k0 & k1 & k2;
             __syncwarp();  // the previous sub-batch's readers are done
             if (br.kind >= 0) {
                 ws.mrec[lane].q[0] = make_float4(__uint_as_float(br.c0), __uint_as_float(br.c1), br.A, br.c2);
@@ -442,7 +509,7 @@ __device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws,
             __syncwarp();
 #pragma unroll 1
             for (int r = 0; r < kBlocksPerTile; ++r) {
-                const int lo = max(r * nm - q0, 0), hi = min((r + 1) * nm - q0, kBatch);
+                const int lo = max(r * n - q0, 0), hi = min((r + 1) * n - q0, kBatch);
                 if (lo >= hi) continue;
                 const unsigned in_r = kv & (0xffffffffu >> (32 - hi)) & (0xffffffffu << lo);
                 if (in_r == 0) continue;
@@ -450,27 +517,43 @@ __device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws,
 #pragma unroll
                 for (int j = 0; j < kPairs; ++j) acc.a[j] = make_float2(0.f, 0.f);
                 if (park_valid & (1u << r)) park_add(ws, r, lane, acc);
-#pragma unroll 1
-                for (int i = lo; i < hi; ++i) {
-                    if (!((in_r >> i) & 1u)) continue;
-                    const float4 a = ws.mrec[i].q[0];
-                    const float4 bq = ws.mrec[i].q[1];
-                    const int kind = ((k0 >> i) & 1u) | (((k1 >> i) & 1u) << 1) | (((k2 >> i) & 1u) << 2);
-                    switch (kind) {
-                        case K_STATIC: mufu_rec<K_STATIC>(a, bq, koff, kf, kk, acc); break;
-                        case K_QUAD: mufu_rec<K_QUAD>(a, bq, koff, kf, kk, acc); break;
-                        case K_DEG4: mufu_rec<K_DEG4>(a, bq, koff, kf, kk, acc); break;
-                        case K_DEG6: mufu_rec<K_DEG6>(a, bq, koff, kf, kk, acc); break;
-                        case K_SBEG: mufu_rec<K_SBEG>(a, bq, koff, kf, kk, acc); break;
-                        case K_SEND: mufu_rec<K_SEND>(a, bq, koff, kf, kk, acc); break;
-                        default: acc = exact_rec(lp.tab, a, tile_base + r * kBlock + lane * kSPT, acc); break;
+                AWG_RUN_KIND(K_STATIC)
+                AWG_RUN_KIND(K_QUAD)
+                AWG_RUN_KIND(K_DEG4)
+                AWG_RUN_KIND(K_DEG6)
+                AWG_RUN_KIND(K_SBEG)
+                AWG_RUN_KIND(K_SEND)
+                {
+                    unsigned m_ = in_r & mk[K_EXACT];
+                    while (m_) {
+                        const int i_ = __ffs(m_) - 1;
+                        m_ &= m_ - 1;
+                        acc = exact_rec(lp.tab, ws.mrec[i_].q[0], tile_base + r * kBlock + lane * kSPT, acc);
                     }
                 }
                 park_store(ws, r, lane, acc);
                 park_valid |= 1u << r;
             }
         }
+        __syncwarp();  // ws.list is rebuilt for the next kListCap tones
     }
+}
+#undef AWG_RUN_KIND
+
+// Draws the team's next tile from the launch counter (leader: lane 0 of rank 0) and hands it to the whole team.
+template <int SPLIT>
+__device__ __forceinline__ int64_t next_unit(const LaunchParams &lp, WarpSmem &ws_leader, int team, int rank, int lane, int64_t n_teams)
+{
+    uint32_t v = 0;
+    if (SPLIT == 1) {
+        if (lane == 0) v = atomicAdd(lp.sched, 1u);
+        v = __shfl_sync(0xffffffffu, v, 0);
+    } else {
+        if (rank == 0 && lane == 0) ws_leader.next = atomicAdd(lp.sched, 1u);
+        team_sync<SPLIT>(team);
+        v = ws_leader.next;
+    }
+    return n_teams + static_cast<int64_t>(v);
 }
 
 // A work unit is one 2048-sample tile (4 blocks of 512) x the tones of one warp.  SPLIT warps (a team) share a
@@ -481,7 +564,7 @@ __device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws,
 // every tone when !ROT) takes the MUFU pass.  Every sample goes through the same arithmetic for every launch
 // geometry because all phases are anchored to absolute tile positions.
 template <int SPLIT, bool ROT>
-__global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchParams lp)
+__global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(const LaunchParams lp)
 {
     constexpr int kTeams = kWarps / SPLIT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -505,7 +588,11 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
     const int t_end = min(lp.n_tones, t_begin + per);
     const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the centre of block 0
 
-    for (int64_t unit = static_cast<int64_t>(team) * gridDim.x + blockIdx.x; unit < n_tiles; unit += n_teams) {
+    // Tile scheduler: every team starts on the tile of its own index and then draws tiles from the launch's
+    // counter lp.sched[0] (tiles that hold moving tones cost several times the others, so a fixed stride leaves
+    // SMs idle at the end).  Which team computes a tile has no effect on its samples.
+    int64_t unit = static_cast<int64_t>(team) * gridDim.x + blockIdx.x;
+    while (unit < n_tiles) {
         const int64_t tile_base = (first_tile + unit) * kTile;
         Acc16 acc[kBlocksPerTile];
         int n_mov = 0;
@@ -520,6 +607,10 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
             const double tb_d = static_cast<double>(tile_base);
             // phase reference: the centre of block 0, minus the half sample of the pair centring
             const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
+            // The records of batch b+1 are requested before the multiply-add loop of batch b runs (v0n..v3n stay in
+            // registers across it, the two carrier tables are pulled into L1), so a batch starts without waiting.
+            uint4 v0n = make_uint4(0, 0, 0, 0), v1n = v0n, v2n = v0n, v3n = v0n;
+            if (t_begin + lane < t_end) fetch_tone(lp.tab + t_begin + lane, v0n, v1n, v2n, v3n);
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int t = tb + lane;
                 bool is_static = false, is_mover = false;
@@ -527,14 +618,11 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
                 const float4 *tabp = nullptr;
                 if (t < t_end) {
                     const ToneRec *tr = lp.tab + t;
-                    const uint4 v0 = ldg16(tr);                                          // A, cls, theta_pre
-                    const uint4 v1 = ldg16(reinterpret_cast<const char *>(tr) + 16);   // w_pre, theta_post
+                    const uint4 v0 = v0n, v1 = v1n, v2 = v2n, v3 = v3n;
                     uint64_t th = u64_of(v0.z, v0.w), w = u64_of(v1.x, v1.y);
                     tabp = reinterpret_cast<const float4 *>(&tr->rot_pre);
                     is_static = true;
                     if ((static_cast<int32_t>(v0.y) & 0xff) != CLS_STATIC) {
-                        const uint4 v2 = ldg16(reinterpret_cast<const char *>(tr) + 32);  // w_post, ns_int
-                        const uint4 v3 = ldg16(reinterpret_cast<const char *>(tr) + 48);  // ns_frac, Tn
                         const double ua = (tb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the tile's first sample
                         const double ub = ua + static_cast<double>(kTile - 1);
                         if (ub <= 0.0) {
@@ -552,6 +640,7 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
                     c1 = round32(w);
                     d = round32(w * static_cast<uint64_t>(kBlock));
                 }
+                if (t + kBatch < t_end) fetch_tone(lp.tab + t + kBatch, v0n, v1n, v2n, v3n);
                 const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
                 const unsigned m_sta = __ballot_sync(0xffffffffu, is_static);
                 if (lane == 0) ws.mov[b] = m_mov;
@@ -565,19 +654,36 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
                     sr.C03 = C03; sr.C47 = C47; sr.S03 = S03; sr.S47 = S47;
                 }
                 __syncwarp();
-                uint4 cc = *reinterpret_cast<const uint4 *>(&ws.st[0]);
+                // Software pipeline, unrolled by two so that the sines/cosines ping-pong between two register sets:
+                // the phase -> I2FP -> FMUL2 -> MUFU chain of tone i+1 (XU and ALU pipes) is issued under the
+                // 32 FFMA2 of tone i.  Scalar fp32 instructions cost the FMA pipe as much as an FFMA2 (measured,
+                // profiles/), hence the packed range multiply and no register moves.
+                float sa[kBlocksPerTile], ca[kBlocksPerTile], sb[kBlocksPerTile], cb[kBlocksPerTile];
+                sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[0]), off, sa, ca);
+                int i = 0;
 #pragma unroll 1
-                for (int i = 0; i < n_sta; ++i) {
+                for (; i + 1 < n_sta; i += 2) {
+                    {
+                        const StageRec &sr = ws.st[i];
+                        const float4 C03 = sr.C03, C47 = sr.C47, S03 = sr.S03, S47 = sr.S47;
+                        sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[i + 1]), off, sb, cb);
+#pragma unroll
+                        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
+                    }
+                    {
+                        const StageRec &sr = ws.st[i + 1];
+                        const float4 C03 = sr.C03, C47 = sr.C47, S03 = sr.S03, S47 = sr.S47;
+                        // slot i + 2 <= kBatch exists; past the last tone it is stale and its result unused
+                        sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[i + 2]), off, sa, ca);
+#pragma unroll
+                        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sb[r], cb[r], C03, C47, S03, S47);
+                    }
+                }
+                if (i < n_sta) {
                     const StageRec &sr = ws.st[i];
                     const float4 C03 = sr.C03, C47 = sr.C47, S03 = sr.S03, S47 = sr.S47;
-                    const uint4 cn = *reinterpret_cast<const uint4 *>(&ws.st[i + 1]);  // next tone's carrier (slot n_sta: unused)
-                    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(off);
-                    float s[kBlocksPerTile], c[kBlocksPerTile];
 #pragma unroll
-                    for (int r = 0; r < kBlocksPerTile; ++r) sincos_turns(p0 + static_cast<uint32_t>(r) * cc.z, s[r], c[r]);
-#pragma unroll
-                    for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], s[r], c[r], C03, C47, S03, S47);
-                    cc = cn;
+                    for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
                 }
             }
 #pragma unroll
@@ -594,6 +700,7 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
         if (SPLIT == 1 && ROT && n_mov == 0) {
 #pragma unroll
             for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, acc[r]);
+            unit = next_unit<SPLIT>(lp, ws_all[warp - rank], team, rank, lane, n_teams);
             continue;
         }
 
@@ -625,7 +732,17 @@ __global__ void __launch_bounds__(kWarps * 32, 2) awg_synth_kernel(const LaunchP
                 store_block(lp, n_thread + r * kBlock, sum);
             }
         }
-        team_sync<SPLIT>(team);  // the next tile's partial sums overwrite the park areas
+        // the closing barrier (the next tile's partial sums overwrite the park areas) also publishes the next tile
+        unit = next_unit<SPLIT>(lp, ws_all[warp - rank], team, rank, lane, n_teams);
+    }
+    // the last team out re-arms the counter for the launch that takes this slot next
+    if (rank == 0 && lane == 0) {
+        __threadfence();
+        if (atomicAdd(lp.sched + 1, 1u) == static_cast<uint32_t>(n_teams - 1)) {
+            lp.sched[0] = 0u;
+            lp.sched[1] = 0u;
+            __threadfence();
+        }
     }
 }
 
@@ -677,6 +794,34 @@ __global__ void awg_scatter_kernel(ToneRec *table, const ToneRec *src, const int
     d4[threadIdx.x] = s4[threadIdx.x];
 }
 
+// Tile-scheduler slots: kSchedSlots pairs of counters per device, zeroed once; every launch takes the next slot
+// and its last team zeroes it again, so a slot is clean when it comes round (kSchedSlots launches later).
+constexpr int kSchedSlots = 256;
+constexpr int kMaxDevices = 64;
+std::mutex g_sched_mutex;
+uint32_t *g_sched[kMaxDevices] = {};
+std::atomic<uint32_t> g_sched_next{0};
+
+cudaError_t sched_slot(uint32_t **slot)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    {
+        std::lock_guard<std::mutex> lock(g_sched_mutex);
+        if (!g_sched[dev]) {
+            uint32_t *p = nullptr;
+            const size_t bytes = static_cast<size_t>(kSchedSlots) * 8 * sizeof(uint32_t);  // 32 bytes per slot
+            if ((e = cudaMalloc(reinterpret_cast<void **>(&p), bytes)) != cudaSuccess) return e;
+            if ((e = cudaMemset(p, 0, bytes)) != cudaSuccess) return e;
+            g_sched[dev] = p;
+        }
+    }
+    *slot = g_sched[dev] + 8 * (g_sched_next.fetch_add(1, std::memory_order_relaxed) % kSchedSlots);
+    return cudaSuccess;
+}
+
 template <int SPLIT, bool ROT>
 cudaError_t launch_one(const LaunchParams &lp, int64_t tiles, int n_sm, cudaStream_t stream)
 {
@@ -689,9 +834,9 @@ cudaError_t launch_one(const LaunchParams &lp, int64_t tiles, int n_sm, cudaStre
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    // persistent grid: two CTAs per SM, fewer when the launch has fewer tiles than teams
+    // persistent grid: kCtasPerSm CTAs per SM, fewer when the launch has fewer tiles than teams
     const int64_t want = (tiles + kTeams - 1) / kTeams;
-    const unsigned grid = static_cast<unsigned>(want < 2 * n_sm ? want : 2 * n_sm);
+    const unsigned grid = static_cast<unsigned>(want < kCtasPerSm * n_sm ? want : kCtasPerSm * n_sm);
     awg_synth_kernel<SPLIT, ROT><<<grid, kWarps * 32, kSmem, stream>>>(lp);
     return cudaGetLastError();
 }
@@ -702,8 +847,7 @@ cudaError_t launch_split(const LaunchParams &lp, int split, int64_t tiles, int n
     switch (split) {
         case 1: return launch_one<1, ROT>(lp, tiles, n_sm, stream);
         case 2: return launch_one<2, ROT>(lp, tiles, n_sm, stream);
-        case 4: return launch_one<4, ROT>(lp, tiles, n_sm, stream);
-        default: return launch_one<8, ROT>(lp, tiles, n_sm, stream);
+        default: return launch_one<kWarps, ROT>(lp, tiles, n_sm, stream);
     }
 }
 
@@ -717,9 +861,10 @@ cudaError_t launch_scatter(ToneRec *table, const ToneRec *src, const int32_t *id
     return cudaGetLastError();
 }
 
-cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream)
+cudaError_t launch_synth(const LaunchParams &lp_in, int engine, cudaStream_t stream)
 {
-    if (lp.n_count <= 0) return cudaSuccess;
+    if (lp_in.n_count <= 0) return cudaSuccess;
+    LaunchParams lp = lp_in;
     cudaError_t e;
     if (engine == AWG_ENGINE_FP64) {
         const int64_t threads = lp.n_count / kSPT64;
@@ -737,11 +882,12 @@ cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream
             else
                 n_sm = 148;
         }
-        // Warps per tile depend on the tone count ONLY (>= 32 tones per warp, at most 8 warps), never on the
+        if ((e = sched_slot(&lp.sched)) != cudaSuccess) return e;
+        // Warps per tile depend on the tone count ONLY (>= 12 tones per warp, at most 8 warps), never on the
         // launch size: the order in which tone partial sums are added is then the same for every chunking,
         // which keeps the output bit-identical across chunk sizes (include/awg.h "pure function").
         int split = 1;
-        while (split < kWarps && lp.n_tones / (split * 2) >= 32) split *= 2;
+        while (split < kWarps && lp.n_tones / (split * 2) >= 12) split *= 2;
         e = (engine == AWG_ENGINE_FMA) ? launch_split<true>(lp, split, tiles, n_sm, stream)
                                        : launch_split<false>(lp, split, tiles, n_sm, stream);
     }

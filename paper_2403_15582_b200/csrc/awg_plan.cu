@@ -266,6 +266,7 @@ awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, voi
     lp.scale = static_cast<float>(p->scale);
     lp.out = dev_out;
     lp.out_f32 = f32 ? 1 : 0;
+    lp.sched = nullptr;  // launch_synth assigns the tile-scheduler slot
     cudaError_t e = launch_synth(lp, p->engine, stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
     if ((e = cudaEventRecord(p->last_use[p->cur_version], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
