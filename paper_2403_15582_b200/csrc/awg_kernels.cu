@@ -592,7 +592,12 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
     // counter lp.sched[0] (tiles that hold moving tones cost several times the others, so a fixed stride leaves
     // SMs idle at the end).  Which team computes a tile has no effect on its samples.
     int64_t unit = static_cast<int64_t>(team) * gridDim.x + blockIdx.x;
+    // The tone records of the next batch are requested before the multiply-add loop of the current batch runs
+    // (v0n..v3n stay in registers across it, the two carrier tables are pulled into L1); after the last batch of a
+    // tile the request wraps round to the first batch, which is what the next tile starts with.
+    uint4 v0n = make_uint4(0, 0, 0, 0), v1n = v0n, v2n = v0n, v3n = v0n;
     while (unit < n_tiles) {
+        if (ROT && t_begin + lane < t_end) fetch_tone(lp.tab + t_begin + lane, v0n, v1n, v2n, v3n);
         const int64_t tile_base = (first_tile + unit) * kTile;
         Acc16 acc[kBlocksPerTile];
         int n_mov = 0;
@@ -607,10 +612,6 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
             const double tb_d = static_cast<double>(tile_base);
             // phase reference: the centre of block 0, minus the half sample of the pair centring
             const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
-            // The records of batch b+1 are requested before the multiply-add loop of batch b runs (v0n..v3n stay in
-            // registers across it, the two carrier tables are pulled into L1), so a batch starts without waiting.
-            uint4 v0n = make_uint4(0, 0, 0, 0), v1n = v0n, v2n = v0n, v3n = v0n;
-            if (t_begin + lane < t_end) fetch_tone(lp.tab + t_begin + lane, v0n, v1n, v2n, v3n);
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int t = tb + lane;
                 bool is_static = false, is_mover = false;
@@ -640,7 +641,10 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                     c1 = round32(w);
                     d = round32(w * static_cast<uint64_t>(kBlock));
                 }
-                if (t + kBatch < t_end) fetch_tone(lp.tab + t + kBatch, v0n, v1n, v2n, v3n);
+                {
+                    const int tn = tb + kBatch + lane;
+                    if (tn < t_end) fetch_tone(lp.tab + tn, v0n, v1n, v2n, v3n);
+                }
                 const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
                 const unsigned m_sta = __ballot_sync(0xffffffffu, is_static);
                 if (lane == 0) ws.mov[b] = m_mov;
@@ -720,15 +724,16 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
             for (int v = 0; v < kSPT / 4; ++v) ws.park[r][v][lane] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         team_sync<SPLIT>(team);
-        if (rank == 0) {
+        // every warp of the team merges and stores its share of the tile's blocks
+        {
 #pragma unroll 1
-            for (int r = 0; r < kBlocksPerTile; ++r) {
+            for (int r = rank; r < kBlocksPerTile; r += SPLIT) {
                 Acc16 sum;
 #pragma unroll
                 for (int j = 0; j < kPairs; ++j) sum.a[j] = make_float2(0.f, 0.f);
                 // fixed summation order (rank 0, 1, ...) keeps the result independent of scheduling
 #pragma unroll
-                for (int r2 = 0; r2 < SPLIT; ++r2) park_add(ws_all[warp + r2], r, lane, sum);
+                for (int r2 = 0; r2 < SPLIT; ++r2) park_add(ws_all[warp - rank + r2], r, lane, sum);
                 store_block(lp, n_thread + r * kBlock, sum);
             }
         }
