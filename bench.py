@@ -12,8 +12,9 @@ buffer.  Metric: tone-samples/s (G).  Rank 0 prints ONE JSON line.
   value      device-timed (CUDA events on the launch stream), inputs resident in HBM
   e2e        the same workload through the C ABI with HOST buffers: awg_set_trajectories from host arrays
              (H2D table upload) + awg_synthesize_range_host into pinned host memory (D2H of the int16 codes)
-  roofline   the synthesis kernel is bound by the XU (MUFU) pipe, one MUFU.SIN per tone-sample:
-             peak = 16 MUFU/clk/SM x 148 SMs x sm_max_mhz; bound "alu"
+  roofline   ALU-bound ("bound": "alu"): a tone-sample needs one fp32 multiply-add where its tone is static (angle
+             addition) and one MUFU.SIN + two multiply-adds inside a move; the pipe (FMA: 128/clk/SM, XU: 16/clk/SM,
+             x 148 SMs x sm_max_mhz) whose roofline time is larger binds; frac = that time / measured launch time
   cpu_baseline  the oracle (oracle/awg_oracle_c.c, as it stands) on this box's host cores, bounded sample
   extras     the other configs (C1, C3, C4 ring, C5 sweep) and the real-time capacity search
 
@@ -41,7 +42,8 @@ import awg_workloads as W  # noqa: E402
 
 METRIC = "tone-samples/s"
 UNIT = "Gtone-samples/s"
-MUFU_PER_CLK_PER_SM = 16  # sm_100: 4 SFU lanes per SM sub-partition (measured 15.85/clk/SM, profiles/)
+MUFU_PER_CLK_PER_SM = 16  # sm_100: 4 SFU lanes per SM sub-partition (measured 15.9/clk/SM, profiles/)
+FMA_PER_CLK_PER_SM = 128  # sm_100: 32 fp32 lanes per SM sub-partition (measured 127/clk/SM with FFMA2, profiles/)
 N_SM = 148
 L2_BYTES = 126 * (1 << 20)
 
@@ -187,6 +189,43 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def moving_tone_samples(w) -> int:
+    """Tone-samples of workload w that fall inside a move (sample granularity; initial trajectory table only)."""
+    fs = float(w.sample_rate)
+    total = 0
+    for k in range(w.n_tones):
+        if int(w.profile[k]) == W.PROFILE_STATIC or float(w.f1[k]) == float(w.f0[k]) or float(w.t_dur[k]) <= 0.0:
+            continue
+        a = max(0.0, float(w.t_start[k]) * fs)
+        b = min(float(w.n_samples), (float(w.t_start[k]) + float(w.t_dur[k])) * fs)
+        if b > a:
+            total += int(b - a)
+    return total
+
+
+def pipe_roofline(w, ms, engine, sm_mhz):
+    """Binding ALU roofline of one launch over workload w.
+
+    Algorithmic work: a tone-sample of a tone that is static there needs ONE fp32 multiply-add (angle addition over a
+    symmetric sample pair); a tone-sample inside a move needs one MUFU.SIN plus two multiply-adds (range multiply,
+    amplitude accumulate).  With --engine mufu every tone-sample takes the MUFU path.  The roofline time is the larger
+    of (multiply-adds / FMA-pipe peak) and (sines / XU-pipe peak) at sm_mhz; frac = that time / the measured time."""
+    n_mov = w.tone_samples if engine == "mufu" else moving_tone_samples(w)
+    n_sta = w.tone_samples - n_mov
+    fma_ops, xu_ops = n_sta + 2 * n_mov, n_mov
+    peak_fma = FMA_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
+    peak_xu = MUFU_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
+    t_fma, t_xu = fma_ops / peak_fma, xu_ops / peak_xu
+    t = ms * 1e-3
+    if t_fma >= t_xu:
+        pipe, ops, peak, unit = "FMA (fp32 multiply-add)", fma_ops, peak_fma, "GFMA/s"
+    else:
+        pipe, ops, peak, unit = "XU (MUFU.SIN)", xu_ops, peak_xu, "Gsin/s"
+    return {"bound": "alu", "pipe": pipe, "achieved": ops / t / 1e9, "peak": peak / 1e9, "unit": unit,
+            "frac": max(t_fma, t_xu) / t, "static_tone_samples": int(n_sta), "moving_tone_samples": int(n_mov),
+            "fma_ops": int(fma_ops), "mufu_ops": int(xu_ops), "t_fma_us": t_fma * 1e6, "t_xu_us": t_xu * 1e6}
+
+
 ENGINES = {"auto": lambda awg: awg.AWG_ENGINE_AUTO, "fma": lambda awg: awg.AWG_ENGINE_FMA,
            "mufu": lambda awg: awg.AWG_ENGINE_MUFU}
 
@@ -290,7 +329,7 @@ def realtime_capacity(torch, awg, fs, chunk_len, mix, host_mirror, seconds, lo=1
     return good
 
 
-def run_extras(torch, awg, peak_sin, quick):
+def run_extras(torch, awg, sm_max_mhz, quick):
     out = {}
     # per-config device throughput (range launch for C1/C3, per-cell chunk launch for C5)
     cfgs = {}
@@ -299,7 +338,7 @@ def run_extras(torch, awg, peak_sin, quick):
         bufs = make_bufs(torch, w.n_samples)
         ms = device_time_range(torch, p, w.n_chunks, bufs, 5 if name == "C3" else 50, 3)
         cfgs[name] = {"tones": w.n_tones, "samples": w.n_samples, "ms": ms, "gts_per_s": w.tone_samples / ms / 1e6,
-                      "out_MS_per_s": w.n_samples / ms / 1e3, "frac_xu_peak": w.tone_samples / (ms * 1e-3) / peak_sin}
+                      "out_MS_per_s": w.n_samples / ms / 1e3, "roofline_frac": pipe_roofline(w, ms, "auto", sm_max_mhz)["frac"]}
         del bufs
         p.close()
     w4 = W.config4(96 if quick else 382)
@@ -359,7 +398,6 @@ def run_ours(args):
 
     peaks, peaks_src = read_peaks()
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
-    peak_sin = MUFU_PER_CLK_PER_SM * N_SM * sm_max_mhz * 1e6  # MUFU.SIN per second at max clock
 
     w, w_desc = pick_workload(args.workload)
     plan = awg.Plan.from_workload(w, engine=ENGINES[args.engine](awg))
@@ -419,23 +457,23 @@ def run_ours(args):
 
     # ---- roofline of the dominant (only) kernel ---------------------------------------------------
     ms_local = ms_total / args.steps
-    achieved = w.tone_samples / (ms_local * 1e-3)  # MUFU.SIN per second = tone-samples per second of one launch
     traffic = None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get("awg_mufu_kernel_C2_dram_bytes_per_launch")
+            traffic = json.load(f).get("awg_synth_kernel_C2_dram_bytes_per_launch")
     except Exception:
         pass
-    roofline = {
-        "bound": "alu", "pipe": "XU (MUFU.SIN), one per tone-sample", "achieved": achieved / 1e9, "peak": peak_sin / 1e9,
-        "unit": "Gsin/s", "frac": achieved / peak_sin, "traffic": traffic,
-        "peak_how": f"16 MUFU/clk/SM x 148 SMs x {sm_max_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peaks_src})",
-        "kernel": "awg_mufu_kernel", "launch_ms": ms_local,
+    roofline = pipe_roofline(w, ms_local, args.engine, sm_max_mhz)
+    roofline.update({
+        "traffic": traffic,
+        "peak_how": f"{FMA_PER_CLK_PER_SM} FMA (or {MUFU_PER_CLK_PER_SM} MUFU) /clk/SM x {N_SM} SMs x {sm_max_mhz:.0f} MHz "
+                    f"(sm_max_mhz of MEASURED_PEAKS.json, {peaks_src}); the pipe whose roofline time is larger binds",
+        "kernel": "awg_synth_kernel", "launch_ms": ms_local,
         "hbm": {"algorithmic_bytes_per_launch": 2 * w.n_samples, "achieved_gbs": 2 * w.n_samples / (ms_local * 1e-3) / 1e9,
                 "peak_gbs": peaks.get("hbm_gbs"), "frac": 2 * w.n_samples / (ms_local * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0))},
-    }
+    })
     if clocks.get("sm_mhz"):
-        roofline["frac_at_achieved_clock"] = achieved / (MUFU_PER_CLK_PER_SM * N_SM * clocks["sm_mhz"] * 1e6)
+        roofline["frac_at_achieved_clock"] = pipe_roofline(w, ms_local, args.engine, clocks["sm_mhz"])["frac"]
 
     # ---- oracle on this box's host cores (bounded sample) ----------------------------------------
     n_cpu = 1 << 22
@@ -458,7 +496,7 @@ def run_ours(args):
         "phase_dtype": "u64 fixed-point turns + fp64 re-centring, u32/fp32 in the inner loop",
     }
     if world == 1 and not args.no_extras:
-        line["extras"] = run_extras(torch, awg, peak_sin, not args.full)
+        line["extras"] = run_extras(torch, awg, sm_max_mhz, not args.full)
     plan.close()
     print(json.dumps(line), flush=True)
     if dist is not None:

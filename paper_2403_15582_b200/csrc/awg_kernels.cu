@@ -235,10 +235,11 @@ struct __align__(16) MovRec {
 struct __align__(16) WarpSmem {
     StageRec st[kBatch + 1];                // +1: the loop prefetches one carrier record ahead
     MovRec mrec[kBatch];
-    float4 park[kBlocksPerTile][kSPT / 4][32];   // partial sums of the tile: [block][4 samples][lane]
+    float4 park[kBlocksPerTile][kSPT / 4][32];   // the warp's static partial sums of the tile: [block][4 samples][lane]
     uint32_t mov[kMaxBatches];              // per batch of 32 tones: which ones take the MUFU pass in this tile
     uint32_t next;                          // (rank-0 warp of a team) the team's next tile, drawn by the leader
-    uint32_t pad_[3];
+    uint32_t n_mov;                         // how many of the warp's tones take the MUFU pass in this tile
+    uint32_t pad_[2];
     uint16_t list[kListCap];                // compacted tone indices (relative to the warp's first tone) of the MUFU pass
 };
 
@@ -432,20 +433,20 @@ __device__ __forceinline__ void sincos_tile(const uint4 cc, int off, float (&s)[
 template <int SPLIT>
 __device__ __forceinline__ void team_sync(int team)
 {
-    if (SPLIT == kWarps) __syncthreads();
-    else if (SPLIT > 1) asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(SPLIT * 32) : "memory");
+    if (SPLIT == 1) __syncwarp();
+    else if (SPLIT == kWarps) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(SPLIT * 32) : "memory");
 }
 
-// MUFU pass of one warp over one tile.  The tones flagged in ws.mov are compacted into ws.list (kListCap at a
-// time); every (tone, block) pair of the list is re-centred (step a1, one lane per pair, block-major so the records
-// of a block are contiguous) and the records of each block are then run KIND BY KIND (warp-uniform loops over ballot
-// masks, no per-record switch) with one MUFU.SIN per tone-sample into that block's 16 samples, which live in ws.park
-// between sub-batches.  Few registers are live here (one block's accumulators), so the 16 sine chains of a record
-// run in parallel.  Which records share a sub-batch depends only on the tile and the tone partition, never on the
-// launch range, so the fp32 summation order is the same for every chunking.
+// MUFU pass of one warp over ONE BLOCK of a tile, for the tones flagged in `mov` (the bit masks one warp of the team
+// left after its static pass; first tone t_begin).  The flagged tones are compacted into ws.list (kListCap at a
+// time); every listed tone is re-centred on the block (step a1, one lane per tone) and the records are then run
+// KIND BY KIND (warp-uniform loops over ballot masks, no per-record switch) with one MUFU.SIN per tone-sample into
+// the block's 16 samples per thread, which stay in registers.  Which records share a sub-batch depends only on the
+// tile and the tone partition, never on the launch range, so the fp32 summation order is the same for every chunking.
 #define AWG_RUN_KIND(K)                                                      \
     {                                                                        \
-        unsigned m_ = in_r & mk[K];                                          \
+        unsigned m_ = kv & mk[K];                                            \
         while (m_) {                                                         \
             const int i_ = __ffs(m_) - 1;                                    \
             m_ &= m_ - 1;                                                    \
@@ -453,8 +454,8 @@ __device__ __forceinline__ void team_sync(int team)
         }                                                                    \
     }
 
-__device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws, int t_begin, int t_end, int64_t tile_base,
-                                           int64_t n_end, int lane, uint32_t &park_valid)
+__device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws, const uint32_t *mov, int t_begin, int t_end,
+                                            int64_t blk_base, int lane, Acc16 &acc)
 {
     const int koff = lane * kSPT - kHalf;
     const unsigned lt = (1u << lane) - 1u;
@@ -469,70 +470,50 @@ __device__ __forceinline__ void mover_pass(const LaunchParams &lp, WarpSmem &ws,
         const int b1 = min(b0 + kListBatches, n_batches);
         int n = 0;
         for (int b = b0; b < b1; ++b) {
-            const unsigned m = ws.mov[b];
+            const unsigned m = mov[b];
             if ((m >> lane) & 1u) ws.list[n + __popc(m & lt)] = static_cast<uint16_t>(b * kBatch + lane);
             n += __popc(m);
         }
         if (n == 0) continue;
         __syncwarp();
-        const int n_pairs = n * kBlocksPerTile;
-        for (int q0 = 0; q0 < n_pairs; q0 += kBatch) {
-            const int idx = q0 + lane;
+        for (int q0 = 0; q0 < n; q0 += kBatch) {
             BlockRec br;
             br.kind = K_NONE;
-            if (idx < n_pairs) {
-                const int r_lane = (idx >= n) + (idx >= 2 * n) + (idx >= 3 * n);
-                static_assert(kBlocksPerTile == 4, "r_lane assumes four blocks per tile");
-                const int64_t blk_base = tile_base + static_cast<int64_t>(r_lane) * kBlock;
-                if (blk_base < n_end && blk_base + kBlock > lp.n_begin) {
-                    const int t = t_begin + ws.list[idx - r_lane * n];
-                    br = block_prologue(lp.tab + t, t, static_cast<uint64_t>(blk_base + kHalf), static_cast<double>(blk_base));
-                }
+            if (q0 + lane < n) {
+                const int t = t_begin + ws.list[q0 + lane];
+                br = block_prologue(lp.tab + t, t, static_cast<uint64_t>(blk_base + kHalf), static_cast<double>(blk_base));
             }
             const unsigned kv = __ballot_sync(0xffffffffu, br.kind >= 0);
             const unsigned k0 = __ballot_sync(0xffffffffu, (br.kind & 1) != 0);
             const unsigned k1 = __ballot_sync(0xffffffffu, (br.kind & 2) != 0);
             const unsigned k2 = __ballot_sync(0xffffffffu, (br.kind & 4) != 0);
             unsigned mk[K_COUNT];
-            mk[K_STATIC] = kv & ~k0 & ~k1 & ~k2;
-            mk[K_QUAD] = kv & k0 & ~k1 & ~k2;
-            mk[K_DEG4] = kv & ~k0 & k1 & ~k2;
-            mk[K_DEG6] = kv & k0 & k1 & ~k2;
-            mk[K_SBEG] = kv & ~k0 & ~k1 & k2;
-            mk[K_SEND] = kv & k0 & ~k1 & k2;
-            mk[K_EXACT] = kv & ~k0 & k1 & k2;
+            mk[K_STATIC] = ~k0 & ~k1 & ~k2;
+            mk[K_QUAD] = k0 & ~k1 & ~k2;
+            mk[K_DEG4] = ~k0 & k1 & ~k2;
+            mk[K_DEG6] = k0 & k1 & ~k2;
+            mk[K_SBEG] = ~k0 & ~k1 & k2;
+            mk[K_SEND] = k0 & ~k1 & k2;
+            mk[K_EXACT] = ~k0 & k1 & k2;
             __syncwarp();  // the previous sub-batch's readers are done
             if (br.kind >= 0) {
                 ws.mrec[lane].q[0] = make_float4(__uint_as_float(br.c0), __uint_as_float(br.c1), br.A, br.c2);
                 ws.mrec[lane].q[1] = make_float4(br.c3, br.c4, br.c5, br.c6);
             }
             __syncwarp();
-#pragma unroll 1
-            for (int r = 0; r < kBlocksPerTile; ++r) {
-                const int lo = max(r * n - q0, 0), hi = min((r + 1) * n - q0, kBatch);
-                if (lo >= hi) continue;
-                const unsigned in_r = kv & (0xffffffffu >> (32 - hi)) & (0xffffffffu << lo);
-                if (in_r == 0) continue;
-                Acc16 acc;
-#pragma unroll
-                for (int j = 0; j < kPairs; ++j) acc.a[j] = make_float2(0.f, 0.f);
-                if (park_valid & (1u << r)) park_add(ws, r, lane, acc);
-                AWG_RUN_KIND(K_STATIC)
-                AWG_RUN_KIND(K_QUAD)
-                AWG_RUN_KIND(K_DEG4)
-                AWG_RUN_KIND(K_DEG6)
-                AWG_RUN_KIND(K_SBEG)
-                AWG_RUN_KIND(K_SEND)
-                {
-                    unsigned m_ = in_r & mk[K_EXACT];
-                    while (m_) {
-                        const int i_ = __ffs(m_) - 1;
-                        m_ &= m_ - 1;
-                        acc = exact_rec(lp.tab, ws.mrec[i_].q[0], tile_base + r * kBlock + lane * kSPT, acc);
-                    }
+            AWG_RUN_KIND(K_STATIC)
+            AWG_RUN_KIND(K_QUAD)
+            AWG_RUN_KIND(K_DEG4)
+            AWG_RUN_KIND(K_DEG6)
+            AWG_RUN_KIND(K_SBEG)
+            AWG_RUN_KIND(K_SEND)
+            {
+                unsigned m_ = kv & mk[K_EXACT];
+                while (m_) {
+                    const int i_ = __ffs(m_) - 1;
+                    m_ &= m_ - 1;
+                    acc = exact_rec(lp.tab, ws.mrec[i_].q[0], blk_base + lane * kSPT, acc);
                 }
-                park_store(ws, r, lane, acc);
-                park_valid |= 1u << r;
             }
         }
         __syncwarp();  // ws.list is rebuilt for the next kListCap tones
@@ -708,32 +689,35 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
             continue;
         }
 
-        // ---- partial sums go to shared memory; the MUFU pass adds the moving tones block by block
-        uint32_t park_valid = 0;
+        // ---- the static partial sums and the lists of moving tones go to shared memory; after the team barrier
+        // warp `rank` owns the blocks rank, rank + SPLIT, ...: it adds the team's partial sums in rank order, runs
+        // the MUFU pass of that block for the moving tones of EVERY warp of the team (so the moving tones load the
+        // team's warps evenly wherever they sit in the tone table), quantises and stores.
         if (ROT) {
 #pragma unroll
             for (int r = 0; r < kBlocksPerTile; ++r) park_store(ws, r, lane, acc[r]);
-            park_valid = (1u << kBlocksPerTile) - 1u;
         }
-        __syncwarp();
-        if (n_mov > 0) mover_pass(lp, ws, t_begin, t_end, tile_base, n_end, lane, park_valid);
-#pragma unroll 1
-        for (int r = 0; r < kBlocksPerTile; ++r) {
-            if (park_valid & (1u << r)) continue;
-#pragma unroll
-            for (int v = 0; v < kSPT / 4; ++v) ws.park[r][v][lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
+        if (lane == 0) ws.n_mov = static_cast<uint32_t>(n_mov);
         team_sync<SPLIT>(team);
-        // every warp of the team merges and stores its share of the tile's blocks
         {
+            WarpSmem *team_ws = ws_all + (warp - rank);
 #pragma unroll 1
             for (int r = rank; r < kBlocksPerTile; r += SPLIT) {
+                const int64_t blk_base = tile_base + static_cast<int64_t>(r) * kBlock;
+                if (blk_base >= n_end || blk_base + kBlock <= lp.n_begin) continue;
                 Acc16 sum;
 #pragma unroll
                 for (int j = 0; j < kPairs; ++j) sum.a[j] = make_float2(0.f, 0.f);
-                // fixed summation order (rank 0, 1, ...) keeps the result independent of scheduling
+                if (ROT) {
 #pragma unroll
-                for (int r2 = 0; r2 < SPLIT; ++r2) park_add(ws_all[warp - rank + r2], r, lane, sum);
+                    for (int r2 = 0; r2 < SPLIT; ++r2) park_add(team_ws[r2], r, lane, sum);
+                }
+#pragma unroll 1
+                for (int r2 = 0; r2 < SPLIT; ++r2) {
+                    if (team_ws[r2].n_mov == 0) continue;
+                    const int tb2 = r2 * per;
+                    mover_block(lp, ws, team_ws[r2].mov, tb2, min(lp.n_tones, tb2 + per), blk_base, lane, sum);
+                }
                 store_block(lp, n_thread + r * kBlock, sum);
             }
         }
