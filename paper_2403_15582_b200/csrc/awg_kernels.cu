@@ -234,7 +234,7 @@ struct __align__(16) MovRec {
 
 struct __align__(16) WarpSmem {
     StageRec st[kBatch + 1];                // +1: the loop prefetches one carrier record ahead
-    MovRec mrec[kBatch];
+    MovRec mrec[kBatch + 1];                // +1: the loops prefetch one record ahead
     float4 park[kBlocksPerTile][kSPT / 4][32];   // the warp's static partial sums of the tile: [block][4 samples][lane]
     uint32_t mov[kMaxBatches];              // per batch of 32 tones: which ones take the MUFU pass in this tile
     uint32_t next;                          // (rank-0 warp of a team) the team's next tile, drawn by the leader
@@ -444,14 +444,18 @@ __device__ __forceinline__ void team_sync(int team)
 // KIND BY KIND (warp-uniform loops over ballot masks, no per-record switch) with one MUFU.SIN per tone-sample into
 // the block's 16 samples per thread, which stay in registers.  Which records share a sub-batch depends only on the
 // tile and the tone partition, never on the launch range, so the fp32 summation order is the same for every chunking.
-#define AWG_RUN_KIND(K)                                                      \
-    {                                                                        \
-        unsigned m_ = kv & mk[K];                                            \
-        while (m_) {                                                         \
-            const int i_ = __ffs(m_) - 1;                                    \
-            m_ &= m_ - 1;                                                    \
-            mufu_rec<K>(ws.mrec[i_].q[0], ws.mrec[i_].q[1], koff, kf, kk, acc); \
-        }                                                                    \
+#define AWG_RUN_KIND(K)                                                                  \
+    {                                                                                    \
+        const int e_ = kbase[K] + kcnt[K];                                               \
+        if (kcnt[K] > 0) {                                                               \
+            float4 a_ = ws.mrec[kbase[K]].q[0], b_ = ws.mrec[kbase[K]].q[1];             \
+            _Pragma("unroll 1") for (int i_ = kbase[K] + 1; i_ <= e_; ++i_) {            \
+                const float4 an_ = ws.mrec[i_].q[0], bn_ = ws.mrec[i_].q[1]; /* next record (slot kBatch: spare) */ \
+                mufu_rec<K>(a_, b_, koff, kf, kk, acc);                                  \
+                a_ = an_;                                                                \
+                b_ = bn_;                                                                \
+            }                                                                            \
+        }                                                                                \
     }
 
 __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws, const uint32_t *mov, int t_begin, int t_end,
@@ -487,18 +491,31 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
             const unsigned k0 = __ballot_sync(0xffffffffu, (br.kind & 1) != 0);
             const unsigned k1 = __ballot_sync(0xffffffffu, (br.kind & 2) != 0);
             const unsigned k2 = __ballot_sync(0xffffffffu, (br.kind & 4) != 0);
+            // records are stored sorted by kind, so every kind's records are contiguous: mrec[kbase[K] .. +kcnt[K])
             unsigned mk[K_COUNT];
-            mk[K_STATIC] = ~k0 & ~k1 & ~k2;
-            mk[K_QUAD] = k0 & ~k1 & ~k2;
-            mk[K_DEG4] = ~k0 & k1 & ~k2;
-            mk[K_DEG6] = k0 & k1 & ~k2;
-            mk[K_SBEG] = ~k0 & ~k1 & k2;
-            mk[K_SEND] = k0 & ~k1 & k2;
-            mk[K_EXACT] = ~k0 & k1 & k2;
+            mk[K_STATIC] = kv & ~k0 & ~k1 & ~k2;
+            mk[K_QUAD] = kv & k0 & ~k1 & ~k2;
+            mk[K_DEG4] = kv & ~k0 & k1 & ~k2;
+            mk[K_DEG6] = kv & k0 & k1 & ~k2;
+            mk[K_SBEG] = kv & ~k0 & ~k1 & k2;
+            mk[K_SEND] = kv & k0 & ~k1 & k2;
+            mk[K_EXACT] = kv & ~k0 & k1 & k2;
+            int kbase[K_COUNT], kcnt[K_COUNT];
+            int slot = 0;
+            {
+                int run = 0;
+#pragma unroll
+                for (int k = 0; k < K_COUNT; ++k) {
+                    kbase[k] = run;
+                    kcnt[k] = __popc(mk[k]);
+                    if (br.kind == k) slot = run + __popc(mk[k] & lt);
+                    run += kcnt[k];
+                }
+            }
             __syncwarp();  // the previous sub-batch's readers are done
             if (br.kind >= 0) {
-                ws.mrec[lane].q[0] = make_float4(__uint_as_float(br.c0), __uint_as_float(br.c1), br.A, br.c2);
-                ws.mrec[lane].q[1] = make_float4(br.c3, br.c4, br.c5, br.c6);
+                ws.mrec[slot].q[0] = make_float4(__uint_as_float(br.c0), __uint_as_float(br.c1), br.A, br.c2);
+                ws.mrec[slot].q[1] = make_float4(br.c3, br.c4, br.c5, br.c6);
             }
             __syncwarp();
             AWG_RUN_KIND(K_STATIC)
@@ -507,14 +524,9 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
             AWG_RUN_KIND(K_DEG6)
             AWG_RUN_KIND(K_SBEG)
             AWG_RUN_KIND(K_SEND)
-            {
-                unsigned m_ = kv & mk[K_EXACT];
-                while (m_) {
-                    const int i_ = __ffs(m_) - 1;
-                    m_ &= m_ - 1;
-                    acc = exact_rec(lp.tab, ws.mrec[i_].q[0], blk_base + lane * kSPT, acc);
-                }
-            }
+#pragma unroll 1
+            for (int i_ = kbase[K_EXACT]; i_ < kbase[K_EXACT] + kcnt[K_EXACT]; ++i_)
+                acc = exact_rec(lp.tab, ws.mrec[i_].q[0], blk_base + lane * kSPT, acc);
         }
         __syncwarp();  // ws.list is rebuilt for the next kListCap tones
     }
