@@ -60,11 +60,11 @@ enum {
 /* sine engine of the synthesis kernel (step a3 of the hot path) */
 enum {
     AWG_ENGINE_AUTO = 0, /* the library picks (currently AWG_ENGINE_FMA)                                    */
-    AWG_ENGINE_MUFU = 1, /* one MUFU.SIN per (tone, sample); phase re-centred per 256-sample tile            */
+    AWG_ENGINE_MUFU = 1, /* one MUFU.SIN per (tone, sample); phase re-centred per 512-sample block           */
     AWG_ENGINE_FP64 = 2, /* reference-grade: closed form and sine in fp64 per (tone, sample); ~50x slower   */
-    AWG_ENGINE_FMA = 3   /* angle addition on the FMA pipe for tiles where a tone is static (one sin + one
-                            cos per 8 samples, then 2 FMA per sample with a per-tone rotation table);
-                            tiles inside a move use the MUFU path                                          */
+    AWG_ENGINE_FMA = 3   /* angle addition on the FMA pipe for 2048-sample tiles where a tone is static (one
+                            sin + one cos per thread, tone and 16 samples, then ONE multiply-add per
+                            tone-sample with a per-tone table); tiles inside a move use the MUFU path      */
 };
 
 /* ---- plan ---------------------------------------------------------------------------------- */
