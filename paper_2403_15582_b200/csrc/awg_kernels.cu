@@ -240,7 +240,7 @@ struct __align__(16) WarpSmem {
     uint32_t next;                          // (rank-0 warp of a team) the team's next tile, drawn by the leader
     uint32_t n_mov;                         // how many of the warp's tones take the MUFU pass in this tile
     uint32_t pad_[2];
-    uint16_t list[kListCap];                // compacted tone indices (relative to the warp's first tone) of the MUFU pass
+    uint16_t list[kListCap];                // compacted tone indices of the MUFU pass (n_tones <= 65536)
 };
 
 // 16 samples of one block of one thread, as 8 packed pairs: a[j] = samples (2j, 2j+1).
@@ -438,8 +438,8 @@ __device__ __forceinline__ void team_sync(int team)
     else asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(SPLIT * 32) : "memory");
 }
 
-// MUFU pass of one warp over ONE BLOCK of a tile, for the tones flagged in `mov` (the bit masks one warp of the team
-// left after its static pass; first tone t_begin).  The flagged tones are compacted into ws.list (kListCap at a
+// MUFU pass of one warp over ONE BLOCK of a tile, for the tones the team's warps flagged in their `mov` bit masks
+// (warp r2 owns tones r2*per ...).  The flagged tones of the whole team are compacted into ws.list (kListCap at a
 // time); every listed tone is re-centred on the block (step a1, one lane per tone) and the records are then run
 // KIND BY KIND (warp-uniform loops over ballot masks, no per-record switch) with one MUFU.SIN per tone-sample into
 // the block's 16 samples per thread, which stay in registers.  Which records share a sub-batch depends only on the
@@ -458,7 +458,8 @@ __device__ __forceinline__ void team_sync(int team)
         }                                                                                \
     }
 
-__device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws, const uint32_t *mov, int t_begin, int t_end,
+template <int SPLIT>
+__device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws, const WarpSmem *team_ws, int per,
                                             int64_t blk_base, int lane, Acc16 &acc)
 {
     const int koff = lane * kSPT - kHalf;
@@ -469,22 +470,30 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
         kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
         kk[j] = __fmul2_rn(kf[j], kf[j]);
     }
-    const int n_batches = (t_end - t_begin + kBatch - 1) / kBatch;
-    for (int b0 = 0; b0 < n_batches; b0 += kListBatches) {
-        const int b1 = min(b0 + kListBatches, n_batches);
+    int r2 = 0, b = 0;
+    while (r2 < SPLIT) {
+        // gather: the moving tones of the team's warps, in (warp, tone) order, up to kListCap at a time
         int n = 0;
-        for (int b = b0; b < b1; ++b) {
-            const unsigned m = mov[b];
-            if ((m >> lane) & 1u) ws.list[n + __popc(m & lt)] = static_cast<uint16_t>(b * kBatch + lane);
+        while (r2 < SPLIT && n + kBatch <= kListCap) {
+            const int tb2 = r2 * per;
+            const int len = min(lp.n_tones, tb2 + per) - tb2;
+            if (team_ws[r2].n_mov == 0 || b * kBatch >= len) {
+                ++r2;
+                b = 0;
+                continue;
+            }
+            const unsigned m = team_ws[r2].mov[b];
+            if ((m >> lane) & 1u) ws.list[n + __popc(m & lt)] = static_cast<uint16_t>(tb2 + b * kBatch + lane);
             n += __popc(m);
+            ++b;
         }
-        if (n == 0) continue;
+        if (n == 0) break;
         __syncwarp();
         for (int q0 = 0; q0 < n; q0 += kBatch) {
             BlockRec br;
             br.kind = K_NONE;
             if (q0 + lane < n) {
-                const int t = t_begin + ws.list[q0 + lane];
+                const int t = ws.list[q0 + lane];
                 br = block_prologue(lp.tab + t, t, static_cast<uint64_t>(blk_base + kHalf), static_cast<double>(blk_base));
             }
             const unsigned kv = __ballot_sync(0xffffffffu, br.kind >= 0);
@@ -628,6 +637,9 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                         } else {
                             is_static = false;
                             is_mover = true;
+                            // the block owners re-centre this tone after the barrier: pull its record towards L1 now
+                            asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char *>(tr)));
+                            asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char *>(tr) + 96));
                         }
                     }
                     c0 = round32(th + w * a0 - (w >> 1));
@@ -724,11 +736,11 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
 #pragma unroll
                     for (int r2 = 0; r2 < SPLIT; ++r2) park_add(team_ws[r2], r, lane, sum);
                 }
-#pragma unroll 1
-                for (int r2 = 0; r2 < SPLIT; ++r2) {
-                    if (team_ws[r2].n_mov == 0) continue;
-                    const int tb2 = r2 * per;
-                    mover_block(lp, ws, team_ws[r2].mov, tb2, min(lp.n_tones, tb2 + per), blk_base, lane, sum);
+                {
+                    uint32_t any = 0;
+#pragma unroll
+                    for (int r2 = 0; r2 < SPLIT; ++r2) any |= team_ws[r2].n_mov;
+                    if (any) mover_block<SPLIT>(lp, ws, team_ws, per, blk_base, lane, sum);
                 }
                 store_block(lp, n_thread + r * kBlock, sum);
             }
