@@ -1,16 +1,18 @@
 // awg_kernels.cu -- sm_100a synthesis kernels: the fused WG + WC (+ quantise) of PAPER.md:158-186.
 //
-// Hot-path steps (SURVEY.md section 8(a) / DESIGN.md):
-//   a1  per (tone, 512-sample block) phase re-centring in 64-bit fixed point + fp64     block_prologue()
-//   a2  per tone-sample phase  c0 + c1*k (u32 turns, wraps exactly) + fp32 polynomial   mufu_loop<KIND>()
-//   a3  sine.  MUFU engine, and every block in which a tone is moving: one MUFU.SIN per tone-sample.
-//       Angle-addition engine, tiles in which a tone is static: one MUFU.SIN + one MUFU.COS per (thread, tone,
-//       2048-sample tile), then per symmetric sample pair centre +- (j + 1/2)
+// Hot-path steps (SURVEY.md section 8(a) / DESIGN.md section 6):
+//   a1  re-centring in 64-bit fixed point + fp64: per (tone, 2048-sample tile) a u32 carrier for tones static there
+//       (stage of the static pass in awg_synth_kernel), per (tone, 512-sample block) c0, c1, c2..c6 and the record
+//       kind for tones moving there                                                          block_prologue()
+//   a2  per tone-sample phase of a moving tone: c0 + c1*k (u32 turns, wraps exactly) + fp32 polynomial  mufu_rec<KIND>()
+//   a3  sine.  Tiles in which a tone is static (angle-addition engine): one MUFU.SIN + one MUFU.COS per (thread, tone,
+//       block), then per symmetric sample pair centre +- (j + 1/2)
 //           A sin(phi +- (j+1/2) w) = sin(phi) [A cos((j+1/2) w)]  +-  cos(phi) [A sin((j+1/2) w)]
-//       i.e. ONE fp32 multiply-add per tone-sample into the even/odd accumulators P_j, Q_j      static_pass()
-//   a4  fp32 register accumulation over tones: 4 blocks x 16 samples per thread
-//   a5  quantise: cvt.rni.sat.s16.f32(scale * acc)                                      store_block()
-//   a6  two 16-byte stores of 8 consecutive int16 per thread and block                  store_block()
+//       i.e. ONE fp32 multiply-add per tone-sample into the even/odd accumulators P_j, Q_j    sincos_tile(), pq_add()
+//       Blocks in which a tone moves (and every tone-sample of the MUFU engine): one MUFU.SIN each   mufu_rec<KIND>()
+//   a4  fp32 register accumulation over tones: 4 blocks x 16 samples per thread (static pass), 16 (MUFU pass)
+//   a5  quantise: cvt.rni.sat.s16.f32(scale * acc)                                           store_block()
+//   a6  two 16-byte stores of 8 consecutive int16 per thread and block                       store_block()
 // No tensor cores (north_star), no per-tone wavetable in DRAM (the paper's limiter); output
 // traffic is 2 bytes per sample.
 #include <cstddef>
