@@ -600,8 +600,14 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
     // (v0n..v3n stay in registers across it, the two carrier tables are pulled into L1); after the last batch of a
     // tile the request wraps round to the first batch, which is what the next tile starts with.
     uint4 v0n = make_uint4(0, 0, 0, 0), v1n = v0n, v2n = v0n, v3n = v0n;
+    // A warp whose tones fit one batch keeps their records in registers for the whole launch, and their tables in
+    // shared memory for as long as the same tones are static on the same carriers (sticky_sta / sticky_post).
+    const bool single = t_end - t_begin <= kBatch;
+    bool have_records = false;
+    unsigned sticky_sta = 0u, sticky_post = 0xffffffffu;   // no tile has post bits outside its static bits
     while (unit < n_tiles) {
-        if (ROT && t_begin + lane < t_end) fetch_tone(lp.tab + t_begin + lane, v0n, v1n, v2n, v3n);
+        if (ROT && t_begin + lane < t_end && !(single && have_records)) fetch_tone(lp.tab + t_begin + lane, v0n, v1n, v2n, v3n);
+        have_records = true;
         const int64_t tile_base = (first_tile + unit) * kTile;
         Acc16 acc[kBlocksPerTile];
         int n_mov = 0;
@@ -618,7 +624,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
             const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int t = tb + lane;
-                bool is_static = false, is_mover = false;
+                bool is_static = false, is_mover = false, is_post = false;
                 uint32_t c0 = 0, c1 = 0, d = 0;
                 const float4 *tabp = nullptr;
                 if (t < t_end) {
@@ -636,6 +642,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                             th = u64_of(v1.z, v1.w);
                             w = u64_of(v2.x, v2.y);
                             tabp = reinterpret_cast<const float4 *>(&tr->rot_post);
+                            is_post = true;
                         } else {
                             is_static = false;
                             is_mover = true;
@@ -658,11 +665,17 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 n_mov += __popc(m_mov);
                 const int n_sta = __popc(m_sta);
                 __syncwarp();  // the previous batch's readers are done
+                const unsigned m_post = __ballot_sync(0xffffffffu, is_post);
+                const bool tables_staged = single && m_sta == sticky_sta && m_post == sticky_post;
+                sticky_sta = m_sta;
+                sticky_post = m_post;
                 if (is_static) {
                     StageRec &sr = ws.st[__popc(m_sta & lt)];
-                    const float4 C03 = __ldg(tabp), C47 = __ldg(tabp + 1), S03 = __ldg(tabp + 2), S47 = __ldg(tabp + 3);
                     *reinterpret_cast<uint4 *>(&sr) = make_uint4(c0, c1, d, 0u);
-                    sr.C03 = C03; sr.C47 = C47; sr.S03 = S03; sr.S47 = S47;
+                    if (!tables_staged) {
+                        const float4 C03 = __ldg(tabp), C47 = __ldg(tabp + 1), S03 = __ldg(tabp + 2), S47 = __ldg(tabp + 3);
+                        sr.C03 = C03; sr.C47 = C47; sr.S03 = S03; sr.S47 = S47;
+                    }
                 }
                 __syncwarp();
                 // Software pipeline, unrolled by two so that the sines/cosines ping-pong between two register sets:
