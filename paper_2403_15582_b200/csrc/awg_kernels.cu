@@ -684,28 +684,27 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 // profiles/), hence the packed range multiply and no register moves.
                 float sa[kBlocksPerTile], ca[kBlocksPerTile], sb[kBlocksPerTile], cb[kBlocksPerTile];
                 sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[0]), off, sa, ca);
-                int i = 0;
+                // a running pointer keeps the loop free of index arithmetic (IMAD shares the FMA pipe)
+                const StageRec *sp = ws.st;
+                const StageRec *const sp_end = ws.st + n_sta;
 #pragma unroll 1
-                for (; i + 1 < n_sta; i += 2) {
+                for (; sp + 1 < sp_end; sp += 2) {
                     {
-                        const StageRec &sr = ws.st[i];
-                        const float4 C03 = sr.C03, C47 = sr.C47, S03 = sr.S03, S47 = sr.S47;
-                        sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[i + 1]), off, sb, cb);
+                        const float4 C03 = sp[0].C03, C47 = sp[0].C47, S03 = sp[0].S03, S47 = sp[0].S47;
+                        sincos_tile(*reinterpret_cast<const uint4 *>(sp + 1), off, sb, cb);
 #pragma unroll
                         for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
                     }
                     {
-                        const StageRec &sr = ws.st[i + 1];
-                        const float4 C03 = sr.C03, C47 = sr.C47, S03 = sr.S03, S47 = sr.S47;
+                        const float4 C03 = sp[1].C03, C47 = sp[1].C47, S03 = sp[1].S03, S47 = sp[1].S47;
                         // slot i + 2 <= kBatch exists; past the last tone it is stale and its result unused
-                        sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[i + 2]), off, sa, ca);
+                        sincos_tile(*reinterpret_cast<const uint4 *>(sp + 2), off, sa, ca);
 #pragma unroll
                         for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sb[r], cb[r], C03, C47, S03, S47);
                     }
                 }
-                if (i < n_sta) {
-                    const StageRec &sr = ws.st[i];
-                    const float4 C03 = sr.C03, C47 = sr.C47, S03 = sr.S03, S47 = sr.S47;
+                if (sp < sp_end) {
+                    const float4 C03 = sp[0].C03, C47 = sp[0].C47, S03 = sp[0].S03, S47 = sp[0].S47;
 #pragma unroll
                     for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
                 }
