@@ -283,6 +283,21 @@ def test_max_tone_count_4096_and_more(awg, torch_cuda, eng):
     p.close()
 
 
+def test_plan_limit_65536_tones(awg, torch_cuda, eng):
+    """The largest plan (include/awg.h: n_tones <= 65536): every warp walks 512 batches of 32 tones; a third of the
+    tones is inside a move in the synthesised chunk, so the moving-tone lists are rebuilt many times per block."""
+    N = 65536
+    rng = np.random.default_rng(7)
+    f0 = rng.uniform(20e6, 250e6, N)
+    rows = [(f0[k], f0[k] + (2e6 if k % 3 == 1 else 0.0), 1.0 / N, rng.uniform(0, 6.28), 0.0, 20e-6,
+             MINJERK if k % 3 == 1 else STATIC) for k in range(N)]
+    p, op = _single(awg, 560e6, 2048, rows, engine=eng)
+    V = oracle.c_waveform(op, 2 * 2048, 3 * 2048)
+    assert_f32_close(_np(p.synthesize_chunk_f32(2)), V, "N=65536")
+    assert_codes_close(_np(p.synthesize_chunk(2)), op.quantise(V), "N=65536")
+    p.close()
+
+
 def test_special_moves(awg, torch_cuda, eng):
     fs = 560e6
     rows = [
