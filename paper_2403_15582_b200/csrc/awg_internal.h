@@ -15,7 +15,8 @@ enum : int32_t {
     CLS_QUAD = 2,    // moving tiles need the k^2 term only (LINEAR always; slow MINJERK)
     CLS_DEG4 = 4,    // k^2..k^4
     CLS_DEG6 = 6,    // k^2..k^6 (exact Taylor series of the degree-6 min-jerk phase)
-    CLS_EXACT = 7    // fp32 in-tile polynomial not accurate enough: moving tiles use the fp64 path
+    CLS_EXACT = 7,   // fp32 in-tile polynomial not accurate enough: moving tiles use the fp64 path
+    CLS_SLOW_FLAG = 1 << 16  // OR-ed into ToneRec::cls: tiles wholly inside the move may take the slow pass (FMA pipe)
 };
 
 // Kernel geometry.  A thread owns kSPT consecutive samples of a block; a block is 32 lanes x kSPT = 512 samples

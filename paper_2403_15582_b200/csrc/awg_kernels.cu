@@ -86,7 +86,7 @@ __device__ __forceinline__ uint64_t exact_phase(const ToneRec &r, int64_t n)
     const double u = (static_cast<double>(n) - r.ns_int) - r.ns_frac;
     if (u <= 0.0) return r.theta_pre + r.w_pre * static_cast<uint64_t>(n);
     if (u >= r.Tn) return r.theta_post + r.w_post * static_cast<uint64_t>(n);
-    const double x = r.DT * profile_g(r.cls >> 8, u * r.inv_Tn);
+    const double x = r.DT * profile_g((r.cls >> 8) & 0xff, u * r.inv_Tn);
     return r.theta_pre + r.w_pre * static_cast<uint64_t>(n) + frac_to_fix64(x);
 }
 
@@ -142,7 +142,7 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
         const double Tn = f64_of(v3.z, v3.w);
         const double ua = (bb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the block's first sample
         const double ub = ua + static_cast<double>(kBlock - 1);
-        const bool linear = (cls >> 8) == AWG_PROFILE_LINEAR;
+        const bool linear = ((cls >> 8) & 0xff) == AWG_PROFILE_LINEAR;
         if (ub <= 0.0) {
             w = w_pre;
             ph = theta_pre + w * nc;
@@ -560,6 +560,63 @@ __device__ __forceinline__ int64_t next_unit(const LaunchParams &lp, WarpSmem &w
     return n_teams + static_cast<int64_t>(v);
 }
 
+// Slow pass, staging (one lane per slow mover): the pair tables at the tile-centre frequency c1 come from MUFU
+// (the frequency changes from tile to tile, so they cannot be precomputed), the second record holds their
+// first-order correction: cos((j+1/2)(w + e)) ~ C_j - (j+1/2) e S_j,  sin((j+1/2)(w + e)) ~ S_j + (j+1/2) e C_j.
+__device__ __forceinline__ void stage_slow(StageRec *dst, const MovRec &parked)
+{
+    const float4 a = parked.q[0];
+    const uint32_t c1 = __float_as_uint(a.y);
+    const float A = parked.q[1].x;
+    float C[kPairs], S[kPairs];
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) {
+        const uint32_t ang = c1 * static_cast<uint32_t>(j) + (c1 >> 1);   // (j + 1/2) c1, u32 turns
+        const float x = __int2float_rn(static_cast<int32_t>(ang)) * kTurnToRad;
+        C[j] = A * mufu_cos(x);
+        S[j] = A * mufu_sin(x);
+    }
+    *reinterpret_cast<float4 *>(&dst[0]) = a;   // {c0 at the tile centre - 1/2, c1, c2, c3}
+    dst[0].C03 = make_float4(C[0], C[1], C[2], C[3]);
+    dst[0].C47 = make_float4(C[4], C[5], C[6], C[7]);
+    dst[0].S03 = make_float4(S[0], S[1], S[2], S[3]);
+    dst[0].S47 = make_float4(S[4], S[5], S[6], S[7]);
+    // correction record: multiplies -sin(phi) e into (j+1/2) S_j and cos(phi) e into (j+1/2) C_j
+    dst[1].C03 = make_float4(0.5f * S[0], 1.5f * S[1], 2.5f * S[2], 3.5f * S[3]);
+    dst[1].C47 = make_float4(4.5f * S[4], 5.5f * S[5], 6.5f * S[6], 7.5f * S[7]);
+    dst[1].S03 = make_float4(0.5f * C[0], 1.5f * C[1], 2.5f * C[2], 3.5f * C[3]);
+    dst[1].S47 = make_float4(4.5f * C[4], 5.5f * C[5], 6.5f * C[6], 7.5f * C[7]);
+}
+
+// Slow pass, one tone: phase polynomial at the thread's pair centre in each block (k = offset from the tile centre),
+// local frequency offset e = d(poly)/dk, then two multiply-adds per tone-sample.
+__device__ __forceinline__ void slow_pair(const StageRec &m, const StageRec &k, int lane, PQ (&pq)[kBlocksPerTile])
+{
+    const uint4 cc = *reinterpret_cast<const uint4 *>(&m);
+    const float c2 = __uint_as_float(cc.z), c3 = __uint_as_float(cc.w);
+    float s[kBlocksPerTile], c[kBlocksPerTile], e[kBlocksPerTile];
+#pragma unroll
+    for (int r = 0; r < kBlocksPerTile; ++r) {
+        const int mr = r * kBlock + lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre
+        const float kf = static_cast<float>(mr) - 0.5f;
+        const uint32_t p = cc.x + cc.y * static_cast<uint32_t>(mr);
+        const float x = fmaf(__int2float_rn(static_cast<int32_t>(p)), kTurnToRad, kf * kf * fmaf(kf, c3, c2));
+        s[r] = mufu_sin(x);
+        c[r] = mufu_cos(x);
+        e[r] = kf * fmaf(3.f * kf, c3, 2.f * c2);
+    }
+    {
+        const float4 C03 = m.C03, C47 = m.C47, S03 = m.S03, S47 = m.S47;
+#pragma unroll
+        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], s[r], c[r], C03, C47, S03, S47);
+    }
+    {
+        const float4 C03 = k.C03, C47 = k.C47, S03 = k.S03, S47 = k.S47;
+#pragma unroll
+        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], -s[r] * e[r], c[r] * e[r], C03, C47, S03, S47);
+    }
+}
+
 // A work unit is one 2048-sample tile (4 blocks of 512) x the tones of one warp.  SPLIT warps (a team) share a
 // tile, each taking 1/SPLIT of the tones; their partial sums meet in shared memory and are added in rank order.
 // The grid is persistent (two CTAs per SM); teams walk the tiles of the launch with a stride of the team count,
@@ -624,7 +681,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
             const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int t = tb + lane;
-                bool is_static = false, is_mover = false, is_post = false;
+                bool is_static = false, is_mover = false, is_post = false, is_slow = false;
                 uint32_t c0 = 0, c1 = 0, d = 0;
                 const float4 *tabp = nullptr;
                 if (t < t_end) {
@@ -643,6 +700,33 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                             w = u64_of(v2.x, v2.y);
                             tabp = reinterpret_cast<const float4 *>(&tr->rot_post);
                             is_post = true;
+                        } else if ((static_cast<int32_t>(v0.y) & CLS_SLOW_FLAG) && ua >= 0.0 && ub <= f64_of(v3.z, v3.w)) {
+                            // Slow mover, tile wholly inside the move: cubic Taylor expansion of the phase about the tile
+                            // centre (phase and frequency in u64 / fp64, curvature terms in fp32 radians); the record is
+                            // parked in ws.mrec (free during the static pass) until the slow pass of this batch.
+                            is_static = false;
+                            is_slow = true;
+                            const uint4 v4 = ldg16(reinterpret_cast<const char *>(tr) + 64);  // inv_Tn, DT
+                            const uint4 v5 = ldg16(reinterpret_cast<const char *>(tr) + 80);  // q1, q[0], q[1]
+                            const double sc = (ua + static_cast<double>(kTile / 2)) * f64_of(v4.x, v4.y);
+                            const float sf = static_cast<float>(sc);
+                            double g0, g1;
+                            float g2, g3;
+                            if (((static_cast<int32_t>(v0.y) >> 8) & 0xff) == AWG_PROFILE_LINEAR) {
+                                g0 = 0.5 * sc * sc; g1 = sc; g2 = 1.f; g3 = 0.f;
+                            } else {
+                                const double s2 = sc * sc;
+                                g0 = s2 * s2 * (2.5 + sc * (sc - 3.0));
+                                g1 = s2 * sc * (10.0 + sc * (6.0 * sc - 15.0));
+                                g2 = sf * sf * (30.f + sf * (30.f * sf - 60.f));
+                                g3 = sf * (60.f + sf * (120.f * sf - 180.f));
+                            }
+                            const uint64_t nc = static_cast<uint64_t>(tile_base + kTile / 2);
+                            const uint64_t wc = w + frac_to_fix64(f64_of(v5.x, v5.y) * g1);
+                            const uint64_t pc = th + w * nc + frac_to_fix64(f64_of(v4.z, v4.w) * g0);
+                            ws.mrec[lane].q[0] = make_float4(__uint_as_float(round32(pc - (wc >> 1))), __uint_as_float(round32(wc)),
+                                                             __uint_as_float(v5.z) * g2, __uint_as_float(v5.w) * g3);
+                            ws.mrec[lane].q[1] = make_float4(__uint_as_float(v0.x), 0.f, 0.f, 0.f);
                         } else {
                             is_static = false;
                             is_mover = true;
@@ -661,6 +745,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 }
                 const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
                 const unsigned m_sta = __ballot_sync(0xffffffffu, is_static);
+                const unsigned m_slow = __ballot_sync(0xffffffffu, is_slow);
                 if (lane == 0) ws.mov[b] = m_mov;
                 n_mov += __popc(m_mov);
                 const int n_sta = __popc(m_sta);
@@ -707,6 +792,23 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                     const float4 C03 = sp[0].C03, C47 = sp[0].C47, S03 = sp[0].S03, S47 = sp[0].S47;
 #pragma unroll
                     for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
+                }
+                // ---- slow pass: the batch's slow movers, 16 lanes at a time (two staged records per tone: the tone
+                // at the tile-centre frequency, and the first-order correction of its pair tables)
+                if (m_slow != 0u) {
+                    sticky_sta = 0u;           // ws.st is overwritten: a single-batch warp restages its tables next tile
+                    sticky_post = 0xffffffffu;
+#pragma unroll 1
+                    for (int half = 0; half < 2; ++half) {
+                        const unsigned mh = m_slow & (0xffffu << (16 * half));
+                        if (mh == 0u) continue;
+                        __syncwarp();  // the readers of ws.st are done
+                        if (is_slow && (lane >> 4) == half) stage_slow(ws.st + 2 * __popc(mh & lt), ws.mrec[lane]);
+                        __syncwarp();
+                        const int n_slow = __popc(mh);
+#pragma unroll 1
+                        for (int i = 0; i < n_slow; ++i) slow_pair(ws.st[2 * i], ws.st[2 * i + 1], lane, pq);
+                    }
                 }
             }
 #pragma unroll

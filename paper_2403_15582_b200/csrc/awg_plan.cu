@@ -85,6 +85,36 @@ int classify(int profile, long double DT, long double Tn)
     return CLS_DEG6;
 }
 
+// Slow movers (flag CLS_SLOW_FLAG): inside its move the tone changes frequency so slowly that, over a whole
+// 2048-sample tile, the angle-addition engine can carry it with a cubic phase polynomial at each thread's pair centre
+// plus a first-order frequency correction of the pair tables (kernel: slow pass).  Bounds with
+// R = 1024 (half a tile) and h = 7.5 (half a thread's 16 samples), Taylor coefficients C_m = a r^(m-1) sup|g^(m)| / m!
+// in turns per sample^m:
+//   dropped phase terms  C4 R^4 + C5 R^5 + C6 R^6            <= 2e-8 turn
+//   dropped frequency    (4 C4 R^3 + 5 C5 R^4 + 6 C6 R^5) h  <= 2e-8 turn
+//   curvature inside a thread's samples (C2 + 3 C3 R + 6 C4 R^2) h^2 <= 2e-7 turn
+//   second order of the table correction  (2 pi h (2 C2 R + 3 C3 R^2))^2 / 2 <= 2e-7
+//   fp32 polynomial magnitude  C2 R^2 + C3 R^3 <= 0.25 turn
+bool is_slow_mover(int profile, long double DT, long double Tn)
+{
+    if (!(Tn >= 2.0L * kTile)) return false;
+    const double a = static_cast<double>(fabsl(DT) / Tn), r = static_cast<double>(1.0L / Tn);
+    const double R = kTile / 2, h = 7.5;
+    const bool lin = profile == AWG_PROFILE_LINEAR;
+    const double C2 = a * r * (lin ? 1.0 : 5.7735) / 2.0;
+    const double C3 = lin ? 0.0 : a * r * r * 60.0 / 6.0;
+    const double C4 = lin ? 0.0 : a * r * r * r * 360.0 / 24.0;
+    const double C5 = lin ? 0.0 : a * r * r * r * r * 720.0 / 120.0;
+    const double C6 = lin ? 0.0 : a * r * r * r * r * r;
+    const double R2 = R * R, R3 = R2 * R, R4 = R3 * R, R5 = R4 * R, R6 = R5 * R;
+    if (C4 * R4 + C5 * R5 + C6 * R6 > 2e-8) return false;
+    if ((4.0 * C4 * R3 + 5.0 * C5 * R4 + 6.0 * C6 * R5) * h > 2e-8) return false;
+    if ((C2 + 3.0 * C3 * R + 6.0 * C4 * R2) * h * h > 2e-7) return false;
+    const double x = 6.283185307179586 * h * (2.0 * C2 * R + 3.0 * C3 * R2);
+    if (0.5 * x * x > 2e-7) return false;
+    return C2 * R2 + C3 * R3 <= 0.25;
+}
+
 // Table of a carrier for the angle-addition engine (RotTable, awg_internal.h): A cos, A sin of (j + 1/2) w for the
 // symmetric sample pairs, and cos, sin of kBlock*w for the block-to-block rotation.  Angles come from the 64-bit
 // fixed-point frequency in long double (the products stay below 2^10 turns: rounding <= 2^-54 turn), the
@@ -149,6 +179,7 @@ void make_move(HostTone &h, long double fs, long double f1, int profile, long do
     //                     = [theta - (f1-f0) t_s - DT/2] + (f1/fs) n
     h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(h.DT / 2.0L);
     h.cls = classify(profile, h.DT, h.Tn);
+    if (h.cls != CLS_EXACT && is_slow_mover(profile, h.DT, h.Tn)) h.cls |= CLS_SLOW_FLAG;
     make_rot(h.rot_pre, h.w_pre, h.A);
     make_rot(h.rot_post, h.w_post, h.A);
 }
@@ -316,7 +347,7 @@ awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int
     for (int i = 0; i < n_upd; ++i) {
         HostTone &h = p->tones[tone_idx[i]];
         // state of the old segment at n_u: instantaneous frequency and a carrier that continues its phase
-        if (h.cls != CLS_STATIC) {
+        if ((h.cls & 0xff) != CLS_STATIC) {
             const long double u = static_cast<long double>(n_u - h.ns_int) - static_cast<long double>(h.ns_frac);
             if (u <= 0.0L) {
                 // move had not started: keep the pre-move carrier
