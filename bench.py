@@ -13,7 +13,7 @@ buffer.  Metric: tone-samples/s (G).  Rank 0 prints ONE JSON line.
   e2e        the same workload through the C ABI with HOST buffers: awg_set_trajectories from host arrays
              (H2D table upload) + awg_synthesize_range_host into pinned host memory (D2H of the int16 codes)
   roofline   ALU-bound ("bound": "alu"): a tone-sample needs one fp32 multiply-add where its tone is static (angle
-             addition) and one MUFU.SIN + two multiply-adds inside a move; the pipe (FMA: 128/clk/SM, XU: 16/clk/SM,
+             addition), two inside a slow move, one MUFU.SIN + two multiply-adds inside any other move; the pipe (FMA: 128/clk/SM, XU: 16/clk/SM,
              x 148 SMs x sm_max_mhz) whose roofline time is larger binds; frac = that time / measured launch time
   cpu_baseline  the oracle (oracle/awg_oracle_c.c, as it stands) on this box's host cores, bounded sample
   extras     the other configs (C1, C3, C4 ring, C5 sweep) and the real-time capacity search
@@ -189,30 +189,61 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def moving_tone_samples(w) -> int:
-    """Tone-samples of workload w that fall inside a move (sample granularity; initial trajectory table only)."""
+def is_slow_mover(profile: int, DT: float, Tn: float) -> bool:
+    """Mirror of is_slow_mover() in csrc/awg_plan.cu (same bounds): a tone whose move the angle-addition engine can carry
+    on the FMA pipe (cubic phase polynomial per thread + first-order table correction)."""
+    if not Tn >= 2.0 * 2048:
+        return False
+    a, r, R, h = abs(DT) / Tn, 1.0 / Tn, 1024.0, 7.5
+    lin = profile == W.PROFILE_LINEAR
+    C2 = a * r * (1.0 if lin else 5.7735) / 2.0
+    C3 = 0.0 if lin else a * r ** 2 * 60.0 / 6.0
+    C4 = 0.0 if lin else a * r ** 3 * 360.0 / 24.0
+    C5 = 0.0 if lin else a * r ** 4 * 720.0 / 120.0
+    C6 = 0.0 if lin else a * r ** 5
+    if C4 * R ** 4 + C5 * R ** 5 + C6 * R ** 6 > 2e-8:
+        return False
+    if (4 * C4 * R ** 3 + 5 * C5 * R ** 4 + 6 * C6 * R ** 5) * h > 2e-8:
+        return False
+    if (C2 + 3 * C3 * R + 6 * C4 * R ** 2) * h * h > 2e-7:
+        return False
+    x = 6.283185307179586 * h * (2 * C2 * R + 3 * C3 * R ** 2)
+    return 0.5 * x * x <= 2e-7 and C2 * R ** 2 + C3 * R ** 3 <= 0.25
+
+
+def moving_tone_samples(w, split: bool = False):
+    """Tone-samples of workload w that fall inside a move (sample granularity; initial trajectory table only).
+    split=True returns (fast, slow): slow movers (is_slow_mover) need no MUFU.SIN per sample."""
     fs = float(w.sample_rate)
-    total = 0
+    fast = slow = 0
     for k in range(w.n_tones):
         if int(w.profile[k]) == W.PROFILE_STATIC or float(w.f1[k]) == float(w.f0[k]) or float(w.t_dur[k]) <= 0.0:
             continue
         a = max(0.0, float(w.t_start[k]) * fs)
         b = min(float(w.n_samples), (float(w.t_start[k]) + float(w.t_dur[k])) * fs)
         if b > a:
-            total += int(b - a)
-    return total
+            DT = (float(w.f1[k]) - float(w.f0[k])) * float(w.t_dur[k])
+            if is_slow_mover(int(w.profile[k]), DT, float(w.t_dur[k]) * fs):
+                slow += int(b - a)
+            else:
+                fast += int(b - a)
+    return (fast, slow) if split else fast + slow
 
 
 def pipe_roofline(w, ms, engine, sm_mhz):
     """Binding ALU roofline of one launch over workload w.
 
     Algorithmic work: a tone-sample of a tone that is static there needs ONE fp32 multiply-add (angle addition over a
-    symmetric sample pair); a tone-sample inside a move needs one MUFU.SIN plus two multiply-adds (range multiply,
-    amplitude accumulate).  With --engine mufu every tone-sample takes the MUFU path.  The roofline time is the larger
-    of (multiply-adds / FMA-pipe peak) and (sines / XU-pipe peak) at sm_mhz; frac = that time / the measured time."""
-    n_mov = w.tone_samples if engine == "mufu" else moving_tone_samples(w)
-    n_sta = w.tone_samples - n_mov
-    fma_ops, xu_ops = n_sta + 2 * n_mov, n_mov
+    symmetric sample pair); inside a slow move TWO multiply-adds (the second is the first-order frequency correction);
+    inside any other move one MUFU.SIN plus two multiply-adds (range multiply, amplitude accumulate).  With
+    --engine mufu every tone-sample takes the MUFU path.  The roofline time is the larger of (multiply-adds / FMA-pipe
+    peak) and (sines / XU-pipe peak) at sm_mhz; frac = that time / the measured time."""
+    if engine == "mufu":
+        n_fast, n_slow = w.tone_samples, 0
+    else:
+        n_fast, n_slow = moving_tone_samples(w, split=True)
+    n_sta = w.tone_samples - n_fast - n_slow
+    fma_ops, xu_ops = n_sta + 2 * n_slow + 2 * n_fast, n_fast
     peak_fma = FMA_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
     peak_xu = MUFU_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
     t_fma, t_xu = fma_ops / peak_fma, xu_ops / peak_xu
@@ -222,8 +253,9 @@ def pipe_roofline(w, ms, engine, sm_mhz):
     else:
         pipe, ops, peak, unit = "XU (MUFU.SIN)", xu_ops, peak_xu, "Gsin/s"
     return {"bound": "alu", "pipe": pipe, "achieved": ops / t / 1e9, "peak": peak / 1e9, "unit": unit,
-            "frac": max(t_fma, t_xu) / t, "static_tone_samples": int(n_sta), "moving_tone_samples": int(n_mov),
-            "fma_ops": int(fma_ops), "mufu_ops": int(xu_ops), "t_fma_us": t_fma * 1e6, "t_xu_us": t_xu * 1e6}
+            "frac": max(t_fma, t_xu) / t, "static_tone_samples": int(n_sta), "moving_tone_samples": int(n_fast + n_slow),
+            "slow_moving_tone_samples": int(n_slow), "fma_ops": int(fma_ops), "mufu_ops": int(xu_ops),
+            "t_fma_us": t_fma * 1e6, "t_xu_us": t_xu * 1e6}
 
 
 ENGINES = {"auto": lambda awg: awg.AWG_ENGINE_AUTO, "fma": lambda awg: awg.AWG_ENGINE_FMA,

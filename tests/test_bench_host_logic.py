@@ -1,6 +1,6 @@
 """Host-side arithmetic of bench.py's roofline accounting (no GPU): which pipe binds, how the algorithmic
-operations are counted (DESIGN.md section 6 "Roofline": 1 multiply-add per static tone-sample, 1 MUFU.SIN +
-2 multiply-adds per moving tone-sample), and that frac = roofline time / measured time."""
+operations are counted (DESIGN.md section 6 "Roofline": 1 multiply-add per static tone-sample, 2 inside a slow
+move, 1 MUFU.SIN + 2 multiply-adds inside any other move), and that frac = roofline time / measured time."""
 import os
 import sys
 
@@ -47,7 +47,14 @@ def test_pipe_roofline_picks_the_binding_pipe_and_scales_with_time():
     rm = bench.pipe_roofline(w2, 0.2, "mufu", sm_mhz)
     assert rm["pipe"].startswith("XU") and rm["mufu_ops"] == w2.tone_samples
     assert np.isclose(rm["frac"], (w2.tone_samples / xu_peak) / 0.2e-3)
-    # C3: all tones moving for 35 ms of a 35.6 ms buffer: XU binds under the default engine too
+    # C3: every tone is a slow mover (10 MHz over 35 ms): two multiply-adds per moving tone-sample, no sine per sample
     w3 = W.config3()
-    r3 = bench.pipe_roofline(w3, 5.5, "auto", sm_mhz)
-    assert r3["pipe"].startswith("XU") and 0.7 < r3["frac"] < 0.8
+    fast, slow = bench.moving_tone_samples(w3, split=True)
+    assert fast == 0 and slow == w3.n_tones * int(35e-3 * 560e6)
+    r3 = bench.pipe_roofline(w3, 2.25, "auto", sm_mhz)
+    assert r3["pipe"].startswith("FMA") and r3["mufu_ops"] == 0
+    assert np.isclose(r3["frac"], ((w3.tone_samples - slow) + 2 * slow) / fma_peak / 2.25e-3)
+    # the fast moves of C2 (0.5-5 MHz in 50-500 us) are not slow movers
+    assert bench.moving_tone_samples(w2, split=True)[1] == 0
+    assert not bench.is_slow_mover(W.PROFILE_MINJERK, 5e6 * 200e-6, 200e-6 * 560e6)
+    assert bench.is_slow_mover(W.PROFILE_MINJERK, 10e6 * 35e-3, 35e-3 * 560e6)

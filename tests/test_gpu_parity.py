@@ -298,6 +298,33 @@ def test_plan_limit_65536_tones(awg, torch_cuda, eng):
     p.close()
 
 
+def test_slow_movers_at_the_class_boundary(awg, torch_cuda):
+    """Slow pass of the angle-addition engine (moves carried on the FMA pipe: cubic phase polynomial per thread +
+    first-order correction of the pair tables).  Sixteen tones sit at ~90 % of the bounds of is_slow_mover()
+    (csrc/awg_plan.cu): LINEAR +-10 MHz and MINJERK +-1.75 MHz over 5 ms at 560 MS/s, sum of amplitudes 1.  Chunks at
+    the start and end of the move (those tiles take the MUFU path), at the largest curvature of the minimum-jerk ramp
+    (s = 0.21, 0.79) and in the middle; the fp32 sum must stay within 1e-5 of full scale, the codes within the bar."""
+    fs, T, cl, N = 560e6, 5e-3, 1 << 14, 16
+    rng = np.random.default_rng(11)
+    f0 = rng.uniform(60e6, 200e6, N)
+    rows = []
+    for k in range(N):
+        sign = 1.0 if k % 2 == 0 else -1.0
+        if k < 8:
+            rows.append((f0[k], f0[k] + sign * 10e6, 1.0 / N, rng.uniform(0, 6.28), 0.0, T, LINEAR))
+        else:
+            rows.append((f0[k], f0[k] + sign * 1.75e6, 1.0 / N, rng.uniform(0, 6.28), 0.0, T, MINJERK))
+    p, op = _single(awg, fs, cl, rows, engine=awg.AWG_ENGINE_FMA)
+    last = int(T * fs) // cl
+    worst = 0.0
+    for c in (0, 1, 35, 36, 85, 134, 135, last - 1, last, last + 1):
+        V = oracle.c_waveform(op, c * cl, (c + 1) * cl)
+        worst = max(worst, assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"slow movers, chunk {c}"))
+        assert_codes_close(_np(p.synthesize_chunk(c)), op.quantise(V), f"slow movers, chunk {c}")
+    print(f"slow movers: f32 max err {worst:.2e} of full scale")
+    p.close()
+
+
 def test_special_moves(awg, torch_cuda, eng):
     fs = 560e6
     rows = [
