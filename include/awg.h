@@ -64,7 +64,8 @@ enum {
     AWG_ENGINE_FP64 = 2, /* reference-grade: closed form and sine in fp64 per (tone, sample); ~50x slower   */
     AWG_ENGINE_FMA = 3   /* angle addition on the FMA pipe for 2048-sample tiles where a tone is static (one
                             sin + one cos per thread, tone and 16 samples, then ONE multiply-add per
-                            tone-sample with a per-tone table); tiles inside a move use the MUFU path      */
+                            tone-sample with a per-tone table); tiles inside a slow move take two
+                            multiply-adds per tone-sample, tiles inside any other move the MUFU path      */
 };
 
 /* ---- plan ---------------------------------------------------------------------------------- */
