@@ -9,7 +9,9 @@
 //       block), then per symmetric sample pair centre +- (j + 1/2)
 //           A sin(phi +- (j+1/2) w) = sin(phi) [A cos((j+1/2) w)]  +-  cos(phi) [A sin((j+1/2) w)]
 //       i.e. ONE fp32 multiply-add per tone-sample into the even/odd accumulators P_j, Q_j    sincos_tile(), pq_add()
-//       Blocks in which a tone moves (and every tone-sample of the MUFU engine): one MUFU.SIN each   mufu_rec<KIND>()
+//       Tiles wholly inside a SLOW move: the same with a cubic phase polynomial per thread and a first-order
+//       frequency correction of the pair tables: TWO multiply-adds per tone-sample              stage_slow(), slow_pair()
+//       Blocks in which a tone moves otherwise (and every tone-sample of the MUFU engine): one MUFU.SIN each   mufu_rec<KIND>()
 //   a4  fp32 register accumulation over tones: 4 blocks x 16 samples per thread (static pass), 16 (MUFU pass)
 //   a5  quantise: cvt.rni.sat.s16.f32(scale * acc)                                           store_block()
 //   a6  two 16-byte stores of 8 consecutive int16 per thread and block                       store_block()
