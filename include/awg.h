@@ -26,7 +26,9 @@
  *  - A plan is not thread-safe; distinct plans are independent.
  *  - Output for (plan, chunk_idx) is a pure function of the trajectory table and of the absolute
  *    sample index; it does not depend on the stream, ring depth, call order or chunk_len
- *    (kernel tiles are anchored to absolute sample indices that are multiples of 256).
+ *    (kernel tiles are anchored to absolute sample indices that are multiples of 4096).
+ *  - A plan belongs to the CUDA device that was current when it was created; calls that enqueue
+ *    work return AWG_ERR_STATE when another device is current.
  */
 #ifndef AWG_H_
 #define AWG_H_
@@ -62,8 +64,8 @@ enum {
     AWG_ENGINE_AUTO = 0, /* the library picks (currently AWG_ENGINE_FMA)                                    */
     AWG_ENGINE_MUFU = 1, /* one MUFU.SIN per (tone, sample); phase re-centred per 512-sample block           */
     AWG_ENGINE_FP64 = 2, /* reference-grade: closed form and sine in fp64 per (tone, sample); ~50x slower   */
-    AWG_ENGINE_FMA = 3   /* angle addition on the FMA pipe for 2048-sample tiles where a tone is static (one
-                            sin + one cos per thread, tone and 16 samples, then ONE multiply-add per
+    AWG_ENGINE_FMA = 3   /* angle addition on the FMA pipe for 4096-sample tiles where a tone is static (one
+                            sin + one cos per thread, tone and 32 samples, then ONE multiply-add per
                             tone-sample with a per-tone table); tiles inside a slow move take two
                             multiply-adds per tone-sample, tiles inside any other move the MUFU path      */
 };
@@ -125,10 +127,10 @@ awg_status awg_synthesize_chunk_f32(awg_plan *p, int64_t chunk_idx, float *dev_o
 awg_status awg_synthesize_range(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *dev_out,
                                 void *stream);
 
-/* End-to-end variant with a HOST destination: synthesises the range chunk by chunk into internal
- * device slots and copies each chunk to host_out (n_chunks*chunk_len int16; pinned memory gives
- * overlap of copy and compute, pageable memory works) -- synchronous, returns when host_out is
- * complete.  Stands in for the paper's pinned-buffer -> DAC transfer. */
+/* End-to-end variant with a HOST destination: synthesises the range in pieces of 2^21 samples into
+ * two internal device slots and copies each piece to host_out (n_chunks*chunk_len int16; pinned
+ * memory gives overlap of copy and compute, pageable memory works) -- synchronous, returns when
+ * host_out is complete.  Stands in for the paper's pinned-buffer -> DAC transfer. */
 awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *host_out);
 
 /* ---- streaming ring (DAC-FIFO stand-in; Fig. 2b, 75, 127) --------------------------- */
@@ -163,6 +165,15 @@ awg_status awg_ring_destroy(awg_ring *r);
 /* Bytes this plan has copied host->device (trajectory table uploads) and device->host (host-destination
  * synthesis and ring mirror) since creation.  Either pointer may be NULL. */
 awg_status awg_plan_io_bytes(awg_plan *p, int64_t *h2d_bytes, int64_t *d2h_bytes);
+
+/* Algorithmic operation counts of the CURRENT trajectory table over chunks first_chunk ..
+ * first_chunk+n_chunks-1, at sample granularity: tone-samples of tones that are static there
+ * (one fp32 multiply-add each on the angle-addition engine), inside a slow move (two multiply-adds:
+ * the kernel's slow pass) and inside any other move (one MUFU.SIN + two multiply-adds).  This is the
+ * library's own classification (the one the kernel acts on); bench.py derives its roofline from it.
+ * Host-only, no CUDA work.  Any pointer may be NULL.  Errors: INVALID_ARG, STATE (no table set). */
+awg_status awg_plan_op_counts(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int64_t *static_ts,
+                              int64_t *slow_ts, int64_t *fast_ts);
 
 /* Number of kernels the library has launched since load (all plans); for launch accounting. */
 int64_t awg_kernel_launch_count(void);

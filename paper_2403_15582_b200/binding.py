@@ -37,7 +37,8 @@ EXPORTED = (
     "awg_plan_create", "awg_plan_destroy", "awg_set_scale", "awg_set_engine", "awg_set_trajectories",
     "awg_update_trajectories", "awg_synthesize_chunk", "awg_synthesize_chunk_f32", "awg_synthesize_range",
     "awg_synthesize_range_host", "awg_ring_create", "awg_ring_submit", "awg_ring_acquire", "awg_ring_release",
-    "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_kernel_launch_count", "awg_last_error",
+    "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_plan_op_counts", "awg_kernel_launch_count",
+    "awg_last_error",
 )
 
 
@@ -66,6 +67,7 @@ def _load() -> ctypes.CDLL:
         "awg_ring_stats": (I32, [P, POINTER(I64), POINTER(I64), POINTER(D)]),
         "awg_ring_destroy": (I32, [P]),
         "awg_plan_io_bytes": (I32, [P, POINTER(I64), POINTER(I64)]),
+        "awg_plan_op_counts": (I32, [P, I64, I64, POINTER(I64), POINTER(I64), POINTER(I64)]),
         "awg_kernel_launch_count": (I64, []),
         "awg_last_error": (c_char_p, []),
     }
@@ -211,6 +213,13 @@ def awg_plan_io_bytes(plan) -> Tuple[int, int]:
     return a.value, b.value
 
 
+def awg_plan_op_counts(plan, first_chunk: int, n_chunks: int) -> Tuple[int, int, int]:
+    """-> (static, slow-moving, fast-moving) tone-samples of the current table over the chunk range."""
+    a, b, c = c_int64(), c_int64(), c_int64()
+    _check(_lib.awg_plan_op_counts(plan, first_chunk, n_chunks, byref(a), byref(b), byref(c)))
+    return a.value, b.value, c.value
+
+
 def awg_kernel_launch_count() -> int:
     return int(_lib.awg_kernel_launch_count())
 
@@ -289,6 +298,9 @@ class Plan:
 
     def io_bytes(self) -> Tuple[int, int]:
         return awg_plan_io_bytes(self._h)
+
+    def op_counts(self, first_chunk: int, n_chunks: int) -> Tuple[int, int, int]:
+        return awg_plan_op_counts(self._h, first_chunk, n_chunks)
 
     def close(self) -> None:
         if self._h is not None:

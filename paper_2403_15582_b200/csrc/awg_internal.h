@@ -8,50 +8,55 @@
 
 namespace awg {
 
-// Tone classes: how the in-tile phase polynomial of a MOVING tile is evaluated (hot-path step a2).
+// Tone classes: how the in-block phase polynomial of a MOVING block is evaluated (hot-path step a2).
 // Chosen per tone on the host from worst-case bounds on the dropped Taylor terms.
 enum : int32_t {
     CLS_STATIC = 0,  // never moves (profile STATIC or f1 == f0): carrier only
-    CLS_QUAD = 2,    // moving tiles need the k^2 term only (LINEAR always; slow MINJERK)
+    CLS_QUAD = 2,    // moving blocks need the k^2 term only (LINEAR always; slow MINJERK)
     CLS_DEG4 = 4,    // k^2..k^4
     CLS_DEG6 = 6,    // k^2..k^6 (exact Taylor series of the degree-6 min-jerk phase)
-    CLS_EXACT = 7,   // fp32 in-tile polynomial not accurate enough: moving tiles use the fp64 path
+    CLS_EXACT = 7,   // fp32 in-block polynomial not accurate enough: moving blocks use the fp64 path
     CLS_SLOW_FLAG = 1 << 16  // OR-ed into ToneRec::cls: tiles wholly inside the move may take the slow pass (FMA pipe)
 };
 
-// Kernel geometry.  A thread owns kSPT consecutive samples of a block; a block is 32 lanes x kSPT = 512 samples
-// (the span of one phase re-centring); a warp tile is kBlocksPerTile consecutive blocks, anchored at absolute
-// sample indices that are multiples of kTile.
-constexpr int kSPT = 16;
+// Kernel geometry.
+//  * A TILE is kTile = 4096 consecutive samples anchored at an absolute multiple of kTile.
+//  * Angle-addition passes (static / slow): a thread owns kSPT = 32 consecutive samples of a kBlock = 1024-sample
+//    block, as kPairs = 16 symmetric pairs centre +- (j + 1/2); a tile is kBlocksPerTile = 4 such blocks.
+//  * MUFU pass: a thread owns kMovSPT = 16 consecutive samples of a kMovBlock = 512-sample block (the span of one
+//    phase re-centring); a tile is kMovBlocksPerTile = 8 such blocks.
+constexpr int kSPT = 32;
 constexpr int kBlock = 32 * kSPT;
 constexpr int kBlocksPerTile = 4;
 constexpr int kTile = kBlocksPerTile * kBlock;
-constexpr int kPairs = kSPT / 2;  // symmetric sample pairs per thread: centre +- (j + 1/2), j = 0..kPairs-1
+constexpr int kPairs = kSPT / 2;
+constexpr int kMovSPT = 16;
+constexpr int kMovBlock = 32 * kMovSPT;
+constexpr int kMovBlocksPerTile = kTile / kMovBlock;
+constexpr int kMovPairs = kMovSPT / 2;
 
-// Carrier table of the angle-addition engine (hot-path step a3, static tiles): with phi the carrier phase at the
-// half-integer centre of a thread's 16 samples, the samples at centre +- (j + 1/2) are
+// Carrier table of the angle-addition engine (hot-path step a3): with phi the carrier phase at the half-integer
+// centre of a thread's 32 samples, the samples at centre +- (j + 1/2) are
 //     A sin(phi +- (j+1/2) w) = sin(phi) * [A cos((j+1/2) w)]  +-  cos(phi) * [A sin((j+1/2) w)]
-// so ONE multiply-add per tone-sample accumulates the even part P_j and the odd part Q_j; the next block of the
-// tile is reached by rotating (sin phi, cos phi) by kBlock*w.
-struct __align__(16) RotTable {
-    float C[kPairs];    // A cos(2 pi (j + 1/2) w)
-    float S[kPairs];    // A sin(2 pi (j + 1/2) w)
-    float cr, sr;       // cos, sin of 2 pi kBlock w
-    float pad_[2];
+// so ONE multiply-add per tone-sample accumulates the even part P_j and the odd part Q_j.  The table is stored as
+// the pairs (C_j, S_j) = (A cos, A sin)(2 pi (j + 1/2) w): one packed FFMA2 (sin phi, cos phi) x (C_j, S_j) updates
+// (P_j, Q_j).  Built on the device (awg_expand_kernel) from the 64-bit fixed-point frequency.
+struct __align__(16) PairTable {
+    float2 cs[kPairs];
 };
-static_assert(sizeof(RotTable) == 80, "RotTable must be 80 bytes");
+static_assert(sizeof(PairTable) == 128, "PairTable must be 128 bytes");
 
-// Device trajectory table (hot-path step a0): one 288-byte record per tone, read by one lane per
-// (tone, tile) with 16-byte loads.  Phases are in TURNS as unsigned 64-bit fixed point (1 turn = 2^64), so
-// the carrier phase theta + w*n wraps exactly mod 1 for any n: the range reduction of Eq. 14
-// done in integer arithmetic.  With u = (n - ns_int) - ns_frac the real number of samples since the move began:
+// What the host uploads per tone (hot-path step a0): carriers, move window, move polynomial.  Phases are in TURNS as
+// unsigned 64-bit fixed point (1 turn = 2^64), so the carrier phase theta + w*n wraps exactly mod 1 for any n: the
+// range reduction of Eq. 14 done in integer arithmetic.  With u = (n - ns_int) - ns_frac the real
+// number of samples since the move began:
 //   before the move   (u <= 0):      phase = theta_pre  + w_pre *n
 //   during the move (0 < u < Tn):    phase = theta_pre  + w_pre *n + DT*g(u/Tn)    g = s^2/2 or 5/2 s^4 - 3 s^5 + s^6
 //   after the move    (u >= Tn):     phase = theta_post + w_post*n
-struct __align__(16) ToneRec {
+struct __align__(16) ToneCore {
     // ---- 64 bytes: carriers and move window
     float A;               // amplitude
-    int32_t cls;           // (profile << 8) | CLS_*
+    int32_t cls;           // (profile << 8) | CLS_* [| CLS_SLOW_FLAG]
     uint64_t theta_pre;    // turns * 2^64
     uint64_t w_pre;        // frac(f0/fs) * 2^64
     uint64_t theta_post;
@@ -65,11 +70,16 @@ struct __align__(16) ToneRec {
     double q1;             // DT/Tn = (f1-f0)/fs, cycles per sample
     float q[5];            // q[k-2] = 2*pi*DT/Tn^k/k!, k = 2..6: radians per sample^k for unit g^(k)
     float pad_[5];
-    // ---- 2 x 80 bytes: tables of the two carriers for the angle-addition engine
-    RotTable rot_pre;
-    RotTable rot_post;
 };
-static_assert(sizeof(ToneRec) == 288, "ToneRec must be 288 bytes");
+static_assert(sizeof(ToneCore) == 128, "ToneCore must be 128 bytes");
+
+// Device trajectory table: one 384-byte record per tone (core + the pair tables of the two carriers).
+struct __align__(16) ToneRec {
+    ToneCore core;
+    PairTable tab_pre;
+    PairTable tab_post;
+};
+static_assert(sizeof(ToneRec) == 384, "ToneRec must be 384 bytes");
 
 struct LaunchParams {
     const ToneRec *tab;
@@ -82,9 +92,14 @@ struct LaunchParams {
     uint32_t *sched;   // {next tile, teams finished}: the launch's tile-scheduler slot (filled in by launch_synth)
 };
 
+// Warps of a team share a tile, each taking 1/split of the tones.  A function of the tone count ONLY, never of the
+// launch size: the order in which tone partial sums are added is then the same for every chunking (bit-identical
+// output across chunk sizes, include/awg.h "pure function").
+int split_for(int n_tones);
+
 cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream);
-// table[idx[j]] = src[j] for j < n (partial trajectory-table update)
-cudaError_t launch_scatter(ToneRec *table, const ToneRec *src, const int32_t *idx, int n, cudaStream_t stream);
+// table[idx ? idx[j] : j] = expand(src[j]) for j < n: copies the core and builds both pair tables (fp64 sincospi)
+cudaError_t launch_expand(ToneRec *table, const ToneCore *src, const int32_t *idx, int n, cudaStream_t stream);
 void count_launch();
 
 }  // namespace awg

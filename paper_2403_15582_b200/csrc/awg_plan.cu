@@ -1,7 +1,8 @@
 // awg_plan.cu -- host side of the C ABI: plan, trajectory table (hot-path step a0), synthesis entry points.
 //
-// The trajectory table is kept on the host in x87 long double / 64-bit fixed point and mirrored to the
-// device as the structure of arrays of awg_internal.h.  Carrier phases are unsigned 64-bit fixed-point
+// The trajectory table is kept on the host in x87 long double / 64-bit fixed point; the host uploads one 128-byte
+// core per tone (carriers, move window, move polynomial) and a device kernel expands it into the 384-byte record of
+// awg_internal.h (it builds the pair tables of the angle-addition engine).  Carrier phases are unsigned 64-bit fixed-point
 // turns, so theta + w*n is exact mod 1 for any absolute sample index n: this is the modf of Eq. 14
 // done in integers, and it is what keeps 35 ms x 560 MS/s (5.6e6 cycles) and 1 s x
 // 100 MS/s (1e8 cycles) phases at full precision.
@@ -38,7 +39,7 @@ awg_status fail_cuda(cudaError_t e, const char *what)
 namespace {
 
 const long double kTwoPiL = 6.283185307179586476925286766559005768L;
-constexpr int kRadius = kBlock / 2;  // half of the kernel's 512-sample block (span of one Taylor re-centring)
+constexpr int kRadius = kMovBlock / 2;  // half of the MUFU pass's 512-sample block (span of one Taylor re-centring)
 
 // frac(x) as 64-bit fixed-point turns.
 uint64_t frac64(long double x)
@@ -86,59 +87,33 @@ int classify(int profile, long double DT, long double Tn)
 }
 
 // Slow movers (flag CLS_SLOW_FLAG): inside its move the tone changes frequency so slowly that, over a whole
-// 2048-sample tile, the angle-addition engine can carry it with a cubic phase polynomial at each thread's pair centre
+// 4096-sample tile, the angle-addition engine can carry it with a cubic phase polynomial at each thread's pair centre
 // plus a first-order frequency correction of the pair tables (kernel: slow pass).  Bounds with
-// R = 1024 (half a tile) and h = 7.5 (half a thread's 16 samples), Taylor coefficients C_m = a r^(m-1) sup|g^(m)| / m!
-// in turns per sample^m:
+// R = 2048 (half a tile) and h = 15.5 (half a thread's 32 samples), Taylor coefficients C_m = a r^(m-1) sup|g^(m)| / m!
+// in turns per sample^m (sup|g^(m)| on [0,1] for the minimum-jerk g: 1.875, 5.7735, 60, 360, 720 for m = 2..6):
 //   dropped phase terms  C4 R^4 + C5 R^5 + C6 R^6            <= 2e-8 turn
 //   dropped frequency    (4 C4 R^3 + 5 C5 R^4 + 6 C6 R^5) h  <= 2e-8 turn
-//   curvature inside a thread's samples (C2 + 3 C3 R + 6 C4 R^2) h^2 <= 2e-7 turn
+//   curvature inside a thread's samples (C2 + 3 C3 R + 6 C4 R^2) h^2 <= 3e-7 turn
 //   second order of the table correction  (2 pi h (2 C2 R + 3 C3 R^2))^2 / 2 <= 2e-7
 //   fp32 polynomial magnitude  C2 R^2 + C3 R^3 <= 0.25 turn
 bool is_slow_mover(int profile, long double DT, long double Tn)
 {
     if (!(Tn >= 2.0L * kTile)) return false;
     const double a = static_cast<double>(fabsl(DT) / Tn), r = static_cast<double>(1.0L / Tn);
-    const double R = kTile / 2, h = 7.5;
+    const double R = kTile / 2, h = 0.5 * (kSPT - 1);
     const bool lin = profile == AWG_PROFILE_LINEAR;
-    const double C2 = a * r * (lin ? 1.0 : 5.7735) / 2.0;
-    const double C3 = lin ? 0.0 : a * r * r * 60.0 / 6.0;
-    const double C4 = lin ? 0.0 : a * r * r * r * 360.0 / 24.0;
-    const double C5 = lin ? 0.0 : a * r * r * r * r * 720.0 / 120.0;
+    const double C2 = a * r * (lin ? 1.0 : 1.875) / 2.0;
+    const double C3 = lin ? 0.0 : a * r * r * 5.7735 / 6.0;
+    const double C4 = lin ? 0.0 : a * r * r * r * 60.0 / 24.0;
+    const double C5 = lin ? 0.0 : a * r * r * r * r * 360.0 / 120.0;
     const double C6 = lin ? 0.0 : a * r * r * r * r * r;
     const double R2 = R * R, R3 = R2 * R, R4 = R3 * R, R5 = R4 * R, R6 = R5 * R;
     if (C4 * R4 + C5 * R5 + C6 * R6 > 2e-8) return false;
     if ((4.0 * C4 * R3 + 5.0 * C5 * R4 + 6.0 * C6 * R5) * h > 2e-8) return false;
-    if ((C2 + 3.0 * C3 * R + 6.0 * C4 * R2) * h * h > 2e-7) return false;
+    if ((C2 + 3.0 * C3 * R + 6.0 * C4 * R2) * h * h > 3e-7) return false;
     const double x = 6.283185307179586 * h * (2.0 * C2 * R + 3.0 * C3 * R2);
     if (0.5 * x * x > 2e-7) return false;
     return C2 * R2 + C3 * R3 <= 0.25;
-}
-
-// Table of a carrier for the angle-addition engine (RotTable, awg_internal.h): A cos, A sin of (j + 1/2) w for the
-// symmetric sample pairs, and cos, sin of kBlock*w for the block-to-block rotation.  Angles come from the 64-bit
-// fixed-point frequency in long double (the products stay below 2^10 turns: rounding <= 2^-54 turn), the
-// trigonometric functions are evaluated in double and rounded once to fp32.
-void make_rot(RotTable &rot, uint64_t w, float A)
-{
-    const long double wl = ldexpl(static_cast<long double>(w), -64);  // turns per sample, exact
-    const double two_pi = 6.283185307179586476925286766559;
-    auto angle = [&](long double mult) {
-        long double t = mult * wl;
-        t -= floorl(t + 0.5L);  // [-1/2, 1/2) turn
-        return two_pi * static_cast<double>(t);
-    };
-    std::memset(&rot, 0, sizeof rot);
-    for (int j = 0; j < kPairs; ++j) {
-        double sn, cs;
-        sincos(angle(static_cast<long double>(j) + 0.5L), &sn, &cs);
-        rot.C[j] = static_cast<float>(static_cast<double>(A) * cs);
-        rot.S[j] = static_cast<float>(static_cast<double>(A) * sn);
-    }
-    double sn, cs;
-    sincos(angle(static_cast<long double>(kBlock)), &sn, &cs);
-    rot.cr = static_cast<float>(cs);
-    rot.sr = static_cast<float>(sn);
 }
 
 void make_static(HostTone &h)
@@ -153,8 +128,6 @@ void make_static(HostTone &h)
     h.DT = 0.0L;
     h.theta_post = h.theta_pre;
     h.w_post = h.w_pre;
-    make_rot(h.rot_pre, h.w_pre, h.A);
-    h.rot_post = h.rot_pre;
 }
 
 // Fills the move part of h (everything but theta_pre/w_pre/f0/A) for a move f0 -> f1 that starts at the
@@ -180,8 +153,6 @@ void make_move(HostTone &h, long double fs, long double f1, int profile, long do
     h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(h.DT / 2.0L);
     h.cls = classify(profile, h.DT, h.Tn);
     if (h.cls != CLS_EXACT && is_slow_mover(profile, h.DT, h.Tn)) h.cls |= CLS_SLOW_FLAG;
-    make_rot(h.rot_pre, h.w_pre, h.A);
-    make_rot(h.rot_post, h.w_post, h.A);
 }
 
 long double profile_h(int profile, long double s)  // frequency ramp 0 -> 1
@@ -200,7 +171,7 @@ long double profile_g(int profile, long double s)  // its integral
 
 // ---- device table versions ---------------------------------------------------------------------
 
-static void fill_record(const HostTone &h, ToneRec &r)
+static void fill_core(const HostTone &h, ToneCore &r)
 {
     std::memset(&r, 0, sizeof r);
     r.A = h.A;
@@ -224,15 +195,13 @@ static void fill_record(const HostTone &h, ToneRec &r)
             r.q[k - 2] = static_cast<float>(q / fact);
         }
     }
-    r.rot_pre = h.rot_pre;
-    r.rot_post = h.rot_post;
 }
 
 // Makes the device table current on `stream`.  A changed table goes to the next of kTableVersions device
-// copies, so kernels still reading the previous version are never disturbed.  After set_trajectories the
-// whole table is uploaded; after per-chunk updates only the changed records travel: the new version is a
-// device-to-device copy of the current one plus a scatter of the updated records (parameters
-// cross the bus only when they change).
+// copies, so kernels still reading the previous version are never disturbed.  The host uploads 128-byte tone cores
+// and the expand kernel builds the records (with their pair tables) on the device.  After set_trajectories every core
+// is uploaded; after per-chunk updates only the changed ones travel: the new version is a device-to-device copy of the
+// current one plus an expand of the updated records (parameters cross the bus only when they change).
 awg_status ensure_table(awg_plan *p, cudaStream_t stream)
 {
     cudaError_t e;
@@ -249,19 +218,22 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
     std::sort(p->dirty_tones.begin(), p->dirty_tones.end());
     p->dirty_tones.erase(std::unique(p->dirty_tones.begin(), p->dirty_tones.end()), p->dirty_tones.end());
     const size_t n_dirty = p->dirty_tones.size();
-    ToneRec *host = reinterpret_cast<ToneRec *>(p->host_table[v]);
-    if (p->dirty_all || n_dirty * 4 > static_cast<size_t>(p->n_tones)) {
+    ToneCore *host = reinterpret_cast<ToneCore *>(p->host_table[v]);
+    ToneRec *table = reinterpret_cast<ToneRec *>(p->dev_table[v]);
+    const ToneCore *stage = reinterpret_cast<const ToneCore *>(p->dev_stage[v]);
+    if (p->dirty_all || n_dirty * 2 > static_cast<size_t>(p->n_tones)) {
         for (int i = 0; i < p->n_pad; ++i) {
-            if (i < p->n_tones) fill_record(p->tones[i], host[i]);
-            else std::memset(&host[i], 0, sizeof(ToneRec));
+            if (i < p->n_tones) fill_core(p->tones[i], host[i]);
+            else std::memset(&host[i], 0, sizeof(ToneCore));
         }
-        if ((e = cudaMemcpyAsync(p->dev_table[v], host, p->table_bytes, cudaMemcpyHostToDevice, stream)) != cudaSuccess)
-            return fail_cuda(e, "cudaMemcpyAsync(table)");
-        p->h2d_bytes += static_cast<int64_t>(p->table_bytes);
+        if ((e = cudaMemcpyAsync(p->dev_stage[v], host, p->core_bytes, cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemcpyAsync(tone cores)");
+        if ((e = launch_expand(table, stage, nullptr, p->n_pad, stream)) != cudaSuccess) return fail_cuda(e, "expand launch");
+        p->h2d_bytes += static_cast<int64_t>(p->core_bytes);
     } else {
-        int32_t *host_idx = reinterpret_cast<int32_t *>(p->host_table[v] + p->table_bytes);
+        int32_t *host_idx = reinterpret_cast<int32_t *>(p->host_table[v] + p->core_bytes);
         for (size_t j = 0; j < n_dirty; ++j) {
-            fill_record(p->tones[p->dirty_tones[j]], host[j]);
+            fill_core(p->tones[p->dirty_tones[j]], host[j]);
             host_idx[j] = p->dirty_tones[j];
         }
         if (p->upload_stream[cur] != stream && (e = cudaStreamWaitEvent(stream, p->uploaded[cur], 0)) != cudaSuccess)
@@ -269,13 +241,13 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
         if ((e = cudaMemcpyAsync(p->dev_table[v], p->dev_table[cur], p->table_bytes, cudaMemcpyDeviceToDevice, stream)) != cudaSuccess)
             return fail_cuda(e, "cudaMemcpyAsync(table d2d)");
         if ((e = cudaEventRecord(p->last_use[cur], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-        if ((e = cudaMemcpyAsync(p->dev_stage[v], host, n_dirty * sizeof(ToneRec), cudaMemcpyHostToDevice, stream)) != cudaSuccess ||
-            (e = cudaMemcpyAsync(p->dev_stage[v] + p->table_bytes, host_idx, n_dirty * sizeof(int32_t), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
-            return fail_cuda(e, "cudaMemcpyAsync(updated records)");
-        if ((e = launch_scatter(reinterpret_cast<ToneRec *>(p->dev_table[v]), reinterpret_cast<const ToneRec *>(p->dev_stage[v]),
-                                reinterpret_cast<const int32_t *>(p->dev_stage[v] + p->table_bytes), static_cast<int>(n_dirty), stream)) != cudaSuccess)
-            return fail_cuda(e, "scatter launch");
-        p->h2d_bytes += static_cast<int64_t>(n_dirty * (sizeof(ToneRec) + sizeof(int32_t)));
+        if ((e = cudaMemcpyAsync(p->dev_stage[v], host, n_dirty * sizeof(ToneCore), cudaMemcpyHostToDevice, stream)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(p->dev_stage[v] + p->core_bytes, host_idx, n_dirty * sizeof(int32_t), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemcpyAsync(updated tone cores)");
+        if ((e = launch_expand(table, stage, reinterpret_cast<const int32_t *>(p->dev_stage[v] + p->core_bytes), static_cast<int>(n_dirty),
+                               stream)) != cudaSuccess)
+            return fail_cuda(e, "expand launch");
+        p->h2d_bytes += static_cast<int64_t>(n_dirty * (sizeof(ToneCore) + sizeof(int32_t)));
     }
     if ((e = cudaEventRecord(p->uploaded[v], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
     p->upload_stream[v] = stream;
@@ -304,10 +276,24 @@ awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, voi
     return AWG_OK;
 }
 
+// A plan lives on the device that was current when it was created; calls that enqueue work must be made with that
+// device current (the library never switches devices behind the caller's back).
+awg_status check_device(const awg_plan *p)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaGetDevice");
+    if (dev != p->device)
+        return fail(AWG_ERR_STATE, "the plan was created on device %d but device %d is current", p->device, dev);
+    return AWG_OK;
+}
+
 awg_status check_chunk_call(awg_plan *p, int64_t first_chunk, int64_t n_chunks, const void *out, size_t align)
 {
     if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
     if (!out) return fail(AWG_ERR_INVALID_ARG, "output pointer is NULL");
+    awg_status dst = check_device(p);
+    if (dst != AWG_OK) return dst;
     if (reinterpret_cast<uintptr_t>(out) % align) return fail(AWG_ERR_INVALID_ARG, "output pointer must be %zu-byte aligned", align);
     if (first_chunk < 0 || n_chunks < 1) return fail(AWG_ERR_INVALID_ARG, "bad chunk range");
     if (first_chunk > (std::numeric_limits<int64_t>::max() / 4) / p->chunk_len - n_chunks)
@@ -406,6 +392,7 @@ awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_h
     p->engine = AWG_ENGINE_FMA;
     p->device = dev;
     p->table_bytes = static_cast<size_t>(p->n_pad) * sizeof(ToneRec);
+    p->core_bytes = static_cast<size_t>(p->n_pad) * sizeof(ToneCore);
     try {
         p->tones.resize(n_tones);
     } catch (...) {
@@ -413,7 +400,7 @@ awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_h
         return fail(AWG_ERR_ALLOC, "out of host memory");
     }
     for (int v = 0; v < kTableVersions; ++v) {
-        const size_t stage_bytes = p->table_bytes + static_cast<size_t>(p->n_pad) * sizeof(int32_t);
+        const size_t stage_bytes = p->core_bytes + static_cast<size_t>(p->n_pad) * sizeof(int32_t);
         if ((e = cudaMalloc(reinterpret_cast<void **>(&p->dev_table[v]), p->table_bytes)) != cudaSuccess ||
             (e = cudaMalloc(reinterpret_cast<void **>(&p->dev_stage[v]), stage_bytes)) != cudaSuccess ||
             (e = cudaMallocHost(reinterpret_cast<void **>(&p->host_table[v]), stage_bytes)) != cudaSuccess ||
@@ -460,6 +447,33 @@ awg_status awg_plan_io_bytes(awg_plan *p, int64_t *h2d_bytes, int64_t *d2h_bytes
     if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
     if (h2d_bytes) *h2d_bytes = p->h2d_bytes;
     if (d2h_bytes) *d2h_bytes = p->d2h_bytes;
+    return AWG_OK;
+}
+
+awg_status awg_plan_op_counts(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int64_t *static_ts, int64_t *slow_ts, int64_t *fast_ts)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (first_chunk < 0 || n_chunks < 0) return fail(AWG_ERR_INVALID_ARG, "bad chunk range");
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    const int64_t n0 = first_chunk * p->chunk_len, n1 = n0 + n_chunks * p->chunk_len;
+    int64_t n_static = 0, n_slow = 0, n_fast = 0;
+    for (const HostTone &h : p->tones) {
+        int64_t moving = 0;
+        if ((h.cls & 0xff) != CLS_STATIC) {
+            // samples n with 0 < u < Tn, u = (n - ns_int) - ns_frac
+            const long double ns = static_cast<long double>(h.ns_int) + static_cast<long double>(h.ns_frac);
+            const int64_t first = static_cast<int64_t>(floorl(ns)) + 1;
+            const int64_t last = static_cast<int64_t>(ceill(ns + h.Tn)) - 1;
+            const int64_t a = first > n0 ? first : n0, b = last < n1 - 1 ? last : n1 - 1;
+            if (b >= a) moving = b - a + 1;
+        }
+        if (h.cls & CLS_SLOW_FLAG) n_slow += moving;
+        else n_fast += moving;
+        n_static += (n1 - n0) - moving;
+    }
+    if (static_ts) *static_ts = n_static;
+    if (slow_ts) *slow_ts = n_slow;
+    if (fast_ts) *fast_ts = n_fast;
     return AWG_OK;
 }
 
@@ -551,17 +565,30 @@ awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n
     awg_status st = check_chunk_call(p, first_chunk, n_chunks, host_out, 2);
     if (st != AWG_OK) return st;
     cudaError_t e;
-    // two device slots; stream 0 synthesises piece i+1 while stream 1 copies piece i to the host
-    constexpr int64_t kPiece = int64_t(1) << 21;  // samples per piece (4 MiB of int16)
-    if (!p->e2e_slot[0]) {
-        for (int s = 0; s < 2; ++s) {
+    // two device slots of 2^21 samples (4 MiB of int16): stream 0 synthesises piece i+1 while stream 1 copies piece i to the host
+    constexpr int64_t kPiece = int64_t(1) << 21;
+    if (!p->e2e_ok) {
+        // both slots or none: a half-built pair is torn down again
+        awg_status bad = AWG_OK;
+        for (int s = 0; s < 2 && bad == AWG_OK; ++s) {
             if ((e = cudaMalloc(reinterpret_cast<void **>(&p->e2e_slot[s]), kPiece * sizeof(int16_t))) != cudaSuccess)
-                return fail(AWG_ERR_ALLOC, "cudaMalloc(e2e slot): %s", cudaGetErrorString(e));
-            if ((e = cudaStreamCreateWithFlags(&p->e2e_stream[s], cudaStreamNonBlocking)) != cudaSuccess ||
-                (e = cudaEventCreateWithFlags(&p->e2e_ready[s], cudaEventDisableTiming)) != cudaSuccess ||
-                (e = cudaEventCreateWithFlags(&p->e2e_done[s], cudaEventDisableTiming)) != cudaSuccess)
-                return fail_cuda(e, "e2e stream/event creation");
+                bad = fail(AWG_ERR_ALLOC, "cudaMalloc(e2e slot): %s", cudaGetErrorString(e));
+            else if ((e = cudaStreamCreateWithFlags(&p->e2e_stream[s], cudaStreamNonBlocking)) != cudaSuccess ||
+                     (e = cudaEventCreateWithFlags(&p->e2e_ready[s], cudaEventDisableTiming)) != cudaSuccess ||
+                     (e = cudaEventCreateWithFlags(&p->e2e_done[s], cudaEventDisableTiming)) != cudaSuccess)
+                bad = fail_cuda(e, "e2e stream/event creation");
         }
+        if (bad != AWG_OK) {
+            for (int s = 0; s < 2; ++s) {
+                if (p->e2e_slot[s]) cudaFree(p->e2e_slot[s]);
+                if (p->e2e_done[s]) cudaEventDestroy(p->e2e_done[s]);
+                if (p->e2e_ready[s]) cudaEventDestroy(p->e2e_ready[s]);
+                if (p->e2e_stream[s]) cudaStreamDestroy(p->e2e_stream[s]);
+                p->e2e_slot[s] = nullptr; p->e2e_done[s] = nullptr; p->e2e_ready[s] = nullptr; p->e2e_stream[s] = nullptr;
+            }
+            return bad;
+        }
+        p->e2e_ok = true;
     }
     const int64_t n0 = first_chunk * p->chunk_len, total = n_chunks * p->chunk_len;
     cudaStream_t s_syn = p->e2e_stream[0], s_cpy = p->e2e_stream[1];

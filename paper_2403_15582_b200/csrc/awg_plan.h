@@ -25,7 +25,6 @@ struct HostTone {
     float A = 0;
     int32_t profile = AWG_PROFILE_STATIC;
     int32_t cls = 0;
-    RotTable rot_pre = {}, rot_post = {};  // angle-addition tables of the two carriers
 };
 
 awg_status fail(awg_status code, const char *fmt, ...);
@@ -49,8 +48,9 @@ struct awg_plan {
     size_t table_bytes = 0;
     int cur_version = 0;
     unsigned char *dev_table[awg::kTableVersions] = {};
-    unsigned char *host_table[awg::kTableVersions] = {};  // pinned staging: records, then int32 indices
-    unsigned char *dev_stage[awg::kTableVersions] = {};   // device staging for partial updates (same layout)
+    size_t core_bytes = 0;                                 // n_pad tone cores (what the host uploads)
+    unsigned char *host_table[awg::kTableVersions] = {};  // pinned staging: tone cores, then int32 indices
+    unsigned char *dev_stage[awg::kTableVersions] = {};   // device staging of the same layout (input of the expand kernel)
     cudaEvent_t last_use[awg::kTableVersions] = {};
     cudaEvent_t uploaded[awg::kTableVersions] = {};
     cudaStream_t upload_stream[awg::kTableVersions] = {};
@@ -58,6 +58,7 @@ struct awg_plan {
     int16_t *e2e_slot[2] = {};
     cudaStream_t e2e_stream[2] = {};
     cudaEvent_t e2e_ready[2] = {}, e2e_done[2] = {};
+    bool e2e_ok = false;                    // both slots, streams and events exist
     // accounting
     int64_t h2d_bytes = 0, d2h_bytes = 0;
     int n_rings = 0;

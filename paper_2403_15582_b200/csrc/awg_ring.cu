@@ -101,9 +101,10 @@ awg_status awg_ring_submit(awg_ring *r, int64_t chunk_idx, int32_t n_upd, const 
     if (chunk_idx <= r->last_chunk) return fail(AWG_ERR_STATE, "chunks must be submitted in increasing order");
     awg_plan *p = r->plan;
     awg_status st;
-    if (n_upd > 0 && (st = apply_update(p, chunk_idx, n_upd, tone_idx, f1, t_dur, profile)) != AWG_OK) return st;
     RingSlot &s = r->slots[r->n_submitted % r->n_slots];
+    // the chunk is validated first: a rejected submit leaves the trajectory table as it was
     if ((st = check_chunk_call(p, chunk_idx, 1, s.dev, 16)) != AWG_OK) return st;
+    if (n_upd > 0 && (st = apply_update(p, chunk_idx, n_upd, tone_idx, f1, t_dur, profile)) != AWG_OK) return st;
     cudaError_t e;
     // table upload (if an update is pending) goes first so that the chunk's device time measures synthesis + mirror
     if ((st = ensure_table(p, r->s_syn)) != AWG_OK) return st;
