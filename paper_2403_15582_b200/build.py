@@ -45,6 +45,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "nvcc")
     tmp = LIB + f".tmp{os.getpid()}"
     cmd = [nvcc] + NVCC_FLAGS + ["-I", INCLUDE, "-I", CSRC, "-o", tmp] + sources()
+    if os.environ.get("AWG_SPT"):  # kernel geometry override (development aid): samples per thread of the angle-addition passes
+        cmd.insert(1, "-DAWG_SPT=" + os.environ["AWG_SPT"])
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd), file=sys.stderr)

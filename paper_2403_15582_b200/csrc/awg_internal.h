@@ -19,32 +19,26 @@ enum : int32_t {
     CLS_SLOW_FLAG = 1 << 16  // OR-ed into ToneRec::cls: tiles wholly inside the move may take the slow pass (FMA pipe)
 };
 
-// Kernel geometry.
-//  * A TILE is kTile = 4096 consecutive samples anchored at an absolute multiple of kTile.
-//  * Angle-addition passes (static / slow): a thread owns kSPT = 32 consecutive samples of a kBlock = 1024-sample
-//    block, as kPairs = 16 symmetric pairs centre +- (j + 1/2); a tile is kBlocksPerTile = 4 such blocks.
-//  * MUFU pass: a thread owns kMovSPT = 16 consecutive samples of a kMovBlock = 512-sample block (the span of one
-//    phase re-centring); a tile is kMovBlocksPerTile = 8 such blocks.
-constexpr int kSPT = 32;
+// Kernel geometry.  A thread owns kSPT consecutive samples of a block; a block is 32 lanes x kSPT = 512 samples
+// (the span of one phase re-centring); a warp tile is kBlocksPerTile consecutive blocks, anchored at absolute
+// sample indices that are multiples of kTile.
+constexpr int kSPT = 16;
 constexpr int kBlock = 32 * kSPT;
 constexpr int kBlocksPerTile = 4;
 constexpr int kTile = kBlocksPerTile * kBlock;
-constexpr int kPairs = kSPT / 2;
-constexpr int kMovSPT = 16;
-constexpr int kMovBlock = 32 * kMovSPT;
-constexpr int kMovBlocksPerTile = kTile / kMovBlock;
-constexpr int kMovPairs = kMovSPT / 2;
+constexpr int kPairs = kSPT / 2;  // symmetric sample pairs per thread: centre +- (j + 1/2), j = 0..kPairs-1
 
-// Carrier table of the angle-addition engine (hot-path step a3): with phi the carrier phase at the half-integer
-// centre of a thread's 32 samples, the samples at centre +- (j + 1/2) are
+// Carrier table of the angle-addition engine (hot-path step a3, static tiles): with phi the carrier phase at the
+// half-integer centre of a thread's 16 samples, the samples at centre +- (j + 1/2) are
 //     A sin(phi +- (j+1/2) w) = sin(phi) * [A cos((j+1/2) w)]  +-  cos(phi) * [A sin((j+1/2) w)]
-// so ONE multiply-add per tone-sample accumulates the even part P_j and the odd part Q_j.  The table is stored as
-// the pairs (C_j, S_j) = (A cos, A sin)(2 pi (j + 1/2) w): one packed FFMA2 (sin phi, cos phi) x (C_j, S_j) updates
-// (P_j, Q_j).  Built on the device (awg_expand_kernel) from the 64-bit fixed-point frequency.
-struct __align__(16) PairTable {
-    float2 cs[kPairs];
+// so ONE multiply-add per tone-sample accumulates the even part P_j and the odd part Q_j.  Built on the device
+// (awg_expand_kernel) from the 64-bit fixed-point frequency.
+struct __align__(16) RotTable {
+    float C[kPairs];    // A cos(2 pi (j + 1/2) w)
+    float S[kPairs];    // A sin(2 pi (j + 1/2) w)
+    float pad_[4];
 };
-static_assert(sizeof(PairTable) == 128, "PairTable must be 128 bytes");
+static_assert(sizeof(RotTable) == 80, "RotTable must be 80 bytes");
 
 // What the host uploads per tone (hot-path step a0): carriers, move window, move polynomial.  Phases are in TURNS as
 // unsigned 64-bit fixed point (1 turn = 2^64), so the carrier phase theta + w*n wraps exactly mod 1 for any n: the
@@ -73,13 +67,14 @@ struct __align__(16) ToneCore {
 };
 static_assert(sizeof(ToneCore) == 128, "ToneCore must be 128 bytes");
 
-// Device trajectory table: one 384-byte record per tone (core + the pair tables of the two carriers).
+// Device trajectory table: one 288-byte record per tone (core + the tables of the two carriers), read by one lane per
+// (tone, tile) with 16-byte loads.
 struct __align__(16) ToneRec {
     ToneCore core;
-    PairTable tab_pre;
-    PairTable tab_post;
+    RotTable rot_pre;
+    RotTable rot_post;
 };
-static_assert(sizeof(ToneRec) == 384, "ToneRec must be 384 bytes");
+static_assert(sizeof(ToneRec) == 288, "ToneRec must be 288 bytes");
 
 struct LaunchParams {
     const ToneRec *tab;
@@ -88,6 +83,7 @@ struct LaunchParams {
     int64_t n_begin;   // absolute index of the first output sample (multiple of 8)
     int64_t n_count;   // samples to produce (multiple of 8)
     float scale;       // int16 full-scale factor
+    float qlo, qhi;    // clamp bounds of the quantiser in units of V (filled in by launch_synth)
     void *out;         // int16* or float* (device)
     uint32_t *sched;   // {next tile, teams finished}: the launch's tile-scheduler slot (filled in by launch_synth)
 };
@@ -98,7 +94,7 @@ struct LaunchParams {
 int split_for(int n_tones);
 
 cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream);
-// table[idx ? idx[j] : j] = expand(src[j]) for j < n: copies the core and builds both pair tables (fp64 sincospi)
+// table[idx ? idx[j] : j] = expand(src[j]) for j < n: copies the core and builds both carrier tables (fp64 sincospi)
 cudaError_t launch_expand(ToneRec *table, const ToneCore *src, const int32_t *idx, int n, cudaStream_t stream);
 void count_launch();
 

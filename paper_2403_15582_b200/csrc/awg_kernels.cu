@@ -1,27 +1,27 @@
 // awg_kernels.cu -- sm_100a synthesis kernels: the fused WG + WC (+ quantise) of PAPER.md:158-186.
 //
 // Hot-path steps (SURVEY.md section 8(a) / DESIGN.md section 6):
-//   a1  re-centring in 64-bit fixed point + fp64: per (tone, 4096-sample tile) a u32 carrier for tones static there
-//       (stage_batch() of the static pass), per (tone, 512-sample block) c0, c1, c2..c6 and the record kind for tones
-//       moving there                                                                          block_prologue()
+//   a1  re-centring in 64-bit fixed point + fp64: per (tone, 2048-sample tile) a u32 carrier for tones static there
+//       (stage of the static pass in awg_synth_kernel), per (tone, 512-sample block) c0, c1, c2..c6 and the record
+//       kind for tones moving there                                                          block_prologue()
 //   a2  per tone-sample phase of a moving tone: c0 + c1*k (u32 turns, wraps exactly) + fp32 polynomial  mufu_rec<KIND>()
 //   a3  sine.  Tiles in which a tone is static (angle-addition engine): one MUFU.SIN + one MUFU.COS per (thread, tone,
-//       1024-sample block), then per symmetric sample pair centre +- (j + 1/2), j = 0..15,
+//       block), then per symmetric sample pair centre +- (j + 1/2)
 //           A sin(phi +- (j+1/2) w) = sin(phi) [A cos((j+1/2) w)]  +-  cos(phi) [A sin((j+1/2) w)]
-//       i.e. ONE fp32 multiply-add per tone-sample: one packed FFMA2 (sin phi, cos phi) x (C_j, S_j) updates the
-//       even/odd accumulators (P_j, Q_j)                                                      sincos4(), tone_fma()
+//       i.e. ONE fp32 multiply-add per tone-sample into the even/odd accumulators P_j, Q_j    sincos_tile(), pq_add()
 //       Tiles wholly inside a SLOW move: the same with a cubic phase polynomial per thread and a first-order
-//       frequency correction of the pair tables: TWO multiply-adds per tone-sample              slow_records(), slow_chain()
+//       frequency correction of the pair tables: TWO multiply-adds per tone-sample              stage_slow(), slow_pair()
 //       Blocks in which a tone moves otherwise (and every tone-sample of the MUFU engine): one MUFU.SIN each   mufu_rec<KIND>()
-//   a4  fp32 register accumulation over tones: 4 blocks x 32 samples per thread (angle-addition passes), 16 (MUFU pass)
+//   a4  fp32 register accumulation over tones: 4 blocks x 16 samples per thread (static pass), 16 (MUFU pass)
 //   a5  quantise: round-half-even and saturate to int16 (fused multiply-add against 1.5*2^23)  pack8()
-//   a6  16-byte stores of 8 consecutive int16                                                 store_block(), store_direct()
+//   a6  two 16-byte stores of 8 consecutive int16 per thread and block                       store_block()
 // No tensor cores (north_star), no per-tone wavetable in DRAM (the paper's limiter); output
 // traffic is 2 bytes per sample.
 #include <cstddef>
 #include <cstdint>
 #include <atomic>
 #include <mutex>
+#include <unordered_map>
 
 #include "awg_internal.h"
 
@@ -32,20 +32,19 @@ void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 int split_for(int n_tones)
 {
-    // <= 32 tones per warp where the tone count allows it (a warp whose tones fit one batch keeps them staged), at
-    // least 17, at most 8 warps (one CTA) per tile
-    if (n_tones <= 32) return 1;
-    if (n_tones <= 64) return 2;
-    if (n_tones <= 128) return 4;
-    return 8;
+    // >= 12 tones per warp, at most one CTA (4 warps) per tile
+    int split = 1;
+    while (split < 4 && n_tones / (split * 2) >= 12) split *= 2;
+    return split;
 }
 
 namespace {
 
-constexpr int kHalf = kMovBlock / 2;  // Taylor expansions of the MUFU pass are centred on the 512-sample block
-constexpr int kWarps = 8;             // warps per CTA; one CTA per SM (255 registers per thread, ~223 KB of shared memory)
-constexpr int kBatch = 32;            // tones (static pass) or (tone, block) items (MUFU pass) per batch: one per lane
-constexpr int kMaxBatches = 65536 / kWarps / kBatch;   // per warp, at the largest tone count (split 8)
+constexpr int kHalf = kBlock / 2;     // Taylor expansions are centred on the block
+constexpr int kWarps = 4;             // warps per CTA
+constexpr int kCtasPerSm = 3;         // 12 warps per SM leave 168 registers per thread: tables and sines double-buffered
+constexpr int kBatch = 32;            // tones (pass 1) or (tone, block) items (pass 2) per batch: one per lane
+constexpr int kMaxBatches = 65536 / kWarps / kBatch;   // per warp, at the largest tone count and widest split
 constexpr float kTurnToRad = 1.4629180792671596e-9f;   // 2*pi / 2^32: int32 phase (turns * 2^32) -> radians
 constexpr double kTwo64 = 18446744073709551616.0;
 constexpr int kListBatches = 8;                        // batches of 32 tones compacted at a time for the MUFU pass
@@ -81,24 +80,8 @@ __device__ __forceinline__ uint64_t frac_to_fix64(double x)
 }
 
 __device__ __forceinline__ uint4 ldg16(const void *p) { return __ldg(reinterpret_cast<const uint4 *>(p)); }
-// a load the compiler may not move: issued where it is written, consumed a whole batch later
-__device__ __forceinline__ uint4 ldg16_pinned(const void *p)
-{
-    uint4 v;
-    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
-    return v;
-}
 __device__ __forceinline__ uint64_t u64_of(uint32_t lo, uint32_t hi) { return (static_cast<uint64_t>(hi) << 32) | lo; }
 __device__ __forceinline__ double f64_of(uint32_t lo, uint32_t hi) { return __hiloint2double(static_cast<int>(hi), static_cast<int>(lo)); }
-
-__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
-{
-    const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst));
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // g(s) of the move profile: phase gained over the carrier is DT*g(s) cycles.
 __device__ __forceinline__ double profile_g(int profile, double s)
@@ -143,8 +126,8 @@ struct BlockRec {
     int kind;
 };
 
-// Step a1.  Lane-private: tone record `rec` (index t) at the 512-sample block whose first sample is blk_base
-// (absolute); bb_d = (double)blk_base, nc = blk_base + kHalf.
+// Step a1.  Lane-private: tone record `rec` (index t) at the block whose first sample is blk_base (absolute);
+// bb_d = (double)blk_base, nc = blk_base + kHalf.
 __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, uint64_t nc, double bb_d)
 {
     BlockRec r;
@@ -170,7 +153,7 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
     } else {
         const double Tn = f64_of(v3.z, v3.w);
         const double ua = (bb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the block's first sample
-        const double ub = ua + static_cast<double>(kMovBlock - 1);
+        const double ub = ua + static_cast<double>(kBlock - 1);
         const bool linear = ((cls >> 8) & 0xff) == AWG_PROFILE_LINEAR;
         if (ub <= 0.0) {
             w = w_pre;
@@ -249,16 +232,13 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
 }
 
 // ---- shared memory of one warp ------------------------------------------------------------------------------
-// One staged record of the angle-addition passes: carrier words and the pair table.
-//   static tone: {c0, c1, d, -}: carrier phase (u32 turns) at the half-integer pair centre of lane 0 in block 0 [c0],
-//                per sample [c1] and per 1024-sample block [d];  T = the tone's (C_j, S_j) table
-//   slow tone, parked by stage_batch(): {c0, c1, c2 bits, c3 bits} about the tile centre, T[0].x = A
-//   slow tone, staged by slow_records(): main record (tables at the tile-centre frequency) and correction record
+// One tile-static tone of the current batch (angle-addition pass): carrier phase (u32 turns) at the half-integer
+// pair centre of lane 0 in block 0 [c0], per sample [c1] and per block [d], and the tone's pair tables.
 struct __align__(16) StageRec {
-    uint32_t c0, c1, d, aux;
-    float4 T[kPairs / 2];   // T[q] = (C_2q, S_2q, C_2q+1, S_2q+1)
+    uint32_t c0, c1, d, pad_;
+    float4 C03, C47, S03, S47;
 };
-static_assert(sizeof(StageRec) == 144, "StageRec must be 144 bytes");
+static_assert(sizeof(StageRec) == 80, "StageRec must be 80 bytes");
 
 // One re-centred (tone, block) record of the MUFU pass: q[0] = {c0 bits, c1 bits, A, c2}; q[1] = {c3, c4, c5, c6}.
 // K_EXACT: c0 = tone index.
@@ -267,9 +247,9 @@ struct __align__(16) MovRec {
 };
 
 struct __align__(16) WarpSmem {
-    StageRec st[2 * kBatch + 2];            // two batches (stage ahead); +2: the loop prefetches up to two records ahead
+    StageRec st[kBatch + 1];                // +1: the loop prefetches one carrier record ahead
     MovRec mrec[kBatch + 1];                // +1: the loops prefetch one record ahead
-    float4 park[kMovBlocksPerTile][kMovSPT / 4][32];   // the warp's static partial sums of the tile: [512-block][4 samples][lane]
+    float4 park[kBlocksPerTile][kSPT / 4][32];   // the warp's static partial sums of the tile: [block][4 samples][lane]
     uint32_t mov[kMaxBatches];              // per batch of 32 tones: which ones take the MUFU pass in this tile
     uint32_t next;                          // (rank-0 warp of a team) the team's next tile, drawn by the leader
     uint32_t n_mov;                         // how many of the warp's tones take the MUFU pass in this tile
@@ -277,16 +257,23 @@ struct __align__(16) WarpSmem {
     uint16_t list[kListCap];                // compacted tone indices of the MUFU pass (n_tones <= 65536)
 };
 
-// 16 samples of one 512-sample block of one thread (MUFU-pass geometry), as 8 packed pairs: a[j] = samples (2j, 2j+1).
+// 16 samples of one block of one thread, as 8 packed pairs: a[j] = samples (2j, 2j+1).
 struct Acc16 {
-    float2 a[kMovPairs];
+    float2 a[kPairs];
 };
 
-__device__ __forceinline__ void park_add(const WarpSmem &ws, int mb, int lane, Acc16 &acc)
+__device__ __forceinline__ void park_store(WarpSmem &ws, int r, int lane, const Acc16 &acc)
 {
 #pragma unroll
-    for (int v = 0; v < kMovSPT / 4; ++v) {
-        const float4 u = ws.park[mb][v][lane];
+    for (int v = 0; v < kSPT / 4; ++v)
+        ws.park[r][v][lane] = make_float4(acc.a[2 * v].x, acc.a[2 * v].y, acc.a[2 * v + 1].x, acc.a[2 * v + 1].y);
+}
+
+__device__ __forceinline__ void park_add(const WarpSmem &ws, int r, int lane, Acc16 &acc)
+{
+#pragma unroll
+    for (int v = 0; v < kSPT / 4; ++v) {
+        const float4 u = ws.park[r][v][lane];
         acc.a[2 * v].x += u.x; acc.a[2 * v].y += u.y;
         acc.a[2 * v + 1].x += u.z; acc.a[2 * v + 1].y += u.w;
     }
@@ -295,15 +282,15 @@ __device__ __forceinline__ void park_add(const WarpSmem &ws, int mb, int lane, A
 // Steps a2-a4, MUFU path, for ONE record of kind KIND.  Samples go in pairs through the packed fp32x2
 // instructions of sm_100 (FMUL2 / FFMA2: one issue slot for two samples); the 16 sine chains are independent.
 template <int KIND>
-__device__ __forceinline__ void mufu_rec(const float4 a, const float4 b, int koff, const float2 (&kfs)[kMovPairs],
-                                         const float2 (&kks)[kMovPairs], Acc16 &acc)
+__device__ __forceinline__ void mufu_rec(const float4 a, const float4 b, int koff, const float2 (&kfs)[kPairs],
+                                         const float2 (&kks)[kPairs], Acc16 &acc)
 {
     const float2 K2 = dup2(kTurnToRad);
     const uint32_t c0 = __float_as_uint(a.x), c1 = __float_as_uint(a.y);
     const float A = a.z;
     const uint32_t base = c0 + c1 * static_cast<uint32_t>(koff);
 #pragma unroll
-    for (int j = 0; j < kMovPairs; ++j) {
+    for (int j = 0; j < kPairs; ++j) {
         const uint32_t p0 = base + c1 * static_cast<uint32_t>(2 * j);
         const uint32_t p1 = base + c1 * static_cast<uint32_t>(2 * j + 1);
         const float2 f = make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1)));
@@ -347,7 +334,7 @@ __device__ __noinline__ Acc16 exact_rec(const ToneRec *tab, const float4 a, int6
     const ToneCore &tr = tab[__float_as_uint(a.x)].core;
     const float A = a.z;
 #pragma unroll 1
-    for (int j = 0; j < kMovPairs; ++j) {
+    for (int j = 0; j < kPairs; ++j) {
         const uint32_t p0 = round32(exact_phase(tr, n_thread + 2 * j));
         const uint32_t p1 = round32(exact_phase(tr, n_thread + 2 * j + 1));
         float2 v = acc.a[0];
@@ -355,8 +342,8 @@ __device__ __noinline__ Acc16 exact_rec(const ToneRec *tab, const float4 a, int6
         v.x = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p0)) * kTurnToRad), v.x);
         v.y = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p1)) * kTurnToRad), v.y);
 #pragma unroll
-        for (int m = 0; m < kMovPairs - 1; ++m) acc.a[m] = acc.a[m + 1];
-        acc.a[kMovPairs - 1] = v;
+        for (int m = 0; m < kPairs - 1; ++m) acc.a[m] = acc.a[m + 1];
+        acc.a[kPairs - 1] = v;
     }
     return acc;
 }
@@ -365,176 +352,105 @@ __device__ __noinline__ Acc16 exact_rec(const ToneRec *tab, const float4 a, int6
 // The clamp is applied to v (bounds -32768/scale, 32767/scale: qlo, qhi); the fused multiply-add against 1.5*2^23 then
 // rounds scale*v ONCE, to nearest-even, into the low mantissa bits: the two's-complement code is the low half-word.
 // Runs on the ALU and FMA pipes (a float-to-int conversion would take the XU pipe the sines need).
-__device__ __forceinline__ uint4 pack8(const LaunchParams &lp, float qlo, float qhi, const float2 (&s)[4])
+__device__ __forceinline__ uint4 pack8(const LaunchParams &lp, const float2 *s)
 {
     uint32_t w[4];
     const float2 sc = dup2(lp.scale), mg = dup2(kRoundMagic);
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        const float2 v = make_float2(fminf(fmaxf(s[j].x, qlo), qhi), fminf(fmaxf(s[j].y, qlo), qhi));
+        const float2 v = make_float2(fminf(fmaxf(s[j].x, lp.qlo), lp.qhi), fminf(fmaxf(s[j].y, lp.qlo), lp.qhi));
         const float2 t = __ffma2_rn(v, sc, mg);
         w[j] = __byte_perm(__float_as_uint(t.x), __float_as_uint(t.y), 0x5410);
     }
     return make_uint4(w[0], w[1], w[2], w[3]);
 }
 
-// Steps a5-a6 for one 512-sample block of one thread (MUFU-pass geometry): 16 consecutive samples starting at absolute
-// index n_thread, as two 8-sample halves (launch ranges are multiples of 8 samples: each half is inside or outside).
-__device__ __forceinline__ void store_block(const LaunchParams &lp, float qlo, float qhi, int64_t n_thread, const Acc16 &acc)
+// Steps a5-a6 for one block of one thread: 16 consecutive samples starting at absolute index n_thread, as two
+// 8-sample halves (launch ranges are multiples of 8 samples, so each half is inside or outside as a whole).
+__device__ __forceinline__ void store_block(const LaunchParams &lp, int64_t n_thread, const Acc16 &acc)
 {
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
         const int64_t off = n_thread + 8 * h - lp.n_begin;
         if (off < 0 || off >= lp.n_count) continue;
-        const float2(&a)[4] = *reinterpret_cast<const float2(*)[4]>(acc.a + 4 * h);
+        const float2 *a = acc.a + 4 * h;
         if (lp.out_f32) {
             float4 *o = reinterpret_cast<float4 *>(static_cast<float *>(lp.out) + off);
             o[0] = make_float4(a[0].x, a[0].y, a[1].x, a[1].y);
             o[1] = make_float4(a[2].x, a[2].y, a[3].x, a[3].y);
         } else {
-            *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = pack8(lp, qlo, qhi, a);
+            *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = pack8(lp, a);
         }
     }
 }
 
-// Even/odd accumulators of the angle-addition passes for one tile: pq[r][j] = (P_j, Q_j) of block r;
-// sample (16 + j) = P_j + Q_j, sample (15 - j) = P_j - Q_j.
-struct TileAcc {
-    float2 pq[kBlocksPerTile][kPairs];
+// Even/odd accumulators of the angle-addition pass for one block: sample (8 + j) = P_j + Q_j, sample (7 - j) = P_j - Q_j.
+struct PQ {
+    float2 P[kPairs / 2], Q[kPairs / 2];  // pairs (j, j+1), j = 0, 2, 4, 6
 };
 
-// The thread's 32 samples of block r, in order, as 16 packed pairs.
-__device__ __forceinline__ void block_samples(const TileAcc &t, int r, float2 (&s)[kPairs])
+__device__ __forceinline__ void pq_add(PQ &pq, float s, float c, const float4 &C03, const float4 &C47, const float4 &S03,
+                                       const float4 &S47)
 {
+    const float2 s2 = dup2(s), c2 = dup2(c);
+    pq.P[0] = __ffma2_rn(s2, make_float2(C03.x, C03.y), pq.P[0]);
+    pq.P[1] = __ffma2_rn(s2, make_float2(C03.z, C03.w), pq.P[1]);
+    pq.P[2] = __ffma2_rn(s2, make_float2(C47.x, C47.y), pq.P[2]);
+    pq.P[3] = __ffma2_rn(s2, make_float2(C47.z, C47.w), pq.P[3]);
+    pq.Q[0] = __ffma2_rn(c2, make_float2(S03.x, S03.y), pq.Q[0]);
+    pq.Q[1] = __ffma2_rn(c2, make_float2(S03.z, S03.w), pq.Q[1]);
+    pq.Q[2] = __ffma2_rn(c2, make_float2(S47.x, S47.y), pq.Q[2]);
+    pq.Q[3] = __ffma2_rn(c2, make_float2(S47.z, S47.w), pq.Q[3]);
+}
+
+__device__ __forceinline__ Acc16 pq_to_samples(const PQ &pq)
+{
+    Acc16 d;
 #pragma unroll
     for (int m = 0; m < kPairs / 2; ++m) {
-        const float2 hi = t.pq[r][kPairs - 1 - 2 * m], lo = t.pq[r][kPairs - 2 - 2 * m];   // j = 15 - 2m, 14 - 2m
-        s[m] = make_float2(hi.x - hi.y, lo.x - lo.y);                                       // samples 2m, 2m + 1
-        const float2 a = t.pq[r][2 * m], b = t.pq[r][2 * m + 1];                            // j = 2m, 2m + 1
-        s[kPairs / 2 + m] = make_float2(a.x + a.y, b.x + b.y);                              // samples 16 + 2m, 17 + 2m
+        const float2 p = pq.P[m], q = pq.Q[m];              // j = 2m, 2m+1
+        d.a[4 + m] = make_float2(p.x + q.x, p.y + q.y);      // samples 8 + 2m, 9 + 2m
+        d.a[3 - m] = make_float2(p.y - q.y, p.x - q.x);      // samples 6 - 2m, 7 - 2m
     }
+    return d;
 }
 
-// Steps a5-a6 straight from the angle-addition geometry (tiles without moving tones, one warp per tile).
-__device__ __forceinline__ void store_direct(const LaunchParams &lp, float qlo, float qhi, int64_t n_thread, const float2 (&s)[kPairs])
+// sin and cos of a u32-turn phase: one range multiply feeds both MUFU operations
+__device__ __forceinline__ void sincos_turns(uint32_t p, float &s, float &c)
 {
-#pragma unroll
-    for (int h = 0; h < kSPT / 8; ++h) {
-        const int64_t off = n_thread + 8 * h - lp.n_begin;
-        if (off < 0 || off >= lp.n_count) continue;
-        const float2(&a)[4] = *reinterpret_cast<const float2(*)[4]>(&s[4 * h]);
-        if (lp.out_f32) {
-            float4 *o = reinterpret_cast<float4 *>(static_cast<float *>(lp.out) + off);
-            o[0] = make_float4(a[0].x, a[0].y, a[1].x, a[1].y);
-            o[1] = make_float4(a[2].x, a[2].y, a[3].x, a[3].y);
-        } else {
-            *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = pack8(lp, qlo, qhi, a);
-        }
-    }
+    const float x = __int2float_rn(static_cast<int32_t>(p)) * kTurnToRad;
+    s = mufu_sin(x);
+    c = mufu_cos(x);
 }
 
-// The warp's partial sums of the tile go to shared memory in the MUFU-pass geometry: thread (block r, lane L, sample i)
-// is thread (512-block 2r + L/16, lane 2(L%16) + i/16, sample i%16) there.
-__device__ __forceinline__ void park_store(WarpSmem &ws, int r, int lane, const float2 (&s)[kPairs])
+// Requests the carrier part of a tone record (A, cls, theta_pre | w_pre, theta_post | w_post, ns_int | ns_frac, Tn) and
+// pulls its two angle-addition tables (bytes 128..287) towards L1.
+__device__ __forceinline__ void fetch_tone(const ToneRec *tr, uint4 &v0, uint4 &v1, uint4 &v2, uint4 &v3)
 {
-    const int mb = 2 * r + (lane >> 4);
-    const int l0 = 2 * (lane & 15);
-#pragma unroll
-    for (int i4 = 0; i4 < kSPT / 4; ++i4)
-        ws.park[mb][i4 & 3][l0 + (i4 >> 2)] = make_float4(s[2 * i4].x, s[2 * i4].y, s[2 * i4 + 1].x, s[2 * i4 + 1].y);
+    const char *p = reinterpret_cast<const char *>(tr);
+    v0 = ldg16(p);
+    v1 = ldg16(p + 16);
+    v2 = ldg16(p + 32);
+    v3 = ldg16(p + 48);
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 128));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 208));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 272));
 }
 
-// sin and cos of the carrier phase at the thread's pair centre in each of the tile's four blocks, as the pairs
-// a[r] = (sin, cos).  cc = {phase at lane 0's centre of block 0, phase per sample, phase per block, -} in u32 turns.
-__device__ __forceinline__ void sincos4(const uint4 cc, int off, float2 (&a)[kBlocksPerTile])
+// Sines and cosines of one tile-static tone at the thread's pair centre in each of the tile's four blocks.
+// cc = {phase at lane 0's centre of block 0, phase per sample, phase per block, -} in u32 turns.
+__device__ __forceinline__ void sincos_tile(const uint4 cc, int off, float (&s)[kBlocksPerTile], float (&c)[kBlocksPerTile])
 {
-    static_assert(kBlocksPerTile == 4, "sincos4 packs the four blocks as two pairs");
+    static_assert(kBlocksPerTile == 4, "sincos_tile packs the four blocks as two pairs");
     const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(off);
     const uint32_t p1 = p0 + cc.z, p2 = p1 + cc.z, p3 = p2 + cc.z;
     const float2 K2 = dup2(kTurnToRad);
     const float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1))), K2);
     const float2 x23 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p2)), __int2float_rn(static_cast<int32_t>(p3))), K2);
-    a[0] = make_float2(mufu_sin(x01.x), mufu_cos(x01.x));
-    a[1] = make_float2(mufu_sin(x01.y), mufu_cos(x01.y));
-    a[2] = make_float2(mufu_sin(x23.x), mufu_cos(x23.x));
-    a[3] = make_float2(mufu_sin(x23.y), mufu_cos(x23.y));
-}
-
-__device__ __forceinline__ void load_table(float4 (&T)[kPairs / 2], const StageRec *sp)
-{
-#pragma unroll
-    for (int q = 0; q < kPairs / 2; ++q) T[q] = sp->T[q];
-}
-
-// Step a4 for one staged record: (P_j, Q_j) += (a.x C_j, a.y S_j) for the 16 pairs of each of the 4 blocks: 64 FFMA2
-// = 128 multiply-adds for 128 tone-samples.  Block-major order: the multiplier pair a[r] stays in the operand reuse
-// cache for 16 instructions, the table T is read from registers (the register file cannot feed three fresh operands
-// per FFMA2 at the pipe's rate; measured).  During the last block every quarter of T is replaced, right after its last
-// use, by the table of the record at `next` (rolling prefetch: no second set of table registers).
-__device__ __forceinline__ void tone_fma(TileAcc &t, const float2 (&a)[kBlocksPerTile], float4 (&T)[kPairs / 2], const StageRec *next)
-{
-#pragma unroll
-    for (int r = 0; r < kBlocksPerTile; ++r) {
-#pragma unroll
-        for (int q = 0; q < kPairs / 2; ++q) {
-            t.pq[r][2 * q] = __ffma2_rn(a[r], make_float2(T[q].x, T[q].y), t.pq[r][2 * q]);
-            t.pq[r][2 * q + 1] = __ffma2_rn(a[r], make_float2(T[q].z, T[q].w), t.pq[r][2 * q + 1]);
-            if (r == kBlocksPerTile - 1) T[q] = next->T[q];
-        }
-    }
-}
-
-// Slow pass, per-thread chain of one tone: cubic phase polynomial about the tile centre at the thread's pair centre
-// in each block (kf = offset from the tile centre), local frequency offset e = d(poly)/dk, and the multiplier pairs of
-// the main record a[r] = (sin, cos) and of the correction record a2[r] = (-e sin, e cos).
-__device__ __forceinline__ void slow_chain(const uint4 cc, int mr0, const float2 (&kf)[2], const float2 (&kf2)[2],
-                                           float2 (&a)[kBlocksPerTile], float2 (&a2)[kBlocksPerTile])
-{
-    const float c2 = __uint_as_float(cc.z), c3 = __uint_as_float(cc.w);
-    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(mr0);
-    const uint32_t dd = cc.y << 10;   // phase per 1024-sample block
-    const uint32_t p1 = p0 + dd, p2 = p1 + dd, p3 = p2 + dd;
-    const float2 K2 = dup2(kTurnToRad);
-    const float2 f01 = make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1)));
-    const float2 f23 = make_float2(__int2float_rn(static_cast<int32_t>(p2)), __int2float_rn(static_cast<int32_t>(p3)));
-    // poly = kf^2 (c2 + c3 kf);  e = kf (2 c2 + 3 c3 kf)
-    const float2 x01 = __ffma2_rn(f01, K2, __fmul2_rn(kf2[0], __ffma2_rn(dup2(c3), kf[0], dup2(c2))));
-    const float2 x23 = __ffma2_rn(f23, K2, __fmul2_rn(kf2[1], __ffma2_rn(dup2(c3), kf[1], dup2(c2))));
-    const float2 e01 = __fmul2_rn(kf[0], __ffma2_rn(dup2(3.f * c3), kf[0], dup2(2.f * c2)));
-    const float2 e23 = __fmul2_rn(kf[1], __ffma2_rn(dup2(3.f * c3), kf[1], dup2(2.f * c2)));
-    a[0] = make_float2(mufu_sin(x01.x), mufu_cos(x01.x));
-    a[1] = make_float2(mufu_sin(x01.y), mufu_cos(x01.y));
-    a[2] = make_float2(mufu_sin(x23.x), mufu_cos(x23.x));
-    a[3] = make_float2(mufu_sin(x23.y), mufu_cos(x23.y));
-    a2[0] = __fmul2_rn(a[0], make_float2(-e01.x, e01.x));
-    a2[1] = __fmul2_rn(a[1], make_float2(-e01.y, e01.y));
-    a2[2] = __fmul2_rn(a[2], make_float2(-e23.x, e23.x));
-    a2[3] = __fmul2_rn(a[3], make_float2(-e23.y, e23.y));
-}
-
-// Slow pass, staging (one lane per slow mover): the pair tables at the tile-centre frequency c1 come from MUFU
-// (the frequency changes from tile to tile, so they cannot be precomputed), the second record holds their
-// first-order correction: cos((j+1/2)(w + e)) ~ C_j - (j+1/2) e S_j,  sin((j+1/2)(w + e)) ~ S_j + (j+1/2) e C_j,
-// i.e. P_j += (-e sin phi) [(j+1/2) S_j],  Q_j += (e cos phi) [(j+1/2) C_j].
-__device__ __forceinline__ void slow_records(StageRec *dst, const uint4 cc, float A)
-{
-    const uint32_t c1 = cc.y;
-    *reinterpret_cast<uint4 *>(&dst[0]) = cc;   // {c0 at the tile centre - 1/2, c1, c2, c3}
-#pragma unroll
-    for (int q = 0; q < kPairs / 2; ++q) {
-        float C[2], S[2];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int j = 2 * q + h;
-            const uint32_t ang = c1 * static_cast<uint32_t>(j) + (c1 >> 1);   // (j + 1/2) c1, u32 turns
-            const float x = __int2float_rn(static_cast<int32_t>(ang)) * kTurnToRad;
-            C[h] = A * mufu_cos(x);
-            S[h] = A * mufu_sin(x);
-        }
-        const float k0 = static_cast<float>(2 * q) + 0.5f, k1 = k0 + 1.f;
-        dst[0].T[q] = make_float4(C[0], S[0], C[1], S[1]);
-        dst[1].T[q] = make_float4(k0 * S[0], k0 * C[0], k1 * S[1], k1 * C[1]);
-    }
+    s[0] = mufu_sin(x01.x); c[0] = mufu_cos(x01.x);
+    s[1] = mufu_sin(x01.y); c[1] = mufu_cos(x01.y);
+    s[2] = mufu_sin(x23.x); c[2] = mufu_cos(x23.x);
+    s[3] = mufu_sin(x23.y); c[3] = mufu_cos(x23.y);
 }
 
 template <int SPLIT>
@@ -545,8 +461,8 @@ __device__ __forceinline__ void team_sync(int team)
     else asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(SPLIT * 32) : "memory");
 }
 
-// MUFU pass of one warp over ONE 512-sample BLOCK of a tile, for the tones the team's warps flagged in their `mov` bit
-// masks (warp r2 owns tones r2*per ...).  The flagged tones of the whole team are compacted into ws.list (kListCap at a
+// MUFU pass of one warp over ONE BLOCK of a tile, for the tones the team's warps flagged in their `mov` bit masks
+// (warp r2 owns tones r2*per ...).  The flagged tones of the whole team are compacted into ws.list (kListCap at a
 // time); every listed tone is re-centred on the block (step a1, one lane per tone) and the records are then run
 // KIND BY KIND (warp-uniform loops over ballot masks, no per-record switch) with one MUFU.SIN per tone-sample into
 // the block's 16 samples per thread, which stay in registers.  Which records share a sub-batch depends only on the
@@ -567,13 +483,13 @@ __device__ __forceinline__ void team_sync(int team)
 
 template <int SPLIT>
 __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws, const WarpSmem *team_ws, int per,
-                                         int64_t blk_base, int lane, Acc16 &acc)
+                                            int64_t blk_base, int lane, Acc16 &acc)
 {
-    const int koff = lane * kMovSPT - kHalf;
+    const int koff = lane * kSPT - kHalf;
     const unsigned lt = (1u << lane) - 1u;
-    float2 kf[kMovPairs], kk[kMovPairs];  // in-block offsets k of the thread's samples, and k^2
+    float2 kf[kPairs], kk[kPairs];  // in-block offsets k of the thread's samples, and k^2
 #pragma unroll
-    for (int j = 0; j < kMovPairs; ++j) {
+    for (int j = 0; j < kPairs; ++j) {
         kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
         kk[j] = __fmul2_rn(kf[j], kf[j]);
     }
@@ -642,7 +558,7 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
             AWG_RUN_KIND(K_SEND)
 #pragma unroll 1
             for (int i_ = kbase[K_EXACT]; i_ < kbase[K_EXACT] + kcnt[K_EXACT]; ++i_)
-                acc = exact_rec(lp.tab, ws.mrec[i_].q[0], blk_base + lane * kMovSPT, acc);
+                acc = exact_rec(lp.tab, ws.mrec[i_].q[0], blk_base + lane * kSPT, acc);
         }
         __syncwarp();  // ws.list is rebuilt for the next kListCap tones
     }
@@ -665,137 +581,72 @@ __device__ __forceinline__ int64_t next_unit(const LaunchParams &lp, WarpSmem &w
     return n_teams + static_cast<int64_t>(v);
 }
 
-// Carrier part of a tone record held by its staging lane (64 bytes: A, cls, theta_pre | w_pre, theta_post | w_post,
-// ns_int | ns_frac, Tn).
-struct CoreRegs {
-    uint4 v0, v1, v2, v3;
-};
-
-__device__ __forceinline__ void fetch_core(const ToneRec *tr, CoreRegs &v)
+// Slow pass, staging (one lane per slow mover): the pair tables at the tile-centre frequency c1 come from MUFU
+// (the frequency changes from tile to tile, so they cannot be precomputed), the second record holds their
+// first-order correction: cos((j+1/2)(w + e)) ~ C_j - (j+1/2) e S_j,  sin((j+1/2)(w + e)) ~ S_j + (j+1/2) e C_j.
+__device__ __forceinline__ void stage_slow(StageRec *dst, const MovRec &parked)
 {
-    const char *p = reinterpret_cast<const char *>(tr);
-    v.v0 = ldg16_pinned(p);
-    v.v1 = ldg16_pinned(p + 16);
-    v.v2 = ldg16_pinned(p + 32);
-    v.v3 = ldg16_pinned(p + 48);
-}
-
-// What stage_batch() leaves behind for the loops of the batch.
-struct BatchInfo {
-    int n_sta;        // static records staged at buf[0 .. n_sta)
-    unsigned m_slow;  // lanes whose tone takes the slow pass; lane L's parameters are parked at buf[kBatch - 1 - rank]
-    unsigned m_sta, m_post;
-};
-
-// Step a1 for one batch of <= 32 tones of the warp (tones tb + lane < t_end) in the tile at tile_base: every lane
-// classifies its tone -- static on the pre- or post-move carrier, inside a slow move, or moving (MUFU pass) -- from the
-// carrier part v it holds in registers, writes the carrier words of a static tone to `buf` and starts the asynchronous
-// copy of its pair table (cp.async, 8 x 16 bytes; `copy_tables` is false when a single-batch warp already has them),
-// parks the cubic expansion of a slow mover at the end of `buf`, and records the movers in ws.mov[b].
-__device__ __forceinline__ BatchInfo stage_batch(const LaunchParams &lp, WarpSmem &ws, StageRec *buf, int b, int tb, int t_end,
-                                                 int lane, int64_t tile_base, const CoreRegs &v, bool sticky, unsigned sticky_sta,
-                                                 unsigned sticky_post, int &n_mov)
-{
-    const unsigned lt = (1u << lane) - 1u;
-    const int t = tb + lane;
-    bool is_static = false, is_mover = false, is_post = false, is_slow = false;
-    uint32_t c0 = 0, c1 = 0, d = 0, aux = 0;
-    float slow_A = 0.f;
-    const float4 *tabp = nullptr;
-    if (t < t_end) {
-        const ToneRec *tr = lp.tab + t;
-        const double tb_d = static_cast<double>(tile_base);
-        // phase reference: the centre of block 0, minus the half sample of the pair centring
-        const uint64_t a0 = static_cast<uint64_t>(tile_base + kBlock / 2);
-        uint64_t th = u64_of(v.v0.z, v.v0.w), w = u64_of(v.v1.x, v.v1.y);
-        tabp = reinterpret_cast<const float4 *>(&tr->tab_pre);
-        is_static = true;
-        const int32_t cls = static_cast<int32_t>(v.v0.y);
-        if ((cls & 0xff) != CLS_STATIC) {
-            const double ua = (tb_d - f64_of(v.v2.z, v.v2.w)) - f64_of(v.v3.x, v.v3.y);  // u of the tile's first sample
-            const double ub = ua + static_cast<double>(kTile - 1);
-            const double Tn = f64_of(v.v3.z, v.v3.w);
-            if (ub <= 0.0) {
-                // whole tile before the move: pre-move carrier
-            } else if (ua >= Tn) {
-                th = u64_of(v.v1.z, v.v1.w);
-                w = u64_of(v.v2.x, v.v2.y);
-                tabp = reinterpret_cast<const float4 *>(&tr->tab_post);
-                is_post = true;
-            } else if ((cls & CLS_SLOW_FLAG) && ua >= 0.0 && ub <= Tn) {
-                // Slow mover, tile wholly inside the move: cubic Taylor expansion of the phase about the tile centre
-                // (phase and frequency in u64 / fp64, curvature terms in fp32 radians).
-                is_static = false;
-                is_slow = true;
-                const uint4 v4 = ldg16(reinterpret_cast<const char *>(tr) + 64);  // inv_Tn, DT
-                const uint4 v5 = ldg16(reinterpret_cast<const char *>(tr) + 80);  // q1, q[0], q[1]
-                const double sc = (ua + static_cast<double>(kTile / 2)) * f64_of(v4.x, v4.y);
-                const float sf = static_cast<float>(sc);
-                double g0, g1;
-                float g2, g3;
-                if (((cls >> 8) & 0xff) == AWG_PROFILE_LINEAR) {
-                    g0 = 0.5 * sc * sc; g1 = sc; g2 = 1.f; g3 = 0.f;
-                } else {
-                    const double s2 = sc * sc;
-                    g0 = s2 * s2 * (2.5 + sc * (sc - 3.0));
-                    g1 = s2 * sc * (10.0 + sc * (6.0 * sc - 15.0));
-                    g2 = sf * sf * (30.f + sf * (30.f * sf - 60.f));
-                    g3 = sf * (60.f + sf * (120.f * sf - 180.f));
-                }
-                const uint64_t nc = static_cast<uint64_t>(tile_base + kTile / 2);
-                const uint64_t wc = w + frac_to_fix64(f64_of(v5.x, v5.y) * g1);
-                const uint64_t pc = th + w * nc + frac_to_fix64(f64_of(v4.z, v4.w) * g0);
-                c0 = round32(pc - (wc >> 1));
-                c1 = round32(wc);
-                d = __float_as_uint(__uint_as_float(v5.z) * g2);
-                aux = __float_as_uint(__uint_as_float(v5.w) * g3);
-                slow_A = __uint_as_float(v.v0.x);
-            } else {
-                is_static = false;
-                is_mover = true;
-                // the block owners re-centre this tone after the barrier: pull its record towards L2/L1 now
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(tr)));
-            }
-        }
-        if (is_static) {
-            c0 = round32(th + w * a0 - (w >> 1));
-            c1 = round32(w);
-            d = round32(w * static_cast<uint64_t>(kBlock));
-        }
-    }
-    BatchInfo bi;
-    const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
-    bi.m_sta = __ballot_sync(0xffffffffu, is_static);
-    bi.m_slow = __ballot_sync(0xffffffffu, is_slow);
-    bi.m_post = __ballot_sync(0xffffffffu, is_post);
-    bi.n_sta = __popc(bi.m_sta);
-    if (lane == 0) ws.mov[b] = m_mov;
-    n_mov += __popc(m_mov);
-    const bool tables_staged = sticky && bi.m_sta == sticky_sta && bi.m_post == sticky_post;
-    if (is_static) {
-        StageRec &sr = buf[__popc(bi.m_sta & lt)];
-        *reinterpret_cast<uint4 *>(&sr) = make_uint4(c0, c1, d, 0u);
-        if (!tables_staged) {
+    const float4 a = parked.q[0];
+    const uint32_t c1 = __float_as_uint(a.y);
+    const float A = parked.q[1].x;
+    float C[kPairs], S[kPairs];
 #pragma unroll
-            for (int q = 0; q < kPairs / 2; ++q) cp_async16(&sr.T[q], tabp + q);
-        }
-    } else if (is_slow) {
-        StageRec &sr = buf[kBatch - 1 - __popc(bi.m_slow & lt)];
-        *reinterpret_cast<uint4 *>(&sr) = make_uint4(c0, c1, d, aux);
-        sr.T[0].x = slow_A;
+    for (int j = 0; j < kPairs; ++j) {
+        const uint32_t ang = c1 * static_cast<uint32_t>(j) + (c1 >> 1);   // (j + 1/2) c1, u32 turns
+        const float x = __int2float_rn(static_cast<int32_t>(ang)) * kTurnToRad;
+        C[j] = A * mufu_cos(x);
+        S[j] = A * mufu_sin(x);
     }
-    cp_async_commit();
-    return bi;
+    *reinterpret_cast<float4 *>(&dst[0]) = a;   // {c0 at the tile centre - 1/2, c1, c2, c3}
+    dst[0].C03 = make_float4(C[0], C[1], C[2], C[3]);
+    dst[0].C47 = make_float4(C[4], C[5], C[6], C[7]);
+    dst[0].S03 = make_float4(S[0], S[1], S[2], S[3]);
+    dst[0].S47 = make_float4(S[4], S[5], S[6], S[7]);
+    // correction record: multiplies -sin(phi) e into (j+1/2) S_j and cos(phi) e into (j+1/2) C_j
+    dst[1].C03 = make_float4(0.5f * S[0], 1.5f * S[1], 2.5f * S[2], 3.5f * S[3]);
+    dst[1].C47 = make_float4(4.5f * S[4], 5.5f * S[5], 6.5f * S[6], 7.5f * S[7]);
+    dst[1].S03 = make_float4(0.5f * C[0], 1.5f * C[1], 2.5f * C[2], 3.5f * C[3]);
+    dst[1].S47 = make_float4(4.5f * C[4], 5.5f * C[5], 6.5f * C[6], 7.5f * C[7]);
 }
 
-// A work unit is one 4096-sample tile x the tones of one warp.  SPLIT warps (a team) share a tile, each taking
-// 1/SPLIT of the tones; their partial sums meet in shared memory and are added in rank order.  The grid is persistent
-// (one 8-warp CTA per SM); teams draw tiles from the launch's counter.
-// ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine), tiles inside a slow move
-// the slow pass, everything else (and every tone when !ROT) the MUFU pass.  Every sample goes through the same
-// arithmetic for every launch geometry because all phases are anchored to absolute tile positions.
+// Slow pass, one tone: phase polynomial at the thread's pair centre in each block (k = offset from the tile centre),
+// local frequency offset e = d(poly)/dk, then two multiply-adds per tone-sample.
+__device__ __forceinline__ void slow_pair(const StageRec &m, const StageRec &k, int lane, PQ (&pq)[kBlocksPerTile])
+{
+    const uint4 cc = *reinterpret_cast<const uint4 *>(&m);
+    const float c2 = __uint_as_float(cc.z), c3 = __uint_as_float(cc.w);
+    float s[kBlocksPerTile], c[kBlocksPerTile], e[kBlocksPerTile];
+#pragma unroll
+    for (int r = 0; r < kBlocksPerTile; ++r) {
+        const int mr = r * kBlock + lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre
+        const float kf = static_cast<float>(mr) - 0.5f;
+        const uint32_t p = cc.x + cc.y * static_cast<uint32_t>(mr);
+        const float x = fmaf(__int2float_rn(static_cast<int32_t>(p)), kTurnToRad, kf * kf * fmaf(kf, c3, c2));
+        s[r] = mufu_sin(x);
+        c[r] = mufu_cos(x);
+        e[r] = kf * fmaf(3.f * kf, c3, 2.f * c2);
+    }
+    {
+        const float4 C03 = m.C03, C47 = m.C47, S03 = m.S03, S47 = m.S47;
+#pragma unroll
+        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], s[r], c[r], C03, C47, S03, S47);
+    }
+    {
+        const float4 C03 = k.C03, C47 = k.C47, S03 = k.S03, S47 = k.S47;
+#pragma unroll
+        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], -s[r] * e[r], c[r] * e[r], C03, C47, S03, S47);
+    }
+}
+
+// A work unit is one 2048-sample tile (4 blocks of 512) x the tones of one warp.  SPLIT warps (a team) share a
+// tile, each taking 1/SPLIT of the tones; their partial sums meet in shared memory and are added in rank order.
+// The grid is persistent (two CTAs per SM); teams walk the tiles of the launch with a stride of the team count,
+// team index = team_in_cta * gridDim.x + blockIdx.x, so a final partial round spreads over all SMs.
+// ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine), everything else (and
+// every tone when !ROT) takes the MUFU pass.  Every sample goes through the same arithmetic for every launch
+// geometry because all phases are anchored to absolute tile positions.
 template <int SPLIT, bool ROT>
-__global__ void __launch_bounds__(kWarps * 32, 1) awg_synth_kernel(const LaunchParams lp, const float qlo, const float qhi)
+__global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(const LaunchParams lp)
 {
     constexpr int kTeams = kWarps / SPLIT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -805,6 +656,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) awg_synth_kernel(const LaunchP
     const int warp = threadIdx.x >> 5;
     const int team = warp / SPLIT;
     const int rank = warp % SPLIT;
+    const unsigned lt = (1u << lane) - 1u;
     WarpSmem &ws = ws_all[warp];
 
     // tiles are anchored to absolute sample indices (chunk-size invariance, SURVEY.md 8(b) "Determinism")
@@ -816,142 +668,172 @@ __global__ void __launch_bounds__(kWarps * 32, 1) awg_synth_kernel(const LaunchP
     const int per = (lp.n_tones + SPLIT - 1) / SPLIT;
     const int t_begin = rank * per;
     const int t_end = min(lp.n_tones, t_begin + per);
-    const int n_batches = (max(t_end - t_begin, 0) + kBatch - 1) / kBatch;
-    const int off = lane * kSPT + kSPT / 2 - kBlock / 2;  // thread's pair centre + 1/2 relative to the centre of block 0
+    const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the centre of block 0
 
     // Tile scheduler: every team starts on the tile of its own index and then draws tiles from the launch's
     // counter lp.sched[0] (tiles that hold moving tones cost several times the others, so a fixed stride leaves
     // SMs idle at the end).  Which team computes a tile has no effect on its samples.
     int64_t unit = static_cast<int64_t>(team) * gridDim.x + blockIdx.x;
-    // The carrier part of the next batch's tone records is requested one staging step ahead and stays in registers
-    // until then; after the last batch of a tile the request wraps round to the first batch (the next tile starts
-    // with it).  A warp whose tones fit one batch keeps them for the whole launch, and their tables in shared memory
-    // for as long as the same tones are static on the same carriers (sticky_sta / sticky_post).
-    CoreRegs core;
-    core.v0 = core.v1 = core.v2 = core.v3 = make_uint4(0, 0, 0, 0);
-    const bool single = n_batches <= 1;
+    // The tone records of the next batch are requested before the multiply-add loop of the current batch runs
+    // (v0n..v3n stay in registers across it, the two carrier tables are pulled into L1); after the last batch of a
+    // tile the request wraps round to the first batch, which is what the next tile starts with.
+    uint4 v0n = make_uint4(0, 0, 0, 0), v1n = v0n, v2n = v0n, v3n = v0n;
+    // A warp whose tones fit one batch keeps their records in registers for the whole launch, and their tables in
+    // shared memory for as long as the same tones are static on the same carriers (sticky_sta / sticky_post).
+    const bool single = t_end - t_begin <= kBatch;
+    bool have_records = false;
     unsigned sticky_sta = 0u, sticky_post = 0xffffffffu;   // no tile has post bits outside its static bits
-    if (ROT && unit < n_tiles && t_begin + lane < t_end) fetch_core(lp.tab + t_begin + lane, core);
-
     while (unit < n_tiles) {
+        if (ROT && t_begin + lane < t_end && !(single && have_records)) fetch_tone(lp.tab + t_begin + lane, v0n, v1n, v2n, v3n);
+        have_records = true;
         const int64_t tile_base = (first_tile + unit) * kTile;
+        Acc16 acc[kBlocksPerTile];
         int n_mov = 0;
-        bool stored = false;
 
         if (ROT) {
-            // ---- angle-addition passes: tones static over the whole tile, then the batch's slow movers; the others
-            // are listed in ws.mov
-            TileAcc acc;
+            // ---- angle-addition pass: tones that are static over the whole tile; the others are listed in ws.mov
+            PQ pq[kBlocksPerTile];
 #pragma unroll
             for (int r = 0; r < kBlocksPerTile; ++r)
 #pragma unroll
-                for (int j = 0; j < kPairs; ++j) acc.pq[r][j] = make_float2(0.f, 0.f);
-            // stage batch 0 (its table copies are awaited below, under the staging of batch 1)
-            BatchInfo cur = stage_batch(lp, ws, ws.st, 0, t_begin, t_end, lane, tile_base, core, single, sticky_sta, sticky_post, n_mov);
-            if (single) {
-                sticky_sta = cur.m_sta;
-                sticky_post = cur.m_post;
-            } else if (t_begin + kBatch + lane < t_end) {
-                fetch_core(lp.tab + t_begin + kBatch + lane, core);
-            }
-            for (int b = 0; b < n_batches; ++b) {
-                StageRec *buf = ws.st + (b & 1) * kBatch;
-                BatchInfo nxt;
-                nxt.n_sta = 0; nxt.m_slow = nxt.m_sta = nxt.m_post = 0u;
-                if (b + 1 < n_batches) {
-                    // stage batch b + 1 into the other buffer (its previous readers finished before batch b - 1 ended)
-                    const int tb1 = t_begin + (b + 1) * kBatch;
-                    nxt = stage_batch(lp, ws, ws.st + ((b + 1) & 1) * kBatch, b + 1, tb1, t_end, lane, tile_base, core, false, 0u, 0u, n_mov);
-                    // request the batch after it: the next one of this tile, or batch 0 for the next tile
-                    const int tn = (b + 2 < n_batches) ? tb1 + kBatch + lane : t_begin + lane;
-                    if (tn < t_end) fetch_core(lp.tab + tn, core);
-                    cp_async_wait<1>();
-                } else {
-                    cp_async_wait<0>();
-                }
-                __syncwarp();
-                // ---- static loop.  Software pipeline, unrolled by two so that the sines/cosines ping-pong between two
-                // register sets: the phase -> I2FP -> FMUL2 -> MUFU chain of tone i+1 (XU and ALU pipes) is issued under
-                // the 64 FFMA2 of tone i.
-                if (cur.n_sta > 0) {
-                    const StageRec *sp = buf;
-                    const StageRec *const sp_end = buf + cur.n_sta;
-                    float4 T[kPairs / 2];
-                    load_table(T, sp);
-                    float2 a[kBlocksPerTile], a2[kBlocksPerTile];
-                    sincos4(*reinterpret_cast<const uint4 *>(sp), off, a);
-#pragma unroll 1
-                    for (; sp + 1 < sp_end; sp += 2) {
-                        sincos4(*reinterpret_cast<const uint4 *>(sp + 1), off, a2);
-                        tone_fma(acc, a, T, sp + 1);
-                        // slot i + 2 exists (kBatch + 2 slots per buffer pair); past the last tone it is stale and unused
-                        sincos4(*reinterpret_cast<const uint4 *>(sp + 2), off, a);
-                        tone_fma(acc, a2, T, sp + 2);
-                    }
-                    if (sp < sp_end) tone_fma(acc, a, T, sp + 1);
-                }
-                // ---- slow pass: the batch's slow movers, 16 at a time (two staged records per tone: the tone at the
-                // tile-centre frequency, and the first-order correction of its pair tables)
-                if (cur.m_slow != 0u) {
-                    sticky_sta = 0u;           // buf is overwritten: a single-batch warp restages its tables next tile
-                    sticky_post = 0xffffffffu;
-                    const int n_slow = __popc(cur.m_slow);
-                    uint4 pc = make_uint4(0, 0, 0, 0);
-                    float pA = 0.f;
-                    if (lane < n_slow) {
-                        const StageRec &sr = buf[kBatch - 1 - lane];
-                        pc = *reinterpret_cast<const uint4 *>(&sr);
-                        pA = sr.T[0].x;
-                    }
-                    const int mr0 = lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre, block 0
-                    float2 kf[2], kf2[2];
-                    kf[0] = make_float2(static_cast<float>(mr0) - 0.5f, static_cast<float>(mr0 + kBlock) - 0.5f);
-                    kf[1] = make_float2(static_cast<float>(mr0 + 2 * kBlock) - 0.5f, static_cast<float>(mr0 + 3 * kBlock) - 0.5f);
-                    kf2[0] = __fmul2_rn(kf[0], kf[0]);
-                    kf2[1] = __fmul2_rn(kf[1], kf[1]);
-#pragma unroll 1
-                    for (int h0 = 0; h0 < n_slow; h0 += 16) {
-                        __syncwarp();  // the readers of buf are done (and every lane holds its parked parameters)
-                        if (lane >= h0 && lane < min(n_slow, h0 + 16)) slow_records(buf + 2 * (lane - h0), pc, pA);
-                        __syncwarp();
-                        const int cnt = min(16, n_slow - h0);
-                        const StageRec *sp = buf;
-                        float4 T[kPairs / 2];
-                        load_table(T, sp);
-                        float2 a[kBlocksPerTile], a2[kBlocksPerTile];
-                        slow_chain(*reinterpret_cast<const uint4 *>(sp), mr0, kf, kf2, a, a2);
-#pragma unroll 1
-                        for (int i = 0; i < cnt; ++i, sp += 2) {
-                            tone_fma(acc, a, T, sp + 1);
-                            float2 an[kBlocksPerTile], a2n[kBlocksPerTile];
-                            slow_chain(*reinterpret_cast<const uint4 *>(sp + 2), mr0, kf, kf2, an, a2n);   // slot 2 cnt <= 32: stale past the end
-                            tone_fma(acc, a2, T, sp + 2);
-#pragma unroll
-                            for (int r = 0; r < kBlocksPerTile; ++r) { a[r] = an[r]; a2[r] = a2n[r]; }
+                for (int m = 0; m < kPairs / 2; ++m) pq[r].P[m] = pq[r].Q[m] = make_float2(0.f, 0.f);
+            const double tb_d = static_cast<double>(tile_base);
+            // phase reference: the centre of block 0, minus the half sample of the pair centring
+            const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
+            for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
+                const int t = tb + lane;
+                bool is_static = false, is_mover = false, is_post = false, is_slow = false;
+                uint32_t c0 = 0, c1 = 0, d = 0;
+                const float4 *tabp = nullptr;
+                if (t < t_end) {
+                    const ToneRec *tr = lp.tab + t;
+                    const uint4 v0 = v0n, v1 = v1n, v2 = v2n, v3 = v3n;
+                    uint64_t th = u64_of(v0.z, v0.w), w = u64_of(v1.x, v1.y);
+                    tabp = reinterpret_cast<const float4 *>(&tr->rot_pre);
+                    is_static = true;
+                    if ((static_cast<int32_t>(v0.y) & 0xff) != CLS_STATIC) {
+                        const double ua = (tb_d - f64_of(v2.z, v2.w)) - f64_of(v3.x, v3.y);  // u of the tile's first sample
+                        const double ub = ua + static_cast<double>(kTile - 1);
+                        if (ub <= 0.0) {
+                            // whole tile before the move: pre-move carrier
+                        } else if (ua >= f64_of(v3.z, v3.w)) {
+                            th = u64_of(v1.z, v1.w);
+                            w = u64_of(v2.x, v2.y);
+                            tabp = reinterpret_cast<const float4 *>(&tr->rot_post);
+                            is_post = true;
+                        } else if ((static_cast<int32_t>(v0.y) & CLS_SLOW_FLAG) && ua >= 0.0 && ub <= f64_of(v3.z, v3.w)) {
+                            // Slow mover, tile wholly inside the move: cubic Taylor expansion of the phase about the tile
+                            // centre (phase and frequency in u64 / fp64, curvature terms in fp32 radians); the record is
+                            // parked in ws.mrec (free during the static pass) until the slow pass of this batch.
+                            is_static = false;
+                            is_slow = true;
+                            const uint4 v4 = ldg16(reinterpret_cast<const char *>(tr) + 64);  // inv_Tn, DT
+                            const uint4 v5 = ldg16(reinterpret_cast<const char *>(tr) + 80);  // q1, q[0], q[1]
+                            const double sc = (ua + static_cast<double>(kTile / 2)) * f64_of(v4.x, v4.y);
+                            const float sf = static_cast<float>(sc);
+                            double g0, g1;
+                            float g2, g3;
+                            if (((static_cast<int32_t>(v0.y) >> 8) & 0xff) == AWG_PROFILE_LINEAR) {
+                                g0 = 0.5 * sc * sc; g1 = sc; g2 = 1.f; g3 = 0.f;
+                            } else {
+                                const double s2 = sc * sc;
+                                g0 = s2 * s2 * (2.5 + sc * (sc - 3.0));
+                                g1 = s2 * sc * (10.0 + sc * (6.0 * sc - 15.0));
+                                g2 = sf * sf * (30.f + sf * (30.f * sf - 60.f));
+                                g3 = sf * (60.f + sf * (120.f * sf - 180.f));
+                            }
+                            const uint64_t nc = static_cast<uint64_t>(tile_base + kTile / 2);
+                            const uint64_t wc = w + frac_to_fix64(f64_of(v5.x, v5.y) * g1);
+                            const uint64_t pc = th + w * nc + frac_to_fix64(f64_of(v4.z, v4.w) * g0);
+                            ws.mrec[lane].q[0] = make_float4(__uint_as_float(round32(pc - (wc >> 1))), __uint_as_float(round32(wc)),
+                                                             __uint_as_float(v5.z) * g2, __uint_as_float(v5.w) * g3);
+                            ws.mrec[lane].q[1] = make_float4(__uint_as_float(v0.x), 0.f, 0.f, 0.f);
+                        } else {
+                            is_static = false;
+                            is_mover = true;
+                            // the block owners re-centre this tone after the barrier: pull its record towards L1 now
+                            asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char *>(tr)));
+                            asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char *>(tr) + 96));
                         }
                     }
-                    __syncwarp();
+                    c0 = round32(th + w * a0 - (w >> 1));
+                    c1 = round32(w);
+                    d = round32(w * static_cast<uint64_t>(kBlock));
                 }
-                cur = nxt;
-            }
-            // ---- tiles without moving tones and one warp per tile: quantise and store straight from the registers
-            const int64_t n_thread = tile_base + lane * kSPT;
-            if (SPLIT == 1 && n_mov == 0) {
+                {
+                    const int tn = tb + kBatch + lane;
+                    if (tn < t_end) fetch_tone(lp.tab + tn, v0n, v1n, v2n, v3n);
+                }
+                const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
+                const unsigned m_sta = __ballot_sync(0xffffffffu, is_static);
+                const unsigned m_slow = __ballot_sync(0xffffffffu, is_slow);
+                if (lane == 0) ws.mov[b] = m_mov;
+                n_mov += __popc(m_mov);
+                const int n_sta = __popc(m_sta);
+                __syncwarp();  // the previous batch's readers are done
+                const unsigned m_post = __ballot_sync(0xffffffffu, is_post);
+                const bool tables_staged = single && m_sta == sticky_sta && m_post == sticky_post;
+                sticky_sta = m_sta;
+                sticky_post = m_post;
+                if (is_static) {
+                    StageRec &sr = ws.st[__popc(m_sta & lt)];
+                    *reinterpret_cast<uint4 *>(&sr) = make_uint4(c0, c1, d, 0u);
+                    if (!tables_staged) {
+                        const float4 C03 = __ldg(tabp), C47 = __ldg(tabp + 1), S03 = __ldg(tabp + 2), S47 = __ldg(tabp + 3);
+                        sr.C03 = C03; sr.C47 = C47; sr.S03 = S03; sr.S47 = S47;
+                    }
+                }
+                __syncwarp();
+                // Software pipeline, unrolled by two so that the sines/cosines ping-pong between two register sets:
+                // the phase -> I2FP -> FMUL2 -> MUFU chain of tone i+1 (XU and ALU pipes) is issued under the
+                // 32 FFMA2 of tone i.  Scalar fp32 instructions cost the FMA pipe as much as an FFMA2 (measured,
+                // profiles/), hence the packed range multiply and no register moves.
+                float sa[kBlocksPerTile], ca[kBlocksPerTile], sb[kBlocksPerTile], cb[kBlocksPerTile];
+                sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[0]), off, sa, ca);
+                // a running pointer keeps the loop free of index arithmetic (IMAD shares the FMA pipe)
+                const StageRec *sp = ws.st;
+                const StageRec *const sp_end = ws.st + n_sta;
+#pragma unroll 1
+                for (; sp + 1 < sp_end; sp += 2) {
+                    {
+                        const float4 C03 = sp[0].C03, C47 = sp[0].C47, S03 = sp[0].S03, S47 = sp[0].S47;
+                        sincos_tile(*reinterpret_cast<const uint4 *>(sp + 1), off, sb, cb);
 #pragma unroll
-                for (int r = 0; r < kBlocksPerTile; ++r) {
-                    float2 s[kPairs];
-                    block_samples(acc, r, s);
-                    store_direct(lp, qlo, qhi, n_thread + r * kBlock, s);
-                }
-                stored = true;
-            } else {
+                        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
+                    }
+                    {
+                        const float4 C03 = sp[1].C03, C47 = sp[1].C47, S03 = sp[1].S03, S47 = sp[1].S47;
+                        // slot i + 2 <= kBatch exists; past the last tone it is stale and its result unused
+                        sincos_tile(*reinterpret_cast<const uint4 *>(sp + 2), off, sa, ca);
 #pragma unroll
-                for (int r = 0; r < kBlocksPerTile; ++r) {
-                    float2 s[kPairs];
-                    block_samples(acc, r, s);
-                    park_store(ws, r, lane, s);
+                        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sb[r], cb[r], C03, C47, S03, S47);
+                    }
+                }
+                if (sp < sp_end) {
+                    const float4 C03 = sp[0].C03, C47 = sp[0].C47, S03 = sp[0].S03, S47 = sp[0].S47;
+#pragma unroll
+                    for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
+                }
+                // ---- slow pass: the batch's slow movers, 16 lanes at a time (two staged records per tone: the tone
+                // at the tile-centre frequency, and the first-order correction of its pair tables)
+                if (m_slow != 0u) {
+                    sticky_sta = 0u;           // ws.st is overwritten: a single-batch warp restages its tables next tile
+                    sticky_post = 0xffffffffu;
+#pragma unroll 1
+                    for (int half = 0; half < 2; ++half) {
+                        const unsigned mh = m_slow & (0xffffu << (16 * half));
+                        if (mh == 0u) continue;
+                        __syncwarp();  // the readers of ws.st are done
+                        if (is_slow && (lane >> 4) == half) stage_slow(ws.st + 2 * __popc(mh & lt), ws.mrec[lane]);
+                        __syncwarp();
+                        const int n_slow = __popc(mh);
+#pragma unroll 1
+                        for (int i = 0; i < n_slow; ++i) slow_pair(ws.st[2 * i], ws.st[2 * i + 1], lane, pq);
+                    }
                 }
             }
+#pragma unroll
+            for (int r = 0; r < kBlocksPerTile; ++r) acc[r] = pq_to_samples(pq[r]);
         } else {
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int left = t_end - tb;
@@ -960,30 +842,44 @@ __global__ void __launch_bounds__(kWarps * 32, 1) awg_synth_kernel(const LaunchP
             n_mov = max(t_end - t_begin, 0);
         }
 
-        if (!stored) {
-            // ---- the static partial sums and the lists of moving tones are in shared memory; after the team barrier
-            // warp `rank` owns the 512-sample blocks rank, rank + SPLIT, ...: it adds the team's partial sums in rank
-            // order, runs the MUFU pass of that block for the moving tones of EVERY warp of the team (so the moving
-            // tones load the team's warps evenly wherever they sit in the tone table), quantises and stores.
-            if (lane == 0) ws.n_mov = static_cast<uint32_t>(n_mov);
-            team_sync<SPLIT>(team);
-            WarpSmem *team_ws = ws_all + (warp - rank);
-            uint32_t any = 0;
+        const int64_t n_thread = tile_base + lane * kSPT;
+        if (SPLIT == 1 && ROT && n_mov == 0) {
 #pragma unroll
-            for (int r2 = 0; r2 < SPLIT; ++r2) any |= team_ws[r2].n_mov;
+            for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, acc[r]);
+            unit = next_unit<SPLIT>(lp, ws_all[warp - rank], team, rank, lane, n_teams);
+            continue;
+        }
+
+        // ---- the static partial sums and the lists of moving tones go to shared memory; after the team barrier
+        // warp `rank` owns the blocks rank, rank + SPLIT, ...: it adds the team's partial sums in rank order, runs
+        // the MUFU pass of that block for the moving tones of EVERY warp of the team (so the moving tones load the
+        // team's warps evenly wherever they sit in the tone table), quantises and stores.
+        if (ROT) {
+#pragma unroll
+            for (int r = 0; r < kBlocksPerTile; ++r) park_store(ws, r, lane, acc[r]);
+        }
+        if (lane == 0) ws.n_mov = static_cast<uint32_t>(n_mov);
+        team_sync<SPLIT>(team);
+        {
+            WarpSmem *team_ws = ws_all + (warp - rank);
 #pragma unroll 1
-            for (int mb = rank; mb < kMovBlocksPerTile; mb += SPLIT) {
-                const int64_t blk_base = tile_base + static_cast<int64_t>(mb) * kMovBlock;
-                if (blk_base >= n_end || blk_base + kMovBlock <= lp.n_begin) continue;
+            for (int r = rank; r < kBlocksPerTile; r += SPLIT) {
+                const int64_t blk_base = tile_base + static_cast<int64_t>(r) * kBlock;
+                if (blk_base >= n_end || blk_base + kBlock <= lp.n_begin) continue;
                 Acc16 sum;
 #pragma unroll
-                for (int j = 0; j < kMovPairs; ++j) sum.a[j] = make_float2(0.f, 0.f);
+                for (int j = 0; j < kPairs; ++j) sum.a[j] = make_float2(0.f, 0.f);
                 if (ROT) {
 #pragma unroll
-                    for (int r2 = 0; r2 < SPLIT; ++r2) park_add(team_ws[r2], mb, lane, sum);
+                    for (int r2 = 0; r2 < SPLIT; ++r2) park_add(team_ws[r2], r, lane, sum);
                 }
-                if (any) mover_block<SPLIT>(lp, ws, team_ws, per, blk_base, lane, sum);
-                store_block(lp, qlo, qhi, blk_base + lane * kMovSPT, sum);
+                {
+                    uint32_t any = 0;
+#pragma unroll
+                    for (int r2 = 0; r2 < SPLIT; ++r2) any |= team_ws[r2].n_mov;
+                    if (any) mover_block<SPLIT>(lp, ws, team_ws, per, blk_base, lane, sum);
+                }
+                store_block(lp, n_thread + r * kBlock, sum);
             }
         }
         // the closing barrier (the next tile's partial sums overwrite the park areas) also publishes the next tile
@@ -1039,7 +935,7 @@ __global__ void __launch_bounds__(256) awg_fp64_kernel(const LaunchParams lp)
 }
 
 // Trajectory-table build on the device (hot-path step a0): one warp per tone record.  Copies the 128-byte core the
-// host computed and builds the pair tables of the two carriers, (C_j, S_j) = A (cos, sin)(2 pi (j + 1/2) w): the angle
+// host computed and builds the tables of the two carriers, C_j, S_j = A cos, A sin(2 pi (j + 1/2) w): the angle
 // (j + 1/2) w is exact in 64-bit fixed-point turns, cosine and sine are evaluated in fp64 and rounded once to fp32.
 __global__ void __launch_bounds__(128) awg_expand_kernel(ToneRec *table, const ToneCore *src, const int32_t *idx, int n)
 {
@@ -1049,27 +945,31 @@ __global__ void __launch_bounds__(128) awg_expand_kernel(ToneRec *table, const T
     const ToneCore &c = src[j];
     ToneRec &dst = table[idx ? idx[j] : j];
     if (lane < 8) reinterpret_cast<uint4 *>(&dst.core)[lane] = reinterpret_cast<const uint4 *>(&c)[lane];
-    const int state = lane >> 4, p = lane & 15;
+    if (lane >= 2 * kPairs) {
+        if (lane < 2 * kPairs + 8) (lane < 2 * kPairs + 4 ? dst.rot_pre : dst.rot_post).pad_[lane & 3] = 0.f;
+        return;
+    }
+    const int state = lane / kPairs, p = lane % kPairs;
     const uint64_t w = state ? c.w_post : c.w_pre;
     const uint64_t ang = w * static_cast<uint64_t>(p) + (w >> 1);              // (p + 1/2) w, turns * 2^64 (wraps exactly)
     const double turns = static_cast<double>(static_cast<int64_t>(ang)) * (1.0 / kTwo64);   // [-1/2, 1/2)
     double sn, cs;
     sincospi(2.0 * turns, &sn, &cs);
     const double A = static_cast<double>(c.A);
-    PairTable &tab = state ? dst.tab_post : dst.tab_pre;
-    tab.cs[p] = make_float2(static_cast<float>(A * cs), static_cast<float>(A * sn));
+    RotTable &tab = state ? dst.rot_post : dst.rot_pre;
+    tab.C[p] = static_cast<float>(A * cs);
+    tab.S[p] = static_cast<float>(A * sn);
 }
 
 // ---- launch state, per device ------------------------------------------------------------------------------------
-// Tile-scheduler slots: kSchedSlots pairs of counters per device, zeroed once; every launch takes the next slot and its
-// last team zeroes it again.  Each slot carries an event recorded behind the launch that used it: the launch that takes
-// the slot next waits on that event in its own stream, so two grids never share a counter, whatever the streams do.
+// Tile-scheduler slots: pairs of counters, zeroed once; the last team of a launch zeroes its slot again.  A slot belongs
+// to ONE stream (keyed by the stream's unique id): launches of a stream run one after the other, so a slot is clean when
+// the next launch of its stream starts, and launches that can overlap (different streams) never share a counter.
 constexpr int kSchedSlots = 1024;
 constexpr int kMaxDevices = 64;
 struct DeviceState {
     uint32_t *sched = nullptr;
-    cudaEvent_t ev[kSchedSlots] = {};
-    uint32_t next = 0;
+    std::unordered_map<unsigned long long, uint32_t> slot_of;   // stream id -> slot
     int n_sm = 0;
     uint32_t configured = 0;   // bit per kernel instantiation: dynamic shared memory opt-in done on this device
 };
@@ -1101,32 +1001,32 @@ cudaError_t device_state(DeviceState **out)
 }
 
 template <int SPLIT, bool ROT>
-cudaError_t launch_one(DeviceState &ds, const LaunchParams &lp, float qlo, float qhi, int64_t tiles, cudaStream_t stream)
+cudaError_t launch_one(DeviceState &ds, const LaunchParams &lp, int64_t tiles, cudaStream_t stream)
 {
     constexpr int kTeams = kWarps / SPLIT;
     constexpr size_t kSmem = sizeof(WarpSmem) * kWarps;
-    constexpr uint32_t kBit = 1u << ((SPLIT == 1 ? 0 : SPLIT == 2 ? 1 : SPLIT == 4 ? 2 : 3) * 2 + (ROT ? 1 : 0));
+    constexpr uint32_t kBit = 1u << ((SPLIT == 1 ? 0 : SPLIT == 2 ? 1 : 2) * 2 + (ROT ? 1 : 0));
     if (!(ds.configured & kBit)) {
         cudaError_t e = cudaFuncSetAttribute(awg_synth_kernel<SPLIT, ROT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              static_cast<int>(kSmem));
         if (e != cudaSuccess) return e;
         ds.configured |= kBit;
     }
-    // persistent grid: one CTA per SM, fewer when the launch has fewer tiles than teams
+    // persistent grid: kCtasPerSm CTAs per SM, fewer when the launch has fewer tiles than teams
     const int64_t want = (tiles + kTeams - 1) / kTeams;
-    const unsigned grid = static_cast<unsigned>(want < ds.n_sm ? want : ds.n_sm);
-    awg_synth_kernel<SPLIT, ROT><<<grid, kWarps * 32, kSmem, stream>>>(lp, qlo, qhi);
+    const int64_t max_grid = static_cast<int64_t>(kCtasPerSm) * ds.n_sm;
+    const unsigned grid = static_cast<unsigned>(want < max_grid ? want : max_grid);
+    awg_synth_kernel<SPLIT, ROT><<<grid, kWarps * 32, kSmem, stream>>>(lp);
     return cudaGetLastError();
 }
 
 template <bool ROT>
-cudaError_t launch_split(DeviceState &ds, const LaunchParams &lp, float qlo, float qhi, int split, int64_t tiles, cudaStream_t stream)
+cudaError_t launch_split(DeviceState &ds, const LaunchParams &lp, int split, int64_t tiles, cudaStream_t stream)
 {
     switch (split) {
-        case 1: return launch_one<1, ROT>(ds, lp, qlo, qhi, tiles, stream);
-        case 2: return launch_one<2, ROT>(ds, lp, qlo, qhi, tiles, stream);
-        case 4: return launch_one<4, ROT>(ds, lp, qlo, qhi, tiles, stream);
-        default: return launch_one<kWarps, ROT>(ds, lp, qlo, qhi, tiles, stream);
+        case 1: return launch_one<1, ROT>(ds, lp, tiles, stream);
+        case 2: return launch_one<2, ROT>(ds, lp, tiles, stream);
+        default: return launch_one<kWarps, ROT>(ds, lp, tiles, stream);
     }
 }
 
@@ -1153,25 +1053,31 @@ cudaError_t launch_synth(const LaunchParams &lp_in, int engine, cudaStream_t str
         const int64_t first_tile = lp.n_begin / kTile;
         const int64_t last_tile = (lp.n_begin + lp.n_count - 1) / kTile;
         const int64_t tiles = last_tile - first_tile + 1;
-        // one launch at a time takes a slot, launches and records the slot's event (the kernel launch is asynchronous)
+        // one launch at a time looks up its stream's slot and launches (the kernel launch is asynchronous)
         std::lock_guard<std::mutex> lock(g_dev_mutex);
         DeviceState *ds = nullptr;
         if ((e = device_state(&ds)) != cudaSuccess) return e;
-        const uint32_t slot = ds->next++ % kSchedSlots;
-        if (ds->ev[slot]) {
-            if ((e = cudaStreamWaitEvent(stream, ds->ev[slot], 0)) != cudaSuccess) return e;
-        } else if ((e = cudaEventCreateWithFlags(&ds->ev[slot], cudaEventDisableTiming)) != cudaSuccess) {
-            return e;
+        unsigned long long sid = 0;
+        if (cudaStreamGetId(stream, &sid) != cudaSuccess) {
+            (void)cudaGetLastError();
+            sid = ~static_cast<unsigned long long>(reinterpret_cast<uintptr_t>(stream));   // no id: key on the handle
         }
-        lp.sched = ds->sched + 8 * slot;
+        auto it = ds->slot_of.find(sid);
+        if (it == ds->slot_of.end()) {
+            if (ds->slot_of.size() >= static_cast<size_t>(kSchedSlots)) {
+                // more streams than slots: wait for everything in flight (every slot is clean then) and start over
+                if ((e = cudaDeviceSynchronize()) != cudaSuccess) return e;
+                ds->slot_of.clear();
+            }
+            it = ds->slot_of.emplace(sid, static_cast<uint32_t>(ds->slot_of.size())).first;
+        }
+        lp.sched = ds->sched + 8 * it->second;
         // clamp bounds of the quantiser in units of V: scale*qlo and scale*qhi round to -32768 and 32767
-        const float qlo = static_cast<float>(-32768.0 / static_cast<double>(lp.scale));
-        const float qhi = static_cast<float>(32767.0 / static_cast<double>(lp.scale));
+        lp.qlo = static_cast<float>(-32768.0 / static_cast<double>(lp.scale));
+        lp.qhi = static_cast<float>(32767.0 / static_cast<double>(lp.scale));
         const int split = split_for(lp.n_tones);
-        e = (engine == AWG_ENGINE_FMA) ? launch_split<true>(*ds, lp, qlo, qhi, split, tiles, stream)
-                                       : launch_split<false>(*ds, lp, qlo, qhi, split, tiles, stream);
-        if (e != cudaSuccess) return e;
-        e = cudaEventRecord(ds->ev[slot], stream);
+        e = (engine == AWG_ENGINE_FMA) ? launch_split<true>(*ds, lp, split, tiles, stream)
+                                       : launch_split<false>(*ds, lp, split, tiles, stream);
     }
     count_launch();
     return e;

@@ -39,7 +39,7 @@ awg_status fail_cuda(cudaError_t e, const char *what)
 namespace {
 
 const long double kTwoPiL = 6.283185307179586476925286766559005768L;
-constexpr int kRadius = kMovBlock / 2;  // half of the MUFU pass's 512-sample block (span of one Taylor re-centring)
+constexpr int kRadius = kBlock / 2;  // half of the 512-sample block (span of one Taylor re-centring)
 
 // frac(x) as 64-bit fixed-point turns.
 uint64_t frac64(long double x)
