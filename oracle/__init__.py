@@ -11,6 +11,8 @@ from .awg_oracle import (  # noqa: F401
     OraclePlan,
     Segment,
     plan_from_workload,
+    snap_frequency,
+    mux_channels,
     segment_phase,
     segment_freq,
 )

@@ -31,9 +31,23 @@ What it computes (paper citations are PAPER.md:<line>):
 * Per-chunk updates (streaming pathway, Fig. 7): at the first sample of chunk c a
   tone starts a new move from its current instantaneous frequency and phase (reading G12).
 
-Every function here is pinned by ``tests/test_oracle_pins.py`` against values the
-paper and the mathematics fix (closed forms, FFT bins, numerical integration of
-the frequency profile, 50-digit arithmetic); nothing is "parity unpinned".
+* Four-channel multiplexed output (the paper's WM kernel, Fig. 4): the codes of the
+  channels' independent tone sets interleaved "in groups of four", ``out[4 i + c] = code_c[i]``
+  (``mux_channels``).
+* Static-buffer pathway (section IV A/B): Eq. 6 frequency snapping (PAPER.md:95-98, ``snap_frequency``);
+  the looped buffer ``X_static[i mod L_s]`` of Eq. 7-8 (``static_buffer``); Eq. 9 with
+  only the other tones evaluated per sample (``waveform_static_pathway``); and the hand-back
+  of Eq. 10 branch 3: after ``L_d`` a moved tone is a looped static wavetable at its
+  final frequency with the phase offset theta' (``handback_theta``, ``fold_into_static_buffer``).
+* Time-varying amplitude ``a_j[i]`` (Eq. 9; constant in the paper's worked case):
+  per tone ``a(t) = A0`` before ``t_a``, ``A0 + (A1 - A0) h((t - t_a)/T_a)`` during the ramp and ``A1`` after,
+  with ``h(s) = s`` (LINEAR) or the minimum-jerk ramp ``10 s^3 - 15 s^4 + 6 s^5`` (MINJERK) -- reading G19 in
+  DESIGN.md: the paper allows ``a_j[i]`` without giving a profile; the frequency ramp's profile is reused
+  (``set_amplitude_ramps``).
+
+Every function here is pinned by ``tests/test_oracle_pins.py`` / ``tests/test_oracle_pins_next.py`` against
+values the paper and the mathematics fix (closed forms, FFT bins, numerical integration of the frequency
+profile, 50-digit arithmetic); nothing is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -135,6 +149,7 @@ class OraclePlan:
         self.scale = float(scale)
         self.A = np.zeros(n_tones)
         self.segments: List[List[Segment]] = [[] for _ in range(n_tones)]
+        self.amp_ramps = None  # (A1, t_a, T_a, profile) arrays once set_amplitude_ramps has been called
 
     # ---- trajectory table -------------------------------------------------------------
     def set_trajectories(self, f0, f1, A, phi0, t_start, t_dur, profile) -> None:
@@ -147,11 +162,46 @@ class OraclePlan:
         if not all(np.all(np.isfinite(a)) for a in arrs) or np.any(t_dur < 0):
             raise ValueError("non-finite input or negative duration")
         self.A = A.copy()
+        self.amp_ramps = None
         self.segments = []
         for k in range(N):
             theta = LD(phi0[k]) / TWO_PI_LD  # radians -> cycles (theta_j of Eq. 8/9)
             self.segments.append([Segment(None, LD(t_start[k]), LD(t_dur[k]), LD(f0[k]), LD(f1[k]),
                                           int(prof[k]), theta)])
+
+    def set_amplitude_ramps(self, A1, t_start, t_dur, profile) -> None:
+        """Time-varying amplitude a_j[i] of Eq. 9: tone k goes from the amplitude given to
+        ``set_trajectories`` to ``A1[k]`` over ``[t_start[k], t_start[k] + t_dur[k]]`` along ``profile[k]``
+        (STATIC = constant amplitude, LINEAR, or MINJERK = 10 s^3 - 15 s^4 + 6 s^5; reading G19)."""
+        N = self.n_tones
+        A1, ts, T = (np.asarray(a, dtype=np.float64) for a in (A1, t_start, t_dur))
+        prof = np.asarray(profile, dtype=np.int64)
+        if A1.shape != (N,) or ts.shape != (N,) or T.shape != (N,) or prof.shape != (N,):
+            raise ValueError("arrays must have length n_tones")
+        if not (np.all(np.isfinite(A1)) and np.all(np.isfinite(ts)) and np.all(np.isfinite(T))) or np.any(T < 0):
+            raise ValueError("non-finite input or negative duration")
+        if np.any((prof < PROFILE_STATIC) | (prof > PROFILE_MINJERK)):
+            raise ValueError("unknown profile")
+        self.amp_ramps = (A1.copy(), ts.copy(), T.copy(), prof.copy())
+
+    def amplitude(self, k: int, n) -> np.ndarray:
+        """a_k at absolute sample indices ``n`` (float64)."""
+        n = np.asarray(n, dtype=np.int64)
+        A0 = float(self.A[k])
+        if self.amp_ramps is None or int(self.amp_ramps[3][k]) == PROFILE_STATIC:
+            return np.full(n.shape, A0)
+        A1, ts, T, prof = (x[k] for x in self.amp_ramps)
+        t = n.astype(LD) / self.fs
+        tau = t - LD(ts)
+        if T > 0:
+            sfrac = np.clip((tau / LD(T)).astype(np.float64), 0.0, 1.0)
+        else:
+            sfrac = (tau >= 0).astype(np.float64)
+        if int(prof) == PROFILE_LINEAR:
+            h = sfrac
+        else:
+            h = sfrac ** 3 * (10.0 + sfrac * (6.0 * sfrac - 15.0))
+        return A0 + (float(A1) - A0) * h
 
     def update_trajectories(self, chunk_idx: int, tone_idx, f1, t_dur, profile) -> None:
         """At the first sample of ``chunk_idx`` each listed tone starts a new move from its
@@ -215,8 +265,56 @@ class OraclePlan:
             for seg, a, b in self._pieces(k, n0, n1):
                 t = np.arange(a, b, dtype=np.int64).astype(LD) / self.fs
                 turns = _frac(segment_phase(seg, t)).astype(np.float64)
-                V[a - n0:b - n0] += self.A[k] * np.sin(TWO_PI * turns)
+                if self.amp_ramps is None:
+                    V[a - n0:b - n0] += self.A[k] * np.sin(TWO_PI * turns)
+                else:
+                    V[a - n0:b - n0] += self.amplitude(k, np.arange(a, b, dtype=np.int64)) * np.sin(TWO_PI * turns)
         return V
+
+    # ---- static-buffer pathway (section IV A/B) ----------------------------------------------
+    def static_buffer(self, tones: Sequence[int], L_s: Optional[int] = None) -> np.ndarray:
+        """X_static[i], i in [0, L_s): sum over the listed tones of a_j sin(2 pi f_j/fs i + theta_j), Eq. 7-8
+        (PAPER.md:102-105).  The tones must be STATIC first segments; L_s defaults to chunk_len."""
+        L = self.chunk_len if L_s is None else int(L_s)
+        X = np.zeros(L, dtype=np.float64)
+        i = np.arange(L, dtype=np.int64).astype(LD)
+        for k in tones:
+            seg = self.segments[int(k)][0]
+            if seg.profile != PROFILE_STATIC or len(self.segments[int(k)]) != 1:
+                raise ValueError("the static buffer holds static tones only")
+            turns = _frac(seg.theta + seg.f0 / self.fs * i).astype(np.float64)
+            X += self.A[int(k)] * np.sin(TWO_PI * turns)
+        return X
+
+    def waveform_static_pathway(self, n0: int, n1: int, X_static: np.ndarray, dynamic_tones: Sequence[int]) -> np.ndarray:
+        """V[i] = X_static[i mod L_s] + sum over the dynamic tones of a_j[i] sin(phi_j[i] + theta_j), Eq. 9."""
+        L = X_static.shape[0]
+        idx = np.arange(n0, n1, dtype=np.int64) % L
+        return X_static[idx] + self.waveform(n0, n1, tones=list(dynamic_tones))
+
+    def handback_theta(self, k: int, L_d: int) -> LD:
+        """theta'_j of Eq. 10 in cycles, reduced mod 1: the phase of tone k at sample L_d, which
+        becomes the phase offset of its looped static wavetable for i > L_d (Eq. 10 branch 3)."""
+        return _frac(self.phase(k, np.array([L_d], dtype=np.int64))[0])
+
+    def fold_into_static_buffer(self, X_static: np.ndarray, tones: Sequence[int], L_d: int) -> np.ndarray:
+        """Eq. 10 branch 3: after L_d each listed tone is a static wavetable at its final frequency,
+        a_j sin(2 pi f_finish/fs (i mod L_s) + theta'_j), added to the looped buffer.  L_d must be a multiple of L_s
+         and the tone's move must have ended by L_d."""
+        L = X_static.shape[0]
+        if L_d % L:
+            raise ValueError("L_d must be a positive integer multiple of L_s (PAPER.md:135)")
+        X = X_static.copy()
+        i = np.arange(L, dtype=np.int64).astype(LD)
+        t_d = LD(L_d) / self.fs
+        for k in tones:
+            seg = self.segments[int(k)][-1]
+            if seg.profile != PROFILE_STATIC and not (t_d - seg.t_s >= seg.T):
+                raise ValueError("the tone is still moving at L_d")
+            f_fin = seg.f0 if seg.profile == PROFILE_STATIC else seg.f1
+            turns = _frac(self.handback_theta(int(k), L_d) + f_fin / self.fs * i).astype(np.float64)
+            X += float(self.amplitude(int(k), np.array([L_d]))[0]) * np.sin(TWO_PI * turns)
+        return X
 
     def quantise(self, V: np.ndarray) -> np.ndarray:
         """int16 DAC codes: rint (half-to-even) of scale*V, saturated (G9)."""
@@ -247,6 +345,23 @@ class OraclePlan:
             reals[:, i] = (s.t_s, s.T, s.f0, s.f1, s.theta)
         prof = np.array([s.profile for s in rows], dtype=np.int32)
         return off, n_begin, np.ascontiguousarray(reals), prof
+
+
+def snap_frequency(f0: float, sample_rate: float, L_s: int) -> float:
+    """Eq. 6: f_j = nint(f0 L_s / fs) fs / L_s, the closest frequency with a whole number of
+    cycles in L_s samples (error below fs / (2 L_s); the paper quotes the grid spacing, "less than 534 Hz")."""
+    j = np.rint(LD(f0) * LD(L_s) / LD(sample_rate))
+    return float(j * LD(sample_rate) / LD(L_s))
+
+
+def mux_channels(plans: Sequence["OraclePlan"], n0: int, n1: int) -> np.ndarray:
+    """The paper's Wavetable Multiplexer (Fig. 4; chunk layout PAPER.md:77): the int16 codes of the
+    channels' waveforms "read sequentially in groups of four": out[C i + c] = code_c[n0 + i] for C channels."""
+    C = len(plans)
+    out = np.empty((n1 - n0) * C, dtype=np.int16)
+    for c, p in enumerate(plans):
+        out[c::C] = p.codes(n0, n1)
+    return out
 
 
 def plan_from_workload(w, apply_updates_upto: Optional[int] = None) -> OraclePlan:

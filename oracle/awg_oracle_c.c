@@ -15,7 +15,9 @@
  *   MINJERK 0<tau<T    :  Phi = theta + f0 t + D T (5/2 s^4 - 3 s^5 + s^6) Eq. 10 / p(i), PAPER.md:141-148,
  *                                                                          prefactor corrected to T (G1)
  *   tau >= T           :  Phi = theta + f0 t_s + f1 tau + T (f0 - f1)/2    Eq. 10 branch 2
- *   V[n] = sum_k A_k sin(2 pi frac(Phi_k[n]))                              Eq. 9, Eq. 14
+ *   V[n] = sum_k a_k[n] sin(2 pi frac(Phi_k[n]))                           Eq. 9, Eq. 14
+ *   a_k[n] = A_k, or with an amplitude ramp (awg_oracle_waveform_amp; Eq. 9 allows a_j[i], reading G19 in DESIGN.md):
+ *            A_k before t_a, A_k + (A1_k - A_k) h((t - t_a)/T_a) during it, A1_k after; h(s) = s or 10 s^3 - 15 s^4 + 6 s^5
  *   code = clamp(rint(scale V), -32768, 32767)                             PAPER.md:77, 196; G9
  *
  * Segment table layout (built by OraclePlan.flat_segments): tone k owns segments
@@ -53,13 +55,32 @@ static long double seg_phase(long double t, long double t_s, long double T, long
     return theta + f0 * t + (f1 - f0) * T * g;
 }
 
-/* V_out[n - n0] for n in [n0, n1).  Returns 0, or -1 on bad arguments. */
-int awg_oracle_waveform(int32_t n_tones, double fs, const int64_t *seg_off, const int64_t *seg_n_begin,
-                        const long double *reals, int64_t n_segs, const int32_t *profile,
-                        const double *A, int64_t n0, int64_t n1, double *V_out, int32_t n_threads)
+static double amp_at(long double t, double A0, double A1, double t_a, double T_a, int prof)
+{
+    if (prof == AWG_STATIC) return A0;
+    long double tau = t - (long double)t_a;
+    double s;
+    if (T_a > 0.0) {
+        s = (double)(tau / (long double)T_a);
+        if (s < 0.0) s = 0.0;
+        if (s > 1.0) s = 1.0;
+    } else {
+        s = tau >= 0.0L ? 1.0 : 0.0;
+    }
+    double h = prof == AWG_LINEAR ? s : s * s * s * (10.0 + s * (6.0 * s - 15.0));
+    return A0 + (A1 - A0) * h;
+}
+
+/* V_out[n - n0] for n in [n0, n1), with optional amplitude ramps (amp_A1 == NULL: constant amplitudes).
+ * Returns 0, or -1 on bad arguments. */
+int awg_oracle_waveform_amp(int32_t n_tones, double fs, const int64_t *seg_off, const int64_t *seg_n_begin,
+                            const long double *reals, int64_t n_segs, const int32_t *profile,
+                            const double *A, const double *amp_A1, const double *amp_ts, const double *amp_T,
+                            const int32_t *amp_prof, int64_t n0, int64_t n1, double *V_out, int32_t n_threads)
 {
     if (n_tones < 1 || !(fs > 0.0) || !seg_off || !seg_n_begin || !reals || !profile || !A || !V_out || n1 < n0)
         return -1;
+    if (amp_A1 && (!amp_ts || !amp_T || !amp_prof)) return -1;
     const long double *t_s = reals, *T = reals + n_segs, *f0 = reals + 2 * n_segs,
                       *f1 = reals + 3 * n_segs, *theta = reals + 4 * n_segs;
     const long double fsl = (long double)fs;
@@ -82,11 +103,20 @@ int awg_oracle_waveform(int32_t n_tones, double fs, const int64_t *seg_off, cons
             }
             long double ph = seg_phase(t, t_s[lo], T[lo], f0[lo], f1[lo], theta[lo], profile[lo]);
             long double fr = ph - floorl(ph);
-            v += A[k] * sin(two_pi * (double)fr);
+            double a = amp_A1 ? amp_at(t, A[k], amp_A1[k], amp_ts[k], amp_T[k], amp_prof[k]) : A[k];
+            v += a * sin(two_pi * (double)fr);
         }
         V_out[n - n0] = v;
     }
     return 0;
+}
+
+int awg_oracle_waveform(int32_t n_tones, double fs, const int64_t *seg_off, const int64_t *seg_n_begin,
+                        const long double *reals, int64_t n_segs, const int32_t *profile,
+                        const double *A, int64_t n0, int64_t n1, double *V_out, int32_t n_threads)
+{
+    return awg_oracle_waveform_amp(n_tones, fs, seg_off, seg_n_begin, reals, n_segs, profile, A, NULL, NULL, NULL, NULL,
+                                   n0, n1, V_out, n_threads);
 }
 
 int awg_oracle_quantise(const double *V, int64_t n, double scale, int16_t *out)

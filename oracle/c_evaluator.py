@@ -39,6 +39,11 @@ def _load():
             ctypes.c_int32, ctypes.c_double, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
             ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64,
             ctypes.c_void_p, ctypes.c_int32]
+        lib.awg_oracle_waveform_amp.restype = ctypes.c_int
+        lib.awg_oracle_waveform_amp.argtypes = [
+            ctypes.c_int32, ctypes.c_double, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int32]
         lib.awg_oracle_quantise.restype = ctypes.c_int
         lib.awg_oracle_quantise.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p]
         lib.awg_oracle_num_threads.restype = ctypes.c_int
@@ -58,9 +63,18 @@ def c_waveform(plan, n0: int, n1: int, n_threads: int = 0) -> np.ndarray:
     off, n_begin, reals, prof = plan.flat_segments()
     A = np.ascontiguousarray(plan.A, dtype=np.float64)
     V = np.empty(n1 - n0, dtype=np.float64)
-    rc = lib.awg_oracle_waveform(plan.n_tones, float(plan.fs), off.ctypes.data, n_begin.ctypes.data,
-                                 reals.ctypes.data, reals.shape[1], prof.ctypes.data, A.ctypes.data,
-                                 n0, n1, V.ctypes.data, n_threads)
+    ramps = getattr(plan, "amp_ramps", None)
+    if ramps is None:
+        rc = lib.awg_oracle_waveform(plan.n_tones, float(plan.fs), off.ctypes.data, n_begin.ctypes.data,
+                                     reals.ctypes.data, reals.shape[1], prof.ctypes.data, A.ctypes.data,
+                                     n0, n1, V.ctypes.data, n_threads)
+    else:
+        A1, ts, T = (np.ascontiguousarray(x, dtype=np.float64) for x in ramps[:3])
+        ap = np.ascontiguousarray(ramps[3], dtype=np.int32)
+        rc = lib.awg_oracle_waveform_amp(plan.n_tones, float(plan.fs), off.ctypes.data, n_begin.ctypes.data,
+                                         reals.ctypes.data, reals.shape[1], prof.ctypes.data, A.ctypes.data,
+                                         A1.ctypes.data, ts.ctypes.data, T.ctypes.data, ap.ctypes.data,
+                                         n0, n1, V.ctypes.data, n_threads)
     if rc != 0:
         raise RuntimeError("awg_oracle_waveform failed")
     return V
