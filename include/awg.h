@@ -133,6 +133,48 @@ awg_status awg_synthesize_range(awg_plan *p, int64_t first_chunk, int64_t n_chun
  * host_out is complete.  Stands in for the paper's pinned-buffer -> DAC transfer. */
 awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *host_out);
 
+/* ---- four-channel multiplexed output (the paper's WM kernel; Fig. 4) ---------- */
+
+/* The paper's streaming chunk is 2^20 samples = 4 DAC channels x 2^18, "read sequentially in groups of
+ * four".  plans: host array of n_channels (1..8) distinct plans on the current device with
+ * the same chunk_len, one independent tone set per channel.  Writes n_channels*chunk_len int16 to dev_out
+ * (device, 16-byte aligned): dev_out[n_channels*i + c] = code of sample chunk_idx*chunk_len + i of
+ * channel c -- bit for bit what awg_synthesize_chunk gives for plans[c].  One kernel launch per channel
+ * on `stream`, each storing its channel's half-words of every group.  Errors: those of
+ * awg_synthesize_chunk for any channel, checked before the first launch; INVALID_ARG (NULL, n_channels,
+ * chunk_len mismatch, repeated plan). */
+awg_status awg_synthesize_chunk_mux(awg_plan *const *plans, int32_t n_channels, int64_t chunk_idx,
+                                    int16_t *dev_out, void *stream);
+
+/* ---- static-buffer pathway (PAPER.md:93-109 section IV A, Eq. 6-8; :133 Eq. 9; :141-146 Eq. 10) -- */
+
+/* Eq. 6: the closest frequency with a whole number of cycles in L_s samples,
+ * f_j = nint(f0 L_s / fs) fs / L_s.  Host-only.  Errors: INVALID_ARG. */
+awg_status awg_snap_frequency(double f0_hz, double sample_rate_hz, int64_t L_s, double *f_snapped_hz);
+
+/* Moves the listed tones (host array of n_static tone indices) out of the per-sample evaluation into the
+ * looped buffer X_static of length L_s = chunk_len (Eq. 7-8): X_static[i] = sum_j a_j sin(2 pi f_j/fs i
+ * + theta_j) is synthesised once on the device (fp32), and every later synthesis call computes
+ * V[n] = X_static[n mod L_s] + (the other tones, evaluated per sample) -- Eq. 9.  The
+ * listed tones must be static and on the fs/L_s grid of Eq. 6 (then the result equals evaluating them
+ * per sample); chunk_len must be >= 2048.  Replaces any earlier buffer; n_static = 0 removes it.
+ * Synchronous on `stream`.  Errors: INVALID_ARG (index out of range or repeated, tone not static or
+ * off the grid, chunk_len too small), STATE (no table set), ALLOC, CUDA. */
+awg_status awg_static_buffer_set(awg_plan *p, int32_t n_static, const int32_t *tone_idx, void *stream);
+
+/* Hand-back of Eq. 10 branch 3: from chunk_idx on (L_d = chunk_idx*chunk_len, a
+ * multiple of L_s) each listed tone is a looped static wavetable at its final frequency
+ * with the phase offset theta'_j = its phase at L_d; its period is added to X_static and the tone leaves
+ * the per-sample evaluation.  Each tone's move must have ended by L_d and its final frequency must be on
+ * the Eq. 6 grid.  Like a trajectory update, this fixes the past: chunks before chunk_idx can no longer
+ * be synthesised.  Synchronous on `stream`.  Errors: INVALID_ARG, STATE (still moving at L_d, already in
+ * the buffer, chunk_idx before the latest update), ALLOC, CUDA. */
+awg_status awg_static_buffer_fold(awg_plan *p, int64_t chunk_idx, int32_t n_fold, const int32_t *tone_idx,
+                                  void *stream);
+
+/* Copies X_static (chunk_len floats, full scale = 1.0) to dev_out (device).  Errors: STATE (no buffer). */
+awg_status awg_static_buffer_read(awg_plan *p, float *dev_out, void *stream);
+
 /* ---- streaming ring (DAC-FIFO stand-in; Fig. 2b, 75, 127) --------------------------- */
 
 /* n_slots >= 2 device slots of chunk_len int16; host_mirror != 0 adds pinned-host slots and a copy

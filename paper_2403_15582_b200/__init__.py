@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     AwgError,
     Plan,
     Ring,
+    synthesize_chunk_mux,
     EXPORTED,
     LIB_PATH,
 )

@@ -37,6 +37,8 @@ EXPORTED = (
     "awg_plan_create", "awg_plan_destroy", "awg_set_scale", "awg_set_engine", "awg_set_trajectories",
     "awg_update_trajectories", "awg_synthesize_chunk", "awg_synthesize_chunk_f32", "awg_synthesize_range",
     "awg_synthesize_range_host", "awg_ring_create", "awg_ring_submit", "awg_ring_acquire", "awg_ring_release",
+    "awg_synthesize_chunk_mux", "awg_snap_frequency", "awg_static_buffer_set", "awg_static_buffer_fold",
+    "awg_static_buffer_read",
     "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_plan_op_counts", "awg_kernel_launch_count",
     "awg_last_error",
 )
@@ -60,6 +62,11 @@ def _load() -> ctypes.CDLL:
         "awg_synthesize_chunk_f32": (I32, [P, I64, P, P]),
         "awg_synthesize_range": (I32, [P, I64, I64, P, P]),
         "awg_synthesize_range_host": (I32, [P, I64, I64, P]),
+        "awg_synthesize_chunk_mux": (I32, [POINTER(P), I32, I64, P, P]),
+        "awg_snap_frequency": (I32, [D, D, I64, POINTER(D)]),
+        "awg_static_buffer_set": (I32, [P, I32, P, P]),
+        "awg_static_buffer_fold": (I32, [P, I64, I32, P, P]),
+        "awg_static_buffer_read": (I32, [P, P, P]),
         "awg_ring_create": (I32, [POINTER(P), P, I32, I32]),
         "awg_ring_submit": (I32, [P, I64, I32, P, P, P, P]),
         "awg_ring_acquire": (I32, [P, POINTER(I64), POINTER(P), POINTER(P)]),
@@ -171,6 +178,31 @@ def awg_synthesize_range(plan, first_chunk: int, n_chunks: int, dev_out_ptr: int
 
 def awg_synthesize_range_host(plan, first_chunk: int, n_chunks: int, host_out_ptr: int) -> None:
     _check(_lib.awg_synthesize_range_host(plan, first_chunk, n_chunks, host_out_ptr))
+
+
+def awg_synthesize_chunk_mux(plans: Sequence, chunk_idx: int, dev_out_ptr: int, stream=None) -> None:
+    arr = (c_void_p * len(plans))(*[p.value if isinstance(p, c_void_p) else p for p in plans])
+    _check(_lib.awg_synthesize_chunk_mux(arr, len(plans), chunk_idx, dev_out_ptr, _stream_handle(stream)))
+
+
+def awg_snap_frequency(f0_hz: float, sample_rate_hz: float, L_s: int) -> float:
+    out = c_double()
+    _check(_lib.awg_snap_frequency(f0_hz, sample_rate_hz, L_s, byref(out)))
+    return out.value
+
+
+def awg_static_buffer_set(plan, tone_idx, stream=None) -> None:
+    idx = _i32(tone_idx)
+    _check(_lib.awg_static_buffer_set(plan, idx.shape[0], idx.ctypes.data, _stream_handle(stream)))
+
+
+def awg_static_buffer_fold(plan, chunk_idx: int, tone_idx, stream=None) -> None:
+    idx = _i32(tone_idx)
+    _check(_lib.awg_static_buffer_fold(plan, chunk_idx, idx.shape[0], idx.ctypes.data, _stream_handle(stream)))
+
+
+def awg_static_buffer_read(plan, dev_out_ptr: int, stream=None) -> None:
+    _check(_lib.awg_static_buffer_read(plan, dev_out_ptr, _stream_handle(stream)))
 
 
 def awg_ring_create(plan, n_slots: int, host_mirror: bool) -> c_void_p:
@@ -296,6 +328,18 @@ class Plan:
         awg_synthesize_range_host(self._h, first_chunk, n_chunks, out.data_ptr())
         return out
 
+    def static_buffer_set(self, tone_idx, stream=None) -> None:
+        awg_static_buffer_set(self._h, tone_idx, stream)
+
+    def static_buffer_fold(self, chunk_idx: int, tone_idx, stream=None) -> None:
+        awg_static_buffer_fold(self._h, chunk_idx, tone_idx, stream)
+
+    def static_buffer(self, out=None, stream=None):
+        import torch
+        out = self._out(self.chunk_len, torch.float32, out)
+        awg_static_buffer_read(self._h, out.data_ptr(), stream)
+        return out
+
     def io_bytes(self) -> Tuple[int, int]:
         return awg_plan_io_bytes(self._h)
 
@@ -318,6 +362,18 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+def synthesize_chunk_mux(plans: Sequence[Plan], chunk_idx: int, out=None, stream=None):
+    """Interleaved int16 codes of the channels' plans: out[C i + c] (torch CUDA tensor of C*chunk_len int16)."""
+    import torch
+    n = plans[0].chunk_len * len(plans)
+    if out is None:
+        out = torch.empty(n, dtype=torch.int16, device="cuda")
+    if out.dtype != torch.int16 or out.numel() != n or not out.is_cuda or not out.is_contiguous():
+        raise ValueError("output tensor has the wrong dtype, size or device")
+    awg_synthesize_chunk_mux([p.handle for p in plans], chunk_idx, out.data_ptr(), stream)
+    return out
 
 
 class Ring:

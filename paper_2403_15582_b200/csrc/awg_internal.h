@@ -85,6 +85,10 @@ struct LaunchParams {
     float scale;       // int16 full-scale factor
     float qlo, qhi;    // clamp bounds of the quantiser in units of V (filled in by launch_synth)
     void *out;         // int16* or float* (device)
+    int32_t out_stride;   // int16 output: code of sample n goes to out[(n - n_begin) * out_stride + out_offset]
+    int32_t out_offset;   //   (channel multiplexing); fp32 output is always contiguous
+    const float *xs;   // looped static buffer X_static (Eq. 9) added before quantisation, or nullptr
+    int64_t xs_len;    //   its length L_s (a multiple of 8, >= kTile)
     uint32_t *sched;   // {next tile, teams finished}: the launch's tile-scheduler slot (filled in by launch_synth)
 };
 

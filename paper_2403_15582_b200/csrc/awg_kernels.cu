@@ -352,7 +352,7 @@ __device__ __noinline__ Acc16 exact_rec(const ToneRec *tab, const float4 a, int6
 // The clamp is applied to v (bounds -32768/scale, 32767/scale: qlo, qhi); the fused multiply-add against 1.5*2^23 then
 // rounds scale*v ONCE, to nearest-even, into the low mantissa bits: the two's-complement code is the low half-word.
 // Runs on the ALU and FMA pipes (a float-to-int conversion would take the XU pipe the sines need).
-__device__ __forceinline__ uint4 pack8(const LaunchParams &lp, const float2 *s)
+__device__ __forceinline__ uint4 pack8(const LaunchParams &lp, const float2 (&s)[4])
 {
     uint32_t w[4];
     const float2 sc = dup2(lp.scale), mg = dup2(kRoundMagic);
@@ -367,19 +367,39 @@ __device__ __forceinline__ uint4 pack8(const LaunchParams &lp, const float2 *s)
 
 // Steps a5-a6 for one block of one thread: 16 consecutive samples starting at absolute index n_thread, as two
 // 8-sample halves (launch ranges are multiples of 8 samples, so each half is inside or outside as a whole).
-__device__ __forceinline__ void store_block(const LaunchParams &lp, int64_t n_thread, const Acc16 &acc)
+// xs_tile: position of the tile's first sample in the looped static buffer (Eq. 9: X_static[i mod L_s] is added
+// before quantisation); tile_off = n_thread - tile_base.
+__device__ __forceinline__ void store_block(const LaunchParams &lp, int64_t n_thread, int64_t xs_tile, int tile_off, const Acc16 &acc)
 {
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
         const int64_t off = n_thread + 8 * h - lp.n_begin;
         if (off < 0 || off >= lp.n_count) continue;
-        const float2 *a = acc.a + 4 * h;
+        float2 a[4] = {acc.a[4 * h], acc.a[4 * h + 1], acc.a[4 * h + 2], acc.a[4 * h + 3]};
+        if (lp.xs) {
+            int64_t i = xs_tile + tile_off + 8 * h;     // < 2 L_s: one wrap at most (L_s >= kTile)
+            if (i >= lp.xs_len) i -= lp.xs_len;
+            const float4 x0 = __ldg(reinterpret_cast<const float4 *>(lp.xs + i)), x1 = __ldg(reinterpret_cast<const float4 *>(lp.xs + i) + 1);
+            a[0].x += x0.x; a[0].y += x0.y; a[1].x += x0.z; a[1].y += x0.w;
+            a[2].x += x1.x; a[2].y += x1.y; a[3].x += x1.z; a[3].y += x1.w;
+        }
         if (lp.out_f32) {
             float4 *o = reinterpret_cast<float4 *>(static_cast<float *>(lp.out) + off);
             o[0] = make_float4(a[0].x, a[0].y, a[1].x, a[1].y);
             o[1] = make_float4(a[2].x, a[2].y, a[3].x, a[3].y);
         } else {
-            *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = pack8(lp, a);
+            const uint4 w = pack8(lp, a);
+            if (lp.out_stride == 1) {
+                *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = w;
+            } else {
+                // multiplexed channels (the paper's WM): this channel's code of every sample index
+                uint16_t *o = static_cast<uint16_t *>(lp.out) + off * lp.out_stride + lp.out_offset;
+                const int st = lp.out_stride;
+                o[0] = static_cast<uint16_t>(w.x); o[st] = static_cast<uint16_t>(w.x >> 16);
+                o[2 * st] = static_cast<uint16_t>(w.y); o[3 * st] = static_cast<uint16_t>(w.y >> 16);
+                o[4 * st] = static_cast<uint16_t>(w.z); o[5 * st] = static_cast<uint16_t>(w.z >> 16);
+                o[6 * st] = static_cast<uint16_t>(w.w); o[7 * st] = static_cast<uint16_t>(w.w >> 16);
+            }
         }
     }
 }
@@ -843,9 +863,10 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
         }
 
         const int64_t n_thread = tile_base + lane * kSPT;
+        const int64_t xs_tile = lp.xs ? tile_base % lp.xs_len : 0;
         if (SPLIT == 1 && ROT && n_mov == 0) {
 #pragma unroll
-            for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, acc[r]);
+            for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, acc[r]);
             unit = next_unit<SPLIT>(lp, ws_all[warp - rank], team, rank, lane, n_teams);
             continue;
         }
@@ -879,7 +900,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                     for (int r2 = 0; r2 < SPLIT; ++r2) any |= team_ws[r2].n_mov;
                     if (any) mover_block<SPLIT>(lp, ws, team_ws, per, blk_base, lane, sum);
                 }
-                store_block(lp, n_thread + r * kBlock, sum);
+                store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, sum);
             }
         }
         // the closing barrier (the next tile's partial sums overwrite the park areas) also publishes the next tile
@@ -917,6 +938,11 @@ __global__ void __launch_bounds__(256) awg_fp64_kernel(const LaunchParams lp)
         }
     }
     const int64_t off = n_thread - lp.n_begin;
+    if (lp.xs) {
+        const int64_t i = n_thread % lp.xs_len;   // 8 consecutive samples never wrap: L_s is a multiple of 8
+#pragma unroll
+        for (int j = 0; j < kSPT64; ++j) acc[j] += static_cast<double>(__ldg(lp.xs + i + j));
+    }
     if (lp.out_f32) {
         float4 *o = reinterpret_cast<float4 *>(static_cast<float *>(lp.out) + off);
         o[0] = make_float4(static_cast<float>(acc[0]), static_cast<float>(acc[1]), static_cast<float>(acc[2]), static_cast<float>(acc[3]));
@@ -930,7 +956,16 @@ __global__ void __launch_bounds__(256) awg_fp64_kernel(const LaunchParams lp)
             asm("cvt.rni.sat.s16.f32 %0, %1;" : "=r"(hi) : "f"(lp.scale * static_cast<float>(acc[2 * j + 1])));
             w[j] = (static_cast<uint32_t>(lo) & 0xffffu) | (static_cast<uint32_t>(hi) << 16);
         }
-        *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = make_uint4(w[0], w[1], w[2], w[3]);
+        if (lp.out_stride == 1) {
+            *reinterpret_cast<uint4 *>(static_cast<int16_t *>(lp.out) + off) = make_uint4(w[0], w[1], w[2], w[3]);
+        } else {
+            uint16_t *o = static_cast<uint16_t *>(lp.out) + off * lp.out_stride + lp.out_offset;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                o[(2 * j) * lp.out_stride] = static_cast<uint16_t>(w[j]);
+                o[(2 * j + 1) * lp.out_stride] = static_cast<uint16_t>(w[j] >> 16);
+            }
+        }
     }
 }
 

@@ -222,19 +222,31 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
     ToneRec *table = reinterpret_cast<ToneRec *>(p->dev_table[v]);
     const ToneCore *stage = reinterpret_cast<const ToneCore *>(p->dev_stage[v]);
     if (p->dirty_all || n_dirty * 2 > static_cast<size_t>(p->n_tones)) {
-        for (int i = 0; i < p->n_pad; ++i) {
-            if (i < p->n_tones) fill_core(p->tones[i], host[i]);
-            else std::memset(&host[i], 0, sizeof(ToneCore));
+        // the device table holds the tones that are evaluated per sample (all of them unless some are served by the
+        // looped static buffer), in tone order
+        int n_act = 0;
+        for (int k = 0; k < p->n_tones; ++k) {
+            if (p->in_buffer[k]) {
+                p->slot_of[k] = -1;
+            } else {
+                p->slot_of[k] = n_act;
+                fill_core(p->tones[k], host[n_act++]);
+            }
         }
-        if ((e = cudaMemcpyAsync(p->dev_stage[v], host, p->core_bytes, cudaMemcpyHostToDevice, stream)) != cudaSuccess)
-            return fail_cuda(e, "cudaMemcpyAsync(tone cores)");
-        if ((e = launch_expand(table, stage, nullptr, p->n_pad, stream)) != cudaSuccess) return fail_cuda(e, "expand launch");
-        p->h2d_bytes += static_cast<int64_t>(p->core_bytes);
+        p->n_active = n_act;
+        const int n_up = (n_act + 31) / 32 * 32;
+        for (int i = n_act; i < n_up; ++i) std::memset(&host[i], 0, sizeof(ToneCore));
+        if (n_up > 0) {
+            if ((e = cudaMemcpyAsync(p->dev_stage[v], host, static_cast<size_t>(n_up) * sizeof(ToneCore), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+                return fail_cuda(e, "cudaMemcpyAsync(tone cores)");
+            if ((e = launch_expand(table, stage, nullptr, n_up, stream)) != cudaSuccess) return fail_cuda(e, "expand launch");
+        }
+        p->h2d_bytes += static_cast<int64_t>(n_up) * static_cast<int64_t>(sizeof(ToneCore));
     } else {
         int32_t *host_idx = reinterpret_cast<int32_t *>(p->host_table[v] + p->core_bytes);
         for (size_t j = 0; j < n_dirty; ++j) {
             fill_core(p->tones[p->dirty_tones[j]], host[j]);
-            host_idx[j] = p->dirty_tones[j];
+            host_idx[j] = p->slot_of[p->dirty_tones[j]];   // updates of tones in the static buffer are rejected earlier
         }
         if (p->upload_stream[cur] != stream && (e = cudaStreamWaitEvent(stream, p->uploaded[cur], 0)) != cudaSuccess)
             return fail_cuda(e, "cudaStreamWaitEvent");
@@ -257,13 +269,18 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
     return AWG_OK;
 }
 
-awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream)
+awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream,
+                              int32_t out_stride, int32_t out_offset)
 {
     awg_status st = ensure_table(p, stream);
     if (st != AWG_OK) return st;
     LaunchParams lp;
     lp.tab = reinterpret_cast<const ToneRec *>(p->dev_table[p->cur_version]);
-    lp.n_tones = p->n_tones;
+    lp.n_tones = p->n_active;
+    lp.out_stride = out_stride;
+    lp.out_offset = out_offset;
+    lp.xs = p->xs_on ? p->xs[p->xs_cur] : nullptr;
+    lp.xs_len = p->chunk_len;
     lp.n_begin = n_begin;
     lp.n_count = n_count;
     lp.scale = static_cast<float>(p->scale);
@@ -323,6 +340,7 @@ awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int
         if (k < 0 || k >= p->n_tones) return fail(AWG_ERR_INVALID_ARG, "tone index %d out of range", k);
         if (seen[k]) return fail(AWG_ERR_INVALID_ARG, "tone %d listed twice in one update", k);
         seen[k] = 1;
+        if (p->in_buffer[k]) return fail(AWG_ERR_STATE, "tone %d is served by the static buffer (clear it with awg_static_buffer_set first)", k);
         if (!std::isfinite(f1[i]) || !std::isfinite(t_dur[i]) || t_dur[i] < 0.0)
             return fail(AWG_ERR_INVALID_ARG, "non-finite value or negative duration in update %d", i);
         if (profile[i] < AWG_PROFILE_STATIC || profile[i] > AWG_PROFILE_MINJERK)
@@ -395,6 +413,8 @@ awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_h
     p->core_bytes = static_cast<size_t>(p->n_pad) * sizeof(ToneCore);
     try {
         p->tones.resize(n_tones);
+        p->in_buffer.assign(n_tones, 0);
+        p->slot_of.assign(n_tones, -1);
     } catch (...) {
         delete p;
         return fail(AWG_ERR_ALLOC, "out of host memory");
@@ -432,6 +452,11 @@ awg_status awg_plan_destroy(awg_plan *p)
         if (p->last_use[v]) cudaEventDestroy(p->last_use[v]);
         if (p->uploaded[v]) cudaEventDestroy(p->uploaded[v]);
     }
+    for (int s = 0; s < 2; ++s)
+        if (p->xs[s]) cudaFree(p->xs[s]);
+    if (p->dev_aux) cudaFree(p->dev_aux);
+    if (p->dev_aux_stage) cudaFree(p->dev_aux_stage);
+    if (p->host_aux) cudaFreeHost(p->host_aux);
     for (int s = 0; s < 2; ++s) {
         if (p->e2e_slot[s]) cudaFree(p->e2e_slot[s]);
         if (p->e2e_done[s]) cudaEventDestroy(p->e2e_done[s]);
@@ -457,7 +482,9 @@ awg_status awg_plan_op_counts(awg_plan *p, int64_t first_chunk, int64_t n_chunks
     if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
     const int64_t n0 = first_chunk * p->chunk_len, n1 = n0 + n_chunks * p->chunk_len;
     int64_t n_static = 0, n_slow = 0, n_fast = 0;
-    for (const HostTone &h : p->tones) {
+    for (int k = 0; k < p->n_tones; ++k) {
+        if (p->in_buffer[k]) continue;   // served by the looped static buffer: no per-sample work
+        const HostTone &h = p->tones[k];
         int64_t moving = 0;
         if ((h.cls & 0xff) != CLS_STATIC) {
             // samples n with 0 < u < Tn, u = (n - ns_int) - ns_frac
@@ -474,6 +501,224 @@ awg_status awg_plan_op_counts(awg_plan *p, int64_t first_chunk, int64_t n_chunks
     if (static_ts) *static_ts = n_static;
     if (slow_ts) *slow_ts = n_slow;
     if (fast_ts) *fast_ts = n_fast;
+    return AWG_OK;
+}
+
+// ---- static-buffer pathway (section IV A/B of the paper) ------------------------------------------------------
+
+awg_status awg_snap_frequency(double f0_hz, double sample_rate_hz, int64_t L_s, double *f_snapped_hz)
+{
+    if (!f_snapped_hz) return fail(AWG_ERR_INVALID_ARG, "f_snapped_hz is NULL");
+    if (!std::isfinite(f0_hz) || !std::isfinite(sample_rate_hz) || sample_rate_hz <= 0.0 || L_s < 1)
+        return fail(AWG_ERR_INVALID_ARG, "bad frequency, rate or buffer length");
+    // Eq. 6: f_j = nint(f0 L_s / fs) fs / L_s
+    const long double fs = sample_rate_hz, L = static_cast<long double>(L_s);
+    *f_snapped_hz = static_cast<double>(rintl(static_cast<long double>(f0_hz) * L / fs) * fs / L);
+    return AWG_OK;
+}
+
+namespace awg {
+namespace {
+
+// does the carrier frequency w (turns * 2^64 per sample) make a whole number of turns in L samples?  (Eq. 5/6)  The
+// frequency arrived as a double: its rounding (2^-53 relative, f/fs < 1) is allowed for, i.e. a phase drift of at most
+// L 2^-53 turns per period, far below anything the output resolves.
+bool periodic_in(uint64_t w, int64_t L)
+{
+    const int64_t r = static_cast<int64_t>(w * static_cast<uint64_t>(L));
+    return r <= 2048 * L && r >= -2048 * L;
+}
+
+awg_status static_buffer_alloc(awg_plan *p)
+{
+    cudaError_t e;
+    const size_t bytes = static_cast<size_t>(p->chunk_len) * sizeof(float);
+    for (int s = 0; s < 2; ++s)
+        if (!p->xs[s] && (e = cudaMalloc(reinterpret_cast<void **>(&p->xs[s]), bytes)) != cudaSuccess)
+            return fail(AWG_ERR_ALLOC, "cudaMalloc(static buffer): %s", cudaGetErrorString(e));
+    const size_t stage_bytes = p->core_bytes + static_cast<size_t>(p->n_pad) * sizeof(int32_t);
+    if (!p->dev_aux && (e = cudaMalloc(reinterpret_cast<void **>(&p->dev_aux), p->table_bytes)) != cudaSuccess)
+        return fail(AWG_ERR_ALLOC, "cudaMalloc(static-buffer table): %s", cudaGetErrorString(e));
+    if (!p->dev_aux_stage && (e = cudaMalloc(reinterpret_cast<void **>(&p->dev_aux_stage), stage_bytes)) != cudaSuccess)
+        return fail(AWG_ERR_ALLOC, "cudaMalloc(static-buffer staging): %s", cudaGetErrorString(e));
+    if (!p->host_aux && (e = cudaMallocHost(reinterpret_cast<void **>(&p->host_aux), stage_bytes)) != cudaSuccess)
+        return fail(AWG_ERR_ALLOC, "cudaMallocHost(static-buffer staging): %s", cudaGetErrorString(e));
+    return AWG_OK;
+}
+
+// One period [0, L_s) of the static carriers `tones` is synthesised as fp32 (the synthesis kernel, fp32 output) into
+// `dst`, on top of `base` when that is not NULL (Eq. 8; Eq. 10 branch 3).  Synchronous.
+awg_status static_buffer_add(awg_plan *p, const std::vector<HostTone> &tones, const float *base, float *dst, cudaStream_t stream)
+{
+    cudaError_t e;
+    const int n = static_cast<int>(tones.size());
+    const int n_up = (n + 31) / 32 * 32;
+    ToneCore *host = reinterpret_cast<ToneCore *>(p->host_aux);
+    for (int i = 0; i < n_up; ++i) {
+        if (i < n) fill_core(tones[i], host[i]);
+        else std::memset(&host[i], 0, sizeof(ToneCore));
+    }
+    if ((e = cudaMemcpyAsync(p->dev_aux_stage, host, static_cast<size_t>(n_up) * sizeof(ToneCore), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
+        return fail_cuda(e, "cudaMemcpyAsync(static-buffer cores)");
+    if ((e = launch_expand(reinterpret_cast<ToneRec *>(p->dev_aux), reinterpret_cast<const ToneCore *>(p->dev_aux_stage), nullptr, n_up,
+                           stream)) != cudaSuccess)
+        return fail_cuda(e, "expand launch");
+    p->h2d_bytes += static_cast<int64_t>(n_up) * static_cast<int64_t>(sizeof(ToneCore));
+    LaunchParams lp;
+    lp.tab = reinterpret_cast<const ToneRec *>(p->dev_aux);
+    lp.n_tones = n;
+    lp.out_f32 = 1;
+    lp.n_begin = 0;
+    lp.n_count = p->chunk_len;
+    lp.scale = static_cast<float>(p->scale);
+    lp.out = dst;
+    lp.out_stride = 1;
+    lp.out_offset = 0;
+    lp.xs = base;
+    lp.xs_len = p->chunk_len;
+    lp.sched = nullptr;
+    if ((e = launch_synth(lp, p->engine, stream)) != cudaSuccess) return fail_cuda(e, "kernel launch");
+    if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return fail_cuda(e, "cudaStreamSynchronize");
+    return AWG_OK;
+}
+
+awg_status check_tone_list(awg_plan *p, int32_t n, const int32_t *tone_idx)
+{
+    if (n < 0 || (n > 0 && !tone_idx)) return fail(AWG_ERR_INVALID_ARG, "bad tone list");
+    std::vector<char> seen(p->n_tones, 0);
+    for (int i = 0; i < n; ++i) {
+        const int k = tone_idx[i];
+        if (k < 0 || k >= p->n_tones) return fail(AWG_ERR_INVALID_ARG, "tone index %d out of range", k);
+        if (seen[k]) return fail(AWG_ERR_INVALID_ARG, "tone %d listed twice", k);
+        seen[k] = 1;
+    }
+    return AWG_OK;
+}
+
+}  // namespace
+}  // namespace awg
+
+awg_status awg_static_buffer_set(awg_plan *p, int32_t n_static, const int32_t *tone_idx, void *stream)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    awg_status st = check_device(p);
+    if (st != AWG_OK) return st;
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    if ((st = check_tone_list(p, n_static, tone_idx)) != AWG_OK) return st;
+    if (n_static == 0) {   // back to evaluating every tone per sample
+        std::fill(p->in_buffer.begin(), p->in_buffer.end(), 0);
+        p->xs_on = false;
+        p->dirty_all = true;
+        return AWG_OK;
+    }
+    if (p->chunk_len < kTile) return fail(AWG_ERR_INVALID_ARG, "the static-buffer pathway needs chunk_len >= %d", kTile);
+    std::vector<HostTone> tones;
+    for (int i = 0; i < n_static; ++i) {
+        const HostTone &h = p->tones[tone_idx[i]];
+        if ((h.cls & 0xff) != CLS_STATIC) return fail(AWG_ERR_INVALID_ARG, "tone %d is not static", tone_idx[i]);
+        if (!periodic_in(h.w_pre, p->chunk_len))
+            return fail(AWG_ERR_INVALID_ARG, "tone %d is off the fs/L_s grid (Eq. 6): snap it with awg_snap_frequency", tone_idx[i]);
+        tones.push_back(h);
+    }
+    if ((st = static_buffer_alloc(p)) != AWG_OK) return st;
+    if ((st = static_buffer_add(p, tones, nullptr, p->xs[0], static_cast<cudaStream_t>(stream))) != AWG_OK) return st;
+    std::fill(p->in_buffer.begin(), p->in_buffer.end(), 0);
+    for (int i = 0; i < n_static; ++i) p->in_buffer[tone_idx[i]] = 1;
+    p->xs_cur = 0;
+    p->xs_on = true;
+    p->dirty_all = true;
+    return AWG_OK;
+}
+
+awg_status awg_static_buffer_fold(awg_plan *p, int64_t chunk_idx, int32_t n_fold, const int32_t *tone_idx, void *stream)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    awg_status st = check_device(p);
+    if (st != AWG_OK) return st;
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    if (chunk_idx < 0 || chunk_idx > (std::numeric_limits<int64_t>::max() / 4) / p->chunk_len)
+        return fail(AWG_ERR_INVALID_ARG, "bad chunk index");
+    if (chunk_idx < p->last_update_chunk) return fail(AWG_ERR_STATE, "the hand-back precedes the latest trajectory update");
+    if ((st = check_tone_list(p, n_fold, tone_idx)) != AWG_OK) return st;
+    if (n_fold == 0) return AWG_OK;
+    if (p->chunk_len < kTile) return fail(AWG_ERR_INVALID_ARG, "the static-buffer pathway needs chunk_len >= %d", kTile);
+    const int64_t n_d = chunk_idx * p->chunk_len;   // L_d: a multiple of L_s
+    std::vector<HostTone> tones;
+    for (int i = 0; i < n_fold; ++i) {
+        const int k = tone_idx[i];
+        if (p->in_buffer[k]) return fail(AWG_ERR_STATE, "tone %d is already in the static buffer", k);
+        HostTone h = p->tones[k];
+        if ((h.cls & 0xff) != CLS_STATIC) {
+            const long double u = static_cast<long double>(n_d - h.ns_int) - static_cast<long double>(h.ns_frac);
+            if (u <= 0.0L) {
+                // the move has not begun: the tone is still on its first carrier
+            } else if (u >= h.Tn) {
+                h.theta_pre = h.theta_post;   // theta' of Eq. 10 is this carrier's phase at L_d
+                h.w_pre = h.w_post;
+                h.f0 = h.f1;
+            } else {
+                return fail(AWG_ERR_STATE, "tone %d is still moving at the hand-back (chunk %lld)", k, static_cast<long long>(chunk_idx));
+            }
+            make_static(h);
+        }
+        if (!periodic_in(h.w_pre, p->chunk_len))
+            return fail(AWG_ERR_INVALID_ARG, "tone %d ends off the fs/L_s grid (Eq. 6): its looped wavetable would not be seamless", k);
+        tones.push_back(h);
+    }
+    if ((st = static_buffer_alloc(p)) != AWG_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    if (!p->xs_on) {
+        if ((e = cudaMemsetAsync(p->xs[0], 0, static_cast<size_t>(p->chunk_len) * sizeof(float), s)) != cudaSuccess)
+            return fail_cuda(e, "cudaMemsetAsync");
+        p->xs_cur = 0;
+    }
+    // work in flight may still read the current buffer: the sum goes to the other one
+    if ((st = static_buffer_add(p, tones, p->xs[p->xs_cur], p->xs[p->xs_cur ^ 1], s)) != AWG_OK) return st;
+    p->xs_cur ^= 1;
+    p->xs_on = true;
+    for (int i = 0; i < n_fold; ++i) p->in_buffer[tone_idx[i]] = 1;
+    p->dirty_all = true;
+    p->last_update_chunk = chunk_idx;
+    return AWG_OK;
+}
+
+awg_status awg_static_buffer_read(awg_plan *p, float *dev_out, void *stream)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (!dev_out) return fail(AWG_ERR_INVALID_ARG, "output pointer is NULL");
+    awg_status st = check_device(p);
+    if (st != AWG_OK) return st;
+    if (!p->xs_on) return fail(AWG_ERR_STATE, "the plan has no static buffer");
+    cudaError_t e = cudaMemcpyAsync(dev_out, p->xs[p->xs_cur], static_cast<size_t>(p->chunk_len) * sizeof(float), cudaMemcpyDeviceToDevice,
+                                    static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
+    return AWG_OK;
+}
+
+// ---- four-channel multiplexed output (the paper's WM kernel) ------------------------------------------------------
+
+awg_status awg_synthesize_chunk_mux(awg_plan *const *plans, int32_t n_channels, int64_t chunk_idx, int16_t *dev_out, void *stream)
+{
+    if (!plans) return fail(AWG_ERR_INVALID_ARG, "plans is NULL");
+    if (n_channels < 1 || n_channels > 8) return fail(AWG_ERR_INVALID_ARG, "n_channels must be in [1, 8]");
+    for (int c = 0; c < n_channels; ++c) {
+        if (!plans[c]) return fail(AWG_ERR_INVALID_ARG, "plan of channel %d is NULL", c);
+        if (plans[c]->chunk_len != plans[0]->chunk_len) return fail(AWG_ERR_INVALID_ARG, "the channels' plans must share chunk_len");
+        for (int d = 0; d < c; ++d)
+            if (plans[d] == plans[c]) return fail(AWG_ERR_INVALID_ARG, "channels %d and %d share a plan", d, c);
+    }
+    // validate every channel before the first launch
+    for (int c = 0; c < n_channels; ++c) {
+        awg_status st = check_chunk_call(plans[c], chunk_idx, 1, dev_out, 16);
+        if (st != AWG_OK) return st;
+    }
+    for (int c = 0; c < n_channels; ++c) {
+        awg_plan *p = plans[c];
+        awg_status st = synthesize_samples(p, chunk_idx * p->chunk_len, p->chunk_len, dev_out, false, static_cast<cudaStream_t>(stream),
+                                           n_channels, c);
+        if (st != AWG_OK) return st;
+    }
     return AWG_OK;
 }
 
@@ -530,6 +775,8 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
     p->dirty_all = true;
     p->dirty_tones.clear();
     p->last_update_chunk = 0;
+    std::fill(p->in_buffer.begin(), p->in_buffer.end(), 0);
+    p->xs_on = false;
     return AWG_OK;
 }
 

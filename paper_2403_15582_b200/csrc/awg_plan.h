@@ -44,6 +44,17 @@ struct awg_plan {
     std::vector<int32_t> dirty_tones;       // tones changed by updates since the last upload
     int64_t last_update_chunk = 0;
     std::vector<awg::HostTone> tones;
+    // static-buffer pathway: tones served by the looped buffer X_static are not in the
+    // device table; slot_of[k] is tone k's record in the device table, or -1
+    std::vector<uint8_t> in_buffer;
+    std::vector<int32_t> slot_of;
+    int32_t n_active = 0;
+    float *xs[2] = {};                      // X_static, chunk_len floats each; xs[xs_cur] is current (a fold writes the other)
+    int xs_cur = 0;
+    bool xs_on = false;
+    unsigned char *dev_aux = nullptr;       // table of the tones whose period is being added to X_static
+    unsigned char *dev_aux_stage = nullptr;
+    unsigned char *host_aux = nullptr;      // pinned staging of their cores
     // versioned device tables
     size_t table_bytes = 0;
     int cur_version = 0;
@@ -66,7 +77,8 @@ struct awg_plan {
 
 namespace awg {
 awg_status ensure_table(awg_plan *p, cudaStream_t stream);
-awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream);
+awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream,
+                              int32_t out_stride = 1, int32_t out_offset = 0);
 awg_status check_chunk_call(awg_plan *p, int64_t first_chunk, int64_t n_chunks, const void *out, size_t align);
 awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx, const double *f1,
                         const double *t_dur, const int32_t *profile);

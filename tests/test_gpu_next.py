@@ -1,0 +1,245 @@
+"""GPU parity for the NEXT rows of SURVEY.md section 8(f), through the C ABI, against the oracle:
+NEXT-2 four-channel multiplexed output, NEXT-3 static-buffer pathway (Eq. 6-9 and the theta'
+hand-back of Eq. 10 branch 3), NEXT-4 time-varying amplitudes (Eq. 9).  Same bar as test_gpu_parity.py."""
+import math
+
+import numpy as np
+import pytest
+
+import awg_workloads as W
+import oracle
+from parity_util import assert_codes_close, assert_f32_close
+
+pytestmark = pytest.mark.gpu
+
+STATIC, LINEAR, MINJERK = W.PROFILE_STATIC, W.PROFILE_LINEAR, W.PROFILE_MINJERK
+FS = 560e6
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(params=["fma", "mufu"])
+def eng(request, awg):
+    return {"fma": awg.AWG_ENGINE_FMA, "mufu": awg.AWG_ENGINE_MUFU}[request.param]
+
+
+def _np(t):
+    return t.cpu().numpy()
+
+
+def _pair(awg, fs, chunk_len, rows, engine=None):
+    cols = list(zip(*rows))
+    p = awg.Plan(len(rows), fs, chunk_len, None, engine if engine is not None else awg.AWG_ENGINE_AUTO)
+    p.set_trajectories(*cols)
+    op = oracle.OraclePlan(len(rows), fs, chunk_len)
+    op.set_trajectories(*cols)
+    return p, op
+
+
+# ------------------------------------------------------------------ NEXT-2: multiplexed channels
+def _channel_rows(rng, n_tones, span):
+    rows = []
+    for k in range(n_tones):
+        f0 = rng.uniform(20e6, 250e6)
+        if k % 3 == 2:
+            T = rng.uniform(0.1, 0.5) * span
+            rows.append((f0, f0 + rng.choice([-1, 1]) * rng.uniform(0.5e6, 5e6), 1.0 / n_tones, rng.uniform(0, 6.28),
+                         rng.uniform(0, span - T), T, MINJERK))
+        else:
+            rows.append((f0, f0, 1.0 / n_tones, rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
+    return rows
+
+
+def test_mux4_paper_chunk(awg, torch_cuda, eng):
+    """The paper's streaming chunk: 2^20 samples = 4 channels x 2^18, 20 tones per channel (its
+    560 MS/s streaming figure), groups of four."""
+    L = 1 << 18
+    rng = np.random.default_rng(22)
+    pairs = [_pair(awg, FS, L, _channel_rows(rng, 20, 2 * L / FS), eng) for _ in range(4)]
+    plans, oplans = [p for p, _ in pairs], [o for _, o in pairs]
+    for c in (0, 1):
+        got = _np(awg.synthesize_chunk_mux(plans, c))
+        assert got.shape == (4 * L,)
+        for ch in range(4):
+            single = _np(plans[ch].synthesize_chunk(c))
+            assert np.array_equal(got[ch::4], single), f"channel {ch} of chunk {c} differs from its single-channel synthesis"
+            V = oracle.c_waveform(oplans[ch], c * L, (c + 1) * L)
+            assert_codes_close(got[ch::4], oplans[ch].quantise(V), f"mux chunk {c} channel {ch}")
+    # the oracle's own interleave on a window (first 4096 sample indices of chunk 1)
+    want = oracle.mux_channels(oplans, L, L + 4096)
+    assert_codes_close(_np(awg.synthesize_chunk_mux(plans, 1))[:4 * 4096], want, "mux vs oracle.mux_channels")
+    for p in plans:
+        p.close()
+
+
+def test_mux_other_channel_counts_and_ragged_chunks(awg, torch_cuda, eng):
+    L = 1000   # not a multiple of the 2048-sample tile: partial tiles at both chunk edges
+    rng = np.random.default_rng(23)
+    for C, sizes in ((2, (5, 40)), (3, (1, 33, 7)), (1, (12,))):
+        pairs = [_pair(awg, FS, L, _channel_rows(rng, n, 6 * L / FS), eng) for n in sizes]
+        plans, oplans = [p for p, _ in pairs], [o for _, o in pairs]
+        for c in (0, 3, 5):
+            got = _np(awg.synthesize_chunk_mux(plans, c))
+            assert_codes_close(got, oracle.mux_channels(oplans, c * L, (c + 1) * L), f"mux C={C} chunk {c}")
+            for ch in range(C):
+                assert np.array_equal(got[ch::C], _np(plans[ch].synthesize_chunk(c)))
+        for p in plans:
+            p.close()
+
+
+def test_mux_errors(awg, torch_cuda):
+    torch = torch_cuda
+    a = awg.Plan(2, FS, 1024)
+    b = awg.Plan(2, FS, 2048)
+    z = np.zeros(2)
+    for p in (a, b):
+        p.set_trajectories(z + 1e6, z + 1e6, z + 0.1, z, z, z, np.zeros(2, np.int32))
+    buf = torch.empty(4096, dtype=torch.int16, device="cuda")
+    with pytest.raises(awg.AwgError) as ei:
+        awg.awg_synthesize_chunk_mux([a.handle, b.handle], 0, buf.data_ptr())
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG      # chunk_len mismatch
+    with pytest.raises(awg.AwgError) as ei:
+        awg.awg_synthesize_chunk_mux([a.handle, a.handle], 0, buf.data_ptr())
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG      # the same plan twice
+    c = awg.Plan(2, FS, 1024)                               # no table yet
+    with pytest.raises(awg.AwgError) as ei:
+        awg.awg_synthesize_chunk_mux([a.handle, c.handle], 0, buf.data_ptr())
+    assert ei.value.status == awg.AWG_ERR_STATE
+    a.close(); b.close(); c.close()
+
+
+# ------------------------------------------------------------------ NEXT-3: static-buffer pathway
+def test_snap_frequency_matches_eq6(awg):
+    L = 1 << 20
+    assert awg.awg_snap_frequency(100e6, FS, L) == oracle.snap_frequency(100e6, FS, L)
+    assert abs(awg.awg_snap_frequency(100e6, FS, L) - 100e6) <= FS / L / 2
+    assert abs(FS / L - 534.06) < 0.005
+    with pytest.raises(awg.AwgError):
+        awg.awg_snap_frequency(100e6, -1.0, L)
+
+
+def _static_rows(rng, L, n_static, n_dyn, span):
+    rows = []
+    for k in range(n_static):
+        f = oracle.snap_frequency(rng.uniform(40e6, 240e6), FS, L)
+        rows.append((f, f, 0.8 / (n_static + n_dyn), rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
+    for k in range(n_dyn):
+        f = rng.uniform(40e6, 240e6)
+        T = rng.uniform(0.1, 0.4) * span
+        rows.append((f, f + rng.choice([-1, 1]) * rng.uniform(1e6, 5e6), 0.8 / (n_static + n_dyn), rng.uniform(0, 6.28),
+                     rng.uniform(0, span - T), T, MINJERK if k % 2 else LINEAR))
+    return rows
+
+
+@pytest.mark.parametrize("L,n_static,n_dyn", [(1 << 14, 40, 5), (4096, 3, 70), (6000, 130, 2)])
+def test_static_pathway_equals_per_sample_evaluation(awg, torch_cuda, eng, L, n_static, n_dyn):
+    rng = np.random.default_rng(L + n_static)
+    rows = _static_rows(rng, L, n_static, n_dyn, 5 * L / FS)
+    p, op = _pair(awg, FS, L, rows, eng)
+    chunks = (0, 1, 4, 77)
+    direct = {c: (_np(p.synthesize_chunk(c)), _np(p.synthesize_chunk_f32(c))) for c in chunks}
+    p.static_buffer_set(range(n_static))
+    # the buffer is Eq. 8 over one period
+    X = op.static_buffer(range(n_static))
+    assert_f32_close(_np(p.static_buffer()), X, "X_static", tol=2e-6)
+    assert p.op_counts(0, 1)[0] + sum(p.op_counts(0, 1)[1:]) == n_dyn * L      # only the dynamic tones are evaluated per sample
+    for c in chunks:
+        V = oracle.c_waveform(op, c * L, (c + 1) * L)                            # absolute-time definition
+        Vp = op.waveform_static_pathway(c * L, (c + 1) * L, X, range(n_static, n_static + n_dyn))
+        assert np.max(np.abs(V - Vp)) < 1e-9
+        f = _np(p.synthesize_chunk_f32(c))
+        assert_f32_close(f, V, f"static pathway f32 chunk {c}")
+        got = _np(p.synthesize_chunk(c))
+        assert_codes_close(got, op.quantise(V), f"static pathway chunk {c}")
+        # and within rounding of the plan's own per-sample evaluation
+        assert np.max(np.abs(got.astype(np.int32) - direct[c][0].astype(np.int32))) <= 1
+        assert np.max(np.abs(f - direct[c][1])) < 2e-6
+    # a range launch over several chunks wraps the looped index
+    r = _np(p.synthesize_range(3, 3))
+    assert_codes_close(r, op.quantise(oracle.c_waveform(op, 3 * L, 6 * L)), "static pathway range")
+    # removing the buffer restores the per-sample evaluation bit for bit
+    p.static_buffer_set([])
+    assert np.array_equal(_np(p.synthesize_chunk(4)), direct[4][0])
+    p.close()
+
+
+def test_static_buffer_handback_theta_prime(awg, torch_cuda, eng):
+    """Eq. 10 branch 3: after L_d the moved tones are looped static wavetables with theta'."""
+    L = 8192
+    rng = np.random.default_rng(8)
+    T = 30e-6                                              # 16800 samples: L_d = 3 L
+    L_d_chunks = math.ceil(T * FS / L)
+    rows = []
+    for k in range(10):
+        f = oracle.snap_frequency(rng.uniform(40e6, 240e6), FS, L)
+        rows.append((f, f, 0.05, rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
+    for k in range(6):   # movers that end ON the grid (they can be handed back) ...
+        f1 = oracle.snap_frequency(rng.uniform(40e6, 240e6), FS, L)
+        rows.append((f1 + rng.uniform(-4e6, 4e6), f1, 0.05, rng.uniform(0, 6.28), 0.0, T * rng.uniform(0.5, 1.0), MINJERK))
+    rows.append((100e6, 103.000123e6, 0.05, 0.3, 0.0, T, MINJERK))   # ... and one that ends off the grid
+    p, op = _pair(awg, FS, L, rows, eng)
+    p.static_buffer_set(range(10))
+    X = op.static_buffer(range(10))
+    for c in range(L_d_chunks):                            # the dynamic phase: static buffer + movers
+        V = oracle.c_waveform(op, c * L, (c + 1) * L)
+        assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"before the hand-back, chunk {c}")
+    with pytest.raises(awg.AwgError) as ei:
+        p.static_buffer_fold(1, [10])                      # still moving at chunk 1
+    assert ei.value.status == awg.AWG_ERR_STATE
+    with pytest.raises(awg.AwgError) as ei:
+        p.static_buffer_fold(L_d_chunks, [16])             # ends off the Eq. 6 grid
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    p.static_buffer_fold(L_d_chunks, range(10, 16))
+    X2 = op.fold_into_static_buffer(X, range(10, 16), L_d_chunks * L)
+    assert_f32_close(_np(p.static_buffer()), X2, "X_static after the hand-back", tol=3e-6)
+    assert sum(p.op_counts(L_d_chunks, 1)) == L            # one tone left in the per-sample evaluation
+    for c in (L_d_chunks, L_d_chunks + 1, L_d_chunks + 50):
+        V = oracle.c_waveform(op, c * L, (c + 1) * L)      # absolute time, every tone: the loop is seamless
+        assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"after the hand-back, chunk {c}")
+        assert_codes_close(_np(p.synthesize_chunk(c)), op.quantise(V), f"after the hand-back, chunk {c}")
+    with pytest.raises(awg.AwgError) as ei:
+        p.synthesize_chunk(0)                              # the past is fixed, as after an update
+    assert ei.value.status == awg.AWG_ERR_STATE
+    with pytest.raises(awg.AwgError) as ei:
+        p.update_trajectories(L_d_chunks + 1, [3], [90e6], [1e-6], [MINJERK])   # a tone in the buffer cannot move
+    assert ei.value.status == awg.AWG_ERR_STATE
+    p.close()
+
+
+def test_static_buffer_alone_and_errors(awg, torch_cuda):
+    L = 4096
+    f = [oracle.snap_frequency(x, FS, L) for x in (50e6, 75e6, 111e6)]
+    rows = [(f[k], f[k], 0.3, 0.5 * k, 0.0, 0.0, STATIC) for k in range(3)] + [(60.00001e6, 60.00001e6, 0.1, 0, 0, 0, STATIC)]
+    p, op = _pair(awg, FS, L, rows)
+    with pytest.raises(awg.AwgError) as ei:
+        p.static_buffer_set([0, 3])                        # tone 3 is off the grid
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    with pytest.raises(awg.AwgError) as ei:
+        p.static_buffer_set([0, 0])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    with pytest.raises(awg.AwgError) as ei:
+        p.static_buffer()                                  # no buffer yet
+    assert ei.value.status == awg.AWG_ERR_STATE
+    p.static_buffer_set([0, 1, 2])
+    # every on-grid tone in the buffer; then fold the last one too (it is static: theta' is its phase): nothing is left
+    # to evaluate per sample and the output is the looped buffer, quantised
+    V = oracle.c_waveform(op, 9 * L, 10 * L)
+    assert_codes_close(_np(p.synthesize_chunk(9)), op.quantise(V), "three tones from the buffer")
+    q, oq = _pair(awg, FS, L, rows[:3])
+    q.static_buffer_set([0, 1, 2])
+    assert sum(q.op_counts(0, 1)) == 0
+    X = oq.static_buffer([0, 1, 2])
+    for c in (0, 5):
+        assert_f32_close(_np(q.synthesize_chunk_f32(c)), X, "looped buffer only", tol=2e-6)
+        assert_codes_close(_np(q.synthesize_chunk(c)), oq.quantise(X), "looped buffer only")
+    small = awg.Plan(1, FS, 1024)
+    small.set_trajectories([FS / 8], [FS / 8], [0.5], [0.0], [0.0], [0.0], [STATIC])
+    with pytest.raises(awg.AwgError) as ei:
+        small.static_buffer_set([0])                       # chunk_len < 2048
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    p.close(); q.close(); small.close()
