@@ -101,6 +101,18 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
                                 const double *phi0, const double *t_start, const double *t_dur,
                                 const int32_t *profile);
 
+/* Time-varying amplitudes a_j[i] of Eq. 9 (constant in the paper's worked case,
+ * PAPER.md:137; reading G19): tone k goes from the amplitude given to awg_set_trajectories to
+ * A1[k] over [t_start[k], t_start[k] + t_dur[k]] along profile[k] -- AWG_PROFILE_STATIC (no ramp: A1,
+ * t_start, t_dur ignored), AWG_PROFILE_LINEAR, or AWG_PROFILE_MINJERK (10 s^3 - 15 s^4 + 6 s^5): tone
+ * creation (0 -> A1) and removal (A -> 0) without a click.  Four host arrays of length n_tones.  Replaces
+ * earlier ramps; awg_set_trajectories clears them.  Samples inside a ramp are evaluated one by one in
+ * fp64 phase (slow, exact); before and after it the tone costs what any other tone costs.
+ * Errors: INVALID_ARG (NULL, non-finite, t_dur < 0, unknown profile), STATE (no table set; after a
+ * per-chunk update; tone in the static buffer). */
+awg_status awg_set_amplitude_ramps(awg_plan *p, const double *A1, const double *t_start, const double *t_dur,
+                                   const int32_t *profile);
+
 /* Per-chunk update (streaming pathway, Fig. 7): at the first sample of chunk_idx each
  * listed tone starts a new move from its current instantaneous frequency and phase (phase- and
  * frequency-continuous) to f1[i] over t_dur[i] with profile[i].  Host arrays of length n_upd.

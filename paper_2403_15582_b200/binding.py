@@ -35,7 +35,7 @@ AWG_ENGINE_FMA = 3
 #: every symbol include/awg.h declares (tests check that the library exports each of them)
 EXPORTED = (
     "awg_plan_create", "awg_plan_destroy", "awg_set_scale", "awg_set_engine", "awg_set_trajectories",
-    "awg_update_trajectories", "awg_synthesize_chunk", "awg_synthesize_chunk_f32", "awg_synthesize_range",
+    "awg_set_amplitude_ramps", "awg_update_trajectories", "awg_synthesize_chunk", "awg_synthesize_chunk_f32", "awg_synthesize_range",
     "awg_synthesize_range_host", "awg_ring_create", "awg_ring_submit", "awg_ring_acquire", "awg_ring_release",
     "awg_synthesize_chunk_mux", "awg_snap_frequency", "awg_static_buffer_set", "awg_static_buffer_fold",
     "awg_static_buffer_read",
@@ -57,6 +57,7 @@ def _load() -> ctypes.CDLL:
         "awg_set_scale": (I32, [P, D]),
         "awg_set_engine": (I32, [P, I32]),
         "awg_set_trajectories": (I32, [P, P, P, P, P, P, P, P]),
+        "awg_set_amplitude_ramps": (I32, [P, P, P, P, P]),
         "awg_update_trajectories": (I32, [P, I64, I32, P, P, P, P]),
         "awg_synthesize_chunk": (I32, [P, I64, P, P]),
         "awg_synthesize_chunk_f32": (I32, [P, I64, P, P]),
@@ -154,6 +155,12 @@ def awg_set_trajectories(plan, n_tones, f0, f1, A, phi0, t_start, t_dur, profile
     arrs = [_f64(x, n_tones) for x in (f0, f1, A, phi0, t_start, t_dur)]
     prof = _i32(profile, n_tones)
     _check(_lib.awg_set_trajectories(plan, *[a.ctypes.data for a in arrs], prof.ctypes.data))
+
+
+def awg_set_amplitude_ramps(plan, n_tones, A1, t_start, t_dur, profile) -> None:
+    arrs = [_f64(x, n_tones) for x in (A1, t_start, t_dur)]
+    prof = _i32(profile, n_tones)
+    _check(_lib.awg_set_amplitude_ramps(plan, *[a.ctypes.data for a in arrs], prof.ctypes.data))
 
 
 def awg_update_trajectories(plan, chunk_idx: int, tone_idx, f1, t_dur, profile) -> None:
@@ -287,6 +294,9 @@ class Plan:
 
     def set_trajectories(self, f0, f1, A, phi0, t_start, t_dur, profile) -> None:
         awg_set_trajectories(self._h, self.n_tones, f0, f1, A, phi0, t_start, t_dur, profile)
+
+    def set_amplitude_ramps(self, A1, t_start, t_dur, profile) -> None:
+        awg_set_amplitude_ramps(self._h, self.n_tones, A1, t_start, t_dur, profile)
 
     def update_trajectories(self, chunk_idx: int, tone_idx, f1, t_dur, profile) -> None:
         awg_update_trajectories(self._h, chunk_idx, tone_idx, f1, t_dur, profile)

@@ -16,7 +16,8 @@ enum : int32_t {
     CLS_DEG4 = 4,    // k^2..k^4
     CLS_DEG6 = 6,    // k^2..k^6 (exact Taylor series of the degree-6 min-jerk phase)
     CLS_EXACT = 7,   // fp32 in-block polynomial not accurate enough: moving blocks use the fp64 path
-    CLS_SLOW_FLAG = 1 << 16  // OR-ed into ToneRec::cls: tiles wholly inside the move may take the slow pass (FMA pipe)
+    CLS_SLOW_FLAG = 1 << 16,  // OR-ed into ToneRec::cls: tiles wholly inside the move may take the slow pass (FMA pipe)
+    CLS_AMP_FLAG = 1 << 17    // OR-ed into ToneRec::cls: the tone has an amplitude ramp (A -> A1 over [amp_ns, amp_ns + amp_Tn))
 };
 
 // Kernel geometry.  A thread owns kSPT consecutive samples of a block; a block is 32 lanes x kSPT = 512 samples
@@ -28,6 +29,8 @@ constexpr int kBlocksPerTile = 4;
 constexpr int kTile = kBlocksPerTile * kBlock;
 constexpr int kPairs = kSPT / 2;  // symmetric sample pairs per thread: centre +- (j + 1/2), j = 0..kPairs-1
 
+// (the table of the pre-move carrier carries the amplitude A, the table of the post-move carrier A1: tiles after both
+// the move and the ramp use the latter, tiles before both the former, anything in between takes the MUFU pass)
 // Carrier table of the angle-addition engine (hot-path step a3, static tiles): with phi the carrier phase at the
 // half-integer centre of a thread's 16 samples, the samples at centre +- (j + 1/2) are
 //     A sin(phi +- (j+1/2) w) = sin(phi) * [A cos((j+1/2) w)]  +-  cos(phi) * [A sin((j+1/2) w)]
@@ -63,7 +66,12 @@ struct __align__(16) ToneCore {
     double DT;             // (f1-f0)*t_dur, cycles
     double q1;             // DT/Tn = (f1-f0)/fs, cycles per sample
     float q[5];            // q[k-2] = 2*pi*DT/Tn^k/k!, k = 2..6: radians per sample^k for unit g^(k)
-    float pad_[5];
+    // ---- amplitude ramp a_j[i] of Eq. 9: A before amp_ns, A + (A1 - A) h((n - amp_ns)/amp_Tn) during,
+    // A1 after; h(s) = s or 10 s^3 - 15 s^4 + 6 s^5 (amp_prof).  A1 = A and amp_prof = STATIC without a ramp.
+    float A1;
+    double amp_ns;         // ramp start, samples (real)
+    float amp_Tn;          // ramp duration, samples
+    int32_t amp_prof;      // AWG_PROFILE_*
 };
 static_assert(sizeof(ToneCore) == 128, "ToneCore must be 128 bytes");
 

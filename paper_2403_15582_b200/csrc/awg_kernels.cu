@@ -102,6 +102,17 @@ __device__ __forceinline__ uint64_t exact_phase(const ToneCore &r, int64_t n)
     return r.theta_pre + r.w_pre * static_cast<uint64_t>(n) + frac_to_fix64(x);
 }
 
+// a_j[i] of Eq. 9 for a tone with an amplitude ramp, at absolute sample n.
+__device__ __forceinline__ float amp_at(const ToneCore &r, int64_t n)
+{
+    if (!(r.cls & CLS_AMP_FLAG)) return r.A;
+    const float u = static_cast<float>(static_cast<double>(n) - r.amp_ns);
+    float s = r.amp_Tn > 0.f ? u / r.amp_Tn : (u >= 0.f ? 1.f : 0.f);
+    s = fminf(fmaxf(s, 0.f), 1.f);
+    const float h = r.amp_prof == AWG_PROFILE_LINEAR ? s : s * s * s * (10.f + s * (6.f * s - 15.f));
+    return fmaf(r.A1 - r.A, h, r.A);
+}
+
 // Kinds of (tone, block) record, in the order the inner loops run them.
 enum : int {
     K_NONE = -1,
@@ -144,8 +155,21 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
     const uint4 v3 = ldg16(reinterpret_cast<const char *>(rec) + 48);  // ns_frac, Tn
     const uint4 v4 = ldg16(reinterpret_cast<const char *>(rec) + 64);  // inv_Tn, DT
     const uint4 v5 = ldg16(reinterpret_cast<const char *>(rec) + 80);  // q1, q[0], q[1]
-    const uint4 v6 = ldg16(reinterpret_cast<const char *>(rec) + 96);  // q[2], q[3], q[4]
+    const uint4 v6 = ldg16(reinterpret_cast<const char *>(rec) + 96);  // q[2], q[3], q[4], A1
     const uint64_t w_pre = u64_of(v1.x, v1.y);
+    if (cls & CLS_AMP_FLAG) {
+        // amplitude ramp: a block it overlaps is evaluated per sample (K_EXACT), one after it takes A1
+        const uint4 v7 = ldg16(reinterpret_cast<const char *>(rec) + 112);  // amp_ns, amp_Tn, amp_prof
+        const double aa = bb_d - f64_of(v7.x, v7.y);
+        if (aa >= static_cast<double>(__uint_as_float(v7.z))) {
+            r.A = __uint_as_float(v6.w);
+        } else if (aa + static_cast<double>(kBlock - 1) > 0.0) {
+            r.kind = K_EXACT;
+            r.c0 = static_cast<uint32_t>(t);
+            r.c1 = 0;
+            return r;
+        }
+    }
     uint64_t ph, w;
     if (c == CLS_STATIC) {
         w = w_pre;
@@ -328,19 +352,18 @@ __device__ __forceinline__ void mufu_rec(const float4 a, const float4 b, int kof
 }
 
 // fp64 path for a K_EXACT record (tones whose fp32 polynomial would be inaccurate, moves shorter than a block,
-// instant retunes): exact phase per sample, same sine.
+// instant retunes, blocks inside an amplitude ramp): exact phase and amplitude per sample, same sine.
 __device__ __noinline__ Acc16 exact_rec(const ToneRec *tab, const float4 a, int64_t n_thread, Acc16 acc)
 {
     const ToneCore &tr = tab[__float_as_uint(a.x)].core;
-    const float A = a.z;
 #pragma unroll 1
     for (int j = 0; j < kPairs; ++j) {
         const uint32_t p0 = round32(exact_phase(tr, n_thread + 2 * j));
         const uint32_t p1 = round32(exact_phase(tr, n_thread + 2 * j + 1));
         float2 v = acc.a[0];
         // rotate through the pairs so that the loop body indexes a[] statically
-        v.x = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p0)) * kTurnToRad), v.x);
-        v.y = fmaf(A, mufu_sin(__int2float_rn(static_cast<int32_t>(p1)) * kTurnToRad), v.y);
+        v.x = fmaf(amp_at(tr, n_thread + 2 * j), mufu_sin(__int2float_rn(static_cast<int32_t>(p0)) * kTurnToRad), v.x);
+        v.y = fmaf(amp_at(tr, n_thread + 2 * j + 1), mufu_sin(__int2float_rn(static_cast<int32_t>(p1)) * kTurnToRad), v.y);
 #pragma unroll
         for (int m = 0; m < kPairs - 1; ++m) acc.a[m] = acc.a[m + 1];
         acc.a[kPairs - 1] = v;
@@ -776,6 +799,30 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                             asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char *>(tr) + 96));
                         }
                     }
+                    if (static_cast<int32_t>(v0.y) & CLS_AMP_FLAG) {
+                        // amplitude ramp (Eq. 9's a_j[i]): the pre-move table carries A, the post-move table A1; a tile
+                        // that is not wholly before (or after) both the move and the ramp takes the MUFU pass
+                        const uint4 v7 = ldg16(reinterpret_cast<const char *>(tr) + 112);  // amp_ns, amp_Tn, amp_prof
+                        const double aa = tb_d - f64_of(v7.x, v7.y);
+                        const bool before = aa + static_cast<double>(kTile - 1) <= 0.0;
+                        const bool after = aa >= static_cast<double>(__uint_as_float(v7.z));
+                        if (is_static) {
+                            if ((static_cast<int32_t>(v0.y) & 0xff) == CLS_STATIC && after) {
+                                tabp = reinterpret_cast<const float4 *>(&tr->rot_post);
+                                is_post = true;
+                            } else if (is_post ? !after : !before) {
+                                is_static = false;
+                                is_mover = true;
+                            }
+                        } else if (is_slow) {
+                            if (!before && !after) {
+                                is_slow = false;
+                                is_mover = true;
+                            } else if (after) {
+                                ws.mrec[lane].q[1].x = __ldg(&tr->core.A1);
+                            }
+                        }
+                    }
                     c0 = round32(th + w * a0 - (w >> 1));
                     c1 = round32(w);
                     d = round32(w * static_cast<uint64_t>(kBlock));
@@ -930,11 +977,10 @@ __global__ void __launch_bounds__(256) awg_fp64_kernel(const LaunchParams lp)
     for (int j = 0; j < kSPT64; ++j) acc[j] = 0.0;
     for (int t = 0; t < lp.n_tones; ++t) {
         const ToneCore &tr = lp.tab[t].core;
-        const double A = static_cast<double>(tr.A);
 #pragma unroll
         for (int j = 0; j < kSPT64; ++j) {
             const int64_t ph = static_cast<int64_t>(exact_phase(tr, n_thread + j));  // signed: [-0.5, 0.5) turn
-            acc[j] += A * sinpi(static_cast<double>(ph) * (2.0 / kTwo64));
+            acc[j] += static_cast<double>(amp_at(tr, n_thread + j)) * sinpi(static_cast<double>(ph) * (2.0 / kTwo64));
         }
     }
     const int64_t off = n_thread - lp.n_begin;
@@ -990,7 +1036,7 @@ __global__ void __launch_bounds__(128) awg_expand_kernel(ToneRec *table, const T
     const double turns = static_cast<double>(static_cast<int64_t>(ang)) * (1.0 / kTwo64);   // [-1/2, 1/2)
     double sn, cs;
     sincospi(2.0 * turns, &sn, &cs);
-    const double A = static_cast<double>(c.A);
+    const double A = static_cast<double>(state ? c.A1 : c.A);
     RotTable &tab = state ? dst.rot_post : dst.rot_pre;
     tab.C[p] = static_cast<float>(A * cs);
     tab.S[p] = static_cast<float>(A * sn);

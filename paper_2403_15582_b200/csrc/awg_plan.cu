@@ -176,6 +176,14 @@ static void fill_core(const HostTone &h, ToneCore &r)
     std::memset(&r, 0, sizeof r);
     r.A = h.A;
     r.cls = (h.profile << 8) | h.cls;
+    r.A1 = h.A;
+    if (h.amp_prof != AWG_PROFILE_STATIC) {
+        r.cls |= CLS_AMP_FLAG;
+        r.A1 = h.A1;
+        r.amp_ns = static_cast<double>(h.amp_ns);
+        r.amp_Tn = static_cast<float>(h.amp_Tn);
+        r.amp_prof = h.amp_prof;
+    }
     r.theta_pre = h.theta_pre;
     r.w_pre = h.w_pre;
     r.theta_post = h.theta_post;
@@ -350,6 +358,11 @@ awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int
     const int64_t n_u = chunk_idx * p->chunk_len;
     for (int i = 0; i < n_upd; ++i) {
         HostTone &h = p->tones[tone_idx[i]];
+        // an amplitude ramp that has ended by n_u is folded into the tone's amplitude (the tables then carry it)
+        if (h.amp_prof != AWG_PROFILE_STATIC && static_cast<long double>(n_u) - h.amp_ns >= h.amp_Tn) {
+            h.A = h.A1;
+            h.amp_prof = AWG_PROFILE_STATIC;
+        }
         // state of the old segment at n_u: instantaneous frequency and a carrier that continues its phase
         if ((h.cls & 0xff) != CLS_STATIC) {
             const long double u = static_cast<long double>(n_u - h.ns_int) - static_cast<long double>(h.ns_frac);
@@ -494,8 +507,23 @@ awg_status awg_plan_op_counts(awg_plan *p, int64_t first_chunk, int64_t n_chunks
             const int64_t a = first > n0 ? first : n0, b = last < n1 - 1 ? last : n1 - 1;
             if (b >= a) moving = b - a + 1;
         }
-        if (h.cls & CLS_SLOW_FLAG) n_slow += moving;
-        else n_fast += moving;
+        int64_t ramping = 0;   // samples inside an amplitude ramp are evaluated one by one as well
+        if (h.amp_prof != AWG_PROFILE_STATIC) {
+            const int64_t first = static_cast<int64_t>(floorl(h.amp_ns)) + 1;
+            const int64_t last = static_cast<int64_t>(ceill(h.amp_ns + h.amp_Tn)) - 1;
+            const int64_t a = first > n0 ? first : n0, b = last < n1 - 1 ? last : n1 - 1;
+            if (b >= a) ramping = b - a + 1;
+        }
+        if (ramping > 0) {
+            // (the union of the two windows is what leaves the angle-addition engine; counted as the larger one)
+            if (ramping > moving) { n_fast += ramping; moving = ramping; }
+            else if (h.cls & CLS_SLOW_FLAG) n_fast += moving;
+            else n_fast += moving;
+        } else if (h.cls & CLS_SLOW_FLAG) {
+            n_slow += moving;
+        } else {
+            n_fast += moving;
+        }
         n_static += (n1 - n0) - moving;
     }
     if (static_ts) *static_ts = n_static;
@@ -615,7 +643,8 @@ awg_status awg_static_buffer_set(awg_plan *p, int32_t n_static, const int32_t *t
     std::vector<HostTone> tones;
     for (int i = 0; i < n_static; ++i) {
         const HostTone &h = p->tones[tone_idx[i]];
-        if ((h.cls & 0xff) != CLS_STATIC) return fail(AWG_ERR_INVALID_ARG, "tone %d is not static", tone_idx[i]);
+        if ((h.cls & 0xff) != CLS_STATIC || h.amp_prof != AWG_PROFILE_STATIC)
+            return fail(AWG_ERR_INVALID_ARG, "tone %d is not static", tone_idx[i]);
         if (!periodic_in(h.w_pre, p->chunk_len))
             return fail(AWG_ERR_INVALID_ARG, "tone %d is off the fs/L_s grid (Eq. 6): snap it with awg_snap_frequency", tone_idx[i]);
         tones.push_back(h);
@@ -648,6 +677,14 @@ awg_status awg_static_buffer_fold(awg_plan *p, int64_t chunk_idx, int32_t n_fold
         const int k = tone_idx[i];
         if (p->in_buffer[k]) return fail(AWG_ERR_STATE, "tone %d is already in the static buffer", k);
         HostTone h = p->tones[k];
+        if (h.amp_prof != AWG_PROFILE_STATIC) {
+            const long double ua = static_cast<long double>(n_d) - h.amp_ns;
+            if (ua > 0.0L && ua < h.amp_Tn)
+                return fail(AWG_ERR_STATE, "tone %d is inside its amplitude ramp at the hand-back (chunk %lld)", k, static_cast<long long>(chunk_idx));
+            if (ua >= h.amp_Tn) h.A = h.A1;
+            h.A1 = h.A;
+            h.amp_prof = AWG_PROFILE_STATIC;
+        }
         if ((h.cls & 0xff) != CLS_STATIC) {
             const long double u = static_cast<long double>(n_d - h.ns_int) - static_cast<long double>(h.ns_frac);
             if (u <= 0.0L) {
@@ -761,6 +798,7 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
         HostTone &h = p->tones[k];
         h = HostTone{};
         h.A = static_cast<float>(A[k]);
+        h.A1 = h.A;
         h.f0 = static_cast<long double>(f0[k]);
         h.theta_pre = frac64(static_cast<long double>(phi0[k]) / kTwoPiL);  // radians -> turns (theta_j of Eq. 8/9)
         h.w_pre = frac64(h.f0 / fs);
@@ -777,6 +815,34 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
     p->last_update_chunk = 0;
     std::fill(p->in_buffer.begin(), p->in_buffer.end(), 0);
     p->xs_on = false;
+    return AWG_OK;
+}
+
+awg_status awg_set_amplitude_ramps(awg_plan *p, const double *A1, const double *t_start, const double *t_dur, const int32_t *profile)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (!A1 || !t_start || !t_dur || !profile) return fail(AWG_ERR_INVALID_ARG, "NULL ramp array");
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    if (p->last_update_chunk > 0) return fail(AWG_ERR_STATE, "amplitude ramps are set before the first trajectory update");
+    const int N = p->n_tones;
+    if (!finite_all(A1, N) || !finite_all(t_start, N) || !finite_all(t_dur, N)) return fail(AWG_ERR_INVALID_ARG, "non-finite value in a ramp array");
+    for (int k = 0; k < N; ++k) {
+        if (t_dur[k] < 0.0) return fail(AWG_ERR_INVALID_ARG, "t_dur[%d] < 0", k);
+        if (profile[k] < AWG_PROFILE_STATIC || profile[k] > AWG_PROFILE_MINJERK)
+            return fail(AWG_ERR_INVALID_ARG, "unknown profile %d for tone %d", profile[k], k);
+        if (std::fabs(t_start[k]) * static_cast<double>(p->fs) > 4.0e18) return fail(AWG_ERR_INVALID_ARG, "t_start[%d] out of range", k);
+        if (profile[k] != AWG_PROFILE_STATIC && p->in_buffer[k])
+            return fail(AWG_ERR_STATE, "tone %d is served by the static buffer", k);
+    }
+    for (int k = 0; k < N; ++k) {
+        HostTone &h = p->tones[k];
+        h.amp_prof = profile[k];
+        h.A1 = profile[k] == AWG_PROFILE_STATIC ? h.A : static_cast<float>(A1[k]);
+        h.amp_ns = static_cast<long double>(t_start[k]) * p->fs;
+        h.amp_Tn = static_cast<long double>(t_dur[k]) * p->fs;
+    }
+    p->dirty_all = true;
+    p->dirty_tones.clear();
     return AWG_OK;
 }
 

@@ -25,6 +25,10 @@ struct HostTone {
     float A = 0;
     int32_t profile = AWG_PROFILE_STATIC;
     int32_t cls = 0;
+    // amplitude ramp (Eq. 9's a_j[i]): A -> A1 over [amp_ns, amp_ns + amp_Tn) samples along amp_prof
+    float A1 = 0;
+    int32_t amp_prof = AWG_PROFILE_STATIC;
+    long double amp_ns = 0, amp_Tn = 0;
 };
 
 awg_status fail(awg_status code, const char *fmt, ...);

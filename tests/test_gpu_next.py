@@ -243,3 +243,102 @@ def test_static_buffer_alone_and_errors(awg, torch_cuda):
         small.static_buffer_set([0])                       # chunk_len < 2048
     assert ei.value.status == awg.AWG_ERR_INVALID_ARG
     p.close(); q.close(); small.close()
+
+
+# ------------------------------------------------------------------ NEXT-4: time-varying amplitudes a_j[i]
+def _ramp_pair(awg, L, rows, ramps, engine):
+    p, op = _pair(awg, FS, L, rows, engine)
+    cols = list(zip(*ramps))
+    p.set_amplitude_ramps(*cols)
+    op.set_amplitude_ramps(*cols)
+    return p, op
+
+
+@pytest.mark.parametrize("engine", ["fma", "mufu", "fp64"])
+def test_amplitude_ramps_creation_removal_and_moving_tones(awg, torch_cuda, engine):
+    """Tone creation (0 -> A), removal (A -> 0), a ramp on a moving tone, a ramp shorter than a block, an instant step,
+    linear and minimum-jerk profiles; chunks before, inside and after the ramps."""
+    eng = {"fma": awg.AWG_ENGINE_FMA, "mufu": awg.AWG_ENGINE_MUFU, "fp64": awg.AWG_ENGINE_FP64}[engine]
+    L = 4096
+    us = 1e-6
+    rows = [
+        (100e6, 100e6, 0.0, 0.3, 0.0, 0.0, STATIC),            # created: 0 -> 0.15 over 12 us (min-jerk)
+        (85e6, 85e6, 0.15, 1.3, 0.0, 0.0, STATIC),             # removed: 0.15 -> 0 over 9 us (linear)
+        (120e6, 124e6, 0.15, 2.3, 5 * us, 20 * us, MINJERK),   # moves AND fades 0.15 -> 0.05 while moving
+        (140e6, 140e6, 0.10, 0.7, 0.0, 0.0, STATIC),           # 0.3 us ramp: shorter than a 512-sample block
+        (60e6, 61e6, 0.10, 0.1, 2 * us, 30 * us, LINEAR),      # instant amplitude step at 10.3 us while chirping
+        (200e6, 200e6, 0.15, 0.9, 0.0, 0.0, STATIC),           # untouched
+        (70e6, 75e6, 0.10, 0.2, 30 * us, 8 * us, MINJERK),     # ramp long before its move
+    ]
+    ramps = [(0.15, 4 * us, 12 * us, MINJERK), (0.0, 7.7 * us, 9 * us, LINEAR), (0.05, 11 * us, 10 * us, MINJERK),
+             (0.02, 13.1 * us, 0.3 * us, MINJERK), (0.2, 10.3 * us, 0.0, LINEAR), (0.0, 0.0, 0.0, STATIC),
+             (0.15, 1 * us, 6 * us, LINEAR)]
+    p, op = _ramp_pair(awg, L, rows, ramps, eng)
+    n_chunks = 8                                            # 58 us: every ramp and move ends inside
+    V = oracle.c_waveform(op, 0, n_chunks * L)
+    gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(n_chunks)])
+    emax = assert_f32_close(gotf, V, f"amplitude ramps {engine}", tol=3e-7 if engine == "fp64" else 1e-5)
+    got = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(n_chunks)])
+    assert_codes_close(got, op.quantise(V), f"amplitude ramps {engine}")
+    # one range launch gives the same bits as the chunks
+    assert np.array_equal(_np(p.synthesize_range(0, n_chunks)), got)
+    # long after everything: the tones sit at their final amplitudes (the post-move tables carry A1)
+    c = 500
+    Vl = oracle.c_waveform(op, c * L, (c + 1) * L)
+    assert_f32_close(_np(p.synthesize_chunk_f32(c)), Vl, "after the ramps")
+    assert np.max(np.abs(Vl)) > 0.1
+    print(f"amplitude ramps {engine}: f32 max err {emax:.2e}")
+    p.close()
+
+
+def test_amplitude_ramp_then_update_and_errors(awg, torch_cuda, eng):
+    L = 2048
+    rows = [(90e6, 90e6, 0.0, 0.4, 0.0, 0.0, STATIC), (110e6, 110e6, 0.3, 0.0, 0.0, 0.0, STATIC)]
+    ramps = [(0.3, 1e-6, 4e-6, MINJERK), (0.0, 0.0, 0.0, STATIC)]
+    p, op = _ramp_pair(awg, L, rows, ramps, eng)
+    # chunk 3 starts after the ramp has ended (5 us = 2800 samples): a frequency update there continues at amplitude A1
+    for plan in (p, op):
+        plan.update_trajectories(3, [0], [93e6], [3e-6], [MINJERK])
+    for c in (3, 4, 5, 9):
+        V = oracle.c_waveform(op, c * L, (c + 1) * L)
+        assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"update after a ramp, chunk {c}")
+        assert_codes_close(_np(p.synthesize_chunk(c)), op.quantise(V), f"update after a ramp, chunk {c}")
+    with pytest.raises(awg.AwgError) as ei:
+        p.set_amplitude_ramps([0.1, 0.1], [0, 0], [1e-6, 1e-6], [LINEAR, LINEAR])
+    assert ei.value.status == awg.AWG_ERR_STATE            # after a per-chunk update
+    q = awg.Plan(2, FS, L)
+    with pytest.raises(awg.AwgError) as ei:
+        q.set_amplitude_ramps([0.1, 0.1], [0, 0], [1e-6, 1e-6], [LINEAR, LINEAR])
+    assert ei.value.status == awg.AWG_ERR_STATE            # no table yet
+    q.set_trajectories([1e6, 2e6], [1e6, 2e6], [0.1, 0.1], [0, 0], [0, 0], [0, 0], [STATIC, STATIC])
+    with pytest.raises(awg.AwgError) as ei:
+        q.set_amplitude_ramps([0.1, 0.1], [0, 0], [-1e-6, 1e-6], [LINEAR, LINEAR])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    with pytest.raises(awg.AwgError) as ei:
+        q.set_amplitude_ramps([0.1, 0.1], [0, 0], [1e-6, 1e-6], [LINEAR, 9])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    p.close(); q.close()
+
+
+def test_amplitude_ramps_many_tones_bit_identical_chunkings(awg, torch_cuda, eng):
+    """130 tones over two warps' batches, a third of them fading in or out: chunkings agree bit for bit."""
+    N, L = 130, 1 << 14
+    rng = np.random.default_rng(41)
+    rows = _channel_rows(rng, N, 3 * L / FS)
+    ramps = []
+    for k in range(N):
+        if k % 3 == 0:
+            ramps.append((rows[k][2] * rng.uniform(0, 2), rng.uniform(0, 40e-6), rng.uniform(2e-6, 30e-6), MINJERK if k % 2 else LINEAR))
+        else:
+            ramps.append((0.0, 0.0, 0.0, STATIC))
+    p, op = _ramp_pair(awg, L, rows, ramps, eng)
+    ref = _np(p.synthesize_range(0, 3))
+    V = oracle.c_waveform(op, 0, 3 * L)
+    assert_codes_close(ref, op.quantise(V), "ramps, 130 tones")
+    cols = list(zip(*rows)); rc = list(zip(*ramps))
+    q = awg.Plan(N, FS, 1000, None, eng)
+    q.set_trajectories(*cols)
+    q.set_amplitude_ramps(*rc)
+    for c in (0, 7, 16, 33, 48):
+        assert np.array_equal(_np(q.synthesize_chunk(c)), ref[c * 1000:(c + 1) * 1000]), c
+    p.close(); q.close()
