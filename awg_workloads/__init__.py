@@ -27,5 +27,6 @@ from .configs import (  # noqa: F401
     config5_grid,
     capacity_toneset,
     comb_toneset,
+    fast_mover_stream,
     by_name,
 )

@@ -272,6 +272,33 @@ def capacity_toneset(n_tones: int, sample_rate: float, chunk_len: int, mix: str 
                     seed=(seed, N))
 
 
+def fast_mover_stream(n_tones: int, sample_rate: float = 560e6, chunk_len: int = 1 << 18, n_chunks: int = 8,
+                      seed: int = 6) -> Workload:
+    """Every tone is inside a short minimum-jerk move ALL the time ("chirp indefinitely"): all tones start
+    static; at every chunk boundary every tone starts a new move that lasts exactly one chunk (2^18 samples at 560 MS/s =
+    468 us, inside the 100-500 us range of tweezer moves) to f_now +- U(0.5, 5) MHz, the sign chosen to stay inside
+    [0.05, 0.45] fs.  Draws: f0 = U(0.1, 0.4, N) fs; phi0 = U(0, 2pi, N); then per chunk mag = U(0.5e6, 5e6, N),
+    sign = choice(+-1, N) (flipped where the target would leave the band)."""
+    rng = np.random.default_rng([seed, n_tones])
+    N = n_tones
+    f0 = rng.uniform(0.1, 0.4, N) * sample_rate
+    phi0 = rng.uniform(0.0, 2.0 * math.pi, N)
+    f_now = f0.copy()
+    T = chunk_len / sample_rate
+    updates: List[Update] = []
+    for c in range(n_chunks):
+        mag = rng.uniform(0.5e6, 5e6, N)
+        sign = rng.choice(np.array([-1.0, 1.0]), N)
+        tgt = f_now + sign * mag
+        bad = (tgt < 0.05 * sample_rate) | (tgt > 0.45 * sample_rate)
+        tgt[bad] = f_now[bad] - sign[bad] * mag[bad]
+        f_now = tgt
+        updates.append(Update(c, _i32(np.arange(N)), _f64(tgt), _f64(np.full(N, T)), _i32(np.full(N, PROFILE_MINJERK))))
+    z = np.zeros(N)
+    return Workload(f"FAST[N={N}]", sample_rate, chunk_len, n_chunks, _f64(f0), _f64(f0.copy()), _f64(np.full(N, 1.0 / N)),
+                    _f64(phi0), _f64(z), _f64(z), _i32(np.zeros(N)), updates=updates, seed=(seed, N))
+
+
 def comb_toneset(n_tones: int, n_samples: int, sample_rate: float = 560e6, f_first: float = 50e6,
                  spacing: float = 1e6) -> Workload:
     """The paper's static benchmark signal a*sum_j sin(2pi(f0 + j*df)t), f0 = 50 MHz, df = 1 MHz,

@@ -5,18 +5,22 @@
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 One "step" = one pass of the whole hot path (trajectory table resident -> phase re-centring -> sine ->
-accumulate -> quantise -> int16 stores) over BASELINE.json config 2: 100 tones at 560 MS/s for 10 ms
-(5.6 M samples, 25 chunks of 224 000), synthesised by ONE awg_synthesize_range launch into a device
-buffer.  Metric: tone-samples/s (G).  Rank 0 prints ONE JSON line.
+accumulate -> quantise -> int16 stores) over BASELINE.json config 3, the largest single-GPU configuration: 1000 tones,
+every one minimum-jerk chirping over 35 ms at 560 MS/s, 19 x 2^20 = 19 922 944 samples (the paper's Playback case,
+PAPER.md:246), synthesised by ONE awg_synthesize_range launch into a 39.8 MB device buffer.  Metric: tone-samples/s (G).
+Rank 0 prints ONE JSON line.
 
   value      device-timed (CUDA events on the launch stream), inputs resident in HBM
   e2e        the same workload through the C ABI with HOST buffers: awg_set_trajectories from host arrays
-             (H2D table upload) + awg_synthesize_range_host into pinned host memory (D2H of the int16 codes)
+             (H2D upload of the tone cores) + awg_synthesize_range_host into pinned host memory (D2H of the int16 codes)
   roofline   ALU-bound ("bound": "alu"): a tone-sample needs one fp32 multiply-add where its tone is static (angle
-             addition), two inside a slow move, one MUFU.SIN + two multiply-adds inside any other move; the pipe (FMA: 128/clk/SM, XU: 16/clk/SM,
+             addition), two inside a slow move, one MUFU.SIN + two multiply-adds inside any other move -- counted by the
+             LIBRARY (awg_plan_op_counts: the classification the kernel acts on); the pipe (FMA: 128/clk/SM, XU: 16/clk/SM,
              x 148 SMs x sm_max_mhz) whose roofline time is larger binds; frac = that time / measured launch time
   cpu_baseline  the oracle (oracle/awg_oracle_c.c, as it stands) on this box's host cores, bounded sample
-  extras     the other configs (C1, C3, C4 ring, C5 sweep) and the real-time capacity search
+  extras     the other configs (C1, C2, C4 at its 382 chunks, the 20 C5 cells), a fast-mover set (every tone inside a
+             468 us minimum-jerk move all the time), the static-buffer pathway, four-channel multiplexing and the
+             real-time capacity search -- every line with its fraction of the binding pipe
 
 Multi-GPU (--gpus N under torchrun): the path shards by time with no exchange (every chunk is a pure
 function of the absolute sample index), so each rank synthesises its own replica of the workload --
@@ -27,6 +31,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import sys
 import threading
@@ -40,6 +45,8 @@ import numpy as np  # noqa: E402
 
 import awg_workloads as W  # noqa: E402
 
+C3_DESC = ("C3: 1000 tones, every one minimum-jerk chirping over 35 ms at 560 MS/s, 19 x 2^20 = 19 922 944 samples, "
+           "precomputed pathway (BASELINE.json configs[2], seed 2; the largest single-GPU configuration)")
 METRIC = "tone-samples/s"
 UNIT = "Gtone-samples/s"
 MUFU_PER_CLK_PER_SM = 16  # sm_100: 4 SFU lanes per SM sub-partition (measured 15.9/clk/SM, profiles/)
@@ -160,13 +167,13 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
-    w = W.config2()
+    w = W.config3()
     op = oracle.plan_from_workload(w)
     # warm-up doubles as a rate probe: size the per-step sample so that the K steps end within ~2 minutes
     t0 = time.perf_counter()
     for _ in range(max(1, args.warmup)):
-        oracle.c_waveform(op, 0, 1 << 16)
-    rate = max(1, args.warmup) * (1 << 16) * w.n_tones / (time.perf_counter() - t0)
+        oracle.c_waveform(op, 0, 1 << 14)
+    rate = max(1, args.warmup) * (1 << 14) * w.n_tones / (time.perf_counter() - t0)
     n = int(min(1 << 20, max(4096, rate * 120.0 / args.steps / w.n_tones)))
     n -= n % 4096
     t0 = time.perf_counter()
@@ -179,70 +186,27 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "C2: 100 tones, 560 MS/s, 10 ms (BASELINE.json configs[1])",
-                   "sample": f"first {n} of {w.n_samples} samples per step"},
+        "config": {"workload": C3_DESC, "sample": f"first {n} of {w.n_samples} samples per step"},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": f"first {n} samples x {w.n_tones} tones of C2 per step, {args.steps} steps"},
+                         "sample": f"first {n} samples x {w.n_tones} tones of C3 per step, {args.steps} steps"},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
 
 
-def is_slow_mover(profile: int, DT: float, Tn: float) -> bool:
-    """Mirror of is_slow_mover() in csrc/awg_plan.cu (same bounds): a tone whose move the angle-addition engine can carry
-    on the FMA pipe (cubic phase polynomial per thread + first-order table correction)."""
-    if not Tn >= 2.0 * 2048:
-        return False
-    a, r, R, h = abs(DT) / Tn, 1.0 / Tn, 1024.0, 7.5
-    lin = profile == W.PROFILE_LINEAR
-    C2 = a * r * (1.0 if lin else 5.7735) / 2.0
-    C3 = 0.0 if lin else a * r ** 2 * 60.0 / 6.0
-    C4 = 0.0 if lin else a * r ** 3 * 360.0 / 24.0
-    C5 = 0.0 if lin else a * r ** 4 * 720.0 / 120.0
-    C6 = 0.0 if lin else a * r ** 5
-    if C4 * R ** 4 + C5 * R ** 5 + C6 * R ** 6 > 2e-8:
-        return False
-    if (4 * C4 * R ** 3 + 5 * C5 * R ** 4 + 6 * C6 * R ** 5) * h > 2e-8:
-        return False
-    if (C2 + 3 * C3 * R + 6 * C4 * R ** 2) * h * h > 2e-7:
-        return False
-    x = 6.283185307179586 * h * (2 * C2 * R + 3 * C3 * R ** 2)
-    return 0.5 * x * x <= 2e-7 and C2 * R ** 2 + C3 * R ** 3 <= 0.25
-
-
-def moving_tone_samples(w, split: bool = False):
-    """Tone-samples of workload w that fall inside a move (sample granularity; initial trajectory table only).
-    split=True returns (fast, slow): slow movers (is_slow_mover) need no MUFU.SIN per sample."""
-    fs = float(w.sample_rate)
-    fast = slow = 0
-    for k in range(w.n_tones):
-        if int(w.profile[k]) == W.PROFILE_STATIC or float(w.f1[k]) == float(w.f0[k]) or float(w.t_dur[k]) <= 0.0:
-            continue
-        a = max(0.0, float(w.t_start[k]) * fs)
-        b = min(float(w.n_samples), (float(w.t_start[k]) + float(w.t_dur[k])) * fs)
-        if b > a:
-            DT = (float(w.f1[k]) - float(w.f0[k])) * float(w.t_dur[k])
-            if is_slow_mover(int(w.profile[k]), DT, float(w.t_dur[k]) * fs):
-                slow += int(b - a)
-            else:
-                fast += int(b - a)
-    return (fast, slow) if split else fast + slow
-
-
-def pipe_roofline(w, ms, engine, sm_mhz):
-    """Binding ALU roofline of one launch over workload w.
+def pipe_roofline(counts, ms, engine, sm_mhz):
+    """Binding ALU roofline of launches that took `ms` in total over `counts` = (static, slow, fast) tone-samples as the
+    LIBRARY classifies them (awg_plan_op_counts).
 
     Algorithmic work: a tone-sample of a tone that is static there needs ONE fp32 multiply-add (angle addition over a
     symmetric sample pair); inside a slow move TWO multiply-adds (the second is the first-order frequency correction);
     inside any other move one MUFU.SIN plus two multiply-adds (range multiply, amplitude accumulate).  With
     --engine mufu every tone-sample takes the MUFU path.  The roofline time is the larger of (multiply-adds / FMA-pipe
     peak) and (sines / XU-pipe peak) at sm_mhz; frac = that time / the measured time."""
+    n_sta, n_slow, n_fast = (int(x) for x in counts)
     if engine == "mufu":
-        n_fast, n_slow = w.tone_samples, 0
-    else:
-        n_fast, n_slow = moving_tone_samples(w, split=True)
-    n_sta = w.tone_samples - n_fast - n_slow
+        n_sta, n_slow, n_fast = 0, 0, n_sta + n_slow + n_fast
     fma_ops, xu_ops = n_sta + 2 * n_slow + 2 * n_fast, n_fast
     peak_fma = FMA_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
     peak_xu = MUFU_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
@@ -253,9 +217,14 @@ def pipe_roofline(w, ms, engine, sm_mhz):
     else:
         pipe, ops, peak, unit = "XU (MUFU.SIN)", xu_ops, peak_xu, "Gsin/s"
     return {"bound": "alu", "pipe": pipe, "achieved": ops / t / 1e9, "peak": peak / 1e9, "unit": unit,
-            "frac": max(t_fma, t_xu) / t, "static_tone_samples": int(n_sta), "moving_tone_samples": int(n_fast + n_slow),
-            "slow_moving_tone_samples": int(n_slow), "fma_ops": int(fma_ops), "mufu_ops": int(xu_ops),
+            "frac": max(t_fma, t_xu) / t, "static_tone_samples": n_sta, "moving_tone_samples": n_slow + n_fast,
+            "slow_moving_tone_samples": n_slow, "fma_ops": int(fma_ops), "mufu_ops": int(xu_ops),
             "t_fma_us": t_fma * 1e6, "t_xu_us": t_xu * 1e6}
+
+
+def frac_of(counts, ms, sm_mhz, engine="auto"):
+    r = pipe_roofline(counts, ms, engine, sm_mhz)
+    return {"roofline_frac": round(r["frac"], 4), "pipe": r["pipe"].split()[0]}
 
 
 ENGINES = {"auto": lambda awg: awg.AWG_ENGINE_AUTO, "fma": lambda awg: awg.AWG_ENGINE_FMA,
@@ -263,15 +232,15 @@ ENGINES = {"auto": lambda awg: awg.AWG_ENGINE_AUTO, "fma": lambda awg: awg.AWG_E
 
 
 def pick_workload(name: str):
-    """The timed workload: C2 (the headline, BASELINE.json configs[1]) unless --workload asks for another one
-    (profiling aid: C1, C3, C5:<tones>:<log2 chunk>, CAP:<static|half|moving>:<tones>)."""
+    """The timed workload: C3 (the headline: the largest single-GPU configuration, BASELINE.json configs[2]) unless
+    --workload asks for another one (profiling aid: C1, C2, C5:<tones>:<log2 chunk>, CAP:<static|half|moving>:<tones>)."""
     if name == "C2":
         return W.config2(), ("C2: 100 tones at 560 MS/s for 10 ms = 5.6 M samples, 50 min-jerk movers "
                              "(BASELINE.json configs[1], seed 1)")
     if name == "C1":
         return W.config1(), "C1: 16 tones, 2^20 samples (BASELINE.json configs[0])"
     if name == "C3":
-        return W.config3(), "C3: 1000 tones min-jerk for 35 ms at 560 MS/s, 19 x 2^20 samples (BASELINE.json configs[2])"
+        return W.config3(), C3_DESC
     kind, *rest = name.split(":")
     if kind == "C5":
         n_t, lg = int(rest[0]), int(rest[1])
@@ -305,7 +274,8 @@ def make_bufs(torch, n_samples):
 
 
 def stream_through_ring(awg, w, host_mirror, n_chunks=None, n_slots=4):
-    """Runs workload w (with its per-chunk updates) through the ring as fast as it goes.
+    """Runs workload w (with its per-chunk updates) through the ring as fast as it goes; the ring's virtual DAC consumes
+    one chunk per chunk_len/fs and counts the chunks that were not complete when due.
     Returns (underruns, max_chunk_ms, wall_s, chunks)."""
     p = awg.Plan.from_workload(w)
     ring = awg.Ring(p, n_slots=n_slots, host_mirror=host_mirror)
@@ -326,22 +296,45 @@ def stream_through_ring(awg, w, host_mirror, n_chunks=None, n_slots=4):
     return underruns, max_ms, wall, produced
 
 
-def realtime_capacity(torch, awg, fs, chunk_len, mix, host_mirror, seconds, lo=16, hi=65536):
-    """Largest tone count whose every chunk completes within chunk_len/fs: bisection on N,
-    each probe streams `seconds` of signal through the ring and reads the longest per-chunk device time."""
-    deadline_ms = chunk_len / fs * 1e3
-    n_chunks = max(8, int(round(seconds * fs / chunk_len)))
+def device_time_chunks(torch, awg, w, n_chunks=None):
+    """Device time (ms, CUDA events around every synthesis launch, table uploads outside) of the chunks of a workload with
+    per-chunk updates, and the library's operation counts summed over the chunks."""
+    p = awg.Plan.from_workload(w)
+    ups = w.updates_by_chunk()
+    n_chunks = n_chunks or w.n_chunks
+    out = [torch.empty(w.chunk_len, dtype=torch.int16, device="cuda") for _ in range(4)]
+    stream = torch.cuda.current_stream()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_chunks)]
+    counts = [0, 0, 0]
+    warm = torch.empty(w.chunk_len, dtype=torch.float32, device="cuda")
+    for c in range(n_chunks):
+        if c in ups:
+            u = ups[c]
+            p.update_trajectories(c, u.tone_idx, u.f1, u.t_dur, u.profile)
+            p.synthesize_chunk_f32(c, out=warm, stream=stream)   # carries the table upload; not timed
+        for i, v in enumerate(p.op_counts(c, 1)):
+            counts[i] += v
+        evs[c][0].record(stream)
+        p.synthesize_chunk(c, out=out[c % 4], stream=stream)
+        evs[c][1].record(stream)
+    torch.cuda.synchronize()
+    ms = [a.elapsed_time(b) for a, b in evs]
+    p.close()
+    return sum(ms), max(ms), counts
 
+
+def realtime_capacity(awg, make_workload, host_mirror, lo=16, hi=65536):
+    """Largest tone count that streams in real time: bisection on N; a probe streams >= 1 s of signal
+    through the ring (3 slots) and is sustained when the ring's own underrun counter stays at zero."""
     def ok(n):
-        w = W.capacity_toneset(n, fs, chunk_len, mix, n_chunks=n_chunks)
-        _, max_ms, _, _ = stream_through_ring(awg, w, host_mirror, n_chunks=n_chunks, n_slots=3)
-        return max_ms <= deadline_ms, max_ms
+        w = make_workload(n)
+        und, _, _, _ = stream_through_ring(awg, w, host_mirror, n_slots=3)
+        return und == 0
 
     good, bad = None, None
     n = lo
     while n <= hi:  # exponential search for the first failing count
-        passed, _ = ok(n)
-        if passed:
+        if ok(n):
             good = n
             n *= 2
         else:
@@ -351,57 +344,157 @@ def realtime_capacity(torch, awg, fs, chunk_len, mix, host_mirror, seconds, lo=1
         return 0
     if bad is None:
         return good
-    while bad - good > max(8, good // 64):
+    while bad - good > max(8, good // 32):
         mid = (good + bad) // 2
-        passed, _ = ok(mid)
-        if passed:
+        if ok(mid):
             good = mid
         else:
             bad = mid
     return good
 
 
-def run_extras(torch, awg, sm_max_mhz, quick):
+def fast_mover_capacity(torch, awg, fs, chunk_len, lo=16, hi=65536):
+    """Largest count of tones that are ALL inside short minimum-jerk moves all the time (W.fast_mover_stream) whose
+    every chunk is synthesised within chunk_len/fs of device time.  (Streaming such a set through the ring re-plans
+    every tone every chunk on the host, which the host sustains only up to ~1000 tones per 468 us: the criterion here
+    is the device time of the synthesis launches.)"""
+    deadline_ms = chunk_len / fs * 1e3
+
+    def ok(n):
+        _, worst, _ = device_time_chunks(torch, awg, W.fast_mover_stream(n, fs, chunk_len, 6))
+        return worst <= deadline_ms
+
+    good, bad, n = None, None, lo
+    while n <= hi:
+        if ok(n):
+            good, n = n, n * 2
+        else:
+            bad = n
+            break
+    if good is None:
+        return 0
+    if bad is None:
+        return good
+    while bad - good > max(8, good // 32):
+        mid = (good + bad) // 2
+        if ok(mid):
+            good = mid
+        else:
+            bad = mid
+    return good
+
+
+def run_extras(torch, awg, sm_max_mhz):
     out = {}
-    # per-config device throughput (range launch for C1/C3, per-cell chunk launch for C5)
+    # ---- per-config device throughput (range launch for C1/C2, per-cell chunk launch for C5), each with its fraction
     cfgs = {}
-    for name, w in (("C1", W.config1()), ("C3", W.config3())):
+    for name, w in (("C1", W.config1()), ("C2", W.config2())):
         p = awg.Plan.from_workload(w)
         bufs = make_bufs(torch, w.n_samples)
-        ms = device_time_range(torch, p, w.n_chunks, bufs, 5 if name == "C3" else 50, 3)
+        ms = device_time_range(torch, p, w.n_chunks, bufs, 50, 5)
         cfgs[name] = {"tones": w.n_tones, "samples": w.n_samples, "ms": ms, "gts_per_s": w.tone_samples / ms / 1e6,
-                      "out_MS_per_s": w.n_samples / ms / 1e3, "roofline_frac": pipe_roofline(w, ms, "auto", sm_max_mhz)["frac"]}
+                      "out_MS_per_s": w.n_samples / ms / 1e3, **frac_of(p.op_counts(0, w.n_chunks), ms, sm_max_mhz)}
         del bufs
         p.close()
-    w4 = W.config4(96 if quick else 382)
+    # ---- C4 at its stated length: 382 chunks = 1 s at 100 MS/s, 7 258 moves
+    w4 = W.config4(382)
+    ms4, worst4, counts4 = device_time_chunks(torch, awg, w4)
+    cfgs["C4_device"] = {"tones": w4.n_tones, "chunks": w4.n_chunks, "ms_total": ms4, "max_chunk_ms": worst4,
+                         "gts_per_s": w4.tone_samples / ms4 / 1e6, **frac_of(counts4, ms4, sm_max_mhz)}
     for mirror in (False, True):
         und, max_ms, wall, produced = stream_through_ring(awg, w4, mirror)
         cfgs["C4_ring" + ("_d2h" if mirror else "")] = {
             "tones": w4.n_tones, "chunks": produced, "underruns": und, "max_chunk_ms": max_ms,
             "deadline_ms": w4.chunk_len / w4.sample_rate * 1e3, "wall_s": wall,
             "gts_per_s": w4.n_tones * w4.chunk_len * produced / wall / 1e9,
-            "realtime_margin": (w4.chunk_len / w4.sample_rate) / (wall / produced)}
+            "realtime_margin": (w4.chunk_len / w4.sample_rate) / (wall / produced),
+            "roofline_frac": cfgs["C4_device"]["roofline_frac"], "pipe": cfgs["C4_device"]["pipe"],
+            "frac_note": "fraction of the synthesis launches (C4_device); the ring adds host-side update planning and table uploads"}
+    # ---- fast movers: every tone inside a 468 us minimum-jerk move all the time (the MUFU pass)
+    wf = W.fast_mover_stream(4096, 560e6, 1 << 18, 8)
+    msf, worstf, countsf = device_time_chunks(torch, awg, wf)
+    cfgs["FAST_4096"] = {"tones": wf.n_tones, "chunks": wf.n_chunks, "ms_total": msf, "max_chunk_ms": worstf,
+                         "gts_per_s": wf.tone_samples / msf / 1e6, **frac_of(countsf, msf, sm_max_mhz)}
+    # ---- static set (the paper's comb, PAPER.md:198-206), per-sample and through the looped static buffer
+    ws = W.capacity_toneset(4096, 560e6, 1 << 20, "static", n_chunks=4)
+    p = awg.Plan.from_workload(ws)
+    bufs = make_bufs(torch, ws.n_samples)
+    ms = device_time_range(torch, p, ws.n_chunks, bufs, 10, 3)
+    cfgs["STATIC_4096"] = {"tones": ws.n_tones, "samples": ws.n_samples, "ms": ms, "gts_per_s": ws.tone_samples / ms / 1e6,
+                           **frac_of(p.op_counts(0, ws.n_chunks), ms, sm_max_mhz)}
+    del bufs
+    p.close()
+    # static-buffer pathway (NEXT-3): 4096 tones snapped to the fs/L_s grid live in X_static, 64 movers are evaluated
+    L = 1 << 20
+    rng = np.random.default_rng(9)
+    fsn = [awg.awg_snap_frequency(float(f), 560e6, L) for f in rng.uniform(30e6, 250e6, 4096)]
+    f0 = np.concatenate([fsn, rng.uniform(30e6, 250e6, 64)])
+    n = f0.shape[0]
+    prof = np.zeros(n, np.int32); prof[4096:] = W.PROFILE_MINJERK
+    f1 = f0.copy(); f1[4096:] += 5e6
+    tdur = np.zeros(n); tdur[4096:] = 300e-6
+    p = awg.Plan(n, 560e6, L)
+    p.set_trajectories(f0, f1, np.full(n, 1.0 / n), rng.uniform(0, 6.28, n), np.zeros(n), tdur, prof)
+    p.static_buffer_set(np.arange(4096))
+    bufs = make_bufs(torch, 4 * L)
+    ms = device_time_range(torch, p, 4, bufs, 20, 3)
+    cfgs["STATIC_BUFFER_4096+64"] = {
+        "tones": n, "tones_per_sample": 64, "samples": 4 * L, "ms": ms, "effective_gts_per_s": n * 4 * L / ms / 1e6,
+        **frac_of(p.op_counts(0, 4), ms, sm_max_mhz),
+        "note": "4096 on-grid static tones come from the looped X_static (Eq. 9); the fraction counts the 64 evaluated tones only"}
+    del bufs
+    p.close()
+    # four-channel multiplexing (NEXT-2): the paper's chunk, 4 x 2^18 samples, 20 tones per channel (PAPER.md:77, 227)
+    Lm = 1 << 18
+    plans = [awg.Plan.from_workload(W.config5_cell(20, Lm)) for _ in range(4)]
+    outm = [torch.empty(4 * Lm, dtype=torch.int16, device="cuda") for _ in range(32)]
+    stream = torch.cuda.current_stream()
+    for i in range(5):
+        awg.synthesize_chunk_mux(plans, 0, out=outm[i], stream=stream)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record(stream)
+    for i in range(32):
+        awg.synthesize_chunk_mux(plans, 0, out=outm[i], stream=stream)
+    b.record(stream)
+    b.synchronize()
+    ms = a.elapsed_time(b) / 32
+    cm = [sum(x) for x in zip(*[pl.op_counts(0, 1) for pl in plans])]
+    cfgs["MUX4_20x4"] = {"tones_per_channel": 20, "samples_per_channel": Lm, "ms": ms, "gts_per_s": 80 * Lm / ms / 1e6,
+                         "out_MS_per_s_per_channel": Lm / ms / 1e3, "deadline_ms": Lm / 560e6 * 1e3, **frac_of(cm, ms, sm_max_mhz)}
+    for pl in plans:
+        pl.close()
     out["configs"] = cfgs
+    # ---- C5: all 20 cells
     sweep = {}
     for n_t, cl in W.config5_grid():
         w = W.config5_cell(n_t, cl)
         p = awg.Plan.from_workload(w)
         bufs = make_bufs(torch, cl)
         ms = device_time_range(torch, p, 1, bufs, 20, 3)
-        sweep[f"N{n_t}_L{cl.bit_length() - 1}"] = round(w.tone_samples / ms / 1e6, 2)
+        sweep[f"N{n_t}_L{cl.bit_length() - 1}"] = {"gts_per_s": round(w.tone_samples / ms / 1e6, 2), "us": round(ms * 1e3, 2),
+                                                   **frac_of(p.op_counts(0, 1), ms, sm_max_mhz)}
         del bufs
         p.close()
-    out["C5_gts_per_s"] = sweep
-    secs = 0.2 if quick else 1.0
+    out["C5"] = sweep
+    # ---- real-time capacity: ring underruns == 0 over >= 1 s of signal
     cap = {}
     for fs, cl, tag in ((560e6, 1 << 20, "560MS"), (100e6, 1 << 18, "100MS")):
-        for mix in ("static", "half", "moving"):
-            for mirror in (False, True):
-                key = f"{tag}_{mix}" + ("_d2h" if mirror else "")
-                cap[key] = realtime_capacity(torch, awg, fs, cl, mix, mirror, secs)
+        n_chunks = int(math.ceil(1.0 * fs / cl))
+        for mix, key in (("static", "static"), ("half", "half_static_half_fast"), ("moving", "all_slow_movers")):
+            mk = (lambda n, fs=fs, cl=cl, mix=mix, n_chunks=n_chunks: W.capacity_toneset(n, fs, cl, mix, n_chunks=n_chunks))
+            cap[f"{tag}_{key}"] = realtime_capacity(awg, mk, False)
+        cap[f"{tag}_static_d2h"] = realtime_capacity(awg, (lambda n, fs=fs, cl=cl, n_chunks=n_chunks:
+                                                           W.capacity_toneset(n, fs, cl, "static", n_chunks=n_chunks)), True)
+    cap["560MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 560e6, 1 << 18)
+    cap["100MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 100e6, 1 << 15)
     out["max_realtime_tones"] = cap
-    out["max_realtime_tones_note"] = (f"largest N with every chunk's device time <= chunk_len/fs over {secs:g} s of "
-                                      "signal through the ring (3 slots); tone sets drawn like C5; _d2h = pinned-host mirror on")
+    out["max_realtime_tones_note"] = (
+        "largest N streamed through the ring (3 slots) for >= 1 s of signal with the ring's underrun counter at zero; tone sets "
+        "drawn like C5 (2^20-sample chunks at 560 MS/s, 2^18 at 100 MS/s); 'all_slow_movers' = one +-5 MHz minimum-jerk move "
+        "spanning the probe (the slow pass); '_d2h' = pinned-host mirror on; 'all_fast_movers_device_time' = every tone "
+        "inside a one-chunk minimum-jerk move all the time (2^18-sample chunks = 468 us at 560 MS/s, 2^15 = 328 us at "
+        "100 MS/s), criterion: every chunk's synthesis within chunk_len/fs of device time")
     out["paper_context"] = {"hardware": "Quadro RTX 6000 + PCIe 2.0 DAC (PAPER.md:69)", "streaming_tones_560MS": 20,
                             "streaming_tones_100MS": 194, "playback_tones_35ms_560MS": 1000,
                             "static_fp32_gts_per_s": 79.4}
@@ -492,10 +585,11 @@ def run_ours(args):
     traffic = None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get("awg_synth_kernel_C2_dram_bytes_per_launch")
+            traffic = json.load(f).get("awg_synth_kernel_C3_dram_bytes_per_launch")
     except Exception:
         pass
-    roofline = pipe_roofline(w, ms_local, args.engine, sm_max_mhz)
+    counts = plan.op_counts(0, w.n_chunks)
+    roofline = pipe_roofline(counts, ms_local, args.engine, sm_max_mhz)
     roofline.update({
         "traffic": traffic,
         "peak_how": f"{FMA_PER_CLK_PER_SM} FMA (or {MUFU_PER_CLK_PER_SM} MUFU) /clk/SM x {N_SM} SMs x {sm_max_mhz:.0f} MHz "
@@ -505,13 +599,13 @@ def run_ours(args):
                 "peak_gbs": peaks.get("hbm_gbs"), "frac": 2 * w.n_samples / (ms_local * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0))},
     })
     if clocks.get("sm_mhz"):
-        roofline["frac_at_achieved_clock"] = pipe_roofline(w, ms_local, args.engine, clocks["sm_mhz"])["frac"]
+        roofline["frac_at_achieved_clock"] = pipe_roofline(counts, ms_local, args.engine, clocks["sm_mhz"])["frac"]
 
     # ---- oracle on this box's host cores (bounded sample) ----------------------------------------
-    n_cpu = 1 << 22
+    n_cpu = max(1 << 16, min(1 << 22, (1 << 32) // w.n_tones // 4096 * 4096))   # ~4e9 tone-samples: ~10 s on 16 cores
     rate, cores, secs = oracle_rate(w, n_cpu)
     cpu_baseline = {"value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
-                    "sample": f"first {min(n_cpu, w.n_samples)} of {w.n_samples} samples x {w.n_tones} tones of C2, "
+                    "sample": f"first {min(n_cpu, w.n_samples)} of {w.n_samples} samples x {w.n_tones} tones of {w.name}, "
                               f"{secs:.2f} s wall"}
 
     line = {
@@ -521,14 +615,14 @@ def run_ours(args):
         "config": {"workload": w_desc, "engine": args.engine,
                    "tones": w.n_tones, "samples_per_step": w.n_samples, "launch": "one awg_synthesize_range per step",
                    "l2": f"output rotates over {len(bufs)} device buffers ({len(bufs) * 2 * w.n_samples / 1e6:.0f} MB > 126 MB L2); "
-                         "the only input is the 9 KB tone table",
+                         f"the only input is the {w.n_tones * 288 // 1024} KB tone table",
                    "parallelism": "replicas only (no data-path collective)" if world > 1 else "1 GPU"},
         "out_MS_per_s": world * w.n_samples / ms_per_step / 1e3,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu_baseline,
         "phase_dtype": "u64 fixed-point turns + fp64 re-centring, u32/fp32 in the inner loop",
     }
     if world == 1 and not args.no_extras:
-        line["extras"] = run_extras(torch, awg, sm_max_mhz, not args.full)
+        line["extras"] = run_extras(torch, awg, sm_max_mhz)
     plan.close()
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -538,13 +632,12 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", default="C2", help="timed workload (default C2 = the headline; others are profiling aids)")
+    ap.add_argument("--workload", default="C3", help="timed workload (default C3 = the headline; others are profiling aids)")
     ap.add_argument("--engine", choices=sorted(ENGINES), default="auto", help="sine engine of the timed plan")
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs and the capacity search")
-    ap.add_argument("--full", action="store_true", help="extras at full length: 382-chunk C4, 1 s per capacity probe")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
