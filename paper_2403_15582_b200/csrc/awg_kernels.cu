@@ -10,7 +10,7 @@
 //           A sin(phi +- (j+1/2) w) = sin(phi) [A cos((j+1/2) w)]  +-  cos(phi) [A sin((j+1/2) w)]
 //       i.e. ONE fp32 multiply-add per tone-sample into the even/odd accumulators P_j, Q_j    sincos_tile(), pq_add()
 //       Tiles wholly inside a SLOW move: the same with a cubic phase polynomial per thread and a first-order
-//       frequency correction of the pair tables: TWO multiply-adds per tone-sample              stage_slow(), slow_pair()
+//       frequency correction of the pair tables: TWO multiply-adds per tone-sample              stage_slow(), slow_sincos(), slow_fma()
 //       Blocks in which a tone moves otherwise (and every tone-sample of the MUFU engine): one MUFU.SIN each   mufu_rec<KIND>()
 //   a4  fp32 register accumulation over tones: 4 blocks x 16 samples per thread (static pass), 16 (MUFU pass)
 //   a5  quantise: round-half-even and saturate to int16 (fused multiply-add against 1.5*2^23)  pack8()
@@ -257,12 +257,14 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
 
 // ---- shared memory of one warp ------------------------------------------------------------------------------
 // One tile-static tone of the current batch (angle-addition pass): carrier phase (u32 turns) at the half-integer
-// pair centre of lane 0 in block 0 [c0], per sample [c1] and per block [d], and the tone's pair tables.
+// pair centre of lane 0 in block 0 [c0], per sample [c1] and per block [d], the rotation that carries a sine/cosine
+// pair two blocks on, and the tone's pair tables.
 struct __align__(16) StageRec {
     uint32_t c0, c1, d, pad_;
+    float r0, r1, r2, r3;        // static tone: {cos, sin}(2 pi 2 kBlock w), the rotation by two blocks; slow mover: 2 c2, 3 c3
     float4 C03, C47, S03, S47;
 };
-static_assert(sizeof(StageRec) == 80, "StageRec must be 80 bytes");
+static_assert(sizeof(StageRec) == 96, "StageRec must be 96 bytes");
 
 // One re-centred (tone, block) record of the MUFU pass: q[0] = {c0 bits, c1 bits, A, c2}; q[1] = {c3, c4, c5, c6}.
 // K_EXACT: c0 = tone index.
@@ -271,7 +273,7 @@ struct __align__(16) MovRec {
 };
 
 struct __align__(16) WarpSmem {
-    StageRec st[kBatch + 1];                // +1: the loop prefetches one carrier record ahead
+    StageRec st[kBatch + 2];                // +2: the loops prefetch one tone (one or two records) ahead
     MovRec mrec[kBatch + 1];                // +1: the loops prefetch one record ahead
     float4 park[kBlocksPerTile][kSPT / 4][32];   // the warp's static partial sums of the tile: [block][4 samples][lane]
     uint32_t mov[kMaxBatches];              // per batch of 32 tones: which ones take the MUFU pass in this tile
@@ -458,14 +460,6 @@ __device__ __forceinline__ Acc16 pq_to_samples(const PQ &pq)
     return d;
 }
 
-// sin and cos of a u32-turn phase: one range multiply feeds both MUFU operations
-__device__ __forceinline__ void sincos_turns(uint32_t p, float &s, float &c)
-{
-    const float x = __int2float_rn(static_cast<int32_t>(p)) * kTurnToRad;
-    s = mufu_sin(x);
-    c = mufu_cos(x);
-}
-
 // Requests the carrier part of a tone record (A, cls, theta_pre | w_pre, theta_post | w_post, ns_int | ns_frac, Tn) and
 // pulls its two angle-addition tables (bytes 128..287) towards L1.
 __device__ __forceinline__ void fetch_tone(const ToneRec *tr, uint4 &v0, uint4 &v1, uint4 &v2, uint4 &v3)
@@ -481,19 +475,26 @@ __device__ __forceinline__ void fetch_tone(const ToneRec *tr, uint4 &v0, uint4 &
 }
 
 // Sines and cosines of one tile-static tone at the thread's pair centre in each of the tile's four blocks.
-// cc = {phase at lane 0's centre of block 0, phase per sample, phase per block, -} in u32 turns.
-__device__ __forceinline__ void sincos_tile(const uint4 cc, int off, float (&s)[kBlocksPerTile], float (&c)[kBlocksPerTile])
+// rec header = {phase at lane 0's centre of block 0, phase per sample, phase per block, - | cos, sin of the phase of
+// two blocks}.  Blocks 0 and 1 come from MUFU (u32 turns -> radians -> sin.approx, cos.approx); blocks 2 and 3 are those
+// two pairs rotated by two blocks, (s, c) -> (s cd + c sd, c cd - s sd), four packed fp32 instructions for both: a
+// sine/cosine chain through IADD, I2FP, FMUL, FMUL.RZ and two MUFU costs the multiply-add stream more issue slots
+// than the rotation does (profiles/: pipe microbenchmarks).  The rotation constants are rounded once from fp64.
+__device__ __forceinline__ void sincos_tile(const StageRec *rec, int off, float (&s)[kBlocksPerTile], float (&c)[kBlocksPerTile])
 {
-    static_assert(kBlocksPerTile == 4, "sincos_tile packs the four blocks as two pairs");
+    static_assert(kBlocksPerTile == 4, "sincos_tile serves four blocks as two pairs");
+    const uint4 cc = *reinterpret_cast<const uint4 *>(rec);
+    const float2 rot = *reinterpret_cast<const float2 *>(&rec->r0);
     const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(off);
-    const uint32_t p1 = p0 + cc.z, p2 = p1 + cc.z, p3 = p2 + cc.z;
-    const float2 K2 = dup2(kTurnToRad);
-    const float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1))), K2);
-    const float2 x23 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p2)), __int2float_rn(static_cast<int32_t>(p3))), K2);
+    const uint32_t p1 = p0 + cc.z;
+    const float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1))), dup2(kTurnToRad));
     s[0] = mufu_sin(x01.x); c[0] = mufu_cos(x01.x);
     s[1] = mufu_sin(x01.y); c[1] = mufu_cos(x01.y);
-    s[2] = mufu_sin(x23.x); c[2] = mufu_cos(x23.x);
-    s[3] = mufu_sin(x23.y); c[3] = mufu_cos(x23.y);
+    const float2 s01 = make_float2(s[0], s[1]), c01 = make_float2(c[0], c[1]);
+    const float2 s23 = __ffma2_rn(c01, dup2(rot.y), __fmul2_rn(s01, dup2(rot.x)));
+    const float2 c23 = __ffma2_rn(s01, dup2(-rot.y), __fmul2_rn(c01, dup2(rot.x)));
+    s[2] = s23.x; s[3] = s23.y;
+    c[2] = c23.x; c[3] = c23.y;
 }
 
 template <int SPLIT>
@@ -626,7 +627,9 @@ __device__ __forceinline__ int64_t next_unit(const LaunchParams &lp, WarpSmem &w
 
 // Slow pass, staging (one lane per slow mover): the pair tables at the tile-centre frequency c1 come from MUFU
 // (the frequency changes from tile to tile, so they cannot be precomputed), the second record holds their
-// first-order correction: cos((j+1/2)(w + e)) ~ C_j - (j+1/2) e S_j,  sin((j+1/2)(w + e)) ~ S_j + (j+1/2) e C_j.
+// first-order correction: cos((j+1/2)(w + e)) ~ C_j - (j+1/2) e S_j,  sin((j+1/2)(w + e)) ~ S_j + (j+1/2) e C_j,
+// the first record's header also carries the coefficients 2 c2 and 3 c3 of the local frequency offset
+// e(k) = 2 c2 k + 3 c3 k^2.
 __device__ __forceinline__ void stage_slow(StageRec *dst, const MovRec &parked)
 {
     const float4 a = parked.q[0];
@@ -646,38 +649,70 @@ __device__ __forceinline__ void stage_slow(StageRec *dst, const MovRec &parked)
     dst[0].S03 = make_float4(S[0], S[1], S[2], S[3]);
     dst[0].S47 = make_float4(S[4], S[5], S[6], S[7]);
     // correction record: multiplies -sin(phi) e into (j+1/2) S_j and cos(phi) e into (j+1/2) C_j
+    *reinterpret_cast<float4 *>(&dst[0].r0) = make_float4(2.f * a.z, 3.f * a.w, 0.f, 0.f);
     dst[1].C03 = make_float4(0.5f * S[0], 1.5f * S[1], 2.5f * S[2], 3.5f * S[3]);
     dst[1].C47 = make_float4(4.5f * S[4], 5.5f * S[5], 6.5f * S[6], 7.5f * S[7]);
     dst[1].S03 = make_float4(0.5f * C[0], 1.5f * C[1], 2.5f * C[2], 3.5f * C[3]);
     dst[1].S47 = make_float4(4.5f * C[4], 5.5f * C[5], 6.5f * C[6], 7.5f * C[7]);
 }
 
-// Slow pass, one tone: phase polynomial at the thread's pair centre in each block (k = offset from the tile centre),
-// local frequency offset e = d(poly)/dk, then two multiply-adds per tone-sample.
-__device__ __forceinline__ void slow_pair(const StageRec &m, const StageRec &k, int lane, PQ (&pq)[kBlocksPerTile])
+// Slow pass, per-thread constants: offsets of the thread's pair centres from the tile centre in the four blocks
+// (k_r = m_r - 1/2, m_r = r*512 + lane*16 + 8 - 1024), packed over block pairs, and their squares.
+struct SlowK {
+    int m0;
+    float2 kf01, kf23, kk01, kk23;
+};
+
+// Slow pass, one tone at one thread: sines and cosines of the cubic phase polynomial at the thread's pair centre in
+// each block, and the same multiplied by the local frequency offset e = 2 c2 k + 3 c3 k^2 (packed over block pairs:
+// every fp32 instruction here serves two blocks).
+struct SlowSC {
+    float2 s01, s23, c01, c23, se01, se23, ce01, ce23;
+};
+
+__device__ __forceinline__ void slow_sincos(const StageRec *rec, const SlowK &K, SlowSC &o)
 {
-    const uint4 cc = *reinterpret_cast<const uint4 *>(&m);
+    const uint4 cc = *reinterpret_cast<const uint4 *>(rec);                 // c0, c1, c2, c3
+    const float2 g = *reinterpret_cast<const float2 *>(&rec->r0);           // 2 c2, 3 c3
     const float c2 = __uint_as_float(cc.z), c3 = __uint_as_float(cc.w);
-    float s[kBlocksPerTile], c[kBlocksPerTile], e[kBlocksPerTile];
-#pragma unroll
-    for (int r = 0; r < kBlocksPerTile; ++r) {
-        const int mr = r * kBlock + lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre
-        const float kf = static_cast<float>(mr) - 0.5f;
-        const uint32_t p = cc.x + cc.y * static_cast<uint32_t>(mr);
-        const float x = fmaf(__int2float_rn(static_cast<int32_t>(p)), kTurnToRad, kf * kf * fmaf(kf, c3, c2));
-        s[r] = mufu_sin(x);
-        c[r] = mufu_cos(x);
-        e[r] = kf * fmaf(3.f * kf, c3, 2.f * c2);
+    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(K.m0);
+    const uint32_t db = cc.y << 9;                                          // phase per block (kBlock = 512)
+    const uint32_t p1 = p0 + db, p2 = p1 + db, p3 = p2 + db;
+    static_assert(kBlock == 512 && kBlocksPerTile == 4, "slow_sincos assumes four 512-sample blocks");
+    const float2 K2 = dup2(kTurnToRad);
+    const float2 f01 = make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1)));
+    const float2 f23 = make_float2(__int2float_rn(static_cast<int32_t>(p2)), __int2float_rn(static_cast<int32_t>(p3)));
+    const float2 x01 = __ffma2_rn(f01, K2, __fmul2_rn(K.kk01, __ffma2_rn(K.kf01, dup2(c3), dup2(c2))));
+    const float2 x23 = __ffma2_rn(f23, K2, __fmul2_rn(K.kk23, __ffma2_rn(K.kf23, dup2(c3), dup2(c2))));
+    o.s01 = make_float2(mufu_sin(x01.x), mufu_sin(x01.y));
+    o.c01 = make_float2(mufu_cos(x01.x), mufu_cos(x01.y));
+    o.s23 = make_float2(mufu_sin(x23.x), mufu_sin(x23.y));
+    o.c23 = make_float2(mufu_cos(x23.x), mufu_cos(x23.y));
+    const float2 e01 = __fmul2_rn(K.kf01, __ffma2_rn(K.kf01, dup2(g.y), dup2(g.x)));
+    const float2 e23 = __fmul2_rn(K.kf23, __ffma2_rn(K.kf23, dup2(g.y), dup2(g.x)));
+    o.ce01 = __fmul2_rn(o.c01, e01);
+    o.ce23 = __fmul2_rn(o.c23, e23);
+    o.se01 = __fmul2_rn(o.s01, make_float2(-e01.x, -e01.y));
+    o.se23 = __fmul2_rn(o.s23, make_float2(-e23.x, -e23.y));
+}
+
+// Slow pass, the multiply-adds of one tone: two per tone-sample (the tone at the tile-centre frequency, and the
+// first-order frequency correction of its pair tables).
+__device__ __forceinline__ void slow_fma(const StageRec *rec, const SlowSC &v, PQ (&pq)[kBlocksPerTile])
+{
+    {
+        const float4 C03 = rec[0].C03, C47 = rec[0].C47, S03 = rec[0].S03, S47 = rec[0].S47;
+        pq_add(pq[0], v.s01.x, v.c01.x, C03, C47, S03, S47);
+        pq_add(pq[1], v.s01.y, v.c01.y, C03, C47, S03, S47);
+        pq_add(pq[2], v.s23.x, v.c23.x, C03, C47, S03, S47);
+        pq_add(pq[3], v.s23.y, v.c23.y, C03, C47, S03, S47);
     }
     {
-        const float4 C03 = m.C03, C47 = m.C47, S03 = m.S03, S47 = m.S47;
-#pragma unroll
-        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], s[r], c[r], C03, C47, S03, S47);
-    }
-    {
-        const float4 C03 = k.C03, C47 = k.C47, S03 = k.S03, S47 = k.S47;
-#pragma unroll
-        for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], -s[r] * e[r], c[r] * e[r], C03, C47, S03, S47);
+        const float4 C03 = rec[1].C03, C47 = rec[1].C47, S03 = rec[1].S03, S47 = rec[1].S47;
+        pq_add(pq[0], v.se01.x, v.ce01.x, C03, C47, S03, S47);
+        pq_add(pq[1], v.se01.y, v.ce01.y, C03, C47, S03, S47);
+        pq_add(pq[2], v.se23.x, v.ce23.x, C03, C47, S03, S47);
+        pq_add(pq[3], v.se23.y, v.ce23.y, C03, C47, S03, S47);
     }
 }
 
@@ -712,6 +747,15 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
     const int t_begin = rank * per;
     const int t_end = min(lp.n_tones, t_begin + per);
     const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the centre of block 0
+    SlowK slowk;
+    {
+        slowk.m0 = lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre, block 0
+        const float k0 = static_cast<float>(slowk.m0) - 0.5f;
+        slowk.kf01 = make_float2(k0, k0 + static_cast<float>(kBlock));
+        slowk.kf23 = make_float2(k0 + static_cast<float>(2 * kBlock), k0 + static_cast<float>(3 * kBlock));
+        slowk.kk01 = __fmul2_rn(slowk.kf01, slowk.kf01);
+        slowk.kk23 = __fmul2_rn(slowk.kf23, slowk.kf23);
+    }
 
     // Tile scheduler: every team starts on the tile of its own index and then draws tiles from the launch's
     // counter lp.sched[0] (tiles that hold moving tones cost several times the others, so a fixed stride leaves
@@ -847,7 +891,9 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                     *reinterpret_cast<uint4 *>(&sr) = make_uint4(c0, c1, d, 0u);
                     if (!tables_staged) {
                         const float4 C03 = __ldg(tabp), C47 = __ldg(tabp + 1), S03 = __ldg(tabp + 2), S47 = __ldg(tabp + 3);
+                        const float4 R = __ldg(tabp + 4);   // {cos, sin}(two blocks of phase), -, -
                         sr.C03 = C03; sr.C47 = C47; sr.S03 = S03; sr.S47 = S47;
+                        *reinterpret_cast<float4 *>(&sr.r0) = R;
                     }
                 }
                 __syncwarp();
@@ -856,7 +902,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 // 32 FFMA2 of tone i.  Scalar fp32 instructions cost the FMA pipe as much as an FFMA2 (measured,
                 // profiles/), hence the packed range multiply and no register moves.
                 float sa[kBlocksPerTile], ca[kBlocksPerTile], sb[kBlocksPerTile], cb[kBlocksPerTile];
-                sincos_tile(*reinterpret_cast<const uint4 *>(&ws.st[0]), off, sa, ca);
+                sincos_tile(&ws.st[0], off, sa, ca);
                 // a running pointer keeps the loop free of index arithmetic (IMAD shares the FMA pipe)
                 const StageRec *sp = ws.st;
                 const StageRec *const sp_end = ws.st + n_sta;
@@ -864,14 +910,14 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 for (; sp + 1 < sp_end; sp += 2) {
                     {
                         const float4 C03 = sp[0].C03, C47 = sp[0].C47, S03 = sp[0].S03, S47 = sp[0].S47;
-                        sincos_tile(*reinterpret_cast<const uint4 *>(sp + 1), off, sb, cb);
+                        sincos_tile(sp + 1, off, sb, cb);
 #pragma unroll
                         for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
                     }
                     {
                         const float4 C03 = sp[1].C03, C47 = sp[1].C47, S03 = sp[1].S03, S47 = sp[1].S47;
                         // slot i + 2 <= kBatch exists; past the last tone it is stale and its result unused
-                        sincos_tile(*reinterpret_cast<const uint4 *>(sp + 2), off, sa, ca);
+                        sincos_tile(sp + 2, off, sa, ca);
 #pragma unroll
                         for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sb[r], cb[r], C03, C47, S03, S47);
                     }
@@ -893,9 +939,20 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                         __syncwarp();  // the readers of ws.st are done
                         if (is_slow && (lane >> 4) == half) stage_slow(ws.st + 2 * __popc(mh & lt), ws.mrec[lane]);
                         __syncwarp();
-                        const int n_slow = __popc(mh);
+                        // software pipeline over the half's tones, unrolled by two (ping-pong register sets): the phase
+                        // polynomial, sines and cosines of tone i+1 are issued under the 64 FFMA2 of tone i
+                        const StageRec *sp = ws.st;
+                        const StageRec *const sp_end = ws.st + 2 * __popc(mh);
+                        SlowSC va, vb;
+                        slow_sincos(sp, slowk, va);
 #pragma unroll 1
-                        for (int i = 0; i < n_slow; ++i) slow_pair(ws.st[2 * i], ws.st[2 * i + 1], lane, pq);
+                        for (; sp + 2 < sp_end; sp += 4) {
+                            slow_sincos(sp + 2, slowk, vb);
+                            slow_fma(sp, va, pq);
+                            slow_sincos(sp + 4, slowk, va);   // slots up to 2*16 + 1 exist; past the last tone: stale, unused
+                            slow_fma(sp + 2, vb, pq);
+                        }
+                        if (sp < sp_end) slow_fma(sp, va, pq);
                     }
                 }
             }
@@ -1027,7 +1084,19 @@ __global__ void __launch_bounds__(128) awg_expand_kernel(ToneRec *table, const T
     ToneRec &dst = table[idx ? idx[j] : j];
     if (lane < 8) reinterpret_cast<uint4 *>(&dst.core)[lane] = reinterpret_cast<const uint4 *>(&c)[lane];
     if (lane >= 2 * kPairs) {
-        if (lane < 2 * kPairs + 8) (lane < 2 * kPairs + 4 ? dst.rot_pre : dst.rot_post).pad_[lane & 3] = 0.f;
+        // pad_[0], pad_[1] of each table: cosine and sine of the carrier phase of two blocks (the rotation that takes the
+        // sines/cosines of blocks 0, 1 to blocks 2, 3 in the static pass); pad_[2], pad_[3] = 0
+        if (lane < 2 * kPairs + 8) {
+            const int st = (lane - 2 * kPairs) >> 2, q = lane & 3;
+            float v = 0.f;
+            if (q < 2) {
+                const uint64_t ang2 = (st ? c.w_post : c.w_pre) * static_cast<uint64_t>(2 * kBlock);
+                double sn2, cs2;
+                sincospi(2.0 * (static_cast<double>(static_cast<int64_t>(ang2)) * (1.0 / kTwo64)), &sn2, &cs2);
+                v = static_cast<float>(q == 0 ? cs2 : sn2);
+            }
+            (st ? dst.rot_post : dst.rot_pre).pad_[q] = v;
+        }
         return;
     }
     const int state = lane / kPairs, p = lane % kPairs;

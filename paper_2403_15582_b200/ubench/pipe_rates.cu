@@ -1,0 +1,288 @@
+// pipe_rates.cu -- instruction-mix microbenchmarks behind the roofline peaks and the loop design of DESIGN.md section 6.
+//
+// Not part of the library (nothing links it).  Build and run on a B200:
+//     nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -o /tmp/pipe_rates paper_2403_15582_b200/ubench/pipe_rates.cu
+//     /tmp/pipe_rates [warps_per_smsp=4]
+// Every body is an unrolled block of independent instructions (inline PTX, so the mix is what the line says); a warp
+// runs it kIters times, `warps_per_smsp` warps share a scheduler, every SM is filled.  Printed: SM cycles (clock64, the
+// slowest CTA) per body per scheduler (SMSP), i.e. the cycles one SMSP needs for one body of EVERY resident warp divided
+// by the warps -- the reciprocal throughput of the mix, independent of the clock the GPU runs at.
+#include <cstdio>
+#include <cstdlib>
+#include <cuda_runtime.h>
+
+constexpr int kIters = 4096;
+
+#define FFMA2(acc, a, b) asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b))
+#define HFMA2(acc, a, b) asm volatile("fma.rn.f16x2 %0, %1, %2, %0;" : "+r"(acc) : "r"(a), "r"(b))
+#define FFMA(acc, a, b) asm volatile("fma.rn.f32 %0, %1, %2, %0;" : "+f"(acc) : "f"(a), "f"(b))
+#define FMUL(acc, a) asm volatile("mul.rn.f32 %0, %0, %1;" : "+f"(acc) : "f"(a))
+#define FMUL2(acc, a) asm volatile("mul.rn.f32x2 %0, %0, %1;" : "+l"(acc) : "l"(a))
+#define MUFU_SIN(acc) asm volatile("sin.approx.ftz.f32 %0, %0;" : "+f"(acc))
+#define MUFU_EX2(acc) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(acc))
+#define IADD(acc, a) asm volatile("add.u32 %0, %0, %1;" : "+r"(acc) : "r"(a))
+#define IMAD(acc, a, b) asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc) : "r"(a), "r"(b))
+#define I2F(dst, src) asm volatile("cvt.rn.f32.s32 %0, %1;" : "=f"(dst) : "r"(src))
+#define LDS128(dst, addr) asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(dst.x), "=f"(dst.y), "=f"(dst.z), "=f"(dst.w) : "r"(addr))
+
+template <int MODE>
+__global__ void __launch_bounds__(128) bench(float *out, unsigned long long seed, int n_iter, unsigned long long *cycles)
+{
+    const long long t_begin = clock64();
+    __shared__ float4 sm[64];
+    if (threadIdx.x < 64) sm[threadIdx.x] = make_float4(1.f, 1.0001f, 0.9999f, 1.f);
+    __syncthreads();
+    unsigned long long a2[32], x2 = seed | 0x3f8000003f800000ull, y2 = 0x3a0000003a000000ull;
+    unsigned h2[32], hx = 0x3c003c00u, hy = 0x10001000u;
+    float f[16], fa = 1.0001f;
+    unsigned u[16], ua = 3u + threadIdx.x;
+    float4 t[8];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) { a2[i] = seed + i; h2[i] = static_cast<unsigned>(seed) + i; }
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { f[i] = 0.001f * i + threadIdx.x; u[i] = i * 7u + threadIdx.x; }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) t[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    const unsigned sbase = static_cast<unsigned>(__cvta_generic_to_shared(sm));
+#pragma unroll 1
+    for (int it = 0; it < n_iter; ++it) {
+        if (MODE == 0) {          // 32 FFMA2
+#pragma unroll
+            for (int i = 0; i < 32; ++i) FFMA2(a2[i], x2, y2);
+        } else if (MODE == 1) {   // 32 HFMA2
+#pragma unroll
+            for (int i = 0; i < 32; ++i) HFMA2(h2[i], hx, hy);
+        } else if (MODE == 2) {   // 32 FFMA2 + 32 HFMA2 interleaved
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); HFMA2(h2[i], hx, hy); }
+        } else if (MODE == 3) {   // 32 FFMA2 + 16 HFMA2
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if (i & 1) HFMA2(h2[i], hx, hy); }
+        } else if (MODE == 4) {   // 32 FFMA2 + 8 scalar FMUL
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 3) == 3) FMUL(f[i >> 2], fa); }
+        } else if (MODE == 5) {   // 32 FFMA2 + 8 FMUL2
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 3) == 3) FMUL2(a2[i - 1], x2); }
+        } else if (MODE == 6) {   // 32 FFMA2 + 8 pairs of adjacent scalar FMUL (16 FMUL)
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 3) == 3) { FMUL(f[i >> 2], fa); FMUL(f[8 + (i >> 2)], fa); } }
+        } else if (MODE == 7) {   // 32 FFMA2 + 8 MUFU.EX2
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 3) == 3) MUFU_EX2(f[i >> 2]); }
+        } else if (MODE == 8) {   // 32 FFMA2 + 8 sin.approx (FMUL.RZ + MUFU.SIN)
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 3) == 3) MUFU_SIN(f[i >> 2]); }
+        } else if (MODE == 9) {   // 32 FFMA2 + 4 MUFU.EX2
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 7) == 7) MUFU_EX2(f[i >> 3]); }
+        } else if (MODE == 10) {  // 32 FFMA2 + 5 LDS.128 broadcast
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if (i % 6 == 5) LDS128(t[i / 6], sbase + 16 * (i / 6)); }
+        } else if (MODE == 11) {  // 32 FFMA2 + 9 LDS.128 broadcast
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if (i % 4 == 3) LDS128(t[i / 4], sbase + 16 * (i / 4)); }
+        } else if (MODE == 12) {  // 32 FFMA2 + 16 IADD + 8 I2F
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if (i & 1) IADD(u[i >> 1], ua); if ((i & 3) == 3) I2F(f[i >> 2], u[i >> 2]); }
+        } else if (MODE == 13) {  // 32 FFMA2 + 4 IMAD
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 7) == 7) IMAD(u[i >> 3], ua, ua); }
+        } else if (MODE == 14) {  // 64 scalar FFMA
+#pragma unroll
+            for (int i = 0; i < 16; ++i) { FFMA(f[i], fa, fa); FFMA(f[i], fa, fa); FFMA(f[i], fa, fa); FFMA(f[i], fa, fa); }
+        } else if (MODE == 15) {  // static-loop mix: 32 FFMA2 + 5 LDS.128 + 8 MUFU(4 sin.approx pairs ~ 4 FMUL.RZ) + 2 FMUL2 + 4 I2F + 4 IADD + 1 IMAD
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                FFMA2(a2[i], x2, y2);
+                if (i % 6 == 5) LDS128(t[i / 6], sbase + 16 * (i / 6));
+                if ((i & 7) == 3) MUFU_SIN(f[i >> 3]);
+                if ((i & 7) == 7) MUFU_EX2(f[8 + (i >> 3)]);
+                if ((i & 15) == 9) FMUL2(a2[i - 1], x2);
+                if ((i & 7) == 1) { IADD(u[i >> 3], ua); I2F(f[4 + (i >> 3)], u[i >> 3]); }
+                if (i == 20) IMAD(u[8], ua, ua);
+            }
+        } else if (MODE == 16) {  // 16 FFMA2 + 16 HFMA2 (slow-pass idea: correction in half precision)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) { FFMA2(a2[i], x2, y2); HFMA2(h2[i], hx, hy); }
+        } else if (MODE == 18) {  // 32 FFMA2 + 8 I2F
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 3) == 3) I2F(f[i >> 2], u[i >> 2]); }
+        } else if (MODE == 19) {  // 32 FFMA2 + 16 LOP3 (xor)
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if (i & 1) asm volatile("xor.b32 %0, %0, %1;" : "+r"(u[i >> 1]) : "r"(ua)); }
+        } else if (MODE == 20) {  // 32 FFMA2 + 4 I2F
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); if ((i & 7) == 7) I2F(f[i >> 3], u[i >> 3]); }
+        } else if (MODE == 21) {  // 32 FFMA2 + 32 LOP3
+#pragma unroll
+            for (int i = 0; i < 32; ++i) { FFMA2(a2[i], x2, y2); asm volatile("xor.b32 %0, %0, %1;" : "+r"(u[i & 15]) : "r"(ua)); }
+        } else if (MODE == 22) {  // rotation mix: 32 FFMA2 + 5 LDS.128 + 2 sin.approx + 2 MUFU.EX2 + 1 FMUL2 + 4 packed rotation ops (2 FMUL2 + 2 FFMA2) + 2 I2F
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                FFMA2(a2[i], x2, y2);
+                if (i % 6 == 5) LDS128(t[i / 6], sbase + 16 * (i / 6));
+                if ((i & 15) == 3) MUFU_SIN(f[i >> 4]);
+                if ((i & 15) == 7) MUFU_EX2(f[8 + (i >> 4)]);
+                if (i == 9) FMUL2(a2[i - 1], x2);
+                if (i == 13 || i == 21) FMUL2(a2[i - 2], x2);
+                if (i == 17 || i == 25) FFMA2(a2[i - 3], x2, y2);
+                if ((i & 15) == 1) I2F(f[4 + (i >> 4)], u[i >> 4]);
+            }
+        } else if (MODE == 23) {  // slow-pass mix: 64 FFMA2 + 9 LDS.128 + 4 sin.approx + 4 MUFU.EX2 + 10 packed fp32x2 + 4 I2F
+#pragma unroll
+            for (int i = 0; i < 64; ++i) {
+                FFMA2(a2[i & 31], x2, y2);
+                if (i % 7 == 6) LDS128(t[(i / 7) & 7], sbase + 16 * (i / 7));
+                if ((i & 15) == 3) MUFU_SIN(f[i >> 4]);
+                if ((i & 15) == 7) MUFU_EX2(f[8 + (i >> 4)]);
+                if (i % 6 == 2) FMUL2(a2[(i + 5) & 31], x2);
+                if ((i & 15) == 1) I2F(f[4 + (i >> 4)], u[i >> 4]);
+            }
+        } else if (MODE == 17) {  // 8 MUFU.SIN alone
+#pragma unroll
+            for (int i = 0; i < 8; ++i) MUFU_SIN(f[i]);
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 32; ++i) s += static_cast<float>(a2[i] & 0xff) + static_cast<float>(h2[i] & 0xff);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += f[i] + static_cast<float>(u[i]);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += t[i].x + t[i].y + t[i].z + t[i].w;
+    if (s == 123.456f) out[0] = s;
+    if (threadIdx.x == 0) atomicMax(cycles, static_cast<unsigned long long>(clock64() - t_begin));
+}
+
+// The multiply-add block of the angle-addition pass as the library writes it: 4 blocks x (4 P + 4 Q) packed accumulators,
+// one tone's pair tables from shared memory (4 broadcast LDS.128), sines/cosines broadcast from scalar registers.
+// WITH_SINCOS adds the per-tone chain IMAD, IADD, I2F, FMUL2, sin.approx, cos.approx of the four blocks (software-pipelined
+// one tone ahead as in the library).
+template <bool WITH_SINCOS>
+__global__ void __launch_bounds__(128) pq_loop(float *out, int n_iter, unsigned long long *cycles)
+{
+    const long long t_begin = clock64();
+    __shared__ float4 tab[64 * 5];
+    for (int i = threadIdx.x; i < 64 * 5; i += 128) tab[i] = make_float4(1e-3f * i, 1.f, 0.5f, 0.25f);
+    __syncthreads();
+    float2 P[4][4], Q[4][4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int m = 0; m < 4; ++m) P[r][m] = Q[r][m] = make_float2(0.f, 0.f);
+    float sn[4] = {0.1f, 0.2f, 0.3f, 0.4f}, cs[4] = {0.9f, 0.8f, 0.7f, 0.6f};
+    const int lane = threadIdx.x & 31;
+    const float4 *tp = tab;
+#pragma unroll 1
+    for (int it = 0; it < n_iter; ++it) {
+        const float4 *rec = tp + 5 * (it & 63);
+        const float4 C03 = rec[1], C47 = rec[2], S03 = rec[3], S47 = rec[4];
+        float sn2[4], cs2[4];
+        if (WITH_SINCOS) {
+            const uint4 cc = *reinterpret_cast<const uint4 *>(tp + 5 * ((it + 1) & 63));
+            unsigned p0 = cc.x + cc.y * static_cast<unsigned>(lane * 16 - 248);
+            unsigned p1 = p0 + cc.z, p2 = p1 + cc.z, p3 = p2 + cc.z;
+            const float k = 1.4629180792671596e-9f;
+            float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int>(p0)), __int2float_rn(static_cast<int>(p1))), make_float2(k, k));
+            float2 x23 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int>(p2)), __int2float_rn(static_cast<int>(p3))), make_float2(k, k));
+            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[0]) : "f"(x01.x)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[0]) : "f"(x01.x));
+            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[1]) : "f"(x01.y)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[1]) : "f"(x01.y));
+            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[2]) : "f"(x23.x)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[2]) : "f"(x23.x));
+            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[3]) : "f"(x23.y)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[3]) : "f"(x23.y));
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const float2 s2 = make_float2(sn[r], sn[r]), c2 = make_float2(cs[r], cs[r]);
+            P[r][0] = __ffma2_rn(s2, make_float2(C03.x, C03.y), P[r][0]);
+            P[r][1] = __ffma2_rn(s2, make_float2(C03.z, C03.w), P[r][1]);
+            P[r][2] = __ffma2_rn(s2, make_float2(C47.x, C47.y), P[r][2]);
+            P[r][3] = __ffma2_rn(s2, make_float2(C47.z, C47.w), P[r][3]);
+            Q[r][0] = __ffma2_rn(c2, make_float2(S03.x, S03.y), Q[r][0]);
+            Q[r][1] = __ffma2_rn(c2, make_float2(S03.z, S03.w), Q[r][1]);
+            Q[r][2] = __ffma2_rn(c2, make_float2(S47.x, S47.y), Q[r][2]);
+            Q[r][3] = __ffma2_rn(c2, make_float2(S47.z, S47.w), Q[r][3]);
+        }
+        if (WITH_SINCOS) {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) { sn[r] = sn2[r]; cs[r] = cs2[r]; }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int m = 0; m < 4; ++m) s += P[r][m].x + P[r][m].y + Q[r][m].x + Q[r][m].y;
+    if (s == 123.456f) out[0] = s;
+    if (threadIdx.x == 0) atomicMax(cycles, static_cast<unsigned long long>(clock64() - t_begin));
+}
+
+template <bool WITH_SINCOS>
+void run_pq(const char *what, int n_sm, int wps, float *out)
+{
+    unsigned long long *cyc_dev, cyc_host = 0;
+    cudaMalloc(&cyc_dev, sizeof cyc_host);
+    pq_loop<WITH_SINCOS><<<n_sm * wps, 128>>>(out, 64, cyc_dev);
+    cudaMemset(cyc_dev, 0, sizeof cyc_host);
+    pq_loop<WITH_SINCOS><<<n_sm * wps, 128>>>(out, kIters, cyc_dev);
+    cudaMemcpy(&cyc_host, cyc_dev, sizeof cyc_host, cudaMemcpyDeviceToHost);
+    cudaFree(cyc_dev);
+    printf("%-100s %8.2f cycles/body/SMSP\n", what, static_cast<double>(cyc_host) / (static_cast<double>(kIters) * wps));
+}
+
+template <int MODE>
+void run(const char *what, int n_sm, int wps, double mhz, float *out)
+{
+    const int ctas = n_sm * wps;  // 4 warps per CTA: one per scheduler
+    unsigned long long *cyc_dev, cyc_host = 0;
+    cudaMalloc(&cyc_dev, sizeof cyc_host);
+    bench<MODE><<<ctas, 128>>>(out, 1ull, 64, cyc_dev);
+    cudaMemset(cyc_dev, 0, sizeof cyc_host);
+    bench<MODE><<<ctas, 128>>>(out, 1ull, kIters, cyc_dev);
+    cudaMemcpy(&cyc_host, cyc_dev, sizeof cyc_host, cudaMemcpyDeviceToHost);
+    cudaFree(cyc_dev);
+    (void)mhz;
+    // SM cycles (clock64) of the slowest CTA: independent of the clock the GPU happens to run at
+    printf("%-100s %8.2f cycles/body/SMSP\n", what, static_cast<double>(cyc_host) / (static_cast<double>(kIters) * wps));
+}
+
+int main(int argc, char **argv)
+{
+    const int wps = argc > 1 ? atoi(argv[1]) : 4;
+    cudaDeviceProp pr;
+    cudaGetDeviceProperties(&pr, 0);
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, 0);
+    const double mhz = khz / 1e3;
+    float *out;
+    cudaMalloc(&out, 64);
+    printf("%s, %d SMs, %.0f MHz (max SM clock), %d warps per SMSP\n", pr.name, pr.multiProcessorCount, mhz, wps);
+    const int n = pr.multiProcessorCount;
+    run<0>("32 FFMA2", n, wps, mhz, out);
+    run<1>("32 HFMA2", n, wps, mhz, out);
+    run<2>("32 FFMA2 + 32 HFMA2", n, wps, mhz, out);
+    run<3>("32 FFMA2 + 16 HFMA2", n, wps, mhz, out);
+    run<16>("16 FFMA2 + 16 HFMA2", n, wps, mhz, out);
+    run<4>("32 FFMA2 + 8 FMUL (scalar)", n, wps, mhz, out);
+    run<5>("32 FFMA2 + 8 FMUL2", n, wps, mhz, out);
+    run<6>("32 FFMA2 + 8 x 2 adjacent scalar FMUL", n, wps, mhz, out);
+    run<7>("32 FFMA2 + 8 MUFU.EX2", n, wps, mhz, out);
+    run<8>("32 FFMA2 + 8 sin.approx (FMUL.RZ + MUFU.SIN)", n, wps, mhz, out);
+    run<9>("32 FFMA2 + 4 MUFU.EX2", n, wps, mhz, out);
+    run<10>("32 FFMA2 + 5 LDS.128 (broadcast)", n, wps, mhz, out);
+    run<11>("32 FFMA2 + 8 LDS.128 (broadcast)", n, wps, mhz, out);
+    run<12>("32 FFMA2 + 16 IADD + 8 I2F", n, wps, mhz, out);
+    run<13>("32 FFMA2 + 4 IMAD", n, wps, mhz, out);
+    run<14>("64 FFMA (scalar)", n, wps, mhz, out);
+    run<15>("static-loop mix: 32 FFMA2 + 5 LDS.128 + 4 sin.approx + 4 MUFU.EX2 + 2 FMUL2 + 4 IADD + 4 I2F + 1 IMAD", n, wps, mhz, out);
+    run<17>("8 sin.approx", n, wps, mhz, out);
+    run<18>("32 FFMA2 + 8 I2F", n, wps, mhz, out);
+    run<20>("32 FFMA2 + 4 I2F", n, wps, mhz, out);
+    run<19>("32 FFMA2 + 16 LOP3", n, wps, mhz, out);
+    run<21>("32 FFMA2 + 32 LOP3", n, wps, mhz, out);
+    run<22>("rotation mix: 32 FFMA2 + 5 LDS.128 + 2 sin.approx + 2 MUFU.EX2 + 3 FMUL2 + 2 more FFMA2 + 2 I2F", n, wps, mhz, out);
+    run<23>("slow-pass mix: 64 FFMA2 + 9 LDS.128 + 4 sin.approx + 4 MUFU.EX2 + 11 FMUL2 + 4 I2F", n, wps, mhz, out);
+    run_pq<false>("library multiply-add block: 32 FFMA2 (distinct accumulators, tables from 4 LDS.128, broadcast sines)", n, wps, out);
+    run_pq<true>("library static loop: the same + IMAD, 3 IADD, 4 I2F, 2 FMUL2, 4 sin.approx, 4 cos.approx per tone", n, wps, out);
+    return 0;
+}
