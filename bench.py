@@ -253,13 +253,19 @@ def pick_workload(name: str):
 
 
 # --------------------------------------------------------------------------------------------------
-def device_time_range(torch, plan, n_chunks, bufs, steps, warmup):
-    """ms per step of awg_synthesize_range, CUDA events on the launch stream, rotating output buffers."""
+def device_time_range(torch, plan, n_chunks, bufs, steps, warmup, prequeue_ms=0.0):
+    """ms per step of awg_synthesize_range, CUDA events on the launch stream, rotating output buffers.
+
+    prequeue_ms > 0: the timed launches are queued behind a spin kernel of about that length (torch.cuda._sleep), so the
+    host has submitted all of them before the first one starts and the events bracket back-to-back DEVICE execution; used
+    for launches of a few microseconds, where a Python call (~10 us) would otherwise be what the events time."""
     stream = torch.cuda.current_stream()
     for i in range(warmup):
         plan.synthesize_range(0, n_chunks, out=bufs[i % len(bufs)], stream=stream)
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    if prequeue_ms > 0.0:
+        torch.cuda._sleep(int(prequeue_ms * 1e-3 * 1.9e9))
     a.record(stream)
     for i in range(steps):
         plan.synthesize_range(0, n_chunks, out=bufs[i % len(bufs)], stream=stream)
@@ -391,8 +397,9 @@ def run_extras(torch, awg, sm_max_mhz):
     for name, w in (("C1", W.config1()), ("C2", W.config2())):
         p = awg.Plan.from_workload(w)
         bufs = make_bufs(torch, w.n_samples)
-        ms = device_time_range(torch, p, w.n_chunks, bufs, 50, 5)
-        cfgs[name] = {"tones": w.n_tones, "samples": w.n_samples, "ms": ms, "gts_per_s": w.tone_samples / ms / 1e6,
+        ms_host = device_time_range(torch, p, w.n_chunks, bufs, 50, 5)
+        ms = device_time_range(torch, p, w.n_chunks, bufs, 50, 5, prequeue_ms=3.0)
+        cfgs[name] = {"tones": w.n_tones, "samples": w.n_samples, "ms": ms, "ms_host_paced": ms_host, "gts_per_s": w.tone_samples / ms / 1e6,
                       "out_MS_per_s": w.n_samples / ms / 1e3, **frac_of(p.op_counts(0, w.n_chunks), ms, sm_max_mhz)}
         del bufs
         p.close()
@@ -453,6 +460,7 @@ def run_extras(torch, awg, sm_max_mhz):
         awg.synthesize_chunk_mux(plans, 0, out=outm[i], stream=stream)
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    torch.cuda._sleep(int(3e-3 * 1.9e9))   # queue pre-filled behind a 3 ms spin: the events time the device, not the Python caller
     a.record(stream)
     for i in range(32):
         awg.synthesize_chunk_mux(plans, 0, out=outm[i], stream=stream)
@@ -465,14 +473,17 @@ def run_extras(torch, awg, sm_max_mhz):
     for pl in plans:
         pl.close()
     out["configs"] = cfgs
-    # ---- C5: all 20 cells
+    # ---- C5: all 20 cells.  us = device time per launch with the queue pre-filled (launches of a few microseconds are
+    # otherwise paced by the Python caller); us_host_paced = the same launches submitted back to back from Python
     sweep = {}
     for n_t, cl in W.config5_grid():
         w = W.config5_cell(n_t, cl)
         p = awg.Plan.from_workload(w)
         bufs = make_bufs(torch, cl)
-        ms = device_time_range(torch, p, 1, bufs, 20, 3)
+        ms_host = device_time_range(torch, p, 1, bufs, 20, 3)
+        ms = device_time_range(torch, p, 1, bufs, 40, 3, prequeue_ms=max(1.0, 40 * 0.03))
         sweep[f"N{n_t}_L{cl.bit_length() - 1}"] = {"gts_per_s": round(w.tone_samples / ms / 1e6, 2), "us": round(ms * 1e3, 2),
+                                                   "us_host_paced": round(ms_host * 1e3, 2),
                                                    **frac_of(p.op_counts(0, 1), ms, sm_max_mhz)}
         del bufs
         p.close()

@@ -84,6 +84,18 @@ struct __align__(16) ToneRec {
 };
 static_assert(sizeof(ToneRec) == 288, "ToneRec must be 288 bytes");
 
+// Fixed-point grids on which the leaves of a large table are merged (exact integer sums; awg_kernels.cu).  A leaf's fp32
+// sum v is first rounded to its OWN grid 2^-leaf_sh[leaf] (|v 2^leaf_sh| < 2^22: one fused multiply-add against 1.5 * 2^23)
+// whose step follows the leaf's own sum of amplitudes, then shifted on to the common grid 2^-fix_sh on which no partial
+// sum of the table reaches 2^30; quad_sh: the same for the summed moving tones of a quad.
+struct FixGrid {
+    int32_t fix_sh;
+    float fix_inv;       // 2^-fix_sh
+    int8_t leaf_sh[64];  // [quad * 4 + rank]
+    int8_t quad_sh[16];
+    uint32_t bias_q[16]; // bits(1.5 * 2^23) * sum over the quad's leaves of 2^(fix_sh - leaf_sh), mod 2^32: the magic-number bias parked with them
+};
+
 struct LaunchParams {
     const ToneRec *tab;
     int32_t n_tones;
@@ -98,12 +110,24 @@ struct LaunchParams {
     const float *xs;   // looped static buffer X_static (Eq. 9) added before quantisation, or nullptr
     int64_t xs_len;    //   its length L_s (a multiple of 8, >= kTile)
     uint32_t *sched;   // {next tile, teams finished}: the launch's tile-scheduler slot (filled in by launch_synth)
+    // tone groups (tone_groups(); filled in by launch_synth): a team's warp takes `per` tones of quad q, a tile has n_quads quads
+    int32_t per;
+    int32_t n_quads;
+    int32_t cross;       // != 0: the quads of a tile are separate work units (launches with few tiles); their sums meet in `scratch`
+    int32_t *scratch;    //   [tile][block][kBlock] int32 fixed point, this launch's slot (zero before and after the launch)
+    uint32_t *tile_cnt;  //   quads delivered per tile (zero before and after the launch)
+    FixGrid fix;         // fixed-point grids of the leaf merge (fix_grids(); large tables only)
 };
 
 // Warps of a team share a tile, each taking 1/split of the tones.  A function of the tone count ONLY, never of the
 // launch size: the order in which tone partial sums are added is then the same for every chunking (bit-identical
 // output across chunk sizes, include/awg.h "pure function").
 int split_for(int n_tones);
+// Tone groups of the synthesis kernel: `split` warps share a tile, warp `rank` takes `per` tones of each of the `quads`
+// quads.  Functions of the tone count only (see split_for): the grouping fixes the fp32 summation order.
+void tone_groups(int n_tones, int *split, int *per, int *quads);
+// amp: max(|A|, |A1|) per tone of the table (host array, n_tones entries)
+void fix_grids(const float *amp, int n_tones, FixGrid *out);
 
 cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream);
 // table[idx ? idx[j] : j] = expand(src[j]) for j < n: copies the core and builds both carrier tables (fp64 sincospi)

@@ -17,6 +17,8 @@
 //   a6  two 16-byte stores of 8 consecutive int16 per thread and block                       store_block()
 // No tensor cores (north_star), no per-tone wavetable in DRAM (the paper's limiter); output
 // traffic is 2 bytes per sample.
+#include <algorithm>
+#include <cmath>
 #include <cstddef>
 #include <cstdint>
 #include <atomic>
@@ -38,13 +40,72 @@ int split_for(int n_tones)
     return split;
 }
 
+void tone_groups(int n_tones, int *split, int *per, int *quads)
+{
+    const int sp = split_for(n_tones);
+    int q = 1;
+    // Large tables are cut into leaves of <= 64 tones (<= 128 above 2048 tones), four per quad, at most 16 quads: a leaf is
+    // summed from zero in fp32 and the leaves are merged in fixed point (exact), so a launch with few tiles can spread a
+    // tile's quads over CTAs and still produce the same bits as a large launch that walks them inside one CTA.  Measured
+    // cost of the leaf boundaries in a large launch: 1 % (4096 tones, 8 quads) to 3 % (1000 tones, 4 quads).
+    const int leaf = n_tones <= 2048 ? 64 : 128;
+    if (sp == 4 && n_tones > 4 * leaf) {
+        q = (n_tones + 4 * leaf - 1) / (4 * leaf);
+        if (q > 16) q = 16;
+    }
+    int pr = (n_tones + sp * q - 1) / (sp * q);
+    if (pr < 1) pr = 1;                        // (an empty table: every tone is served by the static buffer)
+    q = (n_tones + sp * pr - 1) / (sp * pr);   // no empty quad
+    if (q < 1) q = 1;
+    *split = sp;
+    *per = pr;
+    *quads = q;
+}
+
+static int exponent_above(double a)
+{
+    // smallest e with a (1 + margin) < 2^e; sums of amplitudes down to 2^-64 keep their own grid
+    int ex = 0;
+    a = a * 1.001 + 5e-20;
+    (void)std::frexp(a, &ex);   // a = m 2^ex, m in [1/2, 1)
+    return ex;
+}
+
+void fix_grids(const float *amp, int n_tones, FixGrid *out)
+{
+    int split = 1, per = 1, quads = 1;
+    tone_groups(n_tones, &split, &per, &quads);
+    FixGrid g{};
+    double total = 0.0;
+    for (int t = 0; t < n_tones; ++t) total += static_cast<double>(amp[t]);
+    g.fix_sh = 30 - exponent_above(total);
+    g.fix_inv = static_cast<float>(std::ldexp(1.0, -g.fix_sh));
+    for (int q = 0; q < 16; ++q) {
+        double aq = 0.0;
+        g.bias_q[q] = 0;
+        for (int r = 0; r < 4; ++r) {
+            double al = 0.0;
+            if (q < quads && r < split) {
+                const int t0 = std::min((q * split + r) * per, n_tones), t1 = std::min(n_tones, t0 + per);
+                for (int t = t0; t < t1; ++t) al += static_cast<double>(amp[t]);
+            }
+            aq += al;
+            g.leaf_sh[q * 4 + r] = static_cast<int8_t>(std::min(22 - exponent_above(al), g.fix_sh));
+            if (q < quads && r < split) g.bias_q[q] += 0x4B400000u * (1u << (g.fix_sh - g.leaf_sh[q * 4 + r]));
+        }
+        g.quad_sh[q] = static_cast<int8_t>(std::min(22 - exponent_above(aq), g.fix_sh));
+    }
+    *out = g;
+}
+
 namespace {
 
 constexpr int kHalf = kBlock / 2;     // Taylor expansions are centred on the block
 constexpr int kWarps = 4;             // warps per CTA
 constexpr int kCtasPerSm = 3;         // 12 warps per SM leave 168 registers per thread: tables and sines double-buffered
 constexpr int kBatch = 32;            // tones (pass 1) or (tone, block) items (pass 2) per batch: one per lane
-constexpr int kMaxBatches = 65536 / kWarps / kBatch;   // per warp, at the largest tone count and widest split
+constexpr int kMaxBatches = 65536 / kWarps / kBatch;   // per warp (all its leaves), at the largest tone count and widest split
+constexpr int kMaxQuads = 16;                          // leaves per warp and tile (awg::tone_groups)
 constexpr float kTurnToRad = 1.4629180792671596e-9f;   // 2*pi / 2^32: int32 phase (turns * 2^32) -> radians
 constexpr double kTwo64 = 18446744073709551616.0;
 constexpr int kListBatches = 8;                        // batches of 32 tones compacted at a time for the MUFU pass
@@ -279,7 +340,9 @@ struct __align__(16) WarpSmem {
     uint32_t mov[kMaxBatches];              // per batch of 32 tones: which ones take the MUFU pass in this tile
     uint32_t next;                          // (rank-0 warp of a team) the team's next tile, drawn by the leader
     uint32_t n_mov;                         // how many of the warp's tones take the MUFU pass in this tile
-    uint32_t pad_[2];
+    uint32_t last;                          // (warp 0) this CTA delivered the last quad of its tile: it sums and stores
+    uint32_t pad_[1];
+    uint16_t nm_leaf[kMaxQuads];            // per leaf of the warp: how many of its tones take the MUFU pass in this tile
     uint16_t list[kListCap];                // compacted tone indices of the MUFU pass (n_tones <= 65536)
 };
 
@@ -302,6 +365,59 @@ __device__ __forceinline__ void park_add(const WarpSmem &ws, int r, int lane, Ac
         const float4 u = ws.park[r][v][lane];
         acc.a[2 * v].x += u.x; acc.a[2 * v].y += u.y;
         acc.a[2 * v + 1].x += u.z; acc.a[2 * v + 1].y += u.w;
+    }
+}
+
+// Even/odd accumulators of the angle-addition pass for one block: sample (8 + j) = P_j + Q_j, sample (7 - j) = P_j - Q_j.
+struct PQ {
+    float2 P[kPairs / 2], Q[kPairs / 2];  // pairs (j, j+1), j = 0, 2, 4, 6
+};
+
+// Fixed-point merge of large tables (awg::tone_groups, FixGrid): a leaf's fp32 sums are rounded once to the leaf's grid
+// -- fma(v, 2^sh, 1.5 * 2^23) leaves the integer in the low mantissa bits, |v 2^sh| < 2^22 by the host's choice of sh --
+// and shifted on to the table's common grid; from there on everything is added in integers: exact, so the order in
+// which leaves, warps and CTAs meet does not matter.
+constexpr int kMagicBits = 0x4B400000;   // bits of 1.5 * 2^23
+
+__device__ __forceinline__ float pow2f(int e) { return __int_as_float((127 + e) << 23); }
+
+__device__ __forceinline__ int fix_of(float t, int mul) { return (__float_as_int(t) - kMagicBits) * mul; }
+
+// The even/odd accumulators P_j, Q_j of one block of a leaf join the warp's leaves in its park area (int32 on the common
+// grid).  The magic-number bias stays in: new = bits * mul + old is one IMAD per value, and the bias, kMagicBits * (sum
+// of the leaves' mul), is taken out once when the team's park areas are added up (FixGrid::bias_q; integer arithmetic
+// wraps, so this is exact).  The samples P_j +- Q_j are formed there too, in integers.
+__device__ __forceinline__ void ipark_leaf(WarpSmem &ws, int r, int lane, const PQ &pq, float fscale, int mul, bool first)
+{
+    const float2 sc = dup2(fscale), mg = dup2(kRoundMagic);
+#pragma unroll
+    for (int v = 0; v < kSPT / 4; ++v) {
+        const float2 a = v < 2 ? pq.P[2 * v] : pq.Q[2 * v - 4], b = v < 2 ? pq.P[2 * v + 1] : pq.Q[2 * v - 3];
+        const float2 t0 = __ffma2_rn(a, sc, mg), t1 = __ffma2_rn(b, sc, mg);
+        int4 *slot = reinterpret_cast<int4 *>(&ws.park[r][v][lane]);
+        int4 u = make_int4(0, 0, 0, 0);
+        if (!first) u = *slot;
+        *slot = make_int4(__float_as_int(t0.x) * mul + u.x, __float_as_int(t0.y) * mul + u.y, __float_as_int(t1.x) * mul + u.z,
+                          __float_as_int(t1.y) * mul + u.w);
+    }
+}
+
+// i[0..7] = P_0..P_7, i[8..15] = Q_0..Q_7 (bias removed) -> the block's 16 samples: (8 + j) = P_j + Q_j, (7 - j) = P_j - Q_j
+__device__ __forceinline__ void ipq_to_samples(const int (&i)[kSPT], int (&smp)[kSPT])
+{
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) {
+        smp[kPairs + j] = i[j] + i[kPairs + j];
+        smp[kPairs - 1 - j] = i[j] - i[kPairs + j];
+    }
+}
+
+__device__ __forceinline__ void ipark_add(const WarpSmem &ws, int r, int lane, int (&isum)[kSPT])
+{
+#pragma unroll
+    for (int v = 0; v < kSPT / 4; ++v) {
+        const int4 u = *reinterpret_cast<const int4 *>(&ws.park[r][v][lane]);
+        isum[4 * v] += u.x; isum[4 * v + 1] += u.y; isum[4 * v + 2] += u.z; isum[4 * v + 3] += u.w;
     }
 }
 
@@ -429,11 +545,6 @@ __device__ __forceinline__ void store_block(const LaunchParams &lp, int64_t n_th
     }
 }
 
-// Even/odd accumulators of the angle-addition pass for one block: sample (8 + j) = P_j + Q_j, sample (7 - j) = P_j - Q_j.
-struct PQ {
-    float2 P[kPairs / 2], Q[kPairs / 2];  // pairs (j, j+1), j = 0, 2, 4, 6
-};
-
 __device__ __forceinline__ void pq_add(PQ &pq, float s, float c, const float4 &C03, const float4 &C47, const float4 &S03,
                                        const float4 &S47)
 {
@@ -460,8 +571,7 @@ __device__ __forceinline__ Acc16 pq_to_samples(const PQ &pq)
     return d;
 }
 
-// Requests the carrier part of a tone record (A, cls, theta_pre | w_pre, theta_post | w_post, ns_int | ns_frac, Tn) and
-// pulls its two angle-addition tables (bytes 128..287) towards L1.
+// Loads the carrier part of a tone record (A, cls, theta_pre | w_pre, theta_post | w_post, ns_int | ns_frac, Tn).
 __device__ __forceinline__ void fetch_tone(const ToneRec *tr, uint4 &v0, uint4 &v1, uint4 &v2, uint4 &v3)
 {
     const char *p = reinterpret_cast<const char *>(tr);
@@ -469,6 +579,14 @@ __device__ __forceinline__ void fetch_tone(const ToneRec *tr, uint4 &v0, uint4 &
     v1 = ldg16(p + 16);
     v2 = ldg16(p + 32);
     v3 = ldg16(p + 48);
+}
+
+// Pulls a tone record (carrier part and the two angle-addition tables, bytes 0..63 and 128..287) towards L1: issued one
+// batch ahead, so that the loads of the next batch's staging hit L1 and no register stays live across the multiply-add loop.
+__device__ __forceinline__ void prefetch_tone(const ToneRec *tr)
+{
+    const char *p = reinterpret_cast<const char *>(tr);
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
     asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 128));
     asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 208));
     asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 272));
@@ -526,8 +644,8 @@ __device__ __forceinline__ void team_sync(int team)
     }
 
 template <int SPLIT>
-__device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws, const WarpSmem *team_ws, int per,
-                                            int64_t blk_base, int lane, Acc16 &acc)
+__device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws, const WarpSmem *team_ws, int r2_begin, int r2_end,
+                                            int q, int per, int bpl, int64_t blk_base, int lane, Acc16 &acc)
 {
     const int koff = lane * kSPT - kHalf;
     const unsigned lt = (1u << lane) - 1u;
@@ -537,19 +655,20 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
         kf[j] = make_float2(static_cast<float>(koff + 2 * j), static_cast<float>(koff + 2 * j + 1));
         kk[j] = __fmul2_rn(kf[j], kf[j]);
     }
-    int r2 = 0, b = 0;
-    while (r2 < SPLIT) {
+    // sources: leaf q (tones (q*SPLIT + r2)*per ..., batch masks mov[q*bpl ...]) of the team's warps r2_begin .. r2_end-1
+    int r2 = r2_begin, b = 0;
+    while (r2 < r2_end) {
         // gather: the moving tones of the team's warps, in (warp, tone) order, up to kListCap at a time
         int n = 0;
-        while (r2 < SPLIT && n + kBatch <= kListCap) {
-            const int tb2 = r2 * per;
+        while (r2 < r2_end && n + kBatch <= kListCap) {
+            const int tb2 = min((q * SPLIT + r2) * per, lp.n_tones);   // first tone of warp r2's leaf q
             const int len = min(lp.n_tones, tb2 + per) - tb2;
-            if (team_ws[r2].n_mov == 0 || b * kBatch >= len) {
+            if (team_ws[r2].nm_leaf[q] == 0 || b * kBatch >= len) {
                 ++r2;
                 b = 0;
                 continue;
             }
-            const unsigned m = team_ws[r2].mov[b];
+            const unsigned m = team_ws[r2].mov[q * bpl + b];
             if ((m >> lane) & 1u) ws.list[n + __popc(m & lt)] = static_cast<uint16_t>(tb2 + b * kBatch + lane);
             n += __popc(m);
             ++b;
@@ -723,7 +842,7 @@ __device__ __forceinline__ void slow_fma(const StageRec *rec, const SlowSC &v, P
 // ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine), everything else (and
 // every tone when !ROT) takes the MUFU pass.  Every sample goes through the same arithmetic for every launch
 // geometry because all phases are anchored to absolute tile positions.
-template <int SPLIT, bool ROT>
+template <int SPLIT, bool ROT, bool LEAVES>
 __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(const LaunchParams lp)
 {
     constexpr int kTeams = kWarps / SPLIT;
@@ -743,37 +862,43 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
     const int64_t n_tiles = (n_end - 1) / kTile - first_tile + 1;
     const int64_t n_teams = static_cast<int64_t>(gridDim.x) * kTeams;
 
-    const int per = (lp.n_tones + SPLIT - 1) / SPLIT;
-    const int t_begin = rank * per;
-    const int t_end = min(lp.n_tones, t_begin + per);
+    // Tone groups (awg::tone_groups): the tone table is cut into leaves of `per` tones; warp `rank` of a team takes the
+    // leaves q*SPLIT + rank, q = 0 .. Q-1.  A leaf is summed FROM ZERO over its tones in tone order; a warp adds its
+    // leaves in order (W_rank = ((l_0 + l_1) + l_2) ...), the team adds W_0 .. W_3 in rank order, and the moving tones of
+    // every leaf are summed from zero per leaf and block and added leaf by leaf (S + M).  This fixed tree is what lets a
+    // launch with few tiles hand the leaves of a tile to different CTAs (lp.cross) and still produce the same bits:
+    // there the leaves meet in scratch memory and the CTA that delivers the last one adds them up in the same order.
+    // Small tables (Q == 1) are one leaf per warp with the moving tones chained onto the static sum.
+    constexpr bool kQuads = LEAVES;
+    static_assert(!LEAVES || SPLIT == kWarps, "leaves are the large-table path: one CTA per team");
+    const int per = lp.per;
+    const int Q = kQuads ? lp.n_quads : 1;
+    const int bpl = (per + kBatch - 1) / kBatch;   // batches per leaf
+    const bool cross = kQuads && lp.cross != 0;
+    const int64_t n_units = cross ? n_tiles * Q : n_tiles;
     const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the centre of block 0
-    SlowK slowk;
-    {
-        slowk.m0 = lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre, block 0
-        const float k0 = static_cast<float>(slowk.m0) - 0.5f;
-        slowk.kf01 = make_float2(k0, k0 + static_cast<float>(kBlock));
-        slowk.kf23 = make_float2(k0 + static_cast<float>(2 * kBlock), k0 + static_cast<float>(3 * kBlock));
-        slowk.kk01 = __fmul2_rn(slowk.kf01, slowk.kf01);
-        slowk.kk23 = __fmul2_rn(slowk.kf23, slowk.kf23);
-    }
-
     // Tile scheduler: every team starts on the tile of its own index and then draws tiles from the launch's
     // counter lp.sched[0] (tiles that hold moving tones cost several times the others, so a fixed stride leaves
     // SMs idle at the end).  Which team computes a tile has no effect on its samples.
     int64_t unit = static_cast<int64_t>(team) * gridDim.x + blockIdx.x;
-    // The tone records of the next batch are requested before the multiply-add loop of the current batch runs
-    // (v0n..v3n stay in registers across it, the two carrier tables are pulled into L1); after the last batch of a
-    // tile the request wraps round to the first batch, which is what the next tile starts with.
-    uint4 v0n = make_uint4(0, 0, 0, 0), v1n = v0n, v2n = v0n, v3n = v0n;
-    // A warp whose tones fit one batch keeps their records in registers for the whole launch, and their tables in
-    // shared memory for as long as the same tones are static on the same carriers (sticky_sta / sticky_post).
-    const bool single = t_end - t_begin <= kBatch;
-    bool have_records = false;
+    // The tone records of the next batch are pulled into L1 before the multiply-add loop of the current batch runs.
+    // A warp whose tones fit one batch keeps their tables in shared memory for as long as the same tones are static on
+    // the same carriers (sticky_sta / sticky_post).
+    const bool single = !kQuads && per <= kBatch;
     unsigned sticky_sta = 0u, sticky_post = 0xffffffffu;   // no tile has post bits outside its static bits
-    while (unit < n_tiles) {
-        if (ROT && t_begin + lane < t_end && !(single && have_records)) fetch_tone(lp.tab + t_begin + lane, v0n, v1n, v2n, v3n);
-        have_records = true;
-        const int64_t tile_base = (first_tile + unit) * kTile;
+    while (unit < n_units) {
+      const int64_t tile = cross ? unit / Q : unit;
+      const int q_begin = cross ? static_cast<int>(unit - tile * Q) : 0;
+      const int q_end = cross ? q_begin + 1 : Q;
+      const int64_t tile_base = (first_tile + tile) * kTile;
+      const int64_t n_thread = tile_base + lane * kSPT;
+      const int64_t xs_tile = lp.xs ? tile_base % lp.xs_len : 0;
+      int n_mov_tile = 0;
+#pragma unroll 1
+      for (int q = q_begin; q < q_end; ++q) {
+        const int t_begin = min((q * SPLIT + rank) * per, lp.n_tones);
+        const int t_end = min(lp.n_tones, t_begin + per);
+        uint32_t *const mov_q = ws.mov + q * bpl;
         Acc16 acc[kBlocksPerTile];
         int n_mov = 0;
 
@@ -794,7 +919,8 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 const float4 *tabp = nullptr;
                 if (t < t_end) {
                     const ToneRec *tr = lp.tab + t;
-                    const uint4 v0 = v0n, v1 = v1n, v2 = v2n, v3 = v3n;
+                    uint4 v0, v1, v2, v3;
+                    fetch_tone(tr, v0, v1, v2, v3);
                     uint64_t th = u64_of(v0.z, v0.w), w = u64_of(v1.x, v1.y);
                     tabp = reinterpret_cast<const float4 *>(&tr->rot_pre);
                     is_static = true;
@@ -871,14 +997,22 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                     c1 = round32(w);
                     d = round32(w * static_cast<uint64_t>(kBlock));
                 }
-                {
+                if (tb + kBatch < t_end) {
                     const int tn = tb + kBatch + lane;
-                    if (tn < t_end) fetch_tone(lp.tab + tn, v0n, v1n, v2n, v3n);
+                    if (tn < t_end) prefetch_tone(lp.tab + tn);
+                } else if (q + 1 < q_end) {
+                    // last batch of the leaf: the first batch of the warp's next leaf
+                    const int tn0 = min(((q + 1) * SPLIT + rank) * per, lp.n_tones);
+                    if (tn0 + lane < min(lp.n_tones, tn0 + per)) prefetch_tone(lp.tab + tn0 + lane);
+                } else if (!single) {
+                    // last batch of the tile: the first batch of the next one (the same tones unless the quads are spread over CTAs)
+                    const int tn0 = min(rank * per, lp.n_tones);
+                    if (!cross && tn0 + lane < min(lp.n_tones, tn0 + per)) prefetch_tone(lp.tab + tn0 + lane);
                 }
                 const unsigned m_mov = __ballot_sync(0xffffffffu, is_mover);
                 const unsigned m_sta = __ballot_sync(0xffffffffu, is_static);
                 const unsigned m_slow = __ballot_sync(0xffffffffu, is_slow);
-                if (lane == 0) ws.mov[b] = m_mov;
+                if (lane == 0) mov_q[b] = m_mov;
                 n_mov += __popc(m_mov);
                 const int n_sta = __popc(m_sta);
                 __syncwarp();  // the previous batch's readers are done
@@ -930,6 +1064,15 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 // ---- slow pass: the batch's slow movers, 16 lanes at a time (two staged records per tone: the tone
                 // at the tile-centre frequency, and the first-order correction of its pair tables)
                 if (m_slow != 0u) {
+                    SlowK slowk;
+                    {
+                        slowk.m0 = lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre, block 0
+                        const float k0 = static_cast<float>(slowk.m0) - 0.5f;
+                        slowk.kf01 = make_float2(k0, k0 + static_cast<float>(kBlock));
+                        slowk.kf23 = make_float2(k0 + static_cast<float>(2 * kBlock), k0 + static_cast<float>(3 * kBlock));
+                        slowk.kk01 = __fmul2_rn(slowk.kf01, slowk.kf01);
+                        slowk.kk23 = __fmul2_rn(slowk.kf23, slowk.kf23);
+                    }
                     sticky_sta = 0u;           // ws.st is overwritten: a single-batch warp restages its tables next tile
                     sticky_post = 0xffffffffu;
 #pragma unroll 1
@@ -956,41 +1099,53 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                     }
                 }
             }
+            if (kQuads) {
+                // the leaf's sums, rounded to the leaf's fixed-point grid, join the warp's leaves in its park area (int32)
+                const int sh = lp.fix.leaf_sh[q * 4 + rank];
 #pragma unroll
-            for (int r = 0; r < kBlocksPerTile; ++r) acc[r] = pq_to_samples(pq[r]);
+                for (int r = 0; r < kBlocksPerTile; ++r) ipark_leaf(ws, r, lane, pq[r], pow2f(sh), 1 << (lp.fix.fix_sh - sh), q == q_begin);
+            } else {
+#pragma unroll
+                for (int r = 0; r < kBlocksPerTile; ++r) acc[r] = pq_to_samples(pq[r]);
+            }
         } else {
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int left = t_end - tb;
-                if (lane == 0) ws.mov[b] = left >= 32 ? 0xffffffffu : ((1u << left) - 1u);
+                if (lane == 0) mov_q[b] = left >= 32 ? 0xffffffffu : ((1u << left) - 1u);
             }
             n_mov = max(t_end - t_begin, 0);
         }
 
-        const int64_t n_thread = tile_base + lane * kSPT;
-        const int64_t xs_tile = lp.xs ? tile_base % lp.xs_len : 0;
-        if (SPLIT == 1 && ROT && n_mov == 0) {
+        if (lane == 0) ws.nm_leaf[q] = static_cast<uint16_t>(min(n_mov, 65535));
+        n_mov_tile += n_mov;
+        if (!kQuads) {
+            if (SPLIT == 1 && ROT && n_mov == 0) {
 #pragma unroll
-            for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, acc[r]);
-            unit = next_unit<SPLIT>(lp, ws_all[warp - rank], team, rank, lane, n_teams);
-            continue;
+                for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, acc[r]);
+            } else if (ROT) {
+#pragma unroll
+                for (int r = 0; r < kBlocksPerTile; ++r) park_store(ws, r, lane, acc[r]);
+            }
         }
+      }
 
-        // ---- the static partial sums and the lists of moving tones go to shared memory; after the team barrier
-        // warp `rank` owns the blocks rank, rank + SPLIT, ...: it adds the team's partial sums in rank order, runs
-        // the MUFU pass of that block for the moving tones of EVERY warp of the team (so the moving tones load the
-        // team's warps evenly wherever they sit in the tone table), quantises and stores.
-        if (ROT) {
-#pragma unroll
-            for (int r = 0; r < kBlocksPerTile; ++r) park_store(ws, r, lane, acc[r]);
-        }
-        if (lane == 0) ws.n_mov = static_cast<uint32_t>(n_mov);
+      if (!(SPLIT == 1 && ROT && n_mov_tile == 0)) {
+        // ---- the static partial sums and the lists of moving tones are in shared memory; after the team barrier
+        // warp `rank` owns the blocks rank, rank + SPLIT, ...: it adds the team's partial sums, runs the MUFU pass of
+        // that block for the moving tones of EVERY warp of the team (so the moving tones load the team's warps evenly
+        // wherever they sit in the tone table), quantises and stores.
+        if (lane == 0) ws.n_mov = static_cast<uint32_t>(n_mov_tile);
         team_sync<SPLIT>(team);
-        {
-            WarpSmem *team_ws = ws_all + (warp - rank);
+        WarpSmem *team_ws = ws_all + (warp - rank);
 #pragma unroll 1
-            for (int r = rank; r < kBlocksPerTile; r += SPLIT) {
-                const int64_t blk_base = tile_base + static_cast<int64_t>(r) * kBlock;
-                if (blk_base >= n_end || blk_base + kBlock <= lp.n_begin) continue;
+        for (int r = rank; r < kBlocksPerTile; r += SPLIT) {
+            const int64_t blk_base = tile_base + static_cast<int64_t>(r) * kBlock;
+            if (blk_base >= n_end || blk_base + kBlock <= lp.n_begin) continue;
+            uint32_t any = 0;
+#pragma unroll
+            for (int r2 = 0; r2 < SPLIT; ++r2) any |= team_ws[r2].n_mov;
+            if (!kQuads) {
+                // small tables: fp32 all the way, partial sums in rank order, the moving tones chained on top
                 Acc16 sum;
 #pragma unroll
                 for (int j = 0; j < kPairs; ++j) sum.a[j] = make_float2(0.f, 0.f);
@@ -998,17 +1153,93 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
 #pragma unroll
                     for (int r2 = 0; r2 < SPLIT; ++r2) park_add(team_ws[r2], r, lane, sum);
                 }
-                {
-                    uint32_t any = 0;
-#pragma unroll
-                    for (int r2 = 0; r2 < SPLIT; ++r2) any |= team_ws[r2].n_mov;
-                    if (any) mover_block<SPLIT>(lp, ws, team_ws, per, blk_base, lane, sum);
-                }
+                if (any) mover_block<SPLIT>(lp, ws, team_ws, 0, SPLIT, 0, per, bpl, blk_base, lane, sum);
                 store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, sum);
+            } else {
+                // large tables: leaves and per-quad moving-tone sums meet in fixed point (exact, any order)
+                int isum[kSPT];
+#pragma unroll
+                for (int j = 0; j < kSPT; ++j) isum[j] = 0;
+                if (ROT) {
+                    int ipq[kSPT];
+#pragma unroll
+                    for (int j = 0; j < kSPT; ++j) ipq[j] = 0;
+#pragma unroll
+                    for (int r2 = 0; r2 < SPLIT; ++r2) ipark_add(team_ws[r2], r, lane, ipq);
+                    uint32_t bias = 0;
+                    for (int q = q_begin; q < q_end; ++q) bias += lp.fix.bias_q[q];
+#pragma unroll
+                    for (int j = 0; j < kSPT; ++j) ipq[j] -= static_cast<int>(bias);
+                    ipq_to_samples(ipq, isum);
+                }
+                if (any) {
+#pragma unroll 1
+                    for (int q = q_begin; q < q_end; ++q) {
+                        uint32_t nq = 0;
+#pragma unroll
+                        for (int r2 = 0; r2 < SPLIT; ++r2) nq |= team_ws[r2].nm_leaf[q];
+                        if (nq == 0) continue;
+                        Acc16 mq;
+#pragma unroll
+                        for (int j = 0; j < kPairs; ++j) mq.a[j] = make_float2(0.f, 0.f);
+                        mover_block<SPLIT>(lp, ws, team_ws, 0, SPLIT, q, per, bpl, blk_base, lane, mq);
+                        const int sh = lp.fix.quad_sh[q], mul = 1 << (lp.fix.fix_sh - sh);
+                        const float2 sc = dup2(pow2f(sh)), mg = dup2(kRoundMagic);
+#pragma unroll
+                        for (int j = 0; j < kPairs; ++j) {
+                            const float2 t = __ffma2_rn(mq.a[j], sc, mg);
+                            isum[2 * j] += fix_of(t.x, mul);
+                            isum[2 * j + 1] += fix_of(t.y, mul);
+                        }
+                    }
+                }
+                if (!cross) {
+                    Acc16 sum;
+#pragma unroll
+                    for (int j = 0; j < kPairs; ++j)
+                        sum.a[j] = make_float2(__int2float_rn(isum[2 * j]) * lp.fix.fix_inv, __int2float_rn(isum[2 * j + 1]) * lp.fix.fix_inv);
+                    store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, sum);
+                } else {
+                    // this quad's share of the block joins the other quads' in the launch's scratch tile: [tile][block][sample]
+                    int *dst = lp.scratch + (tile * kBlocksPerTile + r) * kBlock + lane;
+#pragma unroll
+                    for (int j = 0; j < kSPT; ++j) atomicAdd(dst + j * 32, isum[j]);
+                }
             }
         }
-        // the closing barrier (the next tile's partial sums overwrite the park areas) also publishes the next tile
-        unit = next_unit<SPLIT>(lp, ws_all[warp - rank], team, rank, lane, n_teams);
+      }
+      if (cross) {
+          // Quads of one tile arrive from different CTAs in any order; integer sums do not care.  The CTA that delivers
+          // the last quad reads the tile back (warp `rank` takes block `rank`), leaves zeros for the next launch on this
+          // slot, quantises and stores.  No CTA waits for another.
+          __threadfence();
+          __syncthreads();
+          if (threadIdx.x == 0) {
+              const uint32_t old = atomicAdd(lp.tile_cnt + tile, 1u);
+              ws_all[0].last = old == static_cast<uint32_t>(Q - 1) ? 1u : 0u;
+              if (old == static_cast<uint32_t>(Q - 1)) lp.tile_cnt[tile] = 0u;
+          }
+          __syncthreads();
+          if (ws_all[0].last) {
+              __threadfence();
+              const int r = rank;
+              const int64_t blk_base = tile_base + static_cast<int64_t>(r) * kBlock;
+              if (!(blk_base >= n_end || blk_base + kBlock <= lp.n_begin)) {
+                  int *src = lp.scratch + (tile * kBlocksPerTile + r) * kBlock + lane;
+                  Acc16 sum;
+#pragma unroll
+                  for (int j = 0; j < kPairs; ++j) {
+                      const int i0 = __ldcg(src + (2 * j) * 32), i1 = __ldcg(src + (2 * j + 1) * 32);
+                      src[(2 * j) * 32] = 0;
+                      src[(2 * j + 1) * 32] = 0;
+                      sum.a[j] = make_float2(__int2float_rn(i0) * lp.fix.fix_inv, __int2float_rn(i1) * lp.fix.fix_inv);
+                  }
+                  store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, sum);
+              }
+          }
+      }
+      // the closing barrier (the next tile's partial sums overwrite the park areas) also publishes the next unit
+      unit = next_unit<SPLIT>(lp, ws_all[warp - rank], team, rank, lane, n_teams);
     }
     // the last team out re-arms the counter for the launch that takes this slot next
     if (rank == 0 && lane == 0) {
@@ -1112,14 +1343,21 @@ __global__ void __launch_bounds__(128) awg_expand_kernel(ToneRec *table, const T
 }
 
 // ---- launch state, per device ------------------------------------------------------------------------------------
-// Tile-scheduler slots: pairs of counters, zeroed once; the last team of a launch zeroes its slot again.  A slot belongs
-// to ONE stream (keyed by the stream's unique id): launches of a stream run one after the other, so a slot is clean when
-// the next launch of its stream starts, and launches that can overlap (different streams) never share a counter.
+// Launch slots: a tile-scheduler counter pair, the per-tile quad counters and a scratch area, zeroed once; the kernel
+// leaves its counters at zero again.  A slot belongs to ONE stream (keyed by the stream's unique id): launches of a stream
+// run one after the other, so a slot is clean when the next launch of its stream starts, and launches that can overlap
+// (different streams) never share a counter or scratch memory.
 constexpr int kSchedSlots = 1024;
 constexpr int kMaxDevices = 64;
+constexpr int kCrossTiles = 512;                         // launches with fewer tiles than the grid has CTAs (<= 3 x 148) may run cross-CTA
+constexpr int kSlotWords = 8 + kCrossTiles;              // {next unit, teams finished, -...} + per-tile quad counters
+struct LaunchSlot {
+    int32_t *scratch = nullptr;   // kCrossTiles tiles of int32 sums, zero between launches
+};
 struct DeviceState {
     uint32_t *sched = nullptr;
     std::unordered_map<unsigned long long, uint32_t> slot_of;   // stream id -> slot
+    LaunchSlot slots[kSchedSlots];
     int n_sm = 0;
     uint32_t configured = 0;   // bit per kernel instantiation: dynamic shared memory opt-in done on this device
 };
@@ -1137,7 +1375,7 @@ cudaError_t device_state(DeviceState **out)
         int v = 0;
         if ((e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
         uint32_t *p = nullptr;
-        const size_t bytes = static_cast<size_t>(kSchedSlots) * 8 * sizeof(uint32_t);  // 32 bytes per slot
+        const size_t bytes = static_cast<size_t>(kSchedSlots) * kSlotWords * sizeof(uint32_t);
         if ((e = cudaMalloc(reinterpret_cast<void **>(&p), bytes)) != cudaSuccess) return e;
         if ((e = cudaMemset(p, 0, bytes)) != cudaSuccess || (e = cudaDeviceSynchronize()) != cudaSuccess) {
             cudaFree(p);
@@ -1150,23 +1388,23 @@ cudaError_t device_state(DeviceState **out)
     return cudaSuccess;
 }
 
-template <int SPLIT, bool ROT>
+template <int SPLIT, bool ROT, bool LEAVES>
 cudaError_t launch_one(DeviceState &ds, const LaunchParams &lp, int64_t tiles, cudaStream_t stream)
 {
     constexpr int kTeams = kWarps / SPLIT;
     constexpr size_t kSmem = sizeof(WarpSmem) * kWarps;
-    constexpr uint32_t kBit = 1u << ((SPLIT == 1 ? 0 : SPLIT == 2 ? 1 : 2) * 2 + (ROT ? 1 : 0));
+    constexpr uint32_t kBit = 1u << ((LEAVES ? 3 : SPLIT == 1 ? 0 : SPLIT == 2 ? 1 : 2) * 2 + (ROT ? 1 : 0));
     if (!(ds.configured & kBit)) {
-        cudaError_t e = cudaFuncSetAttribute(awg_synth_kernel<SPLIT, ROT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(awg_synth_kernel<SPLIT, ROT, LEAVES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              static_cast<int>(kSmem));
         if (e != cudaSuccess) return e;
         ds.configured |= kBit;
     }
-    // persistent grid: kCtasPerSm CTAs per SM, fewer when the launch has fewer tiles than teams
-    const int64_t want = (tiles + kTeams - 1) / kTeams;
+    // persistent grid: kCtasPerSm CTAs per SM, fewer when the launch has fewer work units than teams
+    const int64_t want = (tiles + kTeams - 1) / kTeams;   // (`tiles` = work units: tiles, or tiles x quads when lp.cross)
     const int64_t max_grid = static_cast<int64_t>(kCtasPerSm) * ds.n_sm;
     const unsigned grid = static_cast<unsigned>(want < max_grid ? want : max_grid);
-    awg_synth_kernel<SPLIT, ROT><<<grid, kWarps * 32, kSmem, stream>>>(lp);
+    awg_synth_kernel<SPLIT, ROT, LEAVES><<<grid, kWarps * 32, kSmem, stream>>>(lp);
     return cudaGetLastError();
 }
 
@@ -1174,9 +1412,10 @@ template <bool ROT>
 cudaError_t launch_split(DeviceState &ds, const LaunchParams &lp, int split, int64_t tiles, cudaStream_t stream)
 {
     switch (split) {
-        case 1: return launch_one<1, ROT>(ds, lp, tiles, stream);
-        case 2: return launch_one<2, ROT>(ds, lp, tiles, stream);
-        default: return launch_one<kWarps, ROT>(ds, lp, tiles, stream);
+        case 1: return launch_one<1, ROT, false>(ds, lp, tiles, stream);
+        case 2: return launch_one<2, ROT, false>(ds, lp, tiles, stream);
+        default: return lp.n_quads > 1 ? launch_one<kWarps, ROT, true>(ds, lp, tiles, stream)
+                                       : launch_one<kWarps, ROT, false>(ds, lp, tiles, stream);
     }
 }
 
@@ -1221,13 +1460,38 @@ cudaError_t launch_synth(const LaunchParams &lp_in, int engine, cudaStream_t str
             }
             it = ds->slot_of.emplace(sid, static_cast<uint32_t>(ds->slot_of.size())).first;
         }
-        lp.sched = ds->sched + 8 * it->second;
+        lp.sched = ds->sched + static_cast<size_t>(kSlotWords) * it->second;
+        lp.tile_cnt = lp.sched + 8;
         // clamp bounds of the quantiser in units of V: scale*qlo and scale*qhi round to -32768 and 32767
         lp.qlo = static_cast<float>(-32768.0 / static_cast<double>(lp.scale));
         lp.qhi = static_cast<float>(32767.0 / static_cast<double>(lp.scale));
-        const int split = split_for(lp.n_tones);
-        e = (engine == AWG_ENGINE_FMA) ? launch_split<true>(*ds, lp, split, tiles, stream)
-                                       : launch_split<false>(*ds, lp, split, tiles, stream);
+        int split = 1, per = lp.n_tones, quads = 1;
+        tone_groups(lp.n_tones, &split, &per, &quads);
+        lp.per = per;
+        lp.n_quads = quads;
+        lp.cross = 0;
+        lp.scratch = nullptr;
+        int64_t units = tiles;
+        if (quads > 1 && tiles < static_cast<int64_t>(kCtasPerSm) * ds->n_sm && tiles <= kCrossTiles) {
+            // fewer tiles than CTAs: a tile's quads become separate work units, their sums meet in the slot's scratch tiles
+            LaunchSlot &sl = ds->slots[it->second];
+            if (!sl.scratch) {
+                int32_t *sp = nullptr;
+                const size_t bytes = static_cast<size_t>(kCrossTiles) * kTile * sizeof(int32_t);
+                if (cudaMalloc(reinterpret_cast<void **>(&sp), bytes) == cudaSuccess) {
+                    if (cudaMemset(sp, 0, bytes) == cudaSuccess && cudaDeviceSynchronize() == cudaSuccess) sl.scratch = sp;
+                    else cudaFree(sp);
+                }
+                if (!sl.scratch) (void)cudaGetLastError();   // no scratch: the quads stay inside one CTA
+            }
+            if (sl.scratch) {
+                lp.cross = 1;
+                lp.scratch = sl.scratch;
+                units = tiles * quads;
+            }
+        }
+        e = (engine == AWG_ENGINE_FMA) ? launch_split<true>(*ds, lp, split, units, stream)
+                                       : launch_split<false>(*ds, lp, split, units, stream);
     }
     count_launch();
     return e;

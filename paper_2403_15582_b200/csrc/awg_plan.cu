@@ -223,6 +223,13 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
     const int v = (cur + 1) % kTableVersions;
     // the slot's previous readers (kernels launched kTableVersions uploads ago) must be done
     if ((e = cudaEventSynchronize(p->last_use[v])) != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
+    {
+        std::vector<float> amp;
+        amp.reserve(p->n_tones);
+        for (int k = 0; k < p->n_tones; ++k)
+            if (!p->in_buffer[k]) amp.push_back(std::max(std::fabs(p->tones[k].A), std::fabs(p->tones[k].A1)));
+        fix_grids(amp.data(), static_cast<int>(amp.size()), &p->fix);
+    }
     std::sort(p->dirty_tones.begin(), p->dirty_tones.end());
     p->dirty_tones.erase(std::unique(p->dirty_tones.begin(), p->dirty_tones.end()), p->dirty_tones.end());
     const size_t n_dirty = p->dirty_tones.size();
@@ -292,6 +299,7 @@ awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, voi
     lp.n_begin = n_begin;
     lp.n_count = n_count;
     lp.scale = static_cast<float>(p->scale);
+    lp.fix = p->fix;
     lp.out = dev_out;
     lp.out_f32 = f32 ? 1 : 0;
     lp.sched = nullptr;  // launch_synth assigns the tile-scheduler slot
@@ -599,6 +607,9 @@ awg_status static_buffer_add(awg_plan *p, const std::vector<HostTone> &tones, co
     lp.n_begin = 0;
     lp.n_count = p->chunk_len;
     lp.scale = static_cast<float>(p->scale);
+    std::vector<float> amp;
+    for (const HostTone &h : tones) amp.push_back(std::max(std::fabs(h.A), std::fabs(h.A1)));
+    fix_grids(amp.data(), n, &lp.fix);
     lp.out = dst;
     lp.out_stride = 1;
     lp.out_offset = 0;

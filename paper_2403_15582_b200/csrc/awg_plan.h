@@ -53,6 +53,7 @@ struct awg_plan {
     std::vector<uint8_t> in_buffer;
     std::vector<int32_t> slot_of;
     int32_t n_active = 0;
+    awg::FixGrid fix{};                 // fixed-point grids of the kernel's leaf merge for the current table (fix_grids())
     float *xs[2] = {};                      // X_static, chunk_len floats each; xs[xs_cur] is current (a fold writes the other)
     int xs_cur = 0;
     bool xs_on = false;

@@ -329,9 +329,50 @@ def test_max_tone_count_4096_and_more(awg, torch_cuda, eng):
     p.close()
 
 
+@pytest.mark.parametrize("n_tones", [300, 1000, 4500])
+def test_quads_across_ctas_match_quads_in_one_cta_bit_for_bit(awg, torch_cuda, eng, n_tones):
+    """Tone tables above 256 tones are summed in quads of 4 x <= 64 tones (awg::tone_groups).  A launch with fewer tiles
+    than the grid has CTAs spreads a tile's quads over CTAs (sums meet in scratch memory, last arriver adds them in quad
+    order); a large launch walks the quads inside one CTA.  Same grouping, same order: the int16 codes and the fp32 sums
+    must be identical bit for bit, and both must match the oracle.  Static tones, slow movers, fast movers, a few
+    amplitude ramps; 2^20 samples as one launch (512 tiles) against 2^15-sample chunks (16 tiles each)."""
+    fs, L = 560e6, 1 << 20
+    rng = np.random.default_rng(1000 + n_tones)
+    f0 = rng.uniform(20e6, 250e6, n_tones)
+    kind = rng.integers(0, 4, n_tones)
+    rows = []
+    for k in range(n_tones):
+        if kind[k] == 0:
+            rows.append((f0[k], f0[k], 1.0 / n_tones, rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
+        elif kind[k] == 1:    # slow mover: 2 MHz over 30 ms
+            rows.append((f0[k], f0[k] + rng.uniform(-2e6, 2e6), 1.0 / n_tones, rng.uniform(0, 6.28), -1e-3, 30e-3, MINJERK))
+        elif kind[k] == 2:    # fast mover inside the range
+            rows.append((f0[k], f0[k] + rng.uniform(-4e6, 4e6), 1.0 / n_tones, rng.uniform(0, 6.28),
+                         rng.uniform(0, 1.2e-3), rng.uniform(50e-6, 400e-6), MINJERK))
+        else:
+            rows.append((f0[k], f0[k] + rng.uniform(-1e6, 1e6), 1.0 / n_tones, rng.uniform(0, 6.28),
+                         rng.uniform(0, 1.0e-3), rng.uniform(100e-6, 600e-6), LINEAR))
+    big, op = _single(awg, fs, L, rows, engine=eng)
+    small, _ = _single(awg, fs, 1 << 15, rows, engine=eng)
+    ref = _np(big.synthesize_chunk(0))
+    reff = _np(big.synthesize_chunk_f32(0))
+    parts = np.concatenate([_np(small.synthesize_chunk(c)) for c in range(L >> 15)])
+    partsf = np.concatenate([_np(small.synthesize_chunk_f32(c)) for c in range(L >> 15)])
+    assert np.array_equal(parts, ref), f"{n_tones} tones: int16 differs between the cross-CTA and the one-CTA path"
+    assert np.array_equal(partsf.view(np.uint32), reff.view(np.uint32)), f"{n_tones} tones: fp32 sums differ"
+    # a range launch of the small plan over 8 chunks (128 tiles) is cross-CTA again, at another launch size
+    assert np.array_equal(_np(small.synthesize_range(8, 8)), ref[8 << 15:16 << 15])
+    for a in (0, 3 << 15, L - (1 << 15)):
+        V = oracle.c_waveform(op, a, a + (1 << 15))
+        assert_f32_close(reff[a:a + (1 << 15)], V, f"quads N={n_tones} @ {a}")
+        assert_codes_close(ref[a:a + (1 << 15)], op.quantise(V), f"quads N={n_tones} @ {a}")
+    big.close()
+    small.close()
+
+
 def test_plan_limit_65536_tones(awg, torch_cuda, eng):
-    """The largest plan (include/awg.h: n_tones <= 65536): every warp walks 512 batches of 32 tones; a third of the
-    tones is inside a move in the synthesised chunk, so the moving-tone lists are rebuilt many times per block."""
+    """The largest plan (include/awg.h: n_tones <= 65536): 16 quads, every warp walks 32 batches of 32 tones per quad; a
+    third of the tones is inside a move in the synthesised chunk, so the moving-tone lists are rebuilt many times per block."""
     N = 65536
     rng = np.random.default_rng(7)
     f0 = rng.uniform(20e6, 250e6, N)
