@@ -195,19 +195,23 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+SLOW_FMA_PER_TONE_SAMPLE = 1.25   # (16 table-correction + 64 accumulate) multiply-adds per 64 tone-samples of a thread
+
+
 def pipe_roofline(counts, ms, engine, sm_mhz):
     """Binding ALU roofline of launches that took `ms` in total over `counts` = (static, slow, fast) tone-samples as the
     LIBRARY classifies them (awg_plan_op_counts).
 
     Algorithmic work: a tone-sample of a tone that is static there needs ONE fp32 multiply-add (angle addition over a
-    symmetric sample pair); inside a slow move TWO multiply-adds (the second is the first-order frequency correction);
+    symmetric sample pair); inside a slow move 1.25 multiply-adds (16 to move the tone's 16 pair-table entries to the thread's
+    local frequency + 64 for the thread's 64 samples);
     inside any other move one MUFU.SIN plus two multiply-adds (range multiply, amplitude accumulate).  With
     --engine mufu every tone-sample takes the MUFU path.  The roofline time is the larger of (multiply-adds / FMA-pipe
     peak) and (sines / XU-pipe peak) at sm_mhz; frac = that time / the measured time."""
     n_sta, n_slow, n_fast = (int(x) for x in counts)
     if engine == "mufu":
         n_sta, n_slow, n_fast = 0, 0, n_sta + n_slow + n_fast
-    fma_ops, xu_ops = n_sta + 2 * n_slow + 2 * n_fast, n_fast
+    fma_ops, xu_ops = n_sta + SLOW_FMA_PER_TONE_SAMPLE * n_slow + 2 * n_fast, n_fast
     peak_fma = FMA_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
     peak_xu = MUFU_PER_CLK_PER_SM * N_SM * sm_mhz * 1e6
     t_fma, t_xu = fma_ops / peak_fma, xu_ops / peak_xu

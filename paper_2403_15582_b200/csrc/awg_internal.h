@@ -39,7 +39,7 @@ constexpr int kPairs = kSPT / 2;  // symmetric sample pairs per thread: centre +
 struct __align__(16) RotTable {
     float C[kPairs];    // A cos(2 pi (j + 1/2) w)
     float S[kPairs];    // A sin(2 pi (j + 1/2) w)
-    float pad_[4];      // {cos, sin}(2 pi 2 kBlock w): rotation by two blocks (static pass), 0, 0
+    float pad_[4];      // {cos, sin}(2 pi 32 w): rotation by two groups of 16 samples (static pass), 0, 0
 };
 static_assert(sizeof(RotTable) == 80, "RotTable must be 80 bytes");
 

@@ -317,12 +317,13 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
 }
 
 // ---- shared memory of one warp ------------------------------------------------------------------------------
-// One tile-static tone of the current batch (angle-addition pass): carrier phase (u32 turns) at the half-integer
-// pair centre of lane 0 in block 0 [c0], per sample [c1] and per block [d], the rotation that carries a sine/cosine
-// pair two blocks on, and the tone's pair tables.
+// One tile-static tone of the current batch (angle-addition pass; a thread owns 64 consecutive samples of the tile, four
+// groups of 16): carrier phase (u32 turns) at the half-integer pair centre of group 0 of lane 16 [c0], per thread
+// (64 samples) [c1] and per group (16 samples) [d], the rotation that carries a sine/cosine pair two groups on, and the
+// tone's pair tables.
 struct __align__(16) StageRec {
     uint32_t c0, c1, d, pad_;
-    float r0, r1, r2, r3;        // static tone: {cos, sin}(2 pi 2 kBlock w), the rotation by two blocks; slow mover: 2 c2, 3 c3
+    float r0, r1, r2, r3;        // static tone: {cos, sin}(2 pi 32 w), the rotation by two groups; slow mover: 2 c2, 3 c3
     float4 C03, C47, S03, S47;
 };
 static_assert(sizeof(StageRec) == 96, "StageRec must be 96 bytes");
@@ -351,18 +352,42 @@ struct Acc16 {
     float2 a[kPairs];
 };
 
-__device__ __forceinline__ void park_store(WarpSmem &ws, int r, int lane, const Acc16 &acc)
+// The park area is indexed [block][4 samples][column] in the BLOCK layout of the MUFU pass and of the stores (thread
+// `lane` of block r holds samples lane*16 .. +15 of the block).  The angle-addition passes work in the GROUP layout: a
+// thread owns 64 consecutive samples of the tile, four groups of 16, so its group g is what thread
+// lane' = (lane % 8) * 4 + g of block lane / 8 holds in the block layout.  park_col() swizzles the column so that both
+// the group-layout writers (column stride 4 across lanes) and the block-layout readers are free of bank conflicts.
+__device__ __forceinline__ int park_col(int lane_blk) { return lane_blk ^ (lane_blk >> 3); }
+__device__ __forceinline__ int group_block(int lane) { return lane >> 3; }
+__device__ __forceinline__ int group_col(int lane, int g) { return park_col(((lane & 7) << 2) | g); }
+
+// group layout: the 16 samples of group g of this thread
+__device__ __forceinline__ void park_store(WarpSmem &ws, int g, int lane, const Acc16 &acc)
 {
+    const int r = group_block(lane), col = group_col(lane, g);
 #pragma unroll
     for (int v = 0; v < kSPT / 4; ++v)
-        ws.park[r][v][lane] = make_float4(acc.a[2 * v].x, acc.a[2 * v].y, acc.a[2 * v + 1].x, acc.a[2 * v + 1].y);
+        ws.park[r][v][col] = make_float4(acc.a[2 * v].x, acc.a[2 * v].y, acc.a[2 * v + 1].x, acc.a[2 * v + 1].y);
+}
+
+// block layout: the 16 samples of this thread in block r
+__device__ __forceinline__ void park_load(const WarpSmem &ws, int r, int lane, Acc16 &acc)
+{
+    const int col = park_col(lane);
+#pragma unroll
+    for (int v = 0; v < kSPT / 4; ++v) {
+        const float4 u = ws.park[r][v][col];
+        acc.a[2 * v] = make_float2(u.x, u.y);
+        acc.a[2 * v + 1] = make_float2(u.z, u.w);
+    }
 }
 
 __device__ __forceinline__ void park_add(const WarpSmem &ws, int r, int lane, Acc16 &acc)
 {
+    const int col = park_col(lane);
 #pragma unroll
     for (int v = 0; v < kSPT / 4; ++v) {
-        const float4 u = ws.park[r][v][lane];
+        const float4 u = ws.park[r][v][col];
         acc.a[2 * v].x += u.x; acc.a[2 * v].y += u.y;
         acc.a[2 * v + 1].x += u.z; acc.a[2 * v + 1].y += u.w;
     }
@@ -387,14 +412,15 @@ __device__ __forceinline__ int fix_of(float t, int mul) { return (__float_as_int
 // grid).  The magic-number bias stays in: new = bits * mul + old is one IMAD per value, and the bias, kMagicBits * (sum
 // of the leaves' mul), is taken out once when the team's park areas are added up (FixGrid::bias_q; integer arithmetic
 // wraps, so this is exact).  The samples P_j +- Q_j are formed there too, in integers.
-__device__ __forceinline__ void ipark_leaf(WarpSmem &ws, int r, int lane, const PQ &pq, float fscale, int mul, bool first)
+__device__ __forceinline__ void ipark_leaf(WarpSmem &ws, int g, int lane, const PQ &pq, float fscale, int mul, bool first)
 {
+    const int r = group_block(lane), col = group_col(lane, g);   // group layout -> the block layout of the park area
     const float2 sc = dup2(fscale), mg = dup2(kRoundMagic);
 #pragma unroll
     for (int v = 0; v < kSPT / 4; ++v) {
         const float2 a = v < 2 ? pq.P[2 * v] : pq.Q[2 * v - 4], b = v < 2 ? pq.P[2 * v + 1] : pq.Q[2 * v - 3];
         const float2 t0 = __ffma2_rn(a, sc, mg), t1 = __ffma2_rn(b, sc, mg);
-        int4 *slot = reinterpret_cast<int4 *>(&ws.park[r][v][lane]);
+        int4 *slot = reinterpret_cast<int4 *>(&ws.park[r][v][col]);
         int4 u = make_int4(0, 0, 0, 0);
         if (!first) u = *slot;
         *slot = make_int4(__float_as_int(t0.x) * mul + u.x, __float_as_int(t0.y) * mul + u.y, __float_as_int(t1.x) * mul + u.z,
@@ -414,9 +440,10 @@ __device__ __forceinline__ void ipq_to_samples(const int (&i)[kSPT], int (&smp)[
 
 __device__ __forceinline__ void ipark_add(const WarpSmem &ws, int r, int lane, int (&isum)[kSPT])
 {
+    const int col = park_col(lane);
 #pragma unroll
     for (int v = 0; v < kSPT / 4; ++v) {
-        const int4 u = *reinterpret_cast<const int4 *>(&ws.park[r][v][lane]);
+        const int4 u = *reinterpret_cast<const int4 *>(&ws.park[r][v][col]);
         isum[4 * v] += u.x; isum[4 * v + 1] += u.y; isum[4 * v + 2] += u.z; isum[4 * v + 3] += u.w;
     }
 }
@@ -592,18 +619,19 @@ __device__ __forceinline__ void prefetch_tone(const ToneRec *tr)
     asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 272));
 }
 
-// Sines and cosines of one tile-static tone at the thread's pair centre in each of the tile's four blocks.
-// rec header = {phase at lane 0's centre of block 0, phase per sample, phase per block, - | cos, sin of the phase of
-// two blocks}.  Blocks 0 and 1 come from MUFU (u32 turns -> radians -> sin.approx, cos.approx); blocks 2 and 3 are those
-// two pairs rotated by two blocks, (s, c) -> (s cd + c sd, c cd - s sd), four packed fp32 instructions for both: a
-// sine/cosine chain through IADD, I2FP, FMUL, FMUL.RZ and two MUFU costs the multiply-add stream more issue slots
-// than the rotation does (profiles/: pipe microbenchmarks).  The rotation constants are rounded once from fp64.
-__device__ __forceinline__ void sincos_tile(const StageRec *rec, int off, float (&s)[kBlocksPerTile], float (&c)[kBlocksPerTile])
+// Sines and cosines of one tile-static tone at the pair centres of the thread's four groups of 16 samples.
+// rec header = {phase at the centre of group 0 of lane 16, phase per thread (64 samples), phase per group (16), - | cos,
+// sin of the phase of two groups}; l16 = lane - 16.  Groups 0 and 1 come from MUFU (u32 turns -> radians -> sin.approx,
+// cos.approx); groups 2 and 3 are those two pairs rotated by two groups, (s, c) -> (s cd + c sd, c cd - s sd), four packed
+// fp32 instructions for both: a sine/cosine chain through IADD, I2FP, FMUL, FMUL.RZ and two MUFU costs the multiply-add
+// stream more issue slots than the rotation does (profiles/: pipe microbenchmarks).  The rotation constants are rounded
+// once from fp64.
+__device__ __forceinline__ void sincos_tile(const StageRec *rec, int l16, float (&s)[kBlocksPerTile], float (&c)[kBlocksPerTile])
 {
-    static_assert(kBlocksPerTile == 4, "sincos_tile serves four blocks as two pairs");
+    static_assert(kBlocksPerTile == 4, "sincos_tile serves four groups as two pairs");
     const uint4 cc = *reinterpret_cast<const uint4 *>(rec);
     const float2 rot = *reinterpret_cast<const float2 *>(&rec->r0);
-    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(off);
+    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(l16);
     const uint32_t p1 = p0 + cc.z;
     const float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1))), dup2(kTurnToRad));
     s[0] = mufu_sin(x01.x); c[0] = mufu_cos(x01.x);
@@ -744,15 +772,16 @@ __device__ __forceinline__ int64_t next_unit(const LaunchParams &lp, WarpSmem &w
     return n_teams + static_cast<int64_t>(v);
 }
 
-// Slow pass, staging (one lane per slow mover): the pair tables at the tile-centre frequency c1 come from MUFU
-// (the frequency changes from tile to tile, so they cannot be precomputed), the second record holds their
-// first-order correction: cos((j+1/2)(w + e)) ~ C_j - (j+1/2) e S_j,  sin((j+1/2)(w + e)) ~ S_j + (j+1/2) e C_j,
+// Slow pass, staging (one lane per slow mover): the pair tables at the tile-centre frequency come from MUFU (the
+// frequency changes from tile to tile, so they cannot be precomputed); the second record holds their derivatives with
+// respect to the frequency, cos((j+1/2)(w + e)) ~ C_j - (j+1/2) e S_j,  sin((j+1/2)(w + e)) ~ S_j + (j+1/2) e C_j;
 // the first record's header also carries the coefficients 2 c2 and 3 c3 of the local frequency offset
-// e(k) = 2 c2 k + 3 c3 k^2.
+// e(k) = 2 c2 k + 3 c3 k^2 and the phase step of a group.
+// parked: q[0] = {c0, phase per thread, c2, c3}, q[1] = {A, phase per group (bits), phase per sample (bits), -}
 __device__ __forceinline__ void stage_slow(StageRec *dst, const MovRec &parked)
 {
     const float4 a = parked.q[0];
-    const uint32_t c1 = __float_as_uint(a.y);
+    const uint32_t c1 = __float_as_uint(parked.q[1].z);
     const float A = parked.q[1].x;
     float C[kPairs], S[kPairs];
 #pragma unroll
@@ -762,42 +791,44 @@ __device__ __forceinline__ void stage_slow(StageRec *dst, const MovRec &parked)
         C[j] = A * mufu_cos(x);
         S[j] = A * mufu_sin(x);
     }
-    *reinterpret_cast<float4 *>(&dst[0]) = a;   // {c0 at the tile centre - 1/2, c1, c2, c3}
+    *reinterpret_cast<float4 *>(&dst[0]) = a;
+    *reinterpret_cast<float4 *>(&dst[0].r0) = make_float4(2.f * a.z, 3.f * a.w, parked.q[1].y, 0.f);
     dst[0].C03 = make_float4(C[0], C[1], C[2], C[3]);
     dst[0].C47 = make_float4(C[4], C[5], C[6], C[7]);
     dst[0].S03 = make_float4(S[0], S[1], S[2], S[3]);
     dst[0].S47 = make_float4(S[4], S[5], S[6], S[7]);
-    // correction record: multiplies -sin(phi) e into (j+1/2) S_j and cos(phi) e into (j+1/2) C_j
-    *reinterpret_cast<float4 *>(&dst[0].r0) = make_float4(2.f * a.z, 3.f * a.w, 0.f, 0.f);
-    dst[1].C03 = make_float4(0.5f * S[0], 1.5f * S[1], 2.5f * S[2], 3.5f * S[3]);
-    dst[1].C47 = make_float4(4.5f * S[4], 5.5f * S[5], 6.5f * S[6], 7.5f * S[7]);
+    // derivative record: dC_j/dw = -(j+1/2) S_j in the C slots, dS_j/dw = (j+1/2) C_j in the S slots
+    dst[1].C03 = make_float4(-0.5f * S[0], -1.5f * S[1], -2.5f * S[2], -3.5f * S[3]);
+    dst[1].C47 = make_float4(-4.5f * S[4], -5.5f * S[5], -6.5f * S[6], -7.5f * S[7]);
     dst[1].S03 = make_float4(0.5f * C[0], 1.5f * C[1], 2.5f * C[2], 3.5f * C[3]);
     dst[1].S47 = make_float4(4.5f * C[4], 5.5f * C[5], 6.5f * C[6], 7.5f * C[7]);
 }
 
-// Slow pass, per-thread constants: offsets of the thread's pair centres from the tile centre in the four blocks
-// (k_r = m_r - 1/2, m_r = r*512 + lane*16 + 8 - 1024), packed over block pairs, and their squares.
+// Slow pass, per-thread constants: offsets (from the tile centre) of the pair centres of the thread's four groups,
+// k_g = 64 (lane - 16) + 16 g + 7.5, packed over group pairs, their squares, and the offset of the thread's own centre.
 struct SlowK {
-    int m0;
+    int l16;
+    float kt;
     float2 kf01, kf23, kk01, kk23;
 };
 
-// Slow pass, one tone at one thread: sines and cosines of the cubic phase polynomial at the thread's pair centre in
-// each block, and the same multiplied by the local frequency offset e = 2 c2 k + 3 c3 k^2 (packed over block pairs:
-// every fp32 instruction here serves two blocks).
+// Slow pass, one tone at one thread: sines and cosines of the cubic phase polynomial at the pair centres of the four
+// groups (packed over group pairs: every fp32 instruction here serves two groups) and the tone's frequency offset from
+// the tile-centre frequency at the thread's own centre, e = 2 c2 k + 3 c3 k^2.
 struct SlowSC {
-    float2 s01, s23, c01, c23, se01, se23, ce01, ce23;
+    float2 s01, s23, c01, c23;
+    float e;
 };
 
 __device__ __forceinline__ void slow_sincos(const StageRec *rec, const SlowK &K, SlowSC &o)
 {
-    const uint4 cc = *reinterpret_cast<const uint4 *>(rec);                 // c0, c1, c2, c3
-    const float2 g = *reinterpret_cast<const float2 *>(&rec->r0);           // 2 c2, 3 c3
+    const uint4 cc = *reinterpret_cast<const uint4 *>(rec);                 // c0, phase per thread, c2, c3
+    const float4 g = *reinterpret_cast<const float4 *>(&rec->r0);           // 2 c2, 3 c3, phase per group (bits), -
     const float c2 = __uint_as_float(cc.z), c3 = __uint_as_float(cc.w);
-    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(K.m0);
-    const uint32_t db = cc.y << 9;                                          // phase per block (kBlock = 512)
+    const uint32_t p0 = cc.x + cc.y * static_cast<uint32_t>(K.l16);
+    const uint32_t db = __float_as_uint(g.z);
     const uint32_t p1 = p0 + db, p2 = p1 + db, p3 = p2 + db;
-    static_assert(kBlock == 512 && kBlocksPerTile == 4, "slow_sincos assumes four 512-sample blocks");
+    static_assert(kBlocksPerTile == 4, "slow_sincos assumes four groups per thread");
     const float2 K2 = dup2(kTurnToRad);
     const float2 f01 = make_float2(__int2float_rn(static_cast<int32_t>(p0)), __int2float_rn(static_cast<int32_t>(p1)));
     const float2 f23 = make_float2(__int2float_rn(static_cast<int32_t>(p2)), __int2float_rn(static_cast<int32_t>(p3)));
@@ -807,32 +838,32 @@ __device__ __forceinline__ void slow_sincos(const StageRec *rec, const SlowK &K,
     o.c01 = make_float2(mufu_cos(x01.x), mufu_cos(x01.y));
     o.s23 = make_float2(mufu_sin(x23.x), mufu_sin(x23.y));
     o.c23 = make_float2(mufu_cos(x23.x), mufu_cos(x23.y));
-    const float2 e01 = __fmul2_rn(K.kf01, __ffma2_rn(K.kf01, dup2(g.y), dup2(g.x)));
-    const float2 e23 = __fmul2_rn(K.kf23, __ffma2_rn(K.kf23, dup2(g.y), dup2(g.x)));
-    o.ce01 = __fmul2_rn(o.c01, e01);
-    o.ce23 = __fmul2_rn(o.c23, e23);
-    o.se01 = __fmul2_rn(o.s01, make_float2(-e01.x, -e01.y));
-    o.se23 = __fmul2_rn(o.s23, make_float2(-e23.x, -e23.y));
+    o.e = K.kt * fmaf(K.kt, g.y, g.x);
 }
 
-// Slow pass, the multiply-adds of one tone: two per tone-sample (the tone at the tile-centre frequency, and the
-// first-order frequency correction of its pair tables).
+// Slow pass, the multiply-adds of one tone: the pair tables are moved to the thread's local frequency once,
+// C'_j = C_j + e dC_j/dw, S'_j = S_j + e dS_j/dw (16 multiply-adds), and serve the thread's four groups (64): 1.25
+// multiply-adds per tone-sample.
 __device__ __forceinline__ void slow_fma(const StageRec *rec, const SlowSC &v, PQ (&pq)[kBlocksPerTile])
 {
+    const float2 e2 = dup2(v.e);
+    float4 C03 = rec[0].C03, C47 = rec[0].C47, S03 = rec[0].S03, S47 = rec[0].S47;
     {
-        const float4 C03 = rec[0].C03, C47 = rec[0].C47, S03 = rec[0].S03, S47 = rec[0].S47;
-        pq_add(pq[0], v.s01.x, v.c01.x, C03, C47, S03, S47);
-        pq_add(pq[1], v.s01.y, v.c01.y, C03, C47, S03, S47);
-        pq_add(pq[2], v.s23.x, v.c23.x, C03, C47, S03, S47);
-        pq_add(pq[3], v.s23.y, v.c23.y, C03, C47, S03, S47);
+        const float4 d0 = rec[1].C03, d1 = rec[1].C47, d2 = rec[1].S03, d3 = rec[1].S47;
+        float2 t;
+        t = __ffma2_rn(e2, make_float2(d0.x, d0.y), make_float2(C03.x, C03.y)); C03.x = t.x; C03.y = t.y;
+        t = __ffma2_rn(e2, make_float2(d0.z, d0.w), make_float2(C03.z, C03.w)); C03.z = t.x; C03.w = t.y;
+        t = __ffma2_rn(e2, make_float2(d1.x, d1.y), make_float2(C47.x, C47.y)); C47.x = t.x; C47.y = t.y;
+        t = __ffma2_rn(e2, make_float2(d1.z, d1.w), make_float2(C47.z, C47.w)); C47.z = t.x; C47.w = t.y;
+        t = __ffma2_rn(e2, make_float2(d2.x, d2.y), make_float2(S03.x, S03.y)); S03.x = t.x; S03.y = t.y;
+        t = __ffma2_rn(e2, make_float2(d2.z, d2.w), make_float2(S03.z, S03.w)); S03.z = t.x; S03.w = t.y;
+        t = __ffma2_rn(e2, make_float2(d3.x, d3.y), make_float2(S47.x, S47.y)); S47.x = t.x; S47.y = t.y;
+        t = __ffma2_rn(e2, make_float2(d3.z, d3.w), make_float2(S47.z, S47.w)); S47.z = t.x; S47.w = t.y;
     }
-    {
-        const float4 C03 = rec[1].C03, C47 = rec[1].C47, S03 = rec[1].S03, S47 = rec[1].S47;
-        pq_add(pq[0], v.se01.x, v.ce01.x, C03, C47, S03, S47);
-        pq_add(pq[1], v.se01.y, v.ce01.y, C03, C47, S03, S47);
-        pq_add(pq[2], v.se23.x, v.ce23.x, C03, C47, S03, S47);
-        pq_add(pq[3], v.se23.y, v.ce23.y, C03, C47, S03, S47);
-    }
+    pq_add(pq[0], v.s01.x, v.c01.x, C03, C47, S03, S47);
+    pq_add(pq[1], v.s01.y, v.c01.y, C03, C47, S03, S47);
+    pq_add(pq[2], v.s23.x, v.c23.x, C03, C47, S03, S47);
+    pq_add(pq[3], v.s23.y, v.c23.y, C03, C47, S03, S47);
 }
 
 // A work unit is one 2048-sample tile (4 blocks of 512) x the tones of one warp.  SPLIT warps (a team) share a
@@ -876,7 +907,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
     const int bpl = (per + kBatch - 1) / kBatch;   // batches per leaf
     const bool cross = kQuads && lp.cross != 0;
     const int64_t n_units = cross ? n_tiles * Q : n_tiles;
-    const int off = lane * kSPT + kSPT / 2 - kHalf;  // thread's pair centre + 1/2 relative to the centre of block 0
+    const int l16 = lane - 16;   // angle-addition passes: the thread owns samples lane*64 .. +63 of the tile; phases are referenced to lane 16
     // Tile scheduler: every team starts on the tile of its own index and then draws tiles from the launch's
     // counter lp.sched[0] (tiles that hold moving tones cost several times the others, so a fixed stride leaves
     // SMs idle at the end).  Which team computes a tile has no effect on its samples.
@@ -910,8 +941,9 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
 #pragma unroll
                 for (int m = 0; m < kPairs / 2; ++m) pq[r].P[m] = pq[r].Q[m] = make_float2(0.f, 0.f);
             const double tb_d = static_cast<double>(tile_base);
-            // phase reference: the centre of block 0, minus the half sample of the pair centring
-            const uint64_t a0 = static_cast<uint64_t>(tile_base + kHalf);
+            // phase reference: the pair centre of group 0 of lane 16 (sample 16*64 + 8 of the tile, minus the half sample of the
+            // pair centring); lanes are 64 samples apart, groups 16
+            const uint64_t a0 = static_cast<uint64_t>(tile_base + kTile / 2 + kSPT / 2);
             for (int tb = t_begin, b = 0; tb < t_end; tb += kBatch, ++b) {
                 const int t = tb + lane;
                 bool is_static = false, is_mover = false, is_post = false, is_slow = false;
@@ -958,9 +990,12 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                             const uint64_t nc = static_cast<uint64_t>(tile_base + kTile / 2);
                             const uint64_t wc = w + frac_to_fix64(f64_of(v5.x, v5.y) * g1);
                             const uint64_t pc = th + w * nc + frac_to_fix64(f64_of(v4.z, v4.w) * g0);
-                            ws.mrec[lane].q[0] = make_float4(__uint_as_float(round32(pc - (wc >> 1))), __uint_as_float(round32(wc)),
+                            // linear part of the phase at the pair centre of group 0 of lane 16 (k = 7.5), per thread, per group, per sample
+                            ws.mrec[lane].q[0] = make_float4(__uint_as_float(round32(pc + wc * static_cast<uint64_t>(kSPT / 2) - (wc >> 1))),
+                                                             __uint_as_float(round32(wc * static_cast<uint64_t>(kBlocksPerTile * kSPT))),
                                                              __uint_as_float(v5.z) * g2, __uint_as_float(v5.w) * g3);
-                            ws.mrec[lane].q[1] = make_float4(__uint_as_float(v0.x), 0.f, 0.f, 0.f);
+                            ws.mrec[lane].q[1] = make_float4(__uint_as_float(v0.x), __uint_as_float(round32(wc * static_cast<uint64_t>(kSPT))),
+                                                             __uint_as_float(round32(wc)), 0.f);
                         } else {
                             is_static = false;
                             is_mover = true;
@@ -994,8 +1029,8 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                         }
                     }
                     c0 = round32(th + w * a0 - (w >> 1));
-                    c1 = round32(w);
-                    d = round32(w * static_cast<uint64_t>(kBlock));
+                    c1 = round32(w * static_cast<uint64_t>(kBlocksPerTile * kSPT));
+                    d = round32(w * static_cast<uint64_t>(kSPT));
                 }
                 if (tb + kBatch < t_end) {
                     const int tn = tb + kBatch + lane;
@@ -1036,7 +1071,7 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 // 32 FFMA2 of tone i.  Scalar fp32 instructions cost the FMA pipe as much as an FFMA2 (measured,
                 // profiles/), hence the packed range multiply and no register moves.
                 float sa[kBlocksPerTile], ca[kBlocksPerTile], sb[kBlocksPerTile], cb[kBlocksPerTile];
-                sincos_tile(&ws.st[0], off, sa, ca);
+                sincos_tile(&ws.st[0], l16, sa, ca);
                 // a running pointer keeps the loop free of index arithmetic (IMAD shares the FMA pipe)
                 const StageRec *sp = ws.st;
                 const StageRec *const sp_end = ws.st + n_sta;
@@ -1044,14 +1079,14 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 for (; sp + 1 < sp_end; sp += 2) {
                     {
                         const float4 C03 = sp[0].C03, C47 = sp[0].C47, S03 = sp[0].S03, S47 = sp[0].S47;
-                        sincos_tile(sp + 1, off, sb, cb);
+                        sincos_tile(sp + 1, l16, sb, cb);
 #pragma unroll
                         for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sa[r], ca[r], C03, C47, S03, S47);
                     }
                     {
                         const float4 C03 = sp[1].C03, C47 = sp[1].C47, S03 = sp[1].S03, S47 = sp[1].S47;
                         // slot i + 2 <= kBatch exists; past the last tone it is stale and its result unused
-                        sincos_tile(sp + 2, off, sa, ca);
+                        sincos_tile(sp + 2, l16, sa, ca);
 #pragma unroll
                         for (int r = 0; r < kBlocksPerTile; ++r) pq_add(pq[r], sb[r], cb[r], C03, C47, S03, S47);
                     }
@@ -1066,12 +1101,13 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                 if (m_slow != 0u) {
                     SlowK slowk;
                     {
-                        slowk.m0 = lane * kSPT + kSPT / 2 - kTile / 2;   // (pair centre + 1/2) - tile centre, block 0
-                        const float k0 = static_cast<float>(slowk.m0) - 0.5f;
-                        slowk.kf01 = make_float2(k0, k0 + static_cast<float>(kBlock));
-                        slowk.kf23 = make_float2(k0 + static_cast<float>(2 * kBlock), k0 + static_cast<float>(3 * kBlock));
+                        slowk.l16 = l16;
+                        const float k0 = static_cast<float>(l16 * (kBlocksPerTile * kSPT)) + (0.5f * kSPT - 0.5f);   // group 0: 64 (lane - 16) + 7.5
+                        slowk.kf01 = make_float2(k0, k0 + static_cast<float>(kSPT));
+                        slowk.kf23 = make_float2(k0 + static_cast<float>(2 * kSPT), k0 + static_cast<float>(3 * kSPT));
                         slowk.kk01 = __fmul2_rn(slowk.kf01, slowk.kf01);
                         slowk.kk23 = __fmul2_rn(slowk.kf23, slowk.kf23);
+                        slowk.kt = static_cast<float>(l16 * (kBlocksPerTile * kSPT)) + (0.5f * (kBlocksPerTile * kSPT) - 0.5f);   // the thread's centre: + 31.5
                     }
                     sticky_sta = 0u;           // ws.st is overwritten: a single-batch warp restages its tables next tile
                     sticky_post = 0xffffffffu;
@@ -1121,7 +1157,16 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
         if (!kQuads) {
             if (SPLIT == 1 && ROT && n_mov == 0) {
 #pragma unroll
-                for (int r = 0; r < kBlocksPerTile; ++r) store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, acc[r]);
+                for (int g = 0; g < kBlocksPerTile; ++g) park_store(ws, g, lane, acc[g]);
+                __syncwarp();
+                // (through the park area: group layout -> block layout, whose 16-byte stores are contiguous across the warp)
+#pragma unroll
+                for (int r = 0; r < kBlocksPerTile; ++r) {
+                    Acc16 blk;
+                    park_load(ws, r, lane, blk);
+                    store_block(lp, n_thread + r * kBlock, xs_tile, lane * kSPT + r * kBlock, blk);
+                }
+                __syncwarp();
             } else if (ROT) {
 #pragma unroll
                 for (int r = 0; r < kBlocksPerTile; ++r) park_store(ws, r, lane, acc[r]);
@@ -1315,13 +1360,13 @@ __global__ void __launch_bounds__(128) awg_expand_kernel(ToneRec *table, const T
     ToneRec &dst = table[idx ? idx[j] : j];
     if (lane < 8) reinterpret_cast<uint4 *>(&dst.core)[lane] = reinterpret_cast<const uint4 *>(&c)[lane];
     if (lane >= 2 * kPairs) {
-        // pad_[0], pad_[1] of each table: cosine and sine of the carrier phase of two blocks (the rotation that takes the
-        // sines/cosines of blocks 0, 1 to blocks 2, 3 in the static pass); pad_[2], pad_[3] = 0
+        // pad_[0], pad_[1] of each table: cosine and sine of the carrier phase of two groups of 16 samples (the rotation that
+        // takes the sines/cosines of a thread's groups 0, 1 to its groups 2, 3 in the static pass); pad_[2], pad_[3] = 0
         if (lane < 2 * kPairs + 8) {
             const int st = (lane - 2 * kPairs) >> 2, q = lane & 3;
             float v = 0.f;
             if (q < 2) {
-                const uint64_t ang2 = (st ? c.w_post : c.w_pre) * static_cast<uint64_t>(2 * kBlock);
+                const uint64_t ang2 = (st ? c.w_post : c.w_pre) * static_cast<uint64_t>(2 * kSPT);
                 double sn2, cs2;
                 sincospi(2.0 * (static_cast<double>(static_cast<int64_t>(ang2)) * (1.0 / kTwo64)), &sn2, &cs2);
                 v = static_cast<float>(q == 0 ? cs2 : sn2);

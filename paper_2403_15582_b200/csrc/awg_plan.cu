@@ -86,14 +86,17 @@ int classify(int profile, long double DT, long double Tn)
     return CLS_DEG6;
 }
 
-// Slow movers (flag CLS_SLOW_FLAG): inside its move the tone changes frequency so slowly that, over a whole
-// 4096-sample tile, the angle-addition engine can carry it with a cubic phase polynomial at each thread's pair centre
-// plus a first-order frequency correction of the pair tables (kernel: slow pass).  Bounds with
-// R = 2048 (half a tile) and h = 15.5 (half a thread's 32 samples), Taylor coefficients C_m = a r^(m-1) sup|g^(m)| / m!
-// in turns per sample^m (sup|g^(m)| on [0,1] for the minimum-jerk g: 1.875, 5.7735, 60, 360, 720 for m = 2..6):
+// Slow movers (flag CLS_SLOW_FLAG): inside its move the tone changes frequency so slowly that, over a whole tile, the
+// angle-addition engine can carry it: a cubic phase polynomial about the tile centre gives the phase at the pair centres
+// of a thread's four groups of 16 samples, and the pair tables (built at the tile-centre frequency) are moved to the
+// frequency at the thread's own centre by a first-order correction (kernel: slow pass).  Bounds with
+// R = kTile/2 (half a tile), h = 7.5 (half a group), g = 24 (distance of the outer groups' centres from the thread's
+// centre), Taylor coefficients C_m = a r^(m-1) sup|g^(m)| / m! in turns per sample^m (sup|g^(m)| on [0,1] for the
+// minimum-jerk g: 1.875, 5.7735, 60, 360, 720 for m = 2..6):
 //   dropped phase terms  C4 R^4 + C5 R^5 + C6 R^6            <= 2e-8 turn
 //   dropped frequency    (4 C4 R^3 + 5 C5 R^4 + 6 C6 R^5) h  <= 2e-8 turn
-//   curvature inside a thread's samples (C2 + 3 C3 R + 6 C4 R^2) h^2 <= 3e-7 turn
+//   frequency drift between the thread's centre and a group's centre  (2 C2 + 6 C3 R) g h <= 4e-7 turn
+//   curvature inside a group  (C2 + 3 C3 R + 6 C4 R^2) h^2   <= 3e-7 turn
 //   second order of the table correction  (2 pi h (2 C2 R + 3 C3 R^2))^2 / 2 <= 2e-7
 //   fp32 polynomial magnitude  C2 R^2 + C3 R^3 <= 0.25 turn
 bool is_slow_mover(int profile, long double DT, long double Tn)
@@ -110,6 +113,7 @@ bool is_slow_mover(int profile, long double DT, long double Tn)
     const double R2 = R * R, R3 = R2 * R, R4 = R3 * R, R5 = R4 * R, R6 = R5 * R;
     if (C4 * R4 + C5 * R5 + C6 * R6 > 2e-8) return false;
     if ((4.0 * C4 * R3 + 5.0 * C5 * R4 + 6.0 * C6 * R5) * h > 2e-8) return false;
+    if ((2.0 * C2 + 6.0 * C3 * R) * (1.5 * kSPT) * h > 4e-7) return false;
     if ((C2 + 3.0 * C3 * R + 6.0 * C4 * R2) * h * h > 3e-7) return false;
     const double x = 6.283185307179586 * h * (2.0 * C2 * R + 3.0 * C3 * R2);
     if (0.5 * x * x > 2e-7) return false;

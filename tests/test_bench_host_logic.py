@@ -1,5 +1,5 @@
 """Host-side arithmetic of bench.py's roofline accounting (no GPU): which pipe binds, how the algorithmic operations
-are turned into a fraction (DESIGN.md section 6 "Roofline": 1 multiply-add per static tone-sample, 2 inside a slow
+are turned into a fraction (DESIGN.md section 6 "Roofline": 1 multiply-add per static tone-sample, 1.25 inside a slow
 move, 1 MUFU.SIN + 2 multiply-adds inside any other move).  The counts themselves come from the LIBRARY
 (awg_plan_op_counts: the classification the kernel acts on); tests/test_gpu_parity.py::test_op_counts_* checks those
 against the workload definitions on the GPU box."""
@@ -32,12 +32,12 @@ def test_pipe_roofline_picks_the_binding_pipe_and_scales_with_time():
     rm = bench.pipe_roofline(counts, 0.2, "mufu", sm_mhz)
     assert rm["pipe"].startswith("XU") and rm["mufu_ops"] == total
     assert np.isclose(rm["frac"], (total / xu_peak) / 0.2e-3)
-    # C3-like: every tone a slow mover for 19.6e6 of 19 922 944 samples: two multiply-adds each, no sine per sample
+    # C3-like: every tone a slow mover for 19.6e6 of 19 922 944 samples: 1.25 multiply-adds each, no sine per sample
     slow = 1000 * 19_600_000
     sta = 1000 * 19_922_944 - slow
     r3 = bench.pipe_roofline((sta, slow, 0), 2.25, "auto", sm_mhz)
     assert r3["pipe"].startswith("FMA") and r3["mufu_ops"] == 0
-    assert np.isclose(r3["frac"], (sta + 2 * slow) / fma_peak / 2.25e-3)
+    assert np.isclose(r3["frac"], (sta + 1.25 * slow) / fma_peak / 2.25e-3)
     # all fast movers: XU binds (1 / 16 per clock against 2 / 128)
     rf = bench.pipe_roofline((0, 0, 10 ** 9), 1.0, "auto", sm_mhz)
     assert rf["pipe"].startswith("XU") and np.isclose(rf["frac"], 1e9 / xu_peak / 1e-3)
