@@ -26,7 +26,8 @@
  *  - A plan is not thread-safe; distinct plans are independent.
  *  - Output for (plan, chunk_idx) is a pure function of the trajectory table and of the absolute
  *    sample index; it does not depend on the stream, ring depth, call order or chunk_len
- *    (kernel tiles are anchored to absolute sample indices that are multiples of 4096).
+ *    (kernel tiles are anchored to absolute sample indices that are multiples of 2048, and
+ *    the order in which tone partial sums are added depends on the tone count only).
  *  - A plan belongs to the CUDA device that was current when it was created; calls that enqueue
  *    work return AWG_ERR_STATE when another device is current.
  */
@@ -64,9 +65,9 @@ enum {
     AWG_ENGINE_AUTO = 0, /* the library picks (currently AWG_ENGINE_FMA)                                    */
     AWG_ENGINE_MUFU = 1, /* one MUFU.SIN per (tone, sample); phase re-centred per 512-sample block           */
     AWG_ENGINE_FP64 = 2, /* reference-grade: closed form and sine in fp64 per (tone, sample); ~50x slower   */
-    AWG_ENGINE_FMA = 3   /* angle addition on the FMA pipe for 4096-sample tiles where a tone is static (one
+    AWG_ENGINE_FMA = 3   /* angle addition on the FMA pipe for 2048-sample tiles where a tone is static (one
                             sin + one cos per thread, tone and 32 samples, then ONE multiply-add per
-                            tone-sample with a per-tone table); tiles inside a slow move take two
+                            tone-sample with a per-tone table); tiles inside a slow move take 1.25
                             multiply-adds per tone-sample, tiles inside any other move the MUFU path      */
 };
 

@@ -325,8 +325,9 @@ struct __align__(16) StageRec {
     uint32_t c0, c1, d, pad_;
     float r0, r1, r2, r3;        // static tone: {cos, sin}(2 pi 32 w), the rotation by two groups; slow mover: 2 c2, 3 c3
     float4 C03, C47, S03, S47;
+    float4 bank_pad_;            // 112-byte stride: the 16-byte stores of eight lanes (one record each) fall on distinct banks
 };
-static_assert(sizeof(StageRec) == 96, "StageRec must be 96 bytes");
+static_assert(sizeof(StageRec) == 112, "StageRec must be 112 bytes");
 
 // One re-centred (tone, block) record of the MUFU pass: q[0] = {c0 bits, c1 bits, A, c2}; q[1] = {c3, c4, c5, c6}.
 // K_EXACT: c0 = tone index.

@@ -157,9 +157,9 @@ __global__ void __launch_bounds__(128) bench(float *out, unsigned long long seed
 
 // The multiply-add block of the angle-addition pass as the library writes it: 4 blocks x (4 P + 4 Q) packed accumulators,
 // one tone's pair tables from shared memory (4 broadcast LDS.128), sines/cosines broadcast from scalar registers.
-// WITH_SINCOS adds the per-tone chain IMAD, IADD, I2F, FMUL2, sin.approx, cos.approx of the four blocks (software-pipelined
-// one tone ahead as in the library).
-template <bool WITH_SINCOS>
+// WITH_SINCOS = 1 adds the per-tone chain IMAD, IADD, I2F, FMUL2, sin.approx, cos.approx of the four blocks (software-
+// pipelined one tone ahead as in the library); = 2 takes two of the four blocks from MUFU and rotates them on to the others.
+template <int WITH_SINCOS>
 __global__ void __launch_bounds__(128) pq_loop(float *out, int n_iter, unsigned long long *cycles)
 {
     const long long t_begin = clock64();
@@ -188,8 +188,17 @@ __global__ void __launch_bounds__(128) pq_loop(float *out, int n_iter, unsigned 
             float2 x23 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int>(p2)), __int2float_rn(static_cast<int>(p3))), make_float2(k, k));
             asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[0]) : "f"(x01.x)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[0]) : "f"(x01.x));
             asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[1]) : "f"(x01.y)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[1]) : "f"(x01.y));
-            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[2]) : "f"(x23.x)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[2]) : "f"(x23.x));
-            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[3]) : "f"(x23.y)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[3]) : "f"(x23.y));
+            if (WITH_SINCOS == 1) {
+                asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[2]) : "f"(x23.x)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[2]) : "f"(x23.x));
+                asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[3]) : "f"(x23.y)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[3]) : "f"(x23.y));
+            } else {
+                // blocks 2, 3 = blocks 0, 1 rotated by a per-tone angle (cc.w, cc.z reused as cos, sin): four packed instructions
+                const float cd = __uint_as_float(cc.w), sd = __uint_as_float(cc.z);
+                const float2 s01 = make_float2(sn2[0], sn2[1]), c01 = make_float2(cs2[0], cs2[1]);
+                const float2 s23 = __ffma2_rn(c01, make_float2(sd, sd), __fmul2_rn(s01, make_float2(cd, cd)));
+                const float2 c23 = __ffma2_rn(s01, make_float2(-sd, -sd), __fmul2_rn(c01, make_float2(cd, cd)));
+                sn2[2] = s23.x; sn2[3] = s23.y; cs2[2] = c23.x; cs2[3] = c23.y;
+            }
         }
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
@@ -217,7 +226,7 @@ __global__ void __launch_bounds__(128) pq_loop(float *out, int n_iter, unsigned 
     if (threadIdx.x == 0) atomicMax(cycles, static_cast<unsigned long long>(clock64() - t_begin));
 }
 
-template <bool WITH_SINCOS>
+template <int WITH_SINCOS>
 void run_pq(const char *what, int n_sm, int wps, float *out)
 {
     unsigned long long *cyc_dev, cyc_host = 0;
@@ -282,7 +291,8 @@ int main(int argc, char **argv)
     run<21>("32 FFMA2 + 32 LOP3", n, wps, mhz, out);
     run<22>("rotation mix: 32 FFMA2 + 5 LDS.128 + 2 sin.approx + 2 MUFU.EX2 + 3 FMUL2 + 2 more FFMA2 + 2 I2F", n, wps, mhz, out);
     run<23>("slow-pass mix: 64 FFMA2 + 9 LDS.128 + 4 sin.approx + 4 MUFU.EX2 + 11 FMUL2 + 4 I2F", n, wps, mhz, out);
-    run_pq<false>("library multiply-add block: 32 FFMA2 (distinct accumulators, tables from 4 LDS.128, broadcast sines)", n, wps, out);
-    run_pq<true>("library static loop: the same + IMAD, 3 IADD, 4 I2F, 2 FMUL2, 4 sin.approx, 4 cos.approx per tone", n, wps, out);
+    run_pq<0>("library multiply-add block: 32 FFMA2 (distinct accumulators, tables from 4 LDS.128, broadcast sines)", n, wps, out);
+    run_pq<1>("library static loop, round 1: the same + IMAD, 3 IADD, 4 I2F, 2 FMUL2, 4 sin.approx, 4 cos.approx per tone", n, wps, out);
+    run_pq<2>("library static loop, round 2: 2 sin.approx + 2 cos.approx, the other two blocks by a packed rotation", n, wps, out);
     return 0;
 }
