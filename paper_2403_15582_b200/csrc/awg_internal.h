@@ -17,6 +17,7 @@ enum : int32_t {
     CLS_DEG6 = 6,    // k^2..k^6 (exact Taylor series of the degree-6 min-jerk phase)
     CLS_EXACT = 7,   // fp32 in-block polynomial not accurate enough: moving blocks use the fp64 path
     CLS_SLOW_FLAG = 1 << 16,  // OR-ed into ToneRec::cls: tiles wholly inside the move may take the slow pass (FMA pipe)
+    CLS_SLOW2_FLAG = 1 << 18, // with CLS_SLOW_FLAG: the slow pass corrects the pair tables per PAIR of groups (two local frequencies per thread)
     CLS_AMP_FLAG = 1 << 17    // OR-ed into ToneRec::cls: the tone has an amplitude ramp (A -> A1 over [amp_ns, amp_ns + amp_Tn))
 };
 
@@ -100,6 +101,7 @@ struct LaunchParams {
     const ToneRec *tab;
     int32_t n_tones;
     int32_t out_f32;   // 0: int16 codes, 1: fp32 sum before quantisation
+    int32_t slow2;     // != 0: some tone of the table carries CLS_SLOW2_FLAG: the slow pass corrects the pair tables per pair of groups
     int64_t n_begin;   // absolute index of the first output sample (multiple of 8)
     int64_t n_count;   // samples to produce (multiple of 8)
     float scale;       // int16 full-scale factor

@@ -818,9 +818,11 @@ struct SlowK {
 // the tile-centre frequency at the thread's own centre, e = 2 c2 k + 3 c3 k^2.
 struct SlowSC {
     float2 s01, s23, c01, c23;
-    float e;
+    float e;         // at the thread's centre (one correction per thread) or at the centre of groups 0, 1
+    float e_hi;      // two corrections per thread (SLOW2): at the centre of groups 2, 3
 };
 
+template <bool SLOW2>
 __device__ __forceinline__ void slow_sincos(const StageRec *rec, const SlowK &K, SlowSC &o)
 {
     const uint4 cc = *reinterpret_cast<const uint4 *>(rec);                 // c0, phase per thread, c2, c3
@@ -839,30 +841,42 @@ __device__ __forceinline__ void slow_sincos(const StageRec *rec, const SlowK &K,
     o.c01 = make_float2(mufu_cos(x01.x), mufu_cos(x01.y));
     o.s23 = make_float2(mufu_sin(x23.x), mufu_sin(x23.y));
     o.c23 = make_float2(mufu_cos(x23.x), mufu_cos(x23.y));
-    o.e = K.kt * fmaf(K.kt, g.y, g.x);
+    if (SLOW2) {
+        const float klo = K.kt - static_cast<float>(kSPT), khi = K.kt + static_cast<float>(kSPT);
+        o.e = klo * fmaf(klo, g.y, g.x);
+        o.e_hi = khi * fmaf(khi, g.y, g.x);
+    } else {
+        o.e = K.kt * fmaf(K.kt, g.y, g.x);
+    }
 }
 
 // Slow pass, the multiply-adds of one tone: the pair tables are moved to the thread's local frequency once,
 // C'_j = C_j + e dC_j/dw, S'_j = S_j + e dS_j/dw (16 multiply-adds), and serve the thread's four groups (64): 1.25
 // multiply-adds per tone-sample.
+__device__ __forceinline__ void slow_tables(const StageRec *rec, float e, float4 &C03, float4 &C47, float4 &S03, float4 &S47)
+{
+    const float2 e2 = dup2(e);
+    C03 = rec[0].C03; C47 = rec[0].C47; S03 = rec[0].S03; S47 = rec[0].S47;
+    const float4 d0 = rec[1].C03, d1 = rec[1].C47, d2 = rec[1].S03, d3 = rec[1].S47;
+    float2 t;
+    t = __ffma2_rn(e2, make_float2(d0.x, d0.y), make_float2(C03.x, C03.y)); C03.x = t.x; C03.y = t.y;
+    t = __ffma2_rn(e2, make_float2(d0.z, d0.w), make_float2(C03.z, C03.w)); C03.z = t.x; C03.w = t.y;
+    t = __ffma2_rn(e2, make_float2(d1.x, d1.y), make_float2(C47.x, C47.y)); C47.x = t.x; C47.y = t.y;
+    t = __ffma2_rn(e2, make_float2(d1.z, d1.w), make_float2(C47.z, C47.w)); C47.z = t.x; C47.w = t.y;
+    t = __ffma2_rn(e2, make_float2(d2.x, d2.y), make_float2(S03.x, S03.y)); S03.x = t.x; S03.y = t.y;
+    t = __ffma2_rn(e2, make_float2(d2.z, d2.w), make_float2(S03.z, S03.w)); S03.z = t.x; S03.w = t.y;
+    t = __ffma2_rn(e2, make_float2(d3.x, d3.y), make_float2(S47.x, S47.y)); S47.x = t.x; S47.y = t.y;
+    t = __ffma2_rn(e2, make_float2(d3.z, d3.w), make_float2(S47.z, S47.w)); S47.z = t.x; S47.w = t.y;
+}
+
+template <bool SLOW2>
 __device__ __forceinline__ void slow_fma(const StageRec *rec, const SlowSC &v, PQ (&pq)[kBlocksPerTile])
 {
-    const float2 e2 = dup2(v.e);
-    float4 C03 = rec[0].C03, C47 = rec[0].C47, S03 = rec[0].S03, S47 = rec[0].S47;
-    {
-        const float4 d0 = rec[1].C03, d1 = rec[1].C47, d2 = rec[1].S03, d3 = rec[1].S47;
-        float2 t;
-        t = __ffma2_rn(e2, make_float2(d0.x, d0.y), make_float2(C03.x, C03.y)); C03.x = t.x; C03.y = t.y;
-        t = __ffma2_rn(e2, make_float2(d0.z, d0.w), make_float2(C03.z, C03.w)); C03.z = t.x; C03.w = t.y;
-        t = __ffma2_rn(e2, make_float2(d1.x, d1.y), make_float2(C47.x, C47.y)); C47.x = t.x; C47.y = t.y;
-        t = __ffma2_rn(e2, make_float2(d1.z, d1.w), make_float2(C47.z, C47.w)); C47.z = t.x; C47.w = t.y;
-        t = __ffma2_rn(e2, make_float2(d2.x, d2.y), make_float2(S03.x, S03.y)); S03.x = t.x; S03.y = t.y;
-        t = __ffma2_rn(e2, make_float2(d2.z, d2.w), make_float2(S03.z, S03.w)); S03.z = t.x; S03.w = t.y;
-        t = __ffma2_rn(e2, make_float2(d3.x, d3.y), make_float2(S47.x, S47.y)); S47.x = t.x; S47.y = t.y;
-        t = __ffma2_rn(e2, make_float2(d3.z, d3.w), make_float2(S47.z, S47.w)); S47.z = t.x; S47.w = t.y;
-    }
+    float4 C03, C47, S03, S47;
+    slow_tables(rec, v.e, C03, C47, S03, S47);
     pq_add(pq[0], v.s01.x, v.c01.x, C03, C47, S03, S47);
     pq_add(pq[1], v.s01.y, v.c01.y, C03, C47, S03, S47);
+    if (SLOW2) slow_tables(rec, v.e_hi, C03, C47, S03, S47);   // plans with faster slow movers: groups 2, 3 get their own local frequency (1.5 per tone-sample)
     pq_add(pq[2], v.s23.x, v.c23.x, C03, C47, S03, S47);
     pq_add(pq[3], v.s23.y, v.c23.y, C03, C47, S03, S47);
 }
@@ -874,7 +888,7 @@ __device__ __forceinline__ void slow_fma(const StageRec *rec, const SlowSC &v, P
 // ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine), everything else (and
 // every tone when !ROT) takes the MUFU pass.  Every sample goes through the same arithmetic for every launch
 // geometry because all phases are anchored to absolute tile positions.
-template <int SPLIT, bool ROT, bool LEAVES>
+template <int SPLIT, bool ROT, bool LEAVES, bool SLOW2>
 __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(const LaunchParams lp)
 {
     constexpr int kTeams = kWarps / SPLIT;
@@ -1124,15 +1138,15 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
                         const StageRec *sp = ws.st;
                         const StageRec *const sp_end = ws.st + 2 * __popc(mh);
                         SlowSC va, vb;
-                        slow_sincos(sp, slowk, va);
+                        slow_sincos<SLOW2>(sp, slowk, va);
 #pragma unroll 1
                         for (; sp + 2 < sp_end; sp += 4) {
-                            slow_sincos(sp + 2, slowk, vb);
-                            slow_fma(sp, va, pq);
-                            slow_sincos(sp + 4, slowk, va);   // slots up to 2*16 + 1 exist; past the last tone: stale, unused
-                            slow_fma(sp + 2, vb, pq);
+                            slow_sincos<SLOW2>(sp + 2, slowk, vb);
+                            slow_fma<SLOW2>(sp, va, pq);
+                            slow_sincos<SLOW2>(sp + 4, slowk, va);   // slots up to 2*16 + 1 exist; past the last tone: stale, unused
+                            slow_fma<SLOW2>(sp + 2, vb, pq);
                         }
-                        if (sp < sp_end) slow_fma(sp, va, pq);
+                        if (sp < sp_end) slow_fma<SLOW2>(sp, va, pq);
                     }
                 }
             }
@@ -1434,14 +1448,14 @@ cudaError_t device_state(DeviceState **out)
     return cudaSuccess;
 }
 
-template <int SPLIT, bool ROT, bool LEAVES>
+template <int SPLIT, bool ROT, bool LEAVES, bool SLOW2>
 cudaError_t launch_one(DeviceState &ds, const LaunchParams &lp, int64_t tiles, cudaStream_t stream)
 {
     constexpr int kTeams = kWarps / SPLIT;
     constexpr size_t kSmem = sizeof(WarpSmem) * kWarps;
-    constexpr uint32_t kBit = 1u << ((LEAVES ? 3 : SPLIT == 1 ? 0 : SPLIT == 2 ? 1 : 2) * 2 + (ROT ? 1 : 0));
+    constexpr uint32_t kBit = 1u << (((LEAVES ? 3 : SPLIT == 1 ? 0 : SPLIT == 2 ? 1 : 2) * 2 + (ROT ? 1 : 0)) * 2 + (SLOW2 ? 1 : 0));
     if (!(ds.configured & kBit)) {
-        cudaError_t e = cudaFuncSetAttribute(awg_synth_kernel<SPLIT, ROT, LEAVES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(awg_synth_kernel<SPLIT, ROT, LEAVES, SLOW2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              static_cast<int>(kSmem));
         if (e != cudaSuccess) return e;
         ds.configured |= kBit;
@@ -1450,18 +1464,18 @@ cudaError_t launch_one(DeviceState &ds, const LaunchParams &lp, int64_t tiles, c
     const int64_t want = (tiles + kTeams - 1) / kTeams;   // (`tiles` = work units: tiles, or tiles x quads when lp.cross)
     const int64_t max_grid = static_cast<int64_t>(kCtasPerSm) * ds.n_sm;
     const unsigned grid = static_cast<unsigned>(want < max_grid ? want : max_grid);
-    awg_synth_kernel<SPLIT, ROT, LEAVES><<<grid, kWarps * 32, kSmem, stream>>>(lp);
+    awg_synth_kernel<SPLIT, ROT, LEAVES, SLOW2><<<grid, kWarps * 32, kSmem, stream>>>(lp);
     return cudaGetLastError();
 }
 
-template <bool ROT>
+template <bool ROT, bool SLOW2>
 cudaError_t launch_split(DeviceState &ds, const LaunchParams &lp, int split, int64_t tiles, cudaStream_t stream)
 {
     switch (split) {
-        case 1: return launch_one<1, ROT, false>(ds, lp, tiles, stream);
-        case 2: return launch_one<2, ROT, false>(ds, lp, tiles, stream);
-        default: return lp.n_quads > 1 ? launch_one<kWarps, ROT, true>(ds, lp, tiles, stream)
-                                       : launch_one<kWarps, ROT, false>(ds, lp, tiles, stream);
+        case 1: return launch_one<1, ROT, false, SLOW2>(ds, lp, tiles, stream);
+        case 2: return launch_one<2, ROT, false, SLOW2>(ds, lp, tiles, stream);
+        default: return lp.n_quads > 1 ? launch_one<kWarps, ROT, true, SLOW2>(ds, lp, tiles, stream)
+                                       : launch_one<kWarps, ROT, false, SLOW2>(ds, lp, tiles, stream);
     }
 }
 
@@ -1536,8 +1550,9 @@ cudaError_t launch_synth(const LaunchParams &lp_in, int engine, cudaStream_t str
                 units = tiles * quads;
             }
         }
-        e = (engine == AWG_ENGINE_FMA) ? launch_split<true>(*ds, lp, split, units, stream)
-                                       : launch_split<false>(*ds, lp, split, units, stream);
+        if (engine != AWG_ENGINE_FMA) e = launch_split<false, false>(*ds, lp, split, units, stream);   // (no slow pass: every tone on MUFU)
+        else if (lp.slow2) e = launch_split<true, true>(*ds, lp, split, units, stream);
+        else e = launch_split<true, false>(*ds, lp, split, units, stream);
     }
     count_launch();
     return e;

@@ -95,13 +95,16 @@ int classify(int profile, long double DT, long double Tn)
 // minimum-jerk g: 1.875, 5.7735, 60, 360, 720 for m = 2..6):
 //   dropped phase terms  C4 R^4 + C5 R^5 + C6 R^6            <= 2e-8 turn
 //   dropped frequency    (4 C4 R^3 + 5 C5 R^4 + 6 C6 R^5) h  <= 2e-8 turn
-//   frequency drift between the thread's centre and a group's centre  (2 C2 + 6 C3 R) g h <= 4e-7 turn
+//   frequency drift between the centre the tables are corrected for and a group's centre  (2 C2 + 6 C3 R) g h <= 4e-7 turn
+//     (g = 24 with one correction per thread; tones that fail it but pass with g = 8 get one correction per pair of groups)
 //   curvature inside a group  (C2 + 3 C3 R + 6 C4 R^2) h^2   <= 3e-7 turn
 //   second order of the table correction  (2 pi h (2 C2 R + 3 C3 R^2))^2 / 2 <= 2e-7
 //   fp32 polynomial magnitude  C2 R^2 + C3 R^3 <= 0.25 turn
-bool is_slow_mover(int profile, long double DT, long double Tn)
+// Returns 0 (not a slow mover), 1 (one table correction per thread: 1.25 multiply-adds per tone-sample) or 2 (the drift bound
+// holds only with one correction per pair of groups, g = 8: 1.5 multiply-adds per tone-sample).
+int is_slow_mover(int profile, long double DT, long double Tn)
 {
-    if (!(Tn >= 2.0L * kTile)) return false;
+    if (!(Tn >= 2.0L * kTile)) return 0;
     const double a = static_cast<double>(fabsl(DT) / Tn), r = static_cast<double>(1.0L / Tn);
     const double R = kTile / 2, h = 0.5 * (kSPT - 1);
     const bool lin = profile == AWG_PROFILE_LINEAR;
@@ -111,13 +114,17 @@ bool is_slow_mover(int profile, long double DT, long double Tn)
     const double C5 = lin ? 0.0 : a * r * r * r * r * 360.0 / 120.0;
     const double C6 = lin ? 0.0 : a * r * r * r * r * r;
     const double R2 = R * R, R3 = R2 * R, R4 = R3 * R, R5 = R4 * R, R6 = R5 * R;
-    if (C4 * R4 + C5 * R5 + C6 * R6 > 2e-8) return false;
-    if ((4.0 * C4 * R3 + 5.0 * C5 * R4 + 6.0 * C6 * R5) * h > 2e-8) return false;
-    if ((2.0 * C2 + 6.0 * C3 * R) * (1.5 * kSPT) * h > 4e-7) return false;
-    if ((C2 + 3.0 * C3 * R + 6.0 * C4 * R2) * h * h > 3e-7) return false;
+    if (C4 * R4 + C5 * R5 + C6 * R6 > 2e-8) return 0;
+    if ((4.0 * C4 * R3 + 5.0 * C5 * R4 + 6.0 * C6 * R5) * h > 2e-8) return 0;
+    int tables = 1;
+    if ((2.0 * C2 + 6.0 * C3 * R) * (1.5 * kSPT) * h > 4e-7) {
+        if ((2.0 * C2 + 6.0 * C3 * R) * (0.5 * kSPT) * h > 4e-7) return 0;
+        tables = 2;
+    }
+    if ((C2 + 3.0 * C3 * R + 6.0 * C4 * R2) * h * h > 3e-7) return 0;
     const double x = 6.283185307179586 * h * (2.0 * C2 * R + 3.0 * C3 * R2);
-    if (0.5 * x * x > 2e-7) return false;
-    return C2 * R2 + C3 * R3 <= 0.25;
+    if (0.5 * x * x > 2e-7) return 0;
+    return C2 * R2 + C3 * R3 <= 0.25 ? tables : 0;
 }
 
 void make_static(HostTone &h)
@@ -156,7 +163,11 @@ void make_move(HostTone &h, long double fs, long double f1, int profile, long do
     //                     = [theta - (f1-f0) t_s - DT/2] + (f1/fs) n
     h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(h.DT / 2.0L);
     h.cls = classify(profile, h.DT, h.Tn);
-    if (h.cls != CLS_EXACT && is_slow_mover(profile, h.DT, h.Tn)) h.cls |= CLS_SLOW_FLAG;
+    if (h.cls != CLS_EXACT) {
+        const int slow = is_slow_mover(profile, h.DT, h.Tn);
+        if (slow >= 1) h.cls |= CLS_SLOW_FLAG;
+        if (slow == 2) h.cls |= CLS_SLOW2_FLAG;
+    }
 }
 
 long double profile_h(int profile, long double s)  // frequency ramp 0 -> 1
@@ -233,6 +244,9 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
         for (int k = 0; k < p->n_tones; ++k)
             if (!p->in_buffer[k]) amp.push_back(std::max(std::fabs(p->tones[k].A), std::fabs(p->tones[k].A1)));
         fix_grids(amp.data(), static_cast<int>(amp.size()), &p->fix);
+        p->slow2 = false;
+        for (int k = 0; k < p->n_tones; ++k)
+            if (!p->in_buffer[k] && (p->tones[k].cls & CLS_SLOW2_FLAG)) p->slow2 = true;
     }
     std::sort(p->dirty_tones.begin(), p->dirty_tones.end());
     p->dirty_tones.erase(std::unique(p->dirty_tones.begin(), p->dirty_tones.end()), p->dirty_tones.end());
@@ -304,6 +318,7 @@ awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, voi
     lp.n_count = n_count;
     lp.scale = static_cast<float>(p->scale);
     lp.fix = p->fix;
+    lp.slow2 = p->slow2 ? 1 : 0;
     lp.out = dev_out;
     lp.out_f32 = f32 ? 1 : 0;
     lp.sched = nullptr;  // launch_synth assigns the tile-scheduler slot
@@ -614,6 +629,7 @@ awg_status static_buffer_add(awg_plan *p, const std::vector<HostTone> &tones, co
     std::vector<float> amp;
     for (const HostTone &h : tones) amp.push_back(std::max(std::fabs(h.A), std::fabs(h.A1)));
     fix_grids(amp.data(), n, &lp.fix);
+    lp.slow2 = 0;   // (static carriers only)
     lp.out = dst;
     lp.out_stride = 1;
     lp.out_offset = 0;

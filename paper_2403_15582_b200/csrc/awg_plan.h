@@ -53,6 +53,7 @@ struct awg_plan {
     std::vector<uint8_t> in_buffer;
     std::vector<int32_t> slot_of;
     int32_t n_active = 0;
+    bool slow2 = false;               // some active tone carries CLS_SLOW2_FLAG (slow pass with two table corrections per thread)
     awg::FixGrid fix{};                 // fixed-point grids of the kernel's leaf merge for the current table (fix_grids())
     float *xs[2] = {};                      // X_static, chunk_len floats each; xs[xs_cur] is current (a fold writes the other)
     int xs_cur = 0;

@@ -155,85 +155,97 @@ __global__ void __launch_bounds__(128) bench(float *out, unsigned long long seed
     if (threadIdx.x == 0) atomicMax(cycles, static_cast<unsigned long long>(clock64() - t_begin));
 }
 
-// The multiply-add block of the angle-addition pass as the library writes it: 4 blocks x (4 P + 4 Q) packed accumulators,
-// one tone's pair tables from shared memory (4 broadcast LDS.128), sines/cosines broadcast from scalar registers.
-// WITH_SINCOS = 1 adds the per-tone chain IMAD, IADD, I2F, FMUL2, sin.approx, cos.approx of the four blocks (software-
-// pipelined one tone ahead as in the library); = 2 takes two of the four blocks from MUFU and rotates them on to the others.
-template <int WITH_SINCOS>
-__global__ void __launch_bounds__(128) pq_loop(float *out, int n_iter, unsigned long long *cycles)
+// The multiply-add loop of the angle-addition pass as the library writes it: 4 groups x (4 P + 4 Q) packed accumulators,
+// one tone's pair tables from shared memory (4 broadcast LDS.128), sines/cosines broadcast from scalar registers,
+// software-pipelined one tone ahead and unrolled by two (ping-pong register sets), 3 CTAs of 128 threads per SM.
+// SC = 0: the multiply-adds alone; 1: plus the round-1 chain IMAD, 3 IADD, 4 I2F, 2 FMUL2, 4 sin.approx, 4 cos.approx per
+// tone; 2: the round-2 chain: two sin/cos pairs from MUFU, the other two by a packed rotation (2 FMUL2 + 2 FFMA2).
+struct PQu { float2 P[4], Q[4]; };
+__device__ __forceinline__ void pq_add_u(PQu &pq, float s, float c, const float4 &C03, const float4 &C47, const float4 &S03, const float4 &S47)
+{
+    const float2 s2 = make_float2(s, s), c2 = make_float2(c, c);
+    pq.P[0] = __ffma2_rn(s2, make_float2(C03.x, C03.y), pq.P[0]);
+    pq.P[1] = __ffma2_rn(s2, make_float2(C03.z, C03.w), pq.P[1]);
+    pq.P[2] = __ffma2_rn(s2, make_float2(C47.x, C47.y), pq.P[2]);
+    pq.P[3] = __ffma2_rn(s2, make_float2(C47.z, C47.w), pq.P[3]);
+    pq.Q[0] = __ffma2_rn(c2, make_float2(S03.x, S03.y), pq.Q[0]);
+    pq.Q[1] = __ffma2_rn(c2, make_float2(S03.z, S03.w), pq.Q[1]);
+    pq.Q[2] = __ffma2_rn(c2, make_float2(S47.x, S47.y), pq.Q[2]);
+    pq.Q[3] = __ffma2_rn(c2, make_float2(S47.z, S47.w), pq.Q[3]);
+}
+__device__ __forceinline__ float usin(float x) { float y; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float ucos(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+template <int SC>
+__device__ __forceinline__ void sincos4_u(const uint4 cc, const float4 rot, int off, float (&s)[4], float (&c)[4])
+{
+    const float k = 1.4629180792671596e-9f;
+    const float2 k2 = make_float2(k, k);
+    const unsigned p0 = cc.x + cc.y * static_cast<unsigned>(off), p1 = p0 + cc.z;
+    const float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int>(p0)), __int2float_rn(static_cast<int>(p1))), k2);
+    s[0] = usin(x01.x); c[0] = ucos(x01.x); s[1] = usin(x01.y); c[1] = ucos(x01.y);
+    if (SC == 1) {
+        const unsigned p2 = p1 + cc.z, p3 = p2 + cc.z;
+        const float2 x23 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int>(p2)), __int2float_rn(static_cast<int>(p3))), k2);
+        s[2] = usin(x23.x); c[2] = ucos(x23.x); s[3] = usin(x23.y); c[3] = ucos(x23.y);
+    } else {
+        const float2 s01 = make_float2(s[0], s[1]), c01 = make_float2(c[0], c[1]);
+        const float2 s23 = __ffma2_rn(c01, make_float2(rot.y, rot.y), __fmul2_rn(s01, make_float2(rot.x, rot.x)));
+        const float2 c23 = __ffma2_rn(s01, make_float2(-rot.y, -rot.y), __fmul2_rn(c01, make_float2(rot.x, rot.x)));
+        s[2] = s23.x; s[3] = s23.y; c[2] = c23.x; c[3] = c23.y;
+    }
+}
+
+// staged record: 6 float4 per tone: {c0, c1, d, -}, C03, C47, S03, S47, {cos, sin of the rotation, -, -}
+template <int SC>
+__global__ void __launch_bounds__(128, 3) pq_loop(float *out, int n_iter, unsigned long long *cycles)
 {
     const long long t_begin = clock64();
-    __shared__ float4 tab[64 * 5];
-    for (int i = threadIdx.x; i < 64 * 5; i += 128) tab[i] = make_float4(1e-3f * i, 1.f, 0.5f, 0.25f);
+    __shared__ float4 tab[67 * 6];
+    for (int i = threadIdx.x; i < 67 * 6; i += 128) tab[i] = make_float4(1e-3f * i, 1.f, 0.5f, 0.25f);
     __syncthreads();
-    float2 P[4][4], Q[4][4];
+    PQu pq[4];
 #pragma unroll
     for (int r = 0; r < 4; ++r)
 #pragma unroll
-        for (int m = 0; m < 4; ++m) P[r][m] = Q[r][m] = make_float2(0.f, 0.f);
-    float sn[4] = {0.1f, 0.2f, 0.3f, 0.4f}, cs[4] = {0.9f, 0.8f, 0.7f, 0.6f};
-    const int lane = threadIdx.x & 31;
-    const float4 *tp = tab;
+        for (int m = 0; m < 4; ++m) pq[r].P[m] = pq[r].Q[m] = make_float2(0.f, 0.f);
+    const int off = (threadIdx.x & 31) - 16;
+    float sa[4] = {0.1f, 0.2f, 0.3f, 0.4f}, ca[4] = {0.9f, 0.8f, 0.7f, 0.6f}, sb[4] = {0.11f, 0.21f, 0.31f, 0.41f}, cb[4] = {0.89f, 0.79f, 0.69f, 0.59f};
+    for (int it = 0; it < n_iter; it += 64) {
+        const float4 *sp = tab;
+        if (SC) sincos4_u<SC ? SC : 1>(*reinterpret_cast<const uint4 *>(sp), sp[5], off, sa, ca);
 #pragma unroll 1
-    for (int it = 0; it < n_iter; ++it) {
-        const float4 *rec = tp + 5 * (it & 63);
-        const float4 C03 = rec[1], C47 = rec[2], S03 = rec[3], S47 = rec[4];
-        float sn2[4], cs2[4];
-        if (WITH_SINCOS) {
-            const uint4 cc = *reinterpret_cast<const uint4 *>(tp + 5 * ((it + 1) & 63));
-            unsigned p0 = cc.x + cc.y * static_cast<unsigned>(lane * 16 - 248);
-            unsigned p1 = p0 + cc.z, p2 = p1 + cc.z, p3 = p2 + cc.z;
-            const float k = 1.4629180792671596e-9f;
-            float2 x01 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int>(p0)), __int2float_rn(static_cast<int>(p1))), make_float2(k, k));
-            float2 x23 = __fmul2_rn(make_float2(__int2float_rn(static_cast<int>(p2)), __int2float_rn(static_cast<int>(p3))), make_float2(k, k));
-            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[0]) : "f"(x01.x)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[0]) : "f"(x01.x));
-            asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[1]) : "f"(x01.y)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[1]) : "f"(x01.y));
-            if (WITH_SINCOS == 1) {
-                asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[2]) : "f"(x23.x)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[2]) : "f"(x23.x));
-                asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn2[3]) : "f"(x23.y)); asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs2[3]) : "f"(x23.y));
-            } else {
-                // blocks 2, 3 = blocks 0, 1 rotated by a per-tone angle (cc.w, cc.z reused as cos, sin): four packed instructions
-                const float cd = __uint_as_float(cc.w), sd = __uint_as_float(cc.z);
-                const float2 s01 = make_float2(sn2[0], sn2[1]), c01 = make_float2(cs2[0], cs2[1]);
-                const float2 s23 = __ffma2_rn(c01, make_float2(sd, sd), __fmul2_rn(s01, make_float2(cd, cd)));
-                const float2 c23 = __ffma2_rn(s01, make_float2(-sd, -sd), __fmul2_rn(c01, make_float2(cd, cd)));
-                sn2[2] = s23.x; sn2[3] = s23.y; cs2[2] = c23.x; cs2[3] = c23.y;
+        for (int i = 0; i < 64; i += 2, sp += 12) {
+            {
+                const float4 C03 = sp[1], C47 = sp[2], S03 = sp[3], S47 = sp[4];
+                if (SC) sincos4_u<SC ? SC : 1>(*reinterpret_cast<const uint4 *>(sp + 6), sp[11], off, sb, cb);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) pq_add_u(pq[r], sa[r], ca[r], C03, C47, S03, S47);
             }
-        }
+            {
+                const float4 C03 = sp[7], C47 = sp[8], S03 = sp[9], S47 = sp[10];
+                if (SC) sincos4_u<SC ? SC : 1>(*reinterpret_cast<const uint4 *>(sp + 12), sp[17], off, sa, ca);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const float2 s2 = make_float2(sn[r], sn[r]), c2 = make_float2(cs[r], cs[r]);
-            P[r][0] = __ffma2_rn(s2, make_float2(C03.x, C03.y), P[r][0]);
-            P[r][1] = __ffma2_rn(s2, make_float2(C03.z, C03.w), P[r][1]);
-            P[r][2] = __ffma2_rn(s2, make_float2(C47.x, C47.y), P[r][2]);
-            P[r][3] = __ffma2_rn(s2, make_float2(C47.z, C47.w), P[r][3]);
-            Q[r][0] = __ffma2_rn(c2, make_float2(S03.x, S03.y), Q[r][0]);
-            Q[r][1] = __ffma2_rn(c2, make_float2(S03.z, S03.w), Q[r][1]);
-            Q[r][2] = __ffma2_rn(c2, make_float2(S47.x, S47.y), Q[r][2]);
-            Q[r][3] = __ffma2_rn(c2, make_float2(S47.z, S47.w), Q[r][3]);
-        }
-        if (WITH_SINCOS) {
-#pragma unroll
-            for (int r = 0; r < 4; ++r) { sn[r] = sn2[r]; cs[r] = cs2[r]; }
+                for (int r = 0; r < 4; ++r) pq_add_u(pq[r], sb[r], cb[r], C03, C47, S03, S47);
+            }
         }
     }
     float s = 0.f;
 #pragma unroll
     for (int r = 0; r < 4; ++r)
 #pragma unroll
-        for (int m = 0; m < 4; ++m) s += P[r][m].x + P[r][m].y + Q[r][m].x + Q[r][m].y;
+        for (int m = 0; m < 4; ++m) s += pq[r].P[m].x + pq[r].P[m].y + pq[r].Q[m].x + pq[r].Q[m].y;
     if (s == 123.456f) out[0] = s;
     if (threadIdx.x == 0) atomicMax(cycles, static_cast<unsigned long long>(clock64() - t_begin));
 }
 
-template <int WITH_SINCOS>
+template <int SC>
 void run_pq(const char *what, int n_sm, int wps, float *out)
 {
     unsigned long long *cyc_dev, cyc_host = 0;
     cudaMalloc(&cyc_dev, sizeof cyc_host);
-    pq_loop<WITH_SINCOS><<<n_sm * wps, 128>>>(out, 64, cyc_dev);
+    pq_loop<SC><<<n_sm * wps, 128>>>(out, 64, cyc_dev);
     cudaMemset(cyc_dev, 0, sizeof cyc_host);
-    pq_loop<WITH_SINCOS><<<n_sm * wps, 128>>>(out, kIters, cyc_dev);
+    pq_loop<SC><<<n_sm * wps, 128>>>(out, kIters, cyc_dev);
     cudaMemcpy(&cyc_host, cyc_dev, sizeof cyc_host, cudaMemcpyDeviceToHost);
     cudaFree(cyc_dev);
     printf("%-100s %8.2f cycles/body/SMSP\n", what, static_cast<double>(cyc_host) / (static_cast<double>(kIters) * wps));
@@ -291,8 +303,8 @@ int main(int argc, char **argv)
     run<21>("32 FFMA2 + 32 LOP3", n, wps, mhz, out);
     run<22>("rotation mix: 32 FFMA2 + 5 LDS.128 + 2 sin.approx + 2 MUFU.EX2 + 3 FMUL2 + 2 more FFMA2 + 2 I2F", n, wps, mhz, out);
     run<23>("slow-pass mix: 64 FFMA2 + 9 LDS.128 + 4 sin.approx + 4 MUFU.EX2 + 11 FMUL2 + 4 I2F", n, wps, mhz, out);
-    run_pq<0>("library multiply-add block: 32 FFMA2 (distinct accumulators, tables from 4 LDS.128, broadcast sines)", n, wps, out);
+    run_pq<0>("library multiply-add loop (body = one tone): 32 FFMA2, distinct accumulators, tables from 4 LDS.128, broadcast sines", n, wps, out);
     run_pq<1>("library static loop, round 1: the same + IMAD, 3 IADD, 4 I2F, 2 FMUL2, 4 sin.approx, 4 cos.approx per tone", n, wps, out);
-    run_pq<2>("library static loop, round 2: 2 sin.approx + 2 cos.approx, the other two blocks by a packed rotation", n, wps, out);
+    run_pq<2>("library static loop, round 2: IMAD, IADD, 2 I2F, FMUL2, 2 sin.approx, 2 cos.approx + packed rotation (2 FMUL2, 2 FFMA2)", n, wps, out);
     return 0;
 }

@@ -387,10 +387,12 @@ def test_plan_limit_65536_tones(awg, torch_cuda, eng):
 
 def test_slow_movers_at_the_class_boundary(awg, torch_cuda):
     """Slow pass of the angle-addition engine (moves carried on the FMA pipe: cubic phase polynomial per thread +
-    first-order correction of the pair tables).  Sixteen tones sit at ~90 % of the bounds of is_slow_mover()
-    (csrc/awg_plan.cu): LINEAR +-10 MHz and MINJERK +-1.75 MHz over 5 ms at 560 MS/s, sum of amplitudes 1.  Chunks at
-    the start and end of the move (those tiles take the MUFU path), at the largest curvature of the minimum-jerk ramp
-    (s = 0.21, 0.79) and in the middle; the fp32 sum must stay within 1e-5 of full scale, the codes within the bar."""
+    first-order correction of the pair tables).  Sixteen tones sit at ~95 % of the bounds of is_slow_mover()
+    (csrc/awg_plan.cu): LINEAR +-10 MHz over 5 ms at 560 MS/s is at 95 % of the drift bound with one table correction per
+    PAIR of groups (CLS_SLOW2_FLAG: the plan runs the SLOW2 instantiation), MINJERK +-1.75 MHz at 94 % of the drift bound
+    with one correction per thread; sum of amplitudes 1.  Chunks at the start and end of the move (those tiles take the MUFU
+    path), at the largest curvature of the minimum-jerk ramp (s = 0.21, 0.79) and in the middle; the fp32 sum must stay
+    within 1e-5 of full scale, the codes within the bar."""
     fs, T, cl, N = 560e6, 5e-3, 1 << 14, 16
     rng = np.random.default_rng(11)
     f0 = rng.uniform(60e6, 200e6, N)
@@ -409,6 +411,27 @@ def test_slow_movers_at_the_class_boundary(awg, torch_cuda):
         worst = max(worst, assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"slow movers, chunk {c}"))
         assert_codes_close(_np(p.synthesize_chunk(c)), op.quantise(V), f"slow movers, chunk {c}")
     print(f"slow movers: f32 max err {worst:.2e} of full scale")
+    p.close()
+
+
+def test_slow_movers_one_correction_per_thread_at_its_bound(awg, torch_cuda):
+    """The 1.25-multiply-add slow pass (one table correction per thread, groups up to 24 samples from the thread's centre):
+    64 minimum-jerk tones +-1.8 MHz over 5 ms, 97 % of the drift bound (2 C2 + 6 C3 R) g h <= 4e-7 with g = 24, none over it
+    (the plan must NOT need the SLOW2 instantiation: checked through the op counts), sum of amplitudes 1, all phases equal so that
+    the errors of the tones can add up; chunks around the largest chirp rate (s = 1/2)."""
+    fs, T, cl, N = 560e6, 5e-3, 1 << 14, 64
+    rng = np.random.default_rng(12)
+    f0 = rng.uniform(60e6, 200e6, N)
+    rows = [(f0[k], f0[k] + (1.8e6 if k % 2 else -1.8e6), 1.0 / N, 0.3, 0.0, T, MINJERK) for k in range(N)]
+    p, op = _single(awg, fs, cl, rows, engine=awg.AWG_ENGINE_FMA)
+    sta, slow, fast = p.op_counts(80, 8)
+    assert slow == N * 8 * cl and fast == 0, "the tones must be slow movers inside their move"
+    worst = 0.0
+    for c in (40, 84, 85, 86, 130):
+        V = oracle.c_waveform(op, c * cl, (c + 1) * cl)
+        worst = max(worst, assert_f32_close(_np(p.synthesize_chunk_f32(c)), V, f"slow movers (one correction), chunk {c}"))
+        assert_codes_close(_np(p.synthesize_chunk(c)), op.quantise(V), f"slow movers (one correction), chunk {c}")
+    print(f"slow movers, one correction per thread: f32 max err {worst:.2e} of full scale")
     p.close()
 
 
