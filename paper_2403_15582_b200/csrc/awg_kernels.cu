@@ -5,14 +5,18 @@
 //       (stage of the static pass in awg_synth_kernel), per (tone, 512-sample block) c0, c1, c2..c6 and the record
 //       kind for tones moving there                                                          block_prologue()
 //   a2  per tone-sample phase of a moving tone: c0 + c1*k (u32 turns, wraps exactly) + fp32 polynomial  mufu_rec<KIND>()
-//   a3  sine.  Tiles in which a tone is static (angle-addition engine): one MUFU.SIN + one MUFU.COS per (thread, tone,
-//       block), then per symmetric sample pair centre +- (j + 1/2)
+//   a3  sine.  Tiles in which a tone is static (angle-addition engine; a thread owns 64 consecutive samples, four groups of
+//       16): per (thread, tone) two MUFU.SIN/COS pairs and a packed rotation give sin, cos at the pair centres of the four
+//       groups, then per symmetric sample pair centre +- (j + 1/2)
 //           A sin(phi +- (j+1/2) w) = sin(phi) [A cos((j+1/2) w)]  +-  cos(phi) [A sin((j+1/2) w)]
 //       i.e. ONE fp32 multiply-add per tone-sample into the even/odd accumulators P_j, Q_j    sincos_tile(), pq_add()
-//       Tiles wholly inside a SLOW move: the same with a cubic phase polynomial per thread and a first-order
-//       frequency correction of the pair tables: TWO multiply-adds per tone-sample              stage_slow(), slow_sincos(), slow_fma()
+//       Tiles wholly inside a SLOW move: a cubic phase polynomial gives the phase at the four pair centres, the pair tables
+//       are moved to the thread's local frequency once (first order): 1.25 multiply-adds per tone-sample (1.5 with one
+//       correction per pair of groups, SLOW2)                                     stage_slow(), slow_sincos(), slow_fma()
 //       Blocks in which a tone moves otherwise (and every tone-sample of the MUFU engine): one MUFU.SIN each   mufu_rec<KIND>()
-//   a4  fp32 register accumulation over tones: 4 blocks x 16 samples per thread (static pass), 16 (MUFU pass)
+//   a4  fp32 register accumulation over tones: 4 groups x 16 samples per thread (angle-addition passes), 16 (MUFU pass);
+//       tables above 256 tones: leaves of <= 64 (128) tones summed from zero, merged in int32 fixed point (exact), so that
+//       launches with few tiles spread a tile's tones over CTAs bit-identically          ipark_leaf(), tone_groups(), fix_grids()
 //   a5  quantise: round-half-even and saturate to int16 (fused multiply-add against 1.5*2^23)  pack8()
 //   a6  two 16-byte stores of 8 consecutive int16 per thread and block                       store_block()
 // No tensor cores (north_star), no per-tone wavetable in DRAM (the paper's limiter); output
@@ -881,10 +885,10 @@ __device__ __forceinline__ void slow_fma(const StageRec *rec, const SlowSC &v, P
     pq_add(pq[3], v.s23.y, v.c23.y, C03, C47, S03, S47);
 }
 
-// A work unit is one 2048-sample tile (4 blocks of 512) x the tones of one warp.  SPLIT warps (a team) share a
-// tile, each taking 1/SPLIT of the tones; their partial sums meet in shared memory and are added in rank order.
-// The grid is persistent (two CTAs per SM); teams walk the tiles of the launch with a stride of the team count,
-// team index = team_in_cta * gridDim.x + blockIdx.x, so a final partial round spreads over all SMs.
+// A work unit is one 2048-sample tile (LEAVES launches with few tiles: one quad of tone leaves of a tile).  SPLIT warps (a
+// team) share a tile, each taking 1/SPLIT of the tones; their partial sums meet in shared memory (the park areas).
+// The grid is persistent (three CTAs per SM); teams start on the unit of their own index, team index = team_in_cta *
+// gridDim.x + blockIdx.x, and then draw units from the launch's counter.
 // ROT: tones that are static over the whole tile take the angle-addition pass (FMA engine), everything else (and
 // every tone when !ROT) takes the MUFU pass.  Every sample goes through the same arithmetic for every launch
 // geometry because all phases are anchored to absolute tile positions.
