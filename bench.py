@@ -501,12 +501,16 @@ def run_extras(torch, awg, sm_max_mhz):
             cap[f"{tag}_{key}"] = realtime_capacity(awg, mk, False)
         cap[f"{tag}_static_d2h"] = realtime_capacity(awg, (lambda n, fs=fs, cl=cl, n_chunks=n_chunks:
                                                            W.capacity_toneset(n, fs, cl, "static", n_chunks=n_chunks)), True)
+    # short chunks (2^18 samples = 468 us at 560 MS/s: 128 tiles per launch, fewer than the grid has CTAs): the launches spread a
+    # tile's tone quads over CTAs
+    n18 = int(math.ceil(0.5 * 560e6 / (1 << 18)))
+    cap["560MS_static_L18_chunks"] = realtime_capacity(awg, (lambda n: W.capacity_toneset(n, 560e6, 1 << 18, "static", n_chunks=n18)), False)
     cap["560MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 560e6, 1 << 18)
     cap["100MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 100e6, 1 << 15)
     out["max_realtime_tones"] = cap
     out["max_realtime_tones_note"] = (
         "largest N streamed through the ring (3 slots) for >= 1 s of signal with the ring's underrun counter at zero; tone sets "
-        "drawn like C5 (2^20-sample chunks at 560 MS/s, 2^18 at 100 MS/s); 'all_slow_movers' = one +-5 MHz minimum-jerk move "
+        "drawn like C5 (2^20-sample chunks at 560 MS/s, 2^18 at 100 MS/s; '_L18_chunks': 2^18-sample chunks at 560 MS/s over 0.5 s); 'all_slow_movers' = one +-5 MHz minimum-jerk move "
         "spanning the probe (the slow pass); '_d2h' = pinned-host mirror on; 'all_fast_movers_device_time' = every tone "
         "inside a one-chunk minimum-jerk move all the time (2^18-sample chunks = 468 us at 560 MS/s, 2^15 = 328 us at "
         "100 MS/s), criterion: every chunk's synthesis within chunk_len/fs of device time")
