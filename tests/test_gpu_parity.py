@@ -370,6 +370,35 @@ def test_quads_across_ctas_match_quads_in_one_cta_bit_for_bit(awg, torch_cuda, e
     small.close()
 
 
+def test_leaf_merge_with_a_wide_amplitude_range(awg, torch_cuda, eng):
+    """The fixed-point merge of large tables rounds every leaf on a grid that follows the leaf's own sum of |A|: two strong
+    tones (one with a negative amplitude), a leaf of zero-amplitude tones and hundreds of tones seven orders of magnitude
+    weaker must come out within the usual bars, saturated samples included, for a large launch and for cross-CTA chunks."""
+    fs, L, N = 560e6, 1 << 17, 900
+    rng = np.random.default_rng(5)
+    f0 = rng.uniform(20e6, 250e6, N)
+    A = rng.uniform(-1.0, 1.0, N) * 10.0 ** rng.uniform(-7, -3, N)
+    A[3], A[700] = 0.75, -0.6          # the sum reaches +-1.35 > 32767/29490.3: some samples saturate
+    A[128:192] = 0.0                    # a whole leaf of silent tones
+    rows = []
+    for k in range(N):
+        if k % 4 == 0:
+            rows.append((f0[k], f0[k] + rng.uniform(-3e6, 3e6), A[k], rng.uniform(0, 6.28), rng.uniform(0, 150e-6), rng.uniform(20e-6, 80e-6), MINJERK))
+        else:
+            rows.append((f0[k], f0[k], A[k], rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
+    big, op = _single(awg, fs, 8 * L, rows, engine=eng)       # 512 tiles: leaves walked inside one CTA
+    small, _ = _single(awg, fs, L, rows, engine=eng)          # 64 tiles: quads spread over CTAs
+    ref, reff = _np(big.synthesize_chunk(0)), _np(big.synthesize_chunk_f32(0))
+    V = oracle.c_waveform(op, 0, L)
+    assert np.abs(op.quantise(V)).max() == 32767 or np.abs(op.quantise(V).astype(np.int32)).max() == 32768, "the case is meant to saturate"
+    assert_f32_close(reff[:L], V, "wide amplitude range")
+    assert_codes_close(ref[:L], op.quantise(V), "wide amplitude range")
+    assert np.array_equal(_np(small.synthesize_chunk(0)), ref[:L])
+    assert np.array_equal(_np(small.synthesize_chunk(5)), ref[5 * L:6 * L])
+    assert np.array_equal(_np(small.synthesize_chunk_f32(5)).view(np.uint32), reff[5 * L:6 * L].view(np.uint32))
+    big.close(); small.close()
+
+
 def test_plan_limit_65536_tones(awg, torch_cuda, eng):
     """The largest plan (include/awg.h: n_tones <= 65536): 16 quads, every warp walks 32 batches of 32 tones per quad; a
     third of the tones is inside a move in the synthesised chunk, so the moving-tone lists are rebuilt many times per block."""
