@@ -370,6 +370,35 @@ def test_quads_across_ctas_match_quads_in_one_cta_bit_for_bit(awg, torch_cuda, e
     small.close()
 
 
+@pytest.mark.parametrize("n_tones,chunk_len", [(257, 8000), (513, 33000), (777, 65544), (2049, 24008)])
+def test_cross_cta_launches_with_ragged_chunks(awg, torch_cuda, eng, n_tones, chunk_len):
+    """Cross-CTA launches whose chunks are not multiples of the 2048-sample tile (partial tiles at both edges: blocks
+    outside the launch are skipped by every quad and by the CTA that finishes the tile), tone counts just above a quad
+    boundary (an almost empty last quad): every chunk equals the same samples of one long launch bit for bit."""
+    fs = 560e6
+    rng = np.random.default_rng(n_tones + chunk_len)
+    f0 = rng.uniform(20e6, 250e6, n_tones)
+    rows = []
+    for k in range(n_tones):
+        if k % 3 == 0:
+            rows.append((f0[k], f0[k] + rng.uniform(-4e6, 4e6), 1.0 / n_tones, rng.uniform(0, 6.28), rng.uniform(0, 1.5e-3),
+                         rng.uniform(30e-6, 500e-6), MINJERK if k % 2 else LINEAR))
+        else:
+            rows.append((f0[k], f0[k], 1.0 / n_tones, rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
+    n_chunks = (1 << 20) // chunk_len
+    total = n_chunks * chunk_len
+    small, op = _single(awg, fs, chunk_len, rows, engine=eng)
+    ref = _np(small.synthesize_range(0, n_chunks))       # >= 444 tiles: one CTA per tile
+    for c in sorted(set([0, 1, n_chunks // 2, n_chunks - 1])):
+        assert np.array_equal(_np(small.synthesize_chunk(c)), ref[c * chunk_len:(c + 1) * chunk_len]), f"chunk {c}"
+    a = (n_chunks // 2) * chunk_len
+    V = oracle.c_waveform(op, a, a + chunk_len)
+    assert_codes_close(ref[a:a + chunk_len], op.quantise(V), f"ragged cross-CTA N={n_tones} L={chunk_len}")
+    assert_f32_close(_np(small.synthesize_chunk_f32(n_chunks // 2)), V, f"ragged cross-CTA f32 N={n_tones} L={chunk_len}")
+    assert total <= (1 << 20)
+    small.close()
+
+
 def test_leaf_merge_with_a_wide_amplitude_range(awg, torch_cuda, eng):
     """The fixed-point merge of large tables rounds every leaf on a grid that follows the leaf's own sum of |A|: two strong
     tones (one with a negative amplitude), a leaf of zero-amplitude tones and hundreds of tones seven orders of magnitude
