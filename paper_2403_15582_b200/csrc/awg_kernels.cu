@@ -1413,7 +1413,7 @@ __global__ void __launch_bounds__(128) awg_expand_kernel(ToneRec *table, const T
 // (different streams) never share a counter or scratch memory.
 constexpr int kSchedSlots = 1024;
 constexpr int kMaxDevices = 64;
-constexpr int kCrossTiles = 512;                         // launches with fewer tiles than the grid has CTAs (<= 3 x 148) may run cross-CTA
+constexpr int kCrossTiles = 1024;                        // launches of fewer tiles than two rounds of the grid's CTAs (< 2 x 3 x 148) run cross-CTA
 constexpr int kSlotWords = 8 + kCrossTiles;              // {next unit, teams finished, -...} + per-tile quad counters
 struct LaunchSlot {
     int32_t *scratch = nullptr;   // kCrossTiles tiles of int32 sums, zero between launches
@@ -1536,8 +1536,9 @@ cudaError_t launch_synth(const LaunchParams &lp_in, int engine, cudaStream_t str
         lp.cross = 0;
         lp.scratch = nullptr;
         int64_t units = tiles;
-        if (quads > 1 && tiles < static_cast<int64_t>(kCtasPerSm) * ds->n_sm && tiles <= kCrossTiles) {
-            // fewer tiles than CTAs: a tile's quads become separate work units, their sums meet in the slot's scratch tiles
+        if (quads > 1 && tiles < 2 * static_cast<int64_t>(kCtasPerSm) * ds->n_sm && tiles <= kCrossTiles) {
+            // fewer tiles than two rounds of CTAs (a second round that is mostly empty wastes up to half the GPU): a tile's quads
+            // become separate work units, their sums meet in the slot's scratch tiles
             LaunchSlot &sl = ds->slots[it->second];
             if (!sl.scratch) {
                 int32_t *sp = nullptr;

@@ -347,10 +347,10 @@ def test_amplitude_ramps_many_tones_bit_identical_chunkings(awg, torch_cuda, eng
 # ------------------------------------------------------------------ the NEXT rows on large tables (leaves, cross-CTA launches)
 def test_next_rows_on_a_large_table_cross_cta_and_one_cta_agree(awg, torch_cuda, eng):
     """700 tones (3 quads of leaves): amplitude ramps on a fifth of the tones, 600 on-grid static tones moved into the looped
-    static buffer, the rest evaluated per sample.  A 2^20-sample chunk (512 tiles: quads walked inside one CTA) and 2^15-sample
+    static buffer, the rest evaluated per sample.  A 2^21-sample chunk (1024 tiles: quads walked inside one CTA) and 2^15-sample
     launches of the same samples (16 tiles: quads spread over CTAs, int32 scratch tiles) must agree bit for bit, and match the
     oracle's static pathway."""
-    N, L, l = 700, 1 << 20, 1 << 15
+    N, L, l = 700, 1 << 21, 1 << 15
     rng = np.random.default_rng(77)
     f_grid = np.array([awg.awg_snap_frequency(float(f), FS, L) for f in rng.uniform(30e6, 250e6, N)])
     rows = []

@@ -335,8 +335,9 @@ def test_quads_across_ctas_match_quads_in_one_cta_bit_for_bit(awg, torch_cuda, e
     than the grid has CTAs spreads a tile's quads over CTAs (sums meet in scratch memory, last arriver adds them in quad
     order); a large launch walks the quads inside one CTA.  Same grouping, same order: the int16 codes and the fp32 sums
     must be identical bit for bit, and both must match the oracle.  Static tones, slow movers, fast movers, a few
-    amplitude ramps; 2^20 samples as one launch (512 tiles) against 2^15-sample chunks (16 tiles each)."""
-    fs, L = 560e6, 1 << 20
+    amplitude ramps; 2^21 samples as one launch (1024 tiles: more than two rounds of the grid's 444 CTAs, so every tile
+    stays in one CTA) against 2^15-sample chunks (16 tiles each)."""
+    fs, L = 560e6, 1 << 21
     rng = np.random.default_rng(1000 + n_tones)
     f0 = rng.uniform(20e6, 250e6, n_tones)
     kind = rng.integers(0, 4, n_tones)
@@ -348,10 +349,10 @@ def test_quads_across_ctas_match_quads_in_one_cta_bit_for_bit(awg, torch_cuda, e
             rows.append((f0[k], f0[k] + rng.uniform(-2e6, 2e6), 1.0 / n_tones, rng.uniform(0, 6.28), -1e-3, 30e-3, MINJERK))
         elif kind[k] == 2:    # fast mover inside the range
             rows.append((f0[k], f0[k] + rng.uniform(-4e6, 4e6), 1.0 / n_tones, rng.uniform(0, 6.28),
-                         rng.uniform(0, 1.2e-3), rng.uniform(50e-6, 400e-6), MINJERK))
+                         rng.uniform(0, 3.0e-3), rng.uniform(50e-6, 400e-6), MINJERK))
         else:
             rows.append((f0[k], f0[k] + rng.uniform(-1e6, 1e6), 1.0 / n_tones, rng.uniform(0, 6.28),
-                         rng.uniform(0, 1.0e-3), rng.uniform(100e-6, 600e-6), LINEAR))
+                         rng.uniform(0, 2.8e-3), rng.uniform(100e-6, 600e-6), LINEAR))
     big, op = _single(awg, fs, L, rows, engine=eng)
     small, _ = _single(awg, fs, 1 << 15, rows, engine=eng)
     ref = _np(big.synthesize_chunk(0))
@@ -385,17 +386,17 @@ def test_cross_cta_launches_with_ragged_chunks(awg, torch_cuda, eng, n_tones, ch
                          rng.uniform(30e-6, 500e-6), MINJERK if k % 2 else LINEAR))
         else:
             rows.append((f0[k], f0[k], 1.0 / n_tones, rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
-    n_chunks = (1 << 20) // chunk_len
+    n_chunks = (1 << 21) // chunk_len
     total = n_chunks * chunk_len
     small, op = _single(awg, fs, chunk_len, rows, engine=eng)
-    ref = _np(small.synthesize_range(0, n_chunks))       # >= 444 tiles: one CTA per tile
+    ref = _np(small.synthesize_range(0, n_chunks))       # >= 888 tiles (two rounds of CTAs): one CTA per tile
     for c in sorted(set([0, 1, n_chunks // 2, n_chunks - 1])):
         assert np.array_equal(_np(small.synthesize_chunk(c)), ref[c * chunk_len:(c + 1) * chunk_len]), f"chunk {c}"
     a = (n_chunks // 2) * chunk_len
     V = oracle.c_waveform(op, a, a + chunk_len)
     assert_codes_close(ref[a:a + chunk_len], op.quantise(V), f"ragged cross-CTA N={n_tones} L={chunk_len}")
     assert_f32_close(_np(small.synthesize_chunk_f32(n_chunks // 2)), V, f"ragged cross-CTA f32 N={n_tones} L={chunk_len}")
-    assert total <= (1 << 20)
+    assert total <= (1 << 21)
     small.close()
 
 
@@ -415,7 +416,7 @@ def test_leaf_merge_with_a_wide_amplitude_range(awg, torch_cuda, eng):
             rows.append((f0[k], f0[k] + rng.uniform(-3e6, 3e6), A[k], rng.uniform(0, 6.28), rng.uniform(0, 150e-6), rng.uniform(20e-6, 80e-6), MINJERK))
         else:
             rows.append((f0[k], f0[k], A[k], rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
-    big, op = _single(awg, fs, 8 * L, rows, engine=eng)       # 512 tiles: leaves walked inside one CTA
+    big, op = _single(awg, fs, 16 * L, rows, engine=eng)      # 1024 tiles: leaves walked inside one CTA
     small, _ = _single(awg, fs, L, rows, engine=eng)          # 64 tiles: quads spread over CTAs
     ref, reff = _np(big.synthesize_chunk(0)), _np(big.synthesize_chunk_f32(0))
     V = oracle.c_waveform(op, 0, L)
