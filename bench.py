@@ -619,6 +619,12 @@ def run_ours(args):
     })
     if clocks.get("sm_mhz"):
         roofline["frac_at_achieved_clock"] = pipe_roofline(counts, ms_local, args.engine, clocks["sm_mhz"])["frac"]
+    if args.engine != "mufu" and counts[1] > 0:
+        # continuity with round 1, whose slow pass needed (and whose bench counted) 2 multiply-adds per slow tone-sample
+        n_sta, n_slow, n_fast = (int(x) for x in counts)
+        roofline["frac_if_slow_tone_samples_counted_as_2_fma"] = (
+            (n_sta + 2 * n_slow + 2 * n_fast) / (FMA_PER_CLK_PER_SM * N_SM * sm_max_mhz * 1e6) / (ms_local * 1e-3))
+        roofline["slow_fma_per_tone_sample"] = SLOW_FMA_PER_TONE_SAMPLE
 
     # ---- oracle on this box's host cores (bounded sample) ----------------------------------------
     n_cpu = max(1 << 16, min(1 << 22, (1 << 32) // w.n_tones // 4096 * 4096))   # ~4e9 tone-samples: ~10 s on 16 cores
