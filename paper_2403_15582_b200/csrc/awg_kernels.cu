@@ -38,9 +38,11 @@ void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 int split_for(int n_tones)
 {
-    // >= 12 tones per warp, at most one CTA (4 warps) per tile
+    // >= 5 tones per warp, at most one CTA (4 warps) per tile: a tile's latency is one warp's walk over its tones and over the
+    // blocks it owns in the MUFU pass, and launches of a few dozen tones are bound by it (20 tones x 2^18 samples: 16.7 us with
+    // one warp per tile, 8.5 us with four; 2^22 samples: 19.0 -> 20.7 us)
     int split = 1;
-    while (split < 4 && n_tones / (split * 2) >= 12) split *= 2;
+    while (split < 4 && n_tones / (split * 2) >= 5) split *= 2;
     return split;
 }
 
