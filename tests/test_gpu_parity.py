@@ -717,3 +717,46 @@ def test_concurrent_launches_on_two_streams(awg, torch_cuda):
     assert all(np.array_equal(_np(o), ref1) for o in outs1)
     assert all(np.array_equal(_np(o), ref2) for o in outs2)
     p1.close(); p2.close()
+
+
+# ------------------------------------------------------------------ seeded random soak
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_random_soak_against_the_oracle(awg, torch_cuda, seed):
+    """Forty random plans per seed: tone counts around every grouping boundary (team split at 10 / 20 tones, leaves above 256,
+    quad boundaries, 128-tone leaves above 2048), ragged and tiny chunk lengths, signed amplitudes, a random mix of static
+    tones, slow movers (both slow classes), fast movers, instant retunes; both engines.  A random window of every case is
+    compared with the oracle at the usual bars (fp32 bar scaled by max(1, sum |A|)), and the range launch over all chunks must
+    equal the chunk launches bit for bit (they can take the one-CTA and the cross-CTA path)."""
+    fs = 560e6
+    for case in range(40):
+        rng = np.random.default_rng(10_000 * seed + case)
+        n = int(rng.choice([1, 3, 9, 10, 19, 20, 33, 100, 129, 256, 257, 300, 511, 512, 513, 700, 1025, 2048, 2049, 3000]))
+        cl = int(rng.choice([8, 264, 2048, 4096, 8000, 32768, 65536, 100000, 1 << 18]))
+        span = max(cl * 6, 40000) / fs
+        rows = []
+        for k in range(n):
+            f0, A, ph = rng.uniform(5e6, 270e6), rng.uniform(-1, 1) / n, rng.uniform(0, 6.28)
+            kind = rng.integers(0, 5)
+            if kind == 0:
+                rows.append((f0, f0, A, ph, 0.0, 0.0, STATIC))
+            elif kind == 1:
+                rows.append((f0, f0 + rng.uniform(-3e6, 3e6), A, ph, rng.uniform(-span, 0), rng.uniform(5e-3, 40e-3), MINJERK if k % 2 else LINEAR))
+            elif kind == 2:
+                rows.append((f0, f0 + rng.uniform(-5e6, 5e6), A, ph, rng.uniform(0, span), rng.uniform(1e-6, span), MINJERK if k % 2 else LINEAR))
+            elif kind == 3:
+                rows.append((f0, f0 + rng.uniform(-5e6, 5e6), A, ph, rng.uniform(0, span), float(rng.choice([0.0, 3e-8, 1e-6])), MINJERK))
+            else:
+                rows.append((f0, f0 + rng.uniform(-2e6, 2e6), A, ph, rng.uniform(-span, 0), rng.uniform(1e-3, 4e-3), LINEAR if k % 2 else MINJERK))
+        p, op = _single(awg, fs, cl, rows, engine=[awg.AWG_ENGINE_FMA, awg.AWG_ENGINE_MUFU][case % 2])
+        n_chunks = 6
+        got = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(n_chunks)])
+        gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(n_chunks)])
+        assert np.array_equal(_np(p.synthesize_range(0, n_chunks)), got), f"seed {seed} case {case}: range launch differs from chunk launches"
+        tot = n_chunks * cl
+        wlen = min(tot, max(2048, int(2e7 // n) // 8 * 8))
+        a = int(rng.integers(0, tot - wlen + 1)) // 8 * 8
+        V = oracle.c_waveform(op, a, a + wlen)
+        sa = sum(abs(r[2]) for r in rows)
+        assert_codes_close(got[a:a + wlen], op.quantise(V), f"soak seed {seed} case {case} (N={n}, L={cl})")
+        assert_f32_close(gotf[a:a + wlen], V, f"soak seed {seed} case {case} (N={n}, L={cl})", tol=1e-5 * max(1.0, sa))
+        p.close()
