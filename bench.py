@@ -508,6 +508,28 @@ def run_extras(torch, awg, sm_max_mhz):
     cap["560MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 560e6, 1 << 18)
     cap["100MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 100e6, 1 << 15)
     out["max_realtime_tones"] = cap
+    # fraction of the binding roofline AT each capacity: roofline time of one chunk of the N_max-tone set / the chunk's deadline
+    def cap_frac(n, make, fs, cl, chunk=1):
+        if not n:
+            return None
+        pl = awg.Plan.from_workload(make(n))
+        r = pipe_roofline(pl.op_counts(chunk, 1), cl / fs * 1e3, "auto", sm_max_mhz)
+        pl.close()
+        return {"roofline_frac": round(r["frac"], 4), "pipe": r["pipe"].split()[0]}
+
+    capf = {}
+    for fs, cl, tag in ((560e6, 1 << 20, "560MS"), (100e6, 1 << 18, "100MS")):
+        n_chunks = int(math.ceil(1.0 * fs / cl))   # the same tone sets as in the search (the slow movers' move spans the probe)
+        for mix, key in (("static", "static"), ("half", "half_static_half_fast"), ("moving", "all_slow_movers"), ("static", "static_d2h")):
+            capf[f"{tag}_{key}"] = cap_frac(cap[f"{tag}_{key}"], (lambda n, fs=fs, cl=cl, mix=mix, n_chunks=n_chunks:
+                                                                  W.capacity_toneset(n, fs, cl, mix, n_chunks=n_chunks)), fs, cl, chunk=n_chunks // 2)
+    capf["560MS_static_L18_chunks"] = cap_frac(cap["560MS_static_L18_chunks"], (lambda n: W.capacity_toneset(n, 560e6, 1 << 18, "static", n_chunks=4)), 560e6, 1 << 18)
+    for fs, cl, key in ((560e6, 1 << 18, "560MS_all_fast_movers_device_time"), (100e6, 1 << 15, "100MS_all_fast_movers_device_time")):
+        n = cap[key]
+        if n:   # every tone-sample of such a set is inside a move: one sine each
+            r = pipe_roofline((0, 0, n * cl), cl / fs * 1e3, "auto", sm_max_mhz)
+            capf[key] = {"roofline_frac": round(r["frac"], 4), "pipe": r["pipe"].split()[0]}
+    out["max_realtime_tones_roofline"] = capf
     out["max_realtime_tones_note"] = (
         "largest N streamed through the ring (3 slots) for >= 1 s of signal with the ring's underrun counter at zero; tone sets "
         "drawn like C5 (2^20-sample chunks at 560 MS/s, 2^18 at 100 MS/s; '_L18_chunks': 2^18-sample chunks at 560 MS/s over 0.5 s); 'all_slow_movers' = one +-5 MHz minimum-jerk move "
