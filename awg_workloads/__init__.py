@@ -16,6 +16,7 @@ from .configs import (  # noqa: F401
     PROFILE_STATIC,
     PROFILE_LINEAR,
     PROFILE_MINJERK,
+    PROFILE_EXP,
     DEFAULT_SCALE,
     Update,
     Workload,

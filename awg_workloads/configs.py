@@ -18,6 +18,7 @@ import numpy as np
 PROFILE_STATIC = 0
 PROFILE_LINEAR = 1
 PROFILE_MINJERK = 2
+PROFILE_EXP = 3      # exponential chirp f(t) = f0 (f1/f0)^(tau/T), named at PAPER.md:137
 
 #: int16 full-scale factor named by BASELINE.json config 1 ("int16 scale 0.9*32767").
 DEFAULT_SCALE = 0.9 * 32767.0

@@ -8,6 +8,7 @@ from .awg_oracle import (  # noqa: F401
     PROFILE_STATIC,
     PROFILE_LINEAR,
     PROFILE_MINJERK,
+    PROFILE_EXP,
     OraclePlan,
     Segment,
     plan_from_workload,

@@ -31,6 +31,9 @@ What it computes (paper citations are PAPER.md:<line>):
 * Per-chunk updates (streaming pathway, Fig. 7): at the first sample of chunk c a
   tone starts a new move from its current instantaneous frequency and phase (reading G12).
 
+* Exponential chirp (PAPER.md:137 names "linear, exponential" frequency chirps and prints no formula; DESIGN.md
+  reading G20): f(tau) = f0 (f1/f0)^(tau/T), phase = its integral, f0 T ((f1/f0)^s - 1)/ln(f1/f0) cycles since the
+  start of the move; f0 and f1 of the same sign.  Pinned in tests/test_oracle_pins_next.py.
 * Four-channel multiplexed output (the paper's WM kernel, Fig. 4): the codes of the
   channels' independent tone sets interleaved "in groups of four", ``out[4 i + c] = code_c[i]``
   (``mux_channels``).
@@ -61,6 +64,7 @@ LD = np.longdouble
 PROFILE_STATIC = 0
 PROFILE_LINEAR = 1
 PROFILE_MINJERK = 2
+PROFILE_EXP = 3
 
 TWO_PI_LD = LD(2) * np.arccos(LD(-1))
 TWO_PI = 2.0 * np.pi
@@ -95,6 +99,24 @@ def segment_phase(seg: Segment, t):
     if seg.profile == PROFILE_STATIC:
         return static
     D = seg.f1 - seg.f0
+    if seg.profile == PROFILE_EXP:
+        # Exponential chirp (named, without a formula, at PAPER.md:137; reading G20): the frequency runs
+        # geometrically, f(tau) = f0 r^(tau/T) with r = f1/f0 > 0, so the phase gained since the start of the move is
+        # the integral f0 T (r^s - 1)/ln r, and T (f1 - f0)/ln r over the whole move.
+        if D == 0 or not seg.T > 0:
+            r_gain_total = seg.f0 * seg.T
+        else:
+            Lr = np.log(seg.f1 / seg.f0)
+            r_gain_total = seg.T * D / Lr
+        after = seg.theta + seg.f0 * seg.t_s + r_gain_total + seg.f1 * (tau - seg.T)
+        if seg.T > 0 and D != 0:
+            s = np.clip(tau / seg.T, LD(0), LD(1))
+            during = seg.theta + seg.f0 * seg.t_s + seg.f0 * seg.T * np.expm1(Lr * s) / Lr
+        elif seg.T > 0:
+            during = static
+        else:
+            during = after
+        return np.where(tau <= 0, static, np.where(tau >= seg.T, after, during))
     after = seg.theta + seg.f0 * seg.t_s + seg.f1 * tau + seg.T * (seg.f0 - seg.f1) / LD(2)  # Eq. 10 branch 2
     if seg.T > 0:
         s = tau / seg.T
@@ -114,13 +136,20 @@ def segment_phase(seg: Segment, t):
 
 def segment_freq(seg: Segment, t):
     """Instantaneous frequency (Hz) of one segment: STATIC f0; LINEAR f0 + D s;
-    MINJERK f0 + D (10 s^3 - 15 s^4 + 6 s^5); after the move f1."""
+    MINJERK f0 + D (10 s^3 - 15 s^4 + 6 s^5); EXP f0 (f1/f0)^s; after the move f1."""
     t = np.asarray(t, dtype=LD)
     tau = t - seg.t_s
     f0 = np.full_like(t, seg.f0)
     if seg.profile == PROFILE_STATIC:
         return f0
     D = seg.f1 - seg.f0
+    if seg.profile == PROFILE_EXP:
+        if seg.T > 0 and D != 0:
+            s = np.clip(tau / seg.T, LD(0), LD(1))
+            during = seg.f0 * np.exp(np.log(seg.f1 / seg.f0) * s)
+        else:
+            during = np.full_like(t, seg.f1 if not seg.T > 0 else seg.f0)
+        return np.where(tau <= 0, f0, np.where(tau >= seg.T, np.full_like(t, seg.f1), during))
     if seg.T > 0:
         s = tau / seg.T
         if seg.profile == PROFILE_LINEAR:

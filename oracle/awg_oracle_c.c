@@ -35,6 +35,7 @@
 #define AWG_STATIC 0
 #define AWG_LINEAR 1
 #define AWG_MINJERK 2
+#define AWG_EXP 3   /* exponential chirp f0 (f1/f0)^(tau/T), named at PAPER.md:137 (reading G20) */
 
 static long double seg_phase(long double t, long double t_s, long double T, long double f0,
                              long double f1, long double theta, int profile)
@@ -42,6 +43,16 @@ static long double seg_phase(long double t, long double t_s, long double T, long
     long double tau = t - t_s;
     if (profile == AWG_STATIC || tau <= 0.0L)
         return theta + f0 * t;
+    if (profile == AWG_EXP) {
+        /* phase gained since the start of the move: f0 T (r^s - 1)/ln r, r = f1/f0; T (f1 - f0)/ln r over the whole move */
+        if (f1 == f0 || !(T > 0.0L)) {
+            if (tau >= T) return theta + f0 * t_s + f0 * T + f1 * (tau - T);
+            return theta + f0 * t;
+        }
+        long double Lr = logl(f1 / f0);
+        if (tau >= T) return theta + f0 * t_s + T * (f1 - f0) / Lr + f1 * (tau - T);
+        return theta + f0 * t_s + f0 * T * expm1l(Lr * (tau / T)) / Lr;
+    }
     if (tau >= T)
         return theta + f0 * t_s + f1 * tau + T * (f0 - f1) / 2.0L;
     long double s = tau / T;

@@ -5,6 +5,7 @@ oracle's own formula retyped."""
 import math
 
 import mpmath
+import mpmath as mp
 import numpy as np
 import pytest
 
@@ -215,3 +216,86 @@ def test_zero_duration_amplitude_step_and_static_profile():
     assert np.allclose(V[:100], 0.2) and np.allclose(V[100:], 0.6)
     p.set_amplitude_ramps([0.6], [0.0], [1e-6], [STATIC])   # STATIC profile: amplitude stays
     assert np.allclose(p.waveform(0, L), 0.2)
+
+
+# ------------------------------------------------------------------ exponential chirp (PAPER.md:137 names it; reading G20)
+def _exp_plan(f0=80e6, f1=120e6, T=200e-6, t_s=10e-6, phi0=0.7, fs=560e6, L=1 << 18):
+    op = oracle.OraclePlan(1, fs, L)
+    op.set_trajectories([f0], [f1], [1.0], [phi0], [t_s], [T], [oracle.awg_oracle.PROFILE_EXP])
+    return op
+
+
+def test_exp_chirp_frequency_is_geometric_and_hits_both_ends():
+    """f(tau) = f0 (f1/f0)^(tau/T): f0 at the start, f1 at the end, the GEOMETRIC mean half way, log f linear in time --
+    read off the oracle's own phase by central differences (the phase is what the oracle computes; the frequency law is the pin)."""
+    f0, f1, T, t_s, fs = 80e6, 120e6, 200e-6, 10e-6, 560e6
+    op = _exp_plan(f0, f1, T, t_s)
+    def freq_at(tau):
+        n = (t_s + tau) * fs
+        ns = np.array([n - 0.5, n + 0.5])
+        ph = oracle.awg_oracle.segment_phase(op.segments[0][0], ns.astype(np.longdouble) / np.longdouble(fs))
+        return float((ph[1] - ph[0]) * fs)
+    assert abs(freq_at(2e-9) - f0) < 2e3
+    assert abs(freq_at(T - 2e-9) - f1) < 2e3
+    assert abs(freq_at(T / 2) - math.sqrt(f0 * f1)) < 1.0          # 97.98 MHz, not the arithmetic 100 MHz
+    lf = [math.log(freq_at(T * s)) for s in (0.2, 0.4, 0.6, 0.8)]
+    assert abs((lf[2] - lf[1]) - (lf[1] - lf[0])) < 1e-7 and abs((lf[3] - lf[2]) - (lf[2] - lf[1])) < 1e-7
+    # before the move the tone is static at f0, after it static at f1
+    assert abs(freq_at(-3e-6) - f0) < 1e-3 and abs(freq_at(T + 3e-6) - f1) < 1e-3
+    assert abs(float(op.inst_freq(0, np.array([int((t_s + T / 2) * fs)]))[0]) - f0 * (f1 / f0) ** ((int((t_s + T / 2) * fs) / fs - t_s) / T)) < 1e-3
+
+
+def test_exp_chirp_phase_is_the_integral_of_the_geometric_frequency():
+    """Closed form in 50-digit arithmetic: cycles gained over the whole move = T (f1 - f0)/ln(f1/f0) (the logarithmic mean of
+    the end frequencies times T); and a brute-force trapezoid integration of f0 r^(t/T) on 10^6 points for a point mid-move."""
+    mp.mp.dps = 50
+    f0, f1, T, t_s, fs, phi0 = 80e6, 120e6, 200e-6, 10e-6, 560e6, 0.7
+    op = _exp_plan(f0, f1, T, t_s, phi0)
+    seg = op.segments[0][0]
+    LD = np.longdouble
+    t_end = LD(t_s) + LD(T)
+    ph_end = oracle.awg_oracle.segment_phase(seg, np.array([t_end], dtype=LD))[0]
+    want = mp.mpf(phi0) / (2 * mp.pi) + mp.mpf(f0) * mp.mpf(t_s) + mp.mpf(T) * (mp.mpf(f1) - mp.mpf(f0)) / mp.log(mp.mpf(f1) / mp.mpf(f0))
+    assert abs(mp.mpf(float(ph_end)) - want) < mp.mpf("1e-8")
+    # continuity at the end of the move and slope f1 afterwards
+    ph_after = oracle.awg_oracle.segment_phase(seg, np.array([t_end + LD(1e-6)], dtype=LD))[0]
+    assert abs(float(ph_after - ph_end) - f1 * 1e-6) < 1e-9
+    # trapezoid integration of the frequency law up to tau = 0.37 T
+    tau = 0.37 * T
+    grid = np.linspace(0.0, tau, 1_000_001)
+    f = f0 * (f1 / f0) ** (grid / T)
+    integral = float(np.sum((f[1:] + f[:-1]) * 0.5) * (grid[1] - grid[0]))
+    ph_mid = oracle.awg_oracle.segment_phase(seg, np.array([LD(t_s) + LD(tau)], dtype=LD))[0]
+    assert abs(float(ph_mid) - (phi0 / (2 * math.pi) + f0 * t_s + integral)) < 1e-7
+    # it is not the linear chirp between the same ends: the two differ by many cycles mid-move
+    lin = oracle.OraclePlan(1, fs, 1 << 18)
+    lin.set_trajectories([f0], [f1], [1.0], [phi0], [t_s], [T], [oracle.awg_oracle.PROFILE_LINEAR])
+    ph_lin = oracle.awg_oracle.segment_phase(lin.segments[0][0], np.array([LD(t_s) + LD(T / 2)], dtype=LD))[0]
+    ph_exp = oracle.awg_oracle.segment_phase(seg, np.array([LD(t_s) + LD(T / 2)], dtype=LD))[0]
+    assert abs(float(ph_lin - ph_exp)) > 50.0
+
+
+def test_exp_chirp_limits_updates_and_c_evaluator():
+    """f1 -> f0: the exponential chirp tends to the static tone; a downward chirp mirrors an upward one; an update mid-move
+    continues phase and frequency; the C evaluator agrees with numpy."""
+    fs, L = 560e6, 1 << 16
+    near = _exp_plan(90e6, 90e6 * (1 + 1e-13), 100e-6, 0.0, 0.3, fs, L)
+    sta = oracle.OraclePlan(1, fs, L)
+    sta.set_trajectories([90e6], [90e6], [1.0], [0.3], [0.0], [0.0], [oracle.awg_oracle.PROFILE_STATIC])
+    assert np.abs(near.waveform(0, 4096) - sta.waveform(0, 4096)).max() < 1e-6
+    down = _exp_plan(120e6, 80e6, 150e-6, 5e-6, 0.1, fs, L)
+    n_mid = int((5e-6 + 75e-6) * fs)
+    assert abs(float(down.inst_freq(0, np.array([n_mid]))[0]) - 120e6 * (80e6 / 120e6) ** ((n_mid / fs - 5e-6) / 150e-6)) < 1e-3
+    # mid-move update: phase- and frequency-continuous (G12)
+    op = _exp_plan(80e6, 120e6, 400e-6, 0.0, 0.2, fs, L)
+    n_u = 1 * L
+    f_before = float(op.inst_freq(0, np.array([n_u]))[0])
+    ph_before = op.phase(0, np.array([n_u]))[0]
+    op.update_trajectories(1, [0], [70e6], [100e-6], [oracle.awg_oracle.PROFILE_EXP])
+    assert abs(float(op.inst_freq(0, np.array([n_u]))[0]) - f_before) < 1e-3
+    d = float(op.phase(0, np.array([n_u]))[0] - ph_before)
+    assert abs(d - round(d)) < 1e-9
+    # numpy vs C on a window that covers the update and the end of the new move
+    V_np = op.waveform(n_u - 64, n_u + 60000)
+    V_c = oracle.c_waveform(op, n_u - 64, n_u + 60000)
+    assert np.abs(V_np - V_c).max() < 1e-12
