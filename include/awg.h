@@ -57,7 +57,9 @@ enum {
 enum {
     AWG_PROFILE_STATIC = 0,  /* f(t) = f0                                                   */
     AWG_PROFILE_LINEAR = 1,  /* f0 -> f1 linearly over [t_start, t_start + t_dur]            */
-    AWG_PROFILE_MINJERK = 2  /* f0 -> f1 along the minimum-jerk quintic 10s^3 - 15s^4 + 6s^5 */
+    AWG_PROFILE_MINJERK = 2, /* f0 -> f1 along the minimum-jerk quintic 10s^3 - 15s^4 + 6s^5 */
+    AWG_PROFILE_EXP = 3      /* exponential chirp f(tau) = f0 (f1/f0)^(tau/t_dur) (named at PAPER.md:137; G20):
+                                f0 and f1 must be > 0.  Evaluated in fp64 per sample inside the move (exact path)   */
 };
 
 /* sine engine of the synthesis kernel (step a3 of the hot path) */
@@ -97,13 +99,13 @@ awg_status awg_set_engine(awg_plan *p, int32_t engine);
  *   profile  AWG_PROFILE_* (STATIC ignores f1, t_start, t_dur)
  * Frequencies above Nyquist or negative are evaluated as given (they alias), sum(A) > 1 saturates.
  * Resets the update history.  Errors: INVALID_ARG (NULL, non-finite value, t_dur < 0, unknown
- * profile). */
+ * profile, AWG_PROFILE_EXP with f0 <= 0 or f1 <= 0). */
 awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1, const double *A,
                                 const double *phi0, const double *t_start, const double *t_dur,
                                 const int32_t *profile);
 
 /* Time-varying amplitudes a_j[i] of Eq. 9 (constant in the paper's worked case,
- * PAPER.md:137; reading G19): tone k goes from the amplitude given to awg_set_trajectories to
+ * PAPER.md:137; reading G7): tone k goes from the amplitude given to awg_set_trajectories to
  * A1[k] over [t_start[k], t_start[k] + t_dur[k]] along profile[k] -- AWG_PROFILE_STATIC (no ramp: A1,
  * t_start, t_dur ignored), AWG_PROFILE_LINEAR, or AWG_PROFILE_MINJERK (10 s^3 - 15 s^4 + 6 s^5): tone
  * creation (0 -> A1) and removal (A -> 0) without a click.  Four host arrays of length n_tones.  Replaces

@@ -44,7 +44,7 @@ What it computes (paper citations are PAPER.md:<line>):
   final frequency with the phase offset theta' (``handback_theta``, ``fold_into_static_buffer``).
 * Time-varying amplitude ``a_j[i]`` (Eq. 9; constant in the paper's worked case):
   per tone ``a(t) = A0`` before ``t_a``, ``A0 + (A1 - A0) h((t - t_a)/T_a)`` during the ramp and ``A1`` after,
-  with ``h(s) = s`` (LINEAR) or the minimum-jerk ramp ``10 s^3 - 15 s^4 + 6 s^5`` (MINJERK) -- reading G19 in
+  with ``h(s) = s`` (LINEAR) or the minimum-jerk ramp ``10 s^3 - 15 s^4 + 6 s^5`` (MINJERK) -- reading G7 in
   DESIGN.md: the paper allows ``a_j[i]`` without giving a profile; the frequency ramp's profile is reused
   (``set_amplitude_ramps``).
 
@@ -201,7 +201,7 @@ class OraclePlan:
     def set_amplitude_ramps(self, A1, t_start, t_dur, profile) -> None:
         """Time-varying amplitude a_j[i] of Eq. 9: tone k goes from the amplitude given to
         ``set_trajectories`` to ``A1[k]`` over ``[t_start[k], t_start[k] + t_dur[k]]`` along ``profile[k]``
-        (STATIC = constant amplitude, LINEAR, or MINJERK = 10 s^3 - 15 s^4 + 6 s^5; reading G19)."""
+        (STATIC = constant amplitude, LINEAR, or MINJERK = 10 s^3 - 15 s^4 + 6 s^5; reading G7)."""
         N = self.n_tones
         A1, ts, T = (np.asarray(a, dtype=np.float64) for a in (A1, t_start, t_dur))
         prof = np.asarray(profile, dtype=np.int64)

@@ -16,7 +16,7 @@
  *                                                                          prefactor corrected to T (G1)
  *   tau >= T           :  Phi = theta + f0 t_s + f1 tau + T (f0 - f1)/2    Eq. 10 branch 2
  *   V[n] = sum_k a_k[n] sin(2 pi frac(Phi_k[n]))                           Eq. 9, Eq. 14
- *   a_k[n] = A_k, or with an amplitude ramp (awg_oracle_waveform_amp; Eq. 9 allows a_j[i], reading G19 in DESIGN.md):
+ *   a_k[n] = A_k, or with an amplitude ramp (awg_oracle_waveform_amp; Eq. 9 allows a_j[i], reading G7 in DESIGN.md):
  *            A_k before t_a, A_k + (A1_k - A_k) h((t - t_a)/T_a) during it, A1_k after; h(s) = s or 10 s^3 - 15 s^4 + 6 s^5
  *   code = clamp(rint(scale V), -32768, 32767)                             PAPER.md:77, 196; G9
  *

@@ -26,6 +26,7 @@ AWG_ERR_UNDERRUN = -5
 AWG_PROFILE_STATIC = 0
 AWG_PROFILE_LINEAR = 1
 AWG_PROFILE_MINJERK = 2
+AWG_PROFILE_EXP = 3
 
 AWG_ENGINE_AUTO = 0
 AWG_ENGINE_MUFU = 1

@@ -67,6 +67,7 @@ struct __align__(16) ToneCore {
     double DT;             // (f1-f0)*t_dur, cycles
     double q1;             // DT/Tn = (f1-f0)/fs, cycles per sample
     float q[5];            // q[k-2] = 2*pi*DT/Tn^k/k!, k = 2..6: radians per sample^k for unit g^(k)
+                           // (AWG_PROFILE_EXP: q[0..3] hold f0*T in cycles and ln(f1/f0) as two doubles)
     // ---- amplitude ramp a_j[i] of Eq. 9: A before amp_ns, A + (A1 - A) h((n - amp_ns)/amp_Tn) during,
     // A1 after; h(s) = s or 10 s^3 - 15 s^4 + 6 s^5 (amp_prof).  A1 = A and amp_prof = STATIC without a ramp.
     float A1;

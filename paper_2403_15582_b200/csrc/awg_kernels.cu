@@ -165,7 +165,17 @@ __device__ __forceinline__ uint64_t exact_phase(const ToneCore &r, int64_t n)
     const double u = (static_cast<double>(n) - r.ns_int) - r.ns_frac;
     if (u <= 0.0) return r.theta_pre + r.w_pre * static_cast<uint64_t>(n);
     if (u >= r.Tn) return r.theta_post + r.w_post * static_cast<uint64_t>(n);
-    const double x = r.DT * profile_g((r.cls >> 8) & 0xff, u * r.inv_Tn);
+    const int profile = (r.cls >> 8) & 0xff;
+    double x;
+    if (profile == AWG_PROFILE_EXP) {
+        // exponential chirp (G20): cycles gained over the carrier = f0 T (expm1(L s)/L - s), L = ln(f1/f0);
+        // q[0..3] hold f0 T and L as two doubles
+        const double F = *reinterpret_cast<const double *>(&r.q[0]), L = *reinterpret_cast<const double *>(&r.q[2]);
+        const double s = u * r.inv_Tn;
+        x = F * (expm1(L * s) / L - s);
+    } else {
+        x = r.DT * profile_g(profile, u * r.inv_Tn);
+    }
     return r.theta_pre + r.w_pre * static_cast<uint64_t>(n) + frac_to_fix64(x);
 }
 

@@ -162,6 +162,15 @@ void make_move(HostTone &h, long double fs, long double f1, int profile, long do
     // after the move: Phi = theta + f0 t_s + f1 (t - t_s) + T (f0 - f1)/2   (Eq. 10 branch 2)
     //                     = [theta - (f1-f0) t_s - DT/2] + (f1/fs) n
     h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(h.DT / 2.0L);
+    h.expL = 0.0L;
+    if (profile == AWG_PROFILE_EXP) {
+        // Exponential chirp (G20): f = f0 r^s, r = f1/f0; cycles over the whole move = DT / ln r, so after it
+        //   Phi = [theta - (f1-f0) t_s - (f1 T - DT/ln r)] + (f1/fs) n.   Inside the move every sample takes the fp64 path.
+        h.expL = log1pl(D / h.f0);
+        h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(f1 * T - h.DT / h.expL);
+        h.cls = CLS_EXACT;
+        return;
+    }
     h.cls = classify(profile, h.DT, h.Tn);
     if (h.cls != CLS_EXACT) {
         const int slow = is_slow_mover(profile, h.DT, h.Tn);
@@ -216,6 +225,13 @@ static void fill_core(const HostTone &h, ToneCore &r)
             q *= rT;
             fact *= k;
             r.q[k - 2] = static_cast<float>(q / fact);
+        }
+        if (h.profile == AWG_PROFILE_EXP) {
+            // exponential chirp: no Taylor scales (every sample of the move takes the fp64 path); q[0..3] carry f0 T (cycles)
+            // and ln(f1/f0) as two doubles instead
+            const double F = static_cast<double>(h.f0 * h.T), Lr = static_cast<double>(h.expL);
+            std::memcpy(&r.q[0], &F, sizeof F);
+            std::memcpy(&r.q[2], &Lr, sizeof Lr);
         }
     }
 }
@@ -378,8 +394,10 @@ awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int
         if (p->in_buffer[k]) return fail(AWG_ERR_STATE, "tone %d is served by the static buffer (clear it with awg_static_buffer_set first)", k);
         if (!std::isfinite(f1[i]) || !std::isfinite(t_dur[i]) || t_dur[i] < 0.0)
             return fail(AWG_ERR_INVALID_ARG, "non-finite value or negative duration in update %d", i);
-        if (profile[i] < AWG_PROFILE_STATIC || profile[i] > AWG_PROFILE_MINJERK)
+        if (profile[i] < AWG_PROFILE_STATIC || profile[i] > AWG_PROFILE_EXP)
             return fail(AWG_ERR_INVALID_ARG, "unknown profile %d", profile[i]);
+        if (profile[i] == AWG_PROFILE_EXP && !(f1[i] > 0.0 && p->tones[k].f0 > 0.0L && p->tones[k].f1 > 0.0L))
+            return fail(AWG_ERR_INVALID_ARG, "exponential chirp of tone %d needs positive frequencies", k);
     }
     const long double fs = p->fs;
     const int64_t n_u = chunk_idx * p->chunk_len;
@@ -402,8 +420,10 @@ awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int
             } else {
                 // mid-move (G12): continue from the instantaneous frequency and phase
                 const long double s = u / h.Tn;
-                const long double f_now = h.f0 + (h.f1 - h.f0) * profile_h(h.profile, s);
-                const uint64_t ph = h.theta_pre + h.w_pre * static_cast<uint64_t>(n_u) + frac64(h.DT * profile_g(h.profile, s));
+                const bool ex = h.profile == AWG_PROFILE_EXP;
+                const long double f_now = ex ? h.f0 * expl(h.expL * s) : h.f0 + (h.f1 - h.f0) * profile_h(h.profile, s);
+                const long double gain = ex ? h.f0 * h.T * (expm1l(h.expL * s) / h.expL - s) : h.DT * profile_g(h.profile, s);
+                const uint64_t ph = h.theta_pre + h.w_pre * static_cast<uint64_t>(n_u) + frac64(gain);
                 h.f0 = f_now;
                 h.w_pre = frac64(f_now / fs);
                 h.theta_pre = ph - h.w_pre * static_cast<uint64_t>(n_u);
@@ -819,8 +839,10 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
         return fail(AWG_ERR_INVALID_ARG, "non-finite value in a trajectory array");
     for (int k = 0; k < N; ++k) {
         if (t_dur[k] < 0.0) return fail(AWG_ERR_INVALID_ARG, "t_dur[%d] < 0", k);
-        if (profile[k] < AWG_PROFILE_STATIC || profile[k] > AWG_PROFILE_MINJERK)
+        if (profile[k] < AWG_PROFILE_STATIC || profile[k] > AWG_PROFILE_EXP)
             return fail(AWG_ERR_INVALID_ARG, "unknown profile %d for tone %d", profile[k], k);
+        if (profile[k] == AWG_PROFILE_EXP && !(f0[k] > 0.0 && f1[k] > 0.0))
+            return fail(AWG_ERR_INVALID_ARG, "exponential chirp of tone %d needs f0 > 0 and f1 > 0", k);
         if (std::fabs(t_start[k]) * static_cast<double>(p->fs) > 4.0e18)
             return fail(AWG_ERR_INVALID_ARG, "t_start[%d] out of range", k);
     }

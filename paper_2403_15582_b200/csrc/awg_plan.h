@@ -18,6 +18,7 @@ struct HostTone {
     long double T = 0;           // move duration, s
     long double Tn = 0;          // move duration, samples (T*fs)
     long double DT = 0;          // (f1-f0)*T, cycles
+    long double expL = 0;        // AWG_PROFILE_EXP: ln(f1/f0); the phase gained over the carrier is f0 T (expm1(L s)/L - s)
     int64_t ns_int = 0;          // move start, samples: floor and
     double ns_frac = 0;          //   fractional part
     uint64_t theta_pre = 0, w_pre = 0;    // carrier before/during the move: turns*2^64, turns/sample*2^64

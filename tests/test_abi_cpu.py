@@ -47,7 +47,7 @@ def test_binding_mirrors_the_header(built):
         assert callable(getattr(m, name)), f"binding lacks {name}"
     src = open(HEADER).read()
     for const in ("AWG_OK", "AWG_ERR_INVALID_ARG", "AWG_ERR_ALLOC", "AWG_ERR_CUDA", "AWG_ERR_STATE", "AWG_ERR_UNDERRUN",
-                  "AWG_PROFILE_STATIC", "AWG_PROFILE_LINEAR", "AWG_PROFILE_MINJERK", "AWG_ENGINE_AUTO",
+                  "AWG_PROFILE_STATIC", "AWG_PROFILE_LINEAR", "AWG_PROFILE_MINJERK", "AWG_PROFILE_EXP", "AWG_ENGINE_AUTO",
                   "AWG_ENGINE_MUFU", "AWG_ENGINE_FP64", "AWG_ENGINE_FMA"):
         mm = re.search(rf"\b{const}\s*=\s*(-?\d+)", src)
         assert mm and int(mm.group(1)) == getattr(m, const)

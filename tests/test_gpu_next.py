@@ -403,3 +403,100 @@ def test_cross_cta_launches_on_two_streams_at_once(awg, torch_cuda):
     assert all(np.array_equal(_np(o), ref1) for o in outs1)
     assert all(np.array_equal(_np(o), ref2) for o in outs2)
     p1.close(); p2.close()
+
+
+# ------------------------------------------------------------------ NEXT-4: exponential chirps (G20)
+EXP = W.PROFILE_EXP
+
+
+@pytest.mark.parametrize("engine", ["fma", "mufu", "fp64"])
+def test_exponential_chirps_on_three_engines(awg, torch_cuda, engine):
+    """Upward, downward, octave-wide, nearly flat, very short, instant and not-yet-started exponential chirps beside
+    tones of the other profiles; chunks before, inside and after the moves; chunkings agree bit for bit."""
+    eng = {"fma": awg.AWG_ENGINE_FMA, "mufu": awg.AWG_ENGINE_MUFU, "fp64": awg.AWG_ENGINE_FP64}[engine]
+    L = 4096
+    us = 1e-6
+    rows = [
+        (100e6, 130e6, 0.12, 0.3, 3 * us, 25 * us, EXP),
+        (90e6, 60e6, 0.12, 1.3, 0.0, 40 * us, EXP),
+        (40e6, 160e6, 0.10, 2.1, 6.5 * us, 17.3 * us, EXP),           # two octaves
+        (150e6, 150e6 * (1 + 1e-9), 0.08, 0.9, 1 * us, 30 * us, EXP),  # ln(f1/f0) ~ 1e-9
+        (70e6, 75e6, 0.08, 0.2, 12 * us, 0.4 * us, EXP),               # shorter than a 512-sample block
+        (200e6, 210e6, 0.08, 0.5, 9 * us, 0.0, EXP),                   # instant retune
+        (55e6, 50e6, 0.08, 0.4, -20 * us, 35 * us, EXP),               # started before sample 0
+        (120e6, 120e6, 0.08, 0.0, 2 * us, 9 * us, EXP),                # f1 = f0: a static tone
+        (180e6, 185e6, 0.08, 1.7, 4 * us, 20 * us, MINJERK),
+        (30e6, 30e6, 0.10, 0.6, 0.0, 0.0, STATIC),
+    ]
+    p, op = _pair(awg, FS, L, rows, eng)
+    n_chunks = 8                                             # 58 us: every move ends inside
+    V = oracle.c_waveform(op, 0, n_chunks * L)
+    gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(n_chunks)])
+    emax = assert_f32_close(gotf, V, f"exponential chirps {engine}", tol=3e-7 if engine == "fp64" else 1e-5)
+    got = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(n_chunks)])
+    assert_codes_close(got, op.quantise(V), f"exponential chirps {engine}")
+    assert np.array_equal(_np(p.synthesize_range(0, n_chunks)), got)
+    q = awg.Plan(len(rows), FS, 1000, None, eng)
+    q.set_trajectories(*list(zip(*rows)))
+    for c in (0, 3, 11, 20, 31):
+        assert np.array_equal(_np(q.synthesize_chunk(c)), got[c * 1000:(c + 1) * 1000]), c
+    # long after the moves: each tone sits at f1 with the phase the whole chirp left behind
+    c = 3000
+    Vl = oracle.c_waveform(op, c * L, (c + 1) * L)
+    assert_f32_close(_np(p.synthesize_chunk_f32(c)), Vl, "after the exponential chirps")
+    print(f"exponential chirps {engine}: f32 max err {emax:.2e}")
+    p.close(); q.close()
+
+
+def test_exponential_chirp_updates_and_errors(awg, torch_cuda, eng):
+    """Per-chunk updates into and out of exponential chirps, one of them landing mid-chirp (continues phase-continuously
+    from the instantaneous frequency f0 r^s); a long chirp among 300 tones (leaf path); argument checks."""
+    L = 2048
+    N = 300
+    rng = np.random.default_rng(77)
+    rows = []
+    for k in range(N):
+        f0 = rng.uniform(20e6, 250e6)
+        if k % 5 == 0:
+            rows.append((f0, f0 * rng.uniform(0.8, 1.25), 1.0 / N, rng.uniform(0, 6.28), rng.uniform(0, 20e-6), rng.uniform(5e-6, 60e-6), EXP))
+        elif k % 5 == 1:
+            rows.append((f0, f0 + rng.uniform(-2e6, 2e6), 1.0 / N, rng.uniform(0, 6.28), -1e-3, 30e-3, MINJERK))
+        else:
+            rows.append((f0, f0, 1.0 / N, rng.uniform(0, 6.28), 0.0, 0.0, STATIC))
+    rows[0] = (110e6, 95e6, 1.0 / N, 0.7, 2e-6, 40e-6, EXP)   # mid-chirp at chunk 4
+    p, op = _pair(awg, FS, L, rows, eng)
+    n_chunks = 16
+    updates = {
+        # chunk 4 = 14.6 us: tone 0 is mid-chirp; tone 2 was static; tone 5 goes from an exponential chirp to minimum jerk
+        4: ([0, 2, 5], [rows[0][0] * 1.1, rows[2][0] * 0.9, rows[5][0] + 1e6], [30e-6, 20e-6, 8e-6], [EXP, EXP, MINJERK]),
+        # chunk 9 = 32.9 us: tone 0 is mid-chirp again and jumps back; tone 10 restarts
+        9: ([0, 10], [rows[0][0], rows[10][0] * 1.05], [0.0, 10e-6], [EXP, EXP]),
+    }
+    gotf, got = [], []
+    for c in range(n_chunks):                                # the CUDA plan takes updates in stream order with the chunks
+        if c in updates:
+            p.update_trajectories(c, *updates[c])
+            op.update_trajectories(c, *updates[c])
+        gotf.append(_np(p.synthesize_chunk_f32(c)))
+        got.append(_np(p.synthesize_chunk(c)))
+    V = oracle.c_waveform(op, 0, n_chunks * L)
+    assert_f32_close(np.concatenate(gotf), V, "exponential chirp updates")
+    assert_codes_close(np.concatenate(got), op.quantise(V), "exponential chirp updates")
+    c = 2000
+    assert_f32_close(_np(p.synthesize_chunk_f32(c)), oracle.c_waveform(op, c * L, (c + 1) * L), "after the updates")
+    # errors: a geometric path needs two frequencies of the same sign, away from zero
+    with pytest.raises(awg.AwgError) as ei:
+        p.update_trajectories(20, [3], [0.0], [1e-6], [EXP])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    with pytest.raises(awg.AwgError) as ei:
+        p.update_trajectories(20, [3], [-5e6], [1e-6], [EXP])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    q = awg.Plan(2, FS, L)
+    for f0, f1 in ((0.0, 1e6), (1e6, 0.0), (1e6, -2e6)):
+        with pytest.raises(awg.AwgError) as ei:
+            q.set_trajectories([f0, 2e6], [f1, 2e6], [0.1, 0.1], [0, 0], [0, 0], [1e-6, 0], [EXP, STATIC])
+        assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    with pytest.raises(awg.AwgError) as ei:
+        q.set_trajectories([1e6, 2e6], [1e6, 2e6], [0.1, 0.1], [0, 0], [0, 0], [1e-6, 0], [4, STATIC])
+    assert ei.value.status == awg.AWG_ERR_INVALID_ARG
+    p.close(); q.close()
