@@ -143,9 +143,10 @@ awg_status awg_synthesize_range(awg_plan *p, int64_t first_chunk, int64_t n_chun
                                 void *stream);
 
 /* End-to-end variant with a HOST destination: synthesises the range in pieces of 2^21 samples into
- * two internal device slots and copies each piece to host_out (n_chunks*chunk_len int16; pinned
- * memory gives overlap of copy and compute, pageable memory works) -- synchronous, returns when
- * host_out is complete.  Stands in for the paper's pinned-buffer -> DAC transfer. */
+ * four internal device slots (pieces alternate between two internal streams, so the next piece takes
+ * over the SMs as the current one runs out of tiles) and copies each finished piece to host_out on a
+ * third stream (n_chunks*chunk_len int16; pinned memory gives overlap of copy and compute, pageable
+ * memory works) -- synchronous, returns when host_out is complete.  Stands in for the paper's pinned-buffer -> DAC transfer. */
 awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int16_t *host_out);
 
 /* ---- four-channel multiplexed output (the paper's WM kernel; Fig. 4) ---------- */

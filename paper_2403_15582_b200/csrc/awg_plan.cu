@@ -496,13 +496,27 @@ awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_h
     return AWG_OK;
 }
 
+static void free_e2e(awg_plan *p)
+{
+    for (int s = 0; s < kE2eSlots; ++s) {
+        if (p->e2e_slot[s]) cudaFree(p->e2e_slot[s]);
+        if (p->e2e_done[s]) cudaEventDestroy(p->e2e_done[s]);
+        if (p->e2e_ready[s]) cudaEventDestroy(p->e2e_ready[s]);
+        p->e2e_slot[s] = nullptr; p->e2e_done[s] = nullptr; p->e2e_ready[s] = nullptr;
+    }
+    for (int s = 0; s < 3; ++s) {
+        if (p->e2e_stream[s]) cudaStreamDestroy(p->e2e_stream[s]);
+        p->e2e_stream[s] = nullptr;
+    }
+}
+
 awg_status awg_plan_destroy(awg_plan *p)
 {
     if (!p) return AWG_OK;
     if (p->n_rings > 0) return fail(AWG_ERR_STATE, "destroy the plan's rings first");
     for (int v = 0; v < kTableVersions; ++v)
         if (p->last_use[v]) cudaEventSynchronize(p->last_use[v]);
-    for (int s = 0; s < 2; ++s) {
+    for (int s = 0; s < kE2eSlots; ++s) {
         if (p->e2e_done[s]) cudaEventSynchronize(p->e2e_done[s]);
     }
     for (int v = 0; v < kTableVersions; ++v) {
@@ -517,12 +531,7 @@ awg_status awg_plan_destroy(awg_plan *p)
     if (p->dev_aux) cudaFree(p->dev_aux);
     if (p->dev_aux_stage) cudaFree(p->dev_aux_stage);
     if (p->host_aux) cudaFreeHost(p->host_aux);
-    for (int s = 0; s < 2; ++s) {
-        if (p->e2e_slot[s]) cudaFree(p->e2e_slot[s]);
-        if (p->e2e_done[s]) cudaEventDestroy(p->e2e_done[s]);
-        if (p->e2e_ready[s]) cudaEventDestroy(p->e2e_ready[s]);
-        if (p->e2e_stream[s]) cudaStreamDestroy(p->e2e_stream[s]);
-    }
+    free_e2e(p);
     delete p;
     return AWG_OK;
 }
@@ -931,38 +940,36 @@ awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n
     awg_status st = check_chunk_call(p, first_chunk, n_chunks, host_out, 2);
     if (st != AWG_OK) return st;
     cudaError_t e;
-    // two device slots of 2^21 samples (4 MiB of int16): stream 0 synthesises piece i+1 while stream 1 copies piece i to the host
+    // kE2eSlots device slots of 2^21 samples (4 MiB of int16).  Pieces alternate between two synthesis streams, so the
+    // persistent CTAs of piece i+1 take over SM by SM as those of piece i run out of tiles (no idle tail between pieces),
+    // while the copy stream moves finished pieces to the host.
     constexpr int64_t kPiece = int64_t(1) << 21;
     if (!p->e2e_ok) {
-        // both slots or none: a half-built pair is torn down again
         awg_status bad = AWG_OK;
-        for (int s = 0; s < 2 && bad == AWG_OK; ++s) {
+        for (int s = 0; s < kE2eSlots && bad == AWG_OK; ++s) {
             if ((e = cudaMalloc(reinterpret_cast<void **>(&p->e2e_slot[s]), kPiece * sizeof(int16_t))) != cudaSuccess)
                 bad = fail(AWG_ERR_ALLOC, "cudaMalloc(e2e slot): %s", cudaGetErrorString(e));
-            else if ((e = cudaStreamCreateWithFlags(&p->e2e_stream[s], cudaStreamNonBlocking)) != cudaSuccess ||
-                     (e = cudaEventCreateWithFlags(&p->e2e_ready[s], cudaEventDisableTiming)) != cudaSuccess ||
+            else if ((e = cudaEventCreateWithFlags(&p->e2e_ready[s], cudaEventDisableTiming)) != cudaSuccess ||
                      (e = cudaEventCreateWithFlags(&p->e2e_done[s], cudaEventDisableTiming)) != cudaSuccess)
-                bad = fail_cuda(e, "e2e stream/event creation");
+                bad = fail_cuda(e, "e2e event creation");
         }
+        for (int s = 0; s < 3 && bad == AWG_OK; ++s)
+            if ((e = cudaStreamCreateWithFlags(&p->e2e_stream[s], cudaStreamNonBlocking)) != cudaSuccess)
+                bad = fail_cuda(e, "e2e stream creation");
         if (bad != AWG_OK) {
-            for (int s = 0; s < 2; ++s) {
-                if (p->e2e_slot[s]) cudaFree(p->e2e_slot[s]);
-                if (p->e2e_done[s]) cudaEventDestroy(p->e2e_done[s]);
-                if (p->e2e_ready[s]) cudaEventDestroy(p->e2e_ready[s]);
-                if (p->e2e_stream[s]) cudaStreamDestroy(p->e2e_stream[s]);
-                p->e2e_slot[s] = nullptr; p->e2e_done[s] = nullptr; p->e2e_ready[s] = nullptr; p->e2e_stream[s] = nullptr;
-            }
+            free_e2e(p);   // all or nothing: a half-built set is torn down again
             return bad;
         }
         p->e2e_ok = true;
     }
     const int64_t n0 = first_chunk * p->chunk_len, total = n_chunks * p->chunk_len;
-    cudaStream_t s_syn = p->e2e_stream[0], s_cpy = p->e2e_stream[1];
+    cudaStream_t s_cpy = p->e2e_stream[2];
     int i = 0;
     for (int64_t off = 0; off < total; off += kPiece, ++i) {
-        const int slot = i & 1;
+        const int slot = i % kE2eSlots;
+        cudaStream_t s_syn = p->e2e_stream[i & 1];
         const int64_t cnt = (total - off < kPiece) ? (total - off) : kPiece;
-        if (i >= 2 && (e = cudaStreamWaitEvent(s_syn, p->e2e_done[slot], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+        if (i >= kE2eSlots && (e = cudaStreamWaitEvent(s_syn, p->e2e_done[slot], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
         if ((st = synthesize_samples(p, n0 + off, cnt, p->e2e_slot[slot], false, s_syn)) != AWG_OK) return st;
         if ((e = cudaEventRecord(p->e2e_ready[slot], s_syn)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
         if ((e = cudaStreamWaitEvent(s_cpy, p->e2e_ready[slot], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");

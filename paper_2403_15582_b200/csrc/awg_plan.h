@@ -37,6 +37,8 @@ awg_status fail_cuda(cudaError_t e, const char *what);
 
 }  // namespace awg
 
+constexpr int kE2eSlots = 4;   // device staging slots of awg_synthesize_range_host
+
 struct awg_plan {
     int32_t n_tones = 0, n_pad = 0;
     long double fs = 0;
@@ -73,10 +75,10 @@ struct awg_plan {
     cudaEvent_t uploaded[awg::kTableVersions] = {};
     cudaStream_t upload_stream[awg::kTableVersions] = {};
     // awg_synthesize_range_host
-    int16_t *e2e_slot[2] = {};
-    cudaStream_t e2e_stream[2] = {};
-    cudaEvent_t e2e_ready[2] = {}, e2e_done[2] = {};
-    bool e2e_ok = false;                    // both slots, streams and events exist
+    int16_t *e2e_slot[kE2eSlots] = {};
+    cudaStream_t e2e_stream[3] = {};        // two synthesis streams (alternating pieces), one copy stream
+    cudaEvent_t e2e_ready[kE2eSlots] = {}, e2e_done[kE2eSlots] = {};
+    bool e2e_ok = false;                    // all slots, streams and events exist
     // accounting
     int64_t h2d_bytes = 0, d2h_bytes = 0;
     int n_rings = 0;

@@ -87,6 +87,28 @@ def test_c2_full_range_and_chunks(awg, torch_cuda, eng):
     p.close()
 
 
+def test_host_destination_call_many_pieces_pinned_and_pageable(awg, torch_cuda):
+    """awg_synthesize_range_host over 11 pieces of 2^21 samples (its four device slots are reused, pieces alternate between
+    two synthesis streams), ragged last piece, into pinned and into pageable host memory, twice in a row, with a table
+    change in between: the same codes as one device launch."""
+    import torch
+    L = 1_000_000                                           # 22 chunks = 10.49 pieces
+    w = W.config1()
+    p = awg.Plan(w.n_tones, w.sample_rate, L)
+    p.set_trajectories(w.f0, w.f1, w.A, w.phi0, w.t_start, w.t_dur, w.profile)
+    ref = _np(p.synthesize_range(0, 22))
+    pinned = p.synthesize_range_host(0, 22)
+    assert pinned.is_pinned() and np.array_equal(pinned.numpy(), ref)
+    pageable = torch.zeros(22 * L, dtype=torch.int16)
+    p.synthesize_range_host(0, 22, out=pageable)
+    assert np.array_equal(pageable.numpy(), ref)
+    p.set_trajectories(w.f0, w.f1, 0.5 * np.asarray(w.A), w.phi0, w.t_start, w.t_dur, w.profile)
+    ref2 = _np(p.synthesize_range(3, 19))
+    assert not np.array_equal(ref2, ref[3 * L:])
+    assert np.array_equal(p.synthesize_range_host(3, 19, out=pinned[:19 * L]).numpy(), ref2)
+    p.close()
+
+
 def test_c2_fp64_engine_window(awg, torch_cuda):
     w = W.config2().rechunked(224_000)
     op = oracle.plan_from_workload(w)
