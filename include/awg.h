@@ -226,12 +226,21 @@ awg_status awg_plan_io_bytes(awg_plan *p, int64_t *h2d_bytes, int64_t *d2h_bytes
 
 /* Algorithmic operation counts of the CURRENT trajectory table over chunks first_chunk ..
  * first_chunk+n_chunks-1, at sample granularity: tone-samples of tones that are static there
- * (one fp32 multiply-add each on the angle-addition engine), inside a slow move (two multiply-adds:
- * the kernel's slow pass) and inside any other move (one MUFU.SIN + two multiply-adds).  This is the
+ * (one fp32 multiply-add each on the angle-addition engine), inside a slow move (1.25 multiply-adds,
+ * 1.5 in plans with faster slow movers: the kernel's slow pass) and inside any other move (one MUFU.SIN + two multiply-adds).  This is the
  * library's own classification (the one the kernel acts on); bench.py derives its roofline from it.
  * Host-only, no CUDA work.  Any pointer may be NULL.  Errors: INVALID_ARG, STATE (no table set). */
 awg_status awg_plan_op_counts(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int64_t *static_ts,
                               int64_t *slow_ts, int64_t *fast_ts);
+
+/* Tile-serving order of a launch over chunks first_chunk .. first_chunk+n_chunks-1 of the CURRENT table:
+ * *n_listed = 2048-sample tiles of the range in which at least max(2, n/16) of the n evaluated tones enter
+ * or leave a slow move at once (such a tile costs several ordinary ones: all those tones take the
+ * one-sine-per-sample pass there), *n_served_first = how many of them the launch hands out before all
+ * other tiles (the heaviest 16; 0 for ranges under 64 tiles, whose units all start at once).  The order
+ * has no effect on any sample.  Host-only.  Either pointer may be NULL.  Errors: INVALID_ARG, STATE. */
+awg_status awg_plan_hot_tiles(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int32_t *n_listed,
+                              int32_t *n_served_first);
 
 /* Number of kernels the library has launched since load (all plans); for launch accounting. */
 int64_t awg_kernel_launch_count(void);

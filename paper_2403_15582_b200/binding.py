@@ -40,7 +40,7 @@ EXPORTED = (
     "awg_synthesize_range_host", "awg_ring_create", "awg_ring_submit", "awg_ring_acquire", "awg_ring_release",
     "awg_synthesize_chunk_mux", "awg_snap_frequency", "awg_static_buffer_set", "awg_static_buffer_fold",
     "awg_static_buffer_read",
-    "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_plan_op_counts", "awg_kernel_launch_count",
+    "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_plan_op_counts", "awg_plan_hot_tiles", "awg_kernel_launch_count",
     "awg_last_error",
 )
 
@@ -77,6 +77,7 @@ def _load() -> ctypes.CDLL:
         "awg_ring_destroy": (I32, [P]),
         "awg_plan_io_bytes": (I32, [P, POINTER(I64), POINTER(I64)]),
         "awg_plan_op_counts": (I32, [P, I64, I64, POINTER(I64), POINTER(I64), POINTER(I64)]),
+        "awg_plan_hot_tiles": (I32, [P, I64, I64, POINTER(I32), POINTER(I32)]),
         "awg_kernel_launch_count": (I64, []),
         "awg_last_error": (c_char_p, []),
     }
@@ -253,6 +254,12 @@ def awg_plan_io_bytes(plan) -> Tuple[int, int]:
     return a.value, b.value
 
 
+def awg_plan_hot_tiles(plan, first_chunk: int, n_chunks: int) -> Tuple[int, int]:
+    a, b = ctypes.c_int32(0), ctypes.c_int32(0)
+    _check(_lib.awg_plan_hot_tiles(plan, first_chunk, n_chunks, byref(a), byref(b)))
+    return a.value, b.value
+
+
 def awg_plan_op_counts(plan, first_chunk: int, n_chunks: int) -> Tuple[int, int, int]:
     """-> (static, slow-moving, fast-moving) tone-samples of the current table over the chunk range."""
     a, b, c = c_int64(), c_int64(), c_int64()
@@ -353,6 +360,10 @@ class Plan:
 
     def io_bytes(self) -> Tuple[int, int]:
         return awg_plan_io_bytes(self._h)
+
+    def hot_tiles(self, first_chunk: int, n_chunks: int) -> Tuple[int, int]:
+        """(tiles of the range where many slow moves start or end at once, how many of them the launch serves first)"""
+        return awg_plan_hot_tiles(self._h, first_chunk, n_chunks)
 
     def op_counts(self, first_chunk: int, n_chunks: int) -> Tuple[int, int, int]:
         return awg_plan_op_counts(self._h, first_chunk, n_chunks)

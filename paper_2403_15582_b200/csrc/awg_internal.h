@@ -98,6 +98,8 @@ struct FixGrid {
     uint32_t bias_q[16]; // bits(1.5 * 2^23) * sum over the quad's leaves of 2^(fix_sh - leaf_sh), mod 2^32: the magic-number bias parked with them
 };
 
+constexpr int kMaxHotTiles = 16;
+
 struct LaunchParams {
     const ToneRec *tab;
     int32_t n_tones;
@@ -120,6 +122,12 @@ struct LaunchParams {
     int32_t *scratch;    //   [tile][block][kBlock] int32 fixed point, this launch's slot (zero before and after the launch)
     uint32_t *tile_cnt;  //   quads delivered per tile (zero before and after the launch)
     FixGrid fix;         // fixed-point grids of the leaf merge (fix_grids(); large tables only)
+    // Tiles in which many tones start or end a move at once (all of them leave the angle-addition passes there) cost several
+    // ordinary tiles; drawn late by the tile scheduler such a tile is the tail of the whole launch.  The host lists them
+    // (ascending, relative to the launch's first tile) and the scheduler serves them first.  Which team computes a tile, and
+    // when, has no effect on its samples.
+    int32_t n_hot = 0;
+    int32_t hot[kMaxHotTiles] = {};
 };
 
 // Warps of a team share a tile, each taking 1/split of the tones.  A function of the tone count ONLY, never of the

@@ -773,6 +773,18 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
 }
 #undef AWG_RUN_KIND
 
+// Serving order of the tiles: the launch's hot tiles (LaunchParams::hot, ascending) first, then the others in ascending order.
+__device__ __forceinline__ int64_t hot_first(const LaunchParams &lp, int64_t seq)
+{
+    const int n_hot = lp.n_hot;
+    if (n_hot == 0) return seq;
+    if (seq < n_hot) return lp.hot[seq];
+    int64_t t = seq - n_hot;
+#pragma unroll 1
+    for (int j = 0; j < n_hot && lp.hot[j] <= t; ++j) ++t;
+    return t;
+}
+
 // Draws the team's next tile from the launch counter (leader: lane 0 of rank 0) and hands it to the whole team.
 template <int SPLIT>
 __device__ __forceinline__ int64_t next_unit(const LaunchParams &lp, WarpSmem &ws_leader, int team, int rank, int lane, int64_t n_teams)
@@ -949,8 +961,9 @@ __global__ void __launch_bounds__(kWarps * 32, kCtasPerSm) awg_synth_kernel(cons
     const bool single = !kQuads && per <= kBatch;
     unsigned sticky_sta = 0u, sticky_post = 0xffffffffu;   // no tile has post bits outside its static bits
     while (unit < n_units) {
-      const int64_t tile = cross ? unit / Q : unit;
-      const int q_begin = cross ? static_cast<int>(unit - tile * Q) : 0;
+      const int64_t tile_seq = cross ? unit / Q : unit;
+      const int q_begin = cross ? static_cast<int>(unit - tile_seq * Q) : 0;
+      const int64_t tile = hot_first(lp, tile_seq);
       const int q_end = cross ? q_begin + 1 : Q;
       const int64_t tile_base = (first_tile + tile) * kTile;
       const int64_t n_thread = tile_base + lane * kSPT;

@@ -11,8 +11,10 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <functional>
 #include <limits>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "awg_internal.h"
@@ -263,6 +265,7 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
         p->slow2 = false;
         for (int k = 0; k < p->n_tones; ++k)
             if (!p->in_buffer[k] && (p->tones[k].cls & CLS_SLOW2_FLAG)) p->slow2 = true;
+        p->hot_dirty = true;
     }
     std::sort(p->dirty_tones.begin(), p->dirty_tones.end());
     p->dirty_tones.erase(std::unique(p->dirty_tones.begin(), p->dirty_tones.end()), p->dirty_tones.end());
@@ -318,6 +321,61 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
     return AWG_OK;
 }
 
+// Hot tiles of a launch (LaunchParams::hot): tiles of the range in which at least max(2, n/16) of the n evaluated tones
+// enter or leave a SLOW move (CLS_SLOW_FLAG).  Inside the move such a tone costs 1.25 multiply-adds per sample; in the tile
+// that holds the boundary it takes the one-sine-per-sample pass for the whole tile: when many do so at once (tweezer
+// rearrangements move their tones in step; C3: 1000 moves end in one tile) the tile costs several ordinary ones, and drawn in
+// its turn it ended 0.15 ms after every other CTA had run out of work (C3: 1.69 -> 1.57 ms with the tile served first).
+// The boundaries are a property of the table: they are listed once per table change (p->hot_tiles, absolute tile indices
+// with their tone counts) and filtered per launch.  Fast movers are left out: their tiles cost the same inside the move.
+static void list_hot_tiles(awg_plan *p)
+{
+    p->hot_tiles.clear();
+    p->hot_dirty = false;
+    if (p->n_active > 16384) return;
+    std::vector<int64_t> at;
+    for (int k = 0; k < p->n_tones; ++k) {
+        const HostTone &h = p->tones[k];
+        if (!(h.cls & CLS_SLOW_FLAG) || p->in_buffer[k]) continue;
+        at.push_back(static_cast<int64_t>(floorl(static_cast<long double>(h.ns_int) / kTile)));
+        at.push_back(static_cast<int64_t>(floorl((static_cast<long double>(h.ns_int) + h.ns_frac + h.Tn) / kTile)));
+    }
+    if (at.empty()) return;
+    std::sort(at.begin(), at.end());
+    const size_t thr = std::max<size_t>(2, static_cast<size_t>(p->n_active) / 16);
+    for (size_t i = 0; i < at.size();) {
+        size_t j = i;
+        while (j < at.size() && at[j] == at[i]) ++j;
+        if (j - i >= thr) p->hot_tiles.emplace_back(at[i], static_cast<int64_t>(j - i));
+        i = j;
+    }
+}
+
+static void find_hot_tiles(awg_plan *p, int64_t n_begin, int64_t n_count, LaunchParams &lp)
+{
+    lp.n_hot = 0;
+    const int64_t first = n_begin / kTile, last = (n_begin + n_count - 1) / kTile;
+    if (last - first + 1 < 64) return;   // every unit of such a launch starts at once anyway
+    if (p->hot_dirty) list_hot_tiles(p);
+    if (p->hot_tiles.empty()) return;
+    std::pair<int64_t, int64_t> in[kMaxHotTiles];   // (tones, tile relative to the launch): the kMaxHotTiles heaviest of the range
+    int n = 0;
+    for (const auto &ht : p->hot_tiles) {
+        if (ht.first < first || ht.first > last) continue;
+        const std::pair<int64_t, int64_t> cand(ht.second, ht.first - first);
+        if (n < kMaxHotTiles) {
+            in[n++] = cand;
+        } else {
+            int m = 0;
+            for (int i = 1; i < n; ++i)
+                if (in[i].first < in[m].first) m = i;
+            if (cand.first > in[m].first) in[m] = cand;
+        }
+    }
+    std::sort(in, in + n, [](const std::pair<int64_t, int64_t> &a, const std::pair<int64_t, int64_t> &b) { return a.second < b.second; });
+    for (int i = 0; i < n; ++i) lp.hot[lp.n_hot++] = static_cast<int32_t>(in[i].second);
+}
+
 awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, void *dev_out, bool f32, cudaStream_t stream,
                               int32_t out_stride, int32_t out_offset)
 {
@@ -338,6 +396,7 @@ awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, voi
     lp.out = dev_out;
     lp.out_f32 = f32 ? 1 : 0;
     lp.sched = nullptr;  // launch_synth assigns the tile-scheduler slot
+    find_hot_tiles(p, n_begin, n_count, lp);
     cudaError_t e = launch_synth(lp, p->engine, stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
     if ((e = cudaEventRecord(p->last_use[p->cur_version], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
@@ -541,6 +600,24 @@ awg_status awg_plan_io_bytes(awg_plan *p, int64_t *h2d_bytes, int64_t *d2h_bytes
     if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
     if (h2d_bytes) *h2d_bytes = p->h2d_bytes;
     if (d2h_bytes) *d2h_bytes = p->d2h_bytes;
+    return AWG_OK;
+}
+
+awg_status awg_plan_hot_tiles(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int32_t *n_listed, int32_t *n_served_first)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (first_chunk < 0 || n_chunks < 1) return fail(AWG_ERR_INVALID_ARG, "bad chunk range");
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    list_hot_tiles(p);   // from the host table as it stands (per-chunk updates included)
+    const int64_t n0 = first_chunk * p->chunk_len, cnt = n_chunks * p->chunk_len;
+    const int64_t first = n0 / kTile, last = (n0 + cnt - 1) / kTile;
+    int32_t listed = 0;
+    for (const auto &ht : p->hot_tiles)
+        if (ht.first >= first && ht.first <= last) ++listed;
+    LaunchParams lp;
+    find_hot_tiles(p, n0, cnt, lp);
+    if (n_listed) *n_listed = listed;
+    if (n_served_first) *n_served_first = lp.n_hot;
     return AWG_OK;
 }
 

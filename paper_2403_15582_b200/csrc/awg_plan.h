@@ -1,6 +1,7 @@
 // awg_plan.h -- host-side plan state (shared by awg_plan.cu and awg_ring.cu).  CUDA path only.
 #pragma once
 #include <cstdint>
+#include <utility>
 #include <vector>
 
 #include <cuda_runtime.h>
@@ -78,6 +79,8 @@ struct awg_plan {
     int16_t *e2e_slot[kE2eSlots] = {};
     cudaStream_t e2e_stream[3] = {};        // two synthesis streams (alternating pieces), one copy stream
     cudaEvent_t e2e_ready[kE2eSlots] = {}, e2e_done[kE2eSlots] = {};
+    std::vector<std::pair<int64_t, int64_t>> hot_tiles;   // (absolute tile, tones) where many slow movers start or end a move at once
+    bool hot_dirty = true;                  //   (listed again after a table change)
     bool e2e_ok = false;                    // all slots, streams and events exist
     // accounting
     int64_t h2d_bytes = 0, d2h_bytes = 0;

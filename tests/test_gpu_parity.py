@@ -516,6 +516,44 @@ def test_slow_movers_one_correction_per_thread_at_its_bound(awg, torch_cuda):
     p.close()
 
 
+@pytest.mark.parametrize("N,per_group", [(320, 20), (48, 4)])
+def test_tiles_where_many_slow_moves_start_or_end_are_served_first(awg, torch_cuda, N, per_group):
+    """Tweezer rearrangements move tones in step: groups of slow movers share their move window, so a handful of tiles
+    hold many move boundaries.  A launch with >= 64 tiles serves those tiles first (LaunchParams::hot; here more such
+    tiles than the list holds, so the heaviest are chosen) -- the serving order must not change a bit: one launch over
+    the range, a launch that starts at another tile, and 32-tile chunk launches (no reordering) agree bit for bit, and
+    windows around the boundaries agree with the oracle."""
+    fs, cl = 560e6, 1 << 16
+    rng = np.random.default_rng(N)
+    rows, marks = [], []
+    n_groups = N // per_group
+    for g in range(n_groups):
+        t0 = (0.3 + 0.31 * g) * 1e-3 + rng.uniform(0, 2e-6)            # groups start 0.31 ms apart ...
+        T = 3e-3 + 0.17e-3 * g                                         # ... and end at their own time: 2 x n_groups boundary tiles
+        marks += [int(t0 * fs), int((t0 + T) * fs)]
+        for k in range(per_group):
+            f0 = rng.uniform(40e6, 240e6)
+            rows.append((f0, f0 + rng.choice([-1.0, 1.0]) * rng.uniform(0.3e6, 1.0e6), 1.0 / N, rng.uniform(0, 6.28), t0, T,
+                         MINJERK if k % 2 else LINEAR))
+    p, op = _single(awg, fs, cl, rows, engine=awg.AWG_ENGINE_FMA)
+    n_chunks = int(max(marks) / cl) + 3
+    c_mid = int(0.5 * (min(marks) + max(marks)) / cl)
+    sta, slow, fast = p.op_counts(c_mid, 1)
+    assert slow > 0.5 * N * cl, "most tones must be slow movers in the middle of the range"
+    listed, first = p.hot_tiles(0, n_chunks)
+    assert listed == 2 * n_groups and first == 16, "every group boundary is a hot tile; the launch serves the 16 heaviest first"
+    assert p.hot_tiles(0, 1) == (0, 0) and p.hot_tiles(marks[0] // cl, 1) == (1, 0), "32-tile launches are not reordered"
+    whole = _np(p.synthesize_range(0, n_chunks))
+    assert np.array_equal(_np(p.synthesize_range(3, n_chunks - 5)), whole[3 * cl:(n_chunks - 2) * cl])
+    for c in sorted({0, n_chunks - 1, *(m // cl for m in marks)}):
+        assert np.array_equal(_np(p.synthesize_chunk(c)), whole[c * cl:(c + 1) * cl]), f"chunk {c}"
+    for m in marks[::3]:
+        a = max(0, m - 2048) // 8 * 8
+        V = oracle.c_waveform(op, a, a + 4096)
+        assert_codes_close(whole[a:a + 4096], op.quantise(V), f"around the boundary at sample {m}")
+    p.close()
+
+
 def test_special_moves(awg, torch_cuda, eng):
     fs = 560e6
     rows = [
