@@ -46,8 +46,14 @@ constexpr int kRadius = kBlock / 2;  // half of the 512-sample block (span of on
 // frac(x) as 64-bit fixed-point turns.
 uint64_t frac64(long double x)
 {
-    long double fr = x - floorl(x);        // [0, 1]
-    long double v = ldexpl(fr, 64);        // [0, 2^64]
+    long double fr;                        // x - floor(x) in [0, 1], rounded once
+    if (fabsl(x) < 9.0e18L) {
+        fr = x - static_cast<long double>(static_cast<int64_t>(x));   // exact; in (-1, 1)  (no libm call on the table-build path)
+        if (fr < 0.0L) fr += 1.0L;
+    } else {
+        fr = x - floorl(x);
+    }
+    const long double v = fr * 18446744073709551616.0L;   // [0, 2^64], exact
     if (!(v < 18446744073709551616.0L)) return 0;  // rounded up to one full turn
     return static_cast<uint64_t>(v);
 }
@@ -222,11 +228,13 @@ static void fill_core(const HostTone &h, ToneCore &r)
         r.inv_Tn = static_cast<double>(rT);
         r.DT = static_cast<double>(h.DT);
         r.q1 = static_cast<double>(h.DT * rT);
-        long double q = kTwoPiL * h.DT * rT, fact = 1.0L;  // 2 pi DT / Tn^k / k!
+        // 2 pi DT / Tn^k / k!, k = 2..6, for fp32 consumers: double arithmetic is ample (and far cheaper than x87 here)
+        static const double inv_fact[5] = {1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0};
+        const double rTd = r.inv_Tn;
+        double q = 6.283185307179586476925286766559 * r.q1;
         for (int k = 2; k <= 6; ++k) {
-            q *= rT;
-            fact *= k;
-            r.q[k - 2] = static_cast<float>(q / fact);
+            q *= rTd;
+            r.q[k - 2] = static_cast<float>(q * inv_fact[k - 2]);
         }
         if (h.profile == AWG_PROFILE_EXP) {
             // exponential chirp: no Taylor scales (every sample of the move takes the fp64 path); q[0..3] carry f0 T (cycles)
@@ -333,22 +341,48 @@ static void list_hot_tiles(awg_plan *p)
     p->hot_tiles.clear();
     p->hot_dirty = false;
     if (p->n_active > 16384) return;
-    std::vector<int64_t> at;
+    static_assert((kTile & (kTile - 1)) == 0, "tile index = sample index >> log2(kTile), also for negative indices");
+    constexpr int kTileShift = 11;
+    static_assert((1 << kTileShift) == kTile, "kTileShift");
+    // move starts and move ends, each in tone order: tones that move in step give long runs of equal keys, already in order
+    std::vector<int64_t> (&at)[2] = p->hot_scratch;
+    bool sorted[2] = {true, true};
+    at[0].clear();
+    at[1].clear();
     for (int k = 0; k < p->n_tones; ++k) {
         const HostTone &h = p->tones[k];
         if (!(h.cls & CLS_SLOW_FLAG) || p->in_buffer[k]) continue;
-        at.push_back(static_cast<int64_t>(floorl(static_cast<long double>(h.ns_int) / kTile)));
-        at.push_back(static_cast<int64_t>(floorl((static_cast<long double>(h.ns_int) + h.ns_frac + h.Tn) / kTile)));
+        // slow moves last >= 2 tiles and |t_start| fs < 4e18 (checked on entry): everything fits int64
+        const int64_t t[2] = {h.ns_int >> kTileShift,
+                              (h.ns_int + static_cast<int64_t>(static_cast<long double>(h.ns_frac) + h.Tn)) >> kTileShift};
+        for (int e = 0; e < 2; ++e) {
+            if (!at[e].empty() && t[e] < at[e].back()) sorted[e] = false;
+            at[e].push_back(t[e]);
+        }
     }
-    if (at.empty()) return;
-    std::sort(at.begin(), at.end());
+    if (at[0].empty()) return;
     const size_t thr = std::max<size_t>(2, static_cast<size_t>(p->n_active) / 16);
-    for (size_t i = 0; i < at.size();) {
+    std::vector<std::pair<int64_t, int64_t>> &runs = p->hot_tiles;   // (tile, tones), starts and ends counted separately at first
+    for (int e = 0; e < 2; ++e) {
+        if (!sorted[e]) std::sort(at[e].begin(), at[e].end());
+        for (size_t i = 0; i < at[e].size();) {
+            size_t j = i;
+            while (j < at[e].size() && at[e][j] == at[e][i]) ++j;
+            runs.emplace_back(at[e][i], static_cast<int64_t>(j - i));
+            i = j;
+        }
+    }
+    // a tile can hold starts and ends: add them up, then keep the tiles at or above the threshold
+    std::sort(runs.begin(), runs.end());
+    size_t n_out = 0;
+    for (size_t i = 0; i < runs.size();) {
         size_t j = i;
-        while (j < at.size() && at[j] == at[i]) ++j;
-        if (j - i >= thr) p->hot_tiles.emplace_back(at[i], static_cast<int64_t>(j - i));
+        int64_t cnt = 0;
+        while (j < runs.size() && runs[j].first == runs[i].first) cnt += runs[j++].second;
+        if (static_cast<size_t>(cnt) >= thr) runs[n_out++] = std::make_pair(runs[i].first, cnt);
         i = j;
     }
+    runs.resize(n_out);
 }
 
 static void find_hot_tiles(awg_plan *p, int64_t n_begin, int64_t n_count, LaunchParams &lp)

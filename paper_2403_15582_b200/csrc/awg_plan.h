@@ -81,6 +81,7 @@ struct awg_plan {
     cudaEvent_t e2e_ready[kE2eSlots] = {}, e2e_done[kE2eSlots] = {};
     std::vector<std::pair<int64_t, int64_t>> hot_tiles;   // (absolute tile, tones) where many slow movers start or end a move at once
     bool hot_dirty = true;                  //   (listed again after a table change)
+    std::vector<int64_t> hot_scratch[2];
     bool e2e_ok = false;                    // all slots, streams and events exist
     // accounting
     int64_t h2d_bytes = 0, d2h_bytes = 0;
