@@ -155,8 +155,10 @@ awg_status awg_synthesize_range_host(awg_plan *p, int64_t first_chunk, int64_t n
  * four".  plans: host array of n_channels (1..8) distinct plans on the current device with
  * the same chunk_len, one independent tone set per channel.  Writes n_channels*chunk_len int16 to dev_out
  * (device, 16-byte aligned): dev_out[n_channels*i + c] = code of sample chunk_idx*chunk_len + i of
- * channel c -- bit for bit what awg_synthesize_chunk gives for plans[c].  One kernel launch per channel
- * on `stream`, each storing its channel's half-words of every group.  Errors: those of
+ * channel c -- bit for bit what awg_synthesize_chunk gives for plans[c].  One kernel launch per channel,
+ * each storing its channel's half-words of every group: channel 0 on `stream`, the others beside it on
+ * internal streams that fork from `stream` and join it again (to the caller everything is ordered on
+ * `stream`).  Errors: those of
  * awg_synthesize_chunk for any channel, checked before the first launch; INVALID_ARG (NULL, n_channels,
  * chunk_len mismatch, repeated plan). */
 awg_status awg_synthesize_chunk_mux(awg_plan *const *plans, int32_t n_channels, int64_t chunk_idx,

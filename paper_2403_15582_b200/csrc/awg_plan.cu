@@ -625,6 +625,12 @@ awg_status awg_plan_destroy(awg_plan *p)
     if (p->dev_aux_stage) cudaFree(p->dev_aux_stage);
     if (p->host_aux) cudaFreeHost(p->host_aux);
     free_e2e(p);
+    for (int i = 0; i < p->mux_n; ++i) {
+        cudaStreamSynchronize(p->mux_stream[i]);
+        cudaStreamDestroy(p->mux_stream[i]);
+        cudaEventDestroy(p->mux_join[i]);
+    }
+    if (p->mux_fork) cudaEventDestroy(p->mux_fork);
     delete p;
     return AWG_OK;
 }
@@ -921,13 +927,49 @@ awg_status awg_synthesize_chunk_mux(awg_plan *const *plans, int32_t n_channels, 
         awg_status st = check_chunk_call(plans[c], chunk_idx, 1, dev_out, 16);
         if (st != AWG_OK) return st;
     }
+    // Channel 0 runs on the caller's stream, the others beside it on streams of their own (forked from and joined back into
+    // the caller's stream with events): a channel of a few dozen tones is a launch of a few microseconds that uses a fraction
+    // of the SMs, and four of them back to back on one stream take four times as long as side by side.
+    awg_plan *p0 = plans[0];
+    cudaStream_t user = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    if (n_channels > 1) {
+        if (!p0->mux_fork && (e = cudaEventCreateWithFlags(&p0->mux_fork, cudaEventDisableTiming)) != cudaSuccess)
+            return fail_cuda(e, "cudaEventCreate(mux)");
+        while (p0->mux_n < n_channels - 1) {
+            const int i = p0->mux_n;
+            if ((e = cudaStreamCreateWithFlags(&p0->mux_stream[i], cudaStreamNonBlocking)) != cudaSuccess) return fail_cuda(e, "cudaStreamCreate(mux)");
+            if ((e = cudaEventCreateWithFlags(&p0->mux_join[i], cudaEventDisableTiming)) != cudaSuccess) {
+                cudaStreamDestroy(p0->mux_stream[i]);
+                p0->mux_stream[i] = nullptr;
+                return fail_cuda(e, "cudaEventCreate(mux)");
+            }
+            p0->mux_n = i + 1;
+        }
+        if ((e = cudaEventRecord(p0->mux_fork, user)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+    }
+    awg_status first_bad = AWG_OK;
+    int n_forked = 0;
     for (int c = 0; c < n_channels; ++c) {
         awg_plan *p = plans[c];
-        awg_status st = synthesize_samples(p, chunk_idx * p->chunk_len, p->chunk_len, dev_out, false, static_cast<cudaStream_t>(stream),
-                                           n_channels, c);
-        if (st != AWG_OK) return st;
+        cudaStream_t s = c == 0 ? user : p0->mux_stream[c - 1];
+        if (c > 0 && (e = cudaStreamWaitEvent(s, p0->mux_fork, 0)) != cudaSuccess) {
+            first_bad = fail_cuda(e, "cudaStreamWaitEvent");
+            break;
+        }
+        awg_status st = synthesize_samples(p, chunk_idx * p->chunk_len, p->chunk_len, dev_out, false, s, n_channels, c);
+        if (c > 0) n_forked = c;   // whatever was enqueued on the side stream is joined below, also after an error
+        if (st != AWG_OK) {
+            first_bad = st;
+            break;
+        }
     }
-    return AWG_OK;
+    for (int c = 1; c <= n_forked; ++c) {
+        if ((e = cudaEventRecord(p0->mux_join[c - 1], p0->mux_stream[c - 1])) != cudaSuccess ||
+            (e = cudaStreamWaitEvent(user, p0->mux_join[c - 1], 0)) != cudaSuccess)
+            return fail_cuda(e, "mux join");
+    }
+    return first_bad;
 }
 
 awg_status awg_set_scale(awg_plan *p, double scale)

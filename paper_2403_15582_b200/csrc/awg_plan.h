@@ -82,7 +82,11 @@ struct awg_plan {
     std::vector<std::pair<int64_t, int64_t>> hot_tiles;   // (absolute tile, tones) where many slow movers start or end a move at once
     bool hot_dirty = true;                  //   (listed again after a table change)
     std::vector<int64_t> hot_scratch[2];
-    bool e2e_ok = false;                    // all slots, streams and events exist
+    bool e2e_ok = false;
+    // awg_synthesize_chunk_mux, held by the plan of channel 0: channels 1.. run on these streams beside channel 0
+    cudaStream_t mux_stream[7] = {};
+    cudaEvent_t mux_fork = nullptr, mux_join[7] = {};
+    int mux_n = 0;                          // streams and join events created so far                    // all slots, streams and events exist
     // accounting
     int64_t h2d_bytes = 0, d2h_bytes = 0;
     int n_rings = 0;
