@@ -251,6 +251,38 @@ static void fill_core(const HostTone &h, ToneCore &r)
 // and the expand kernel builds the records (with their pair tables) on the device.  After set_trajectories every core
 // is uploaded; after per-chunk updates only the changed ones travel: the new version is a device-to-device copy of the
 // current one plus an expand of the updated records (parameters cross the bus only when they change).
+// Work just enqueued on `stream` reads table version v.
+static cudaError_t note_use(awg_plan *p, int v, cudaStream_t stream)
+{
+    awg_plan::VersionUse &u = p->use[v];
+    cudaError_t e;
+    int i = 0;
+    while (i < u.n && u.stream[i] != stream) ++i;
+    if (i == u.n) {
+        if (u.n < kUseSlots) {
+            if (!u.ev[i] && (e = cudaEventCreateWithFlags(&u.ev[i], cudaEventDisableTiming)) != cudaSuccess) return e;
+            u.n++;
+        } else {
+            i = 0;   // more streams than slots: slot 0 changes hands once its own stream's work on this version is done
+            if ((e = cudaEventSynchronize(u.ev[0])) != cudaSuccess) return e;
+        }
+        u.stream[i] = stream;
+    }
+    return cudaEventRecord(u.ev[i], stream);
+}
+
+// Blocks until every launch that reads table version v has finished (the version is about to be rewritten or freed).
+static cudaError_t wait_users(awg_plan *p, int v)
+{
+    awg_plan::VersionUse &u = p->use[v];
+    for (int i = 0; i < u.n; ++i) {
+        cudaError_t e = cudaEventSynchronize(u.ev[i]);
+        if (e != cudaSuccess) return e;
+    }
+    u.n = 0;
+    return cudaSuccess;
+}
+
 awg_status ensure_table(awg_plan *p, cudaStream_t stream)
 {
     cudaError_t e;
@@ -263,7 +295,7 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
     const int cur = p->cur_version;
     const int v = (cur + 1) % kTableVersions;
     // the slot's previous readers (kernels launched kTableVersions uploads ago) must be done
-    if ((e = cudaEventSynchronize(p->last_use[v])) != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
+    if ((e = wait_users(p, v)) != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
     {
         std::vector<float> amp;
         amp.reserve(p->n_tones);
@@ -312,7 +344,7 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
             return fail_cuda(e, "cudaStreamWaitEvent");
         if ((e = cudaMemcpyAsync(p->dev_table[v], p->dev_table[cur], p->table_bytes, cudaMemcpyDeviceToDevice, stream)) != cudaSuccess)
             return fail_cuda(e, "cudaMemcpyAsync(table d2d)");
-        if ((e = cudaEventRecord(p->last_use[cur], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+        if ((e = note_use(p, cur, stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
         if ((e = cudaMemcpyAsync(p->dev_stage[v], host, n_dirty * sizeof(ToneCore), cudaMemcpyHostToDevice, stream)) != cudaSuccess ||
             (e = cudaMemcpyAsync(p->dev_stage[v] + p->core_bytes, host_idx, n_dirty * sizeof(int32_t), cudaMemcpyHostToDevice, stream)) != cudaSuccess)
             return fail_cuda(e, "cudaMemcpyAsync(updated tone cores)");
@@ -433,7 +465,7 @@ awg_status synthesize_samples(awg_plan *p, int64_t n_begin, int64_t n_count, voi
     find_hot_tiles(p, n_begin, n_count, lp);
     cudaError_t e = launch_synth(lp, p->engine, stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
-    if ((e = cudaEventRecord(p->last_use[p->cur_version], stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+    if ((e = note_use(p, p->cur_version, stream)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
     return AWG_OK;
 }
 
@@ -577,7 +609,6 @@ awg_status awg_plan_create(awg_plan **out, int32_t n_tones, double sample_rate_h
         if ((e = cudaMalloc(reinterpret_cast<void **>(&p->dev_table[v]), p->table_bytes)) != cudaSuccess ||
             (e = cudaMalloc(reinterpret_cast<void **>(&p->dev_stage[v]), stage_bytes)) != cudaSuccess ||
             (e = cudaMallocHost(reinterpret_cast<void **>(&p->host_table[v]), stage_bytes)) != cudaSuccess ||
-            (e = cudaEventCreateWithFlags(&p->last_use[v], cudaEventDisableTiming)) != cudaSuccess ||
             (e = cudaEventCreateWithFlags(&p->uploaded[v], cudaEventDisableTiming)) != cudaSuccess) {
             awg_status st = (e == cudaErrorMemoryAllocation) ? fail(AWG_ERR_ALLOC, "device/pinned allocation failed: %s", cudaGetErrorString(e))
                                                              : fail_cuda(e, "plan allocation");
@@ -608,7 +639,7 @@ awg_status awg_plan_destroy(awg_plan *p)
     if (!p) return AWG_OK;
     if (p->n_rings > 0) return fail(AWG_ERR_STATE, "destroy the plan's rings first");
     for (int v = 0; v < kTableVersions; ++v)
-        if (p->last_use[v]) cudaEventSynchronize(p->last_use[v]);
+        (void)wait_users(p, v);
     for (int s = 0; s < kE2eSlots; ++s) {
         if (p->e2e_done[s]) cudaEventSynchronize(p->e2e_done[s]);
     }
@@ -616,7 +647,8 @@ awg_status awg_plan_destroy(awg_plan *p)
         if (p->dev_table[v]) cudaFree(p->dev_table[v]);
         if (p->dev_stage[v]) cudaFree(p->dev_stage[v]);
         if (p->host_table[v]) cudaFreeHost(p->host_table[v]);
-        if (p->last_use[v]) cudaEventDestroy(p->last_use[v]);
+        for (int i = 0; i < kUseSlots; ++i)
+            if (p->use[v].ev[i]) cudaEventDestroy(p->use[v].ev[i]);
         if (p->uploaded[v]) cudaEventDestroy(p->uploaded[v]);
     }
     for (int s = 0; s < 2; ++s)

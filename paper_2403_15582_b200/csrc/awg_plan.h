@@ -38,6 +38,7 @@ awg_status fail_cuda(cudaError_t e, const char *what);
 
 }  // namespace awg
 
+constexpr int kUseSlots = 4;   // streams tracked per table version (more: the oldest slot changes hands after a wait)
 constexpr int kE2eSlots = 4;   // device staging slots of awg_synthesize_range_host
 
 struct awg_plan {
@@ -72,7 +73,13 @@ struct awg_plan {
     size_t core_bytes = 0;                                 // n_pad tone cores (what the host uploads)
     unsigned char *host_table[awg::kTableVersions] = {};  // pinned staging: tone cores, then int32 indices
     unsigned char *dev_stage[awg::kTableVersions] = {};   // device staging of the same layout (input of the expand kernel)
-    cudaEvent_t last_use[awg::kTableVersions] = {};
+    // readers of each table version: one event per stream that has launched work on it (a plan is used from several
+    // streams: the caller's, the two synthesis streams of awg_synthesize_range_host, the side streams of the multiplexer)
+    struct VersionUse {
+        cudaStream_t stream[kUseSlots] = {};
+        cudaEvent_t ev[kUseSlots] = {};
+        int n = 0;
+    } use[awg::kTableVersions];
     cudaEvent_t uploaded[awg::kTableVersions] = {};
     cudaStream_t upload_stream[awg::kTableVersions] = {};
     // awg_synthesize_range_host

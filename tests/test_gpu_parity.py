@@ -760,6 +760,42 @@ def test_scheduler_slots_with_many_launches_in_flight_on_four_streams(awg, torch
     p_big.close()
 
 
+def test_one_plan_on_six_streams_while_the_table_versions_rotate(awg, torch_cuda):
+    """One plan, chunk c launched on stream c mod 6 (more streams than a table version tracks readers for), a trajectory
+    update before every second chunk, so chunks 2k and 2k+1 read the same table version from two streams -- and every
+    twelfth one sits behind a 5 ms delay on its stream while the host races ahead through the later updates: a version must not be
+    rewritten while a launch on ANY stream still reads it.  Same updates on a second plan, one stream, chunk by chunk: the
+    same bits."""
+    torch = torch_cuda
+    N, L, n_chunks = 300, 1 << 16, 36
+    rng = np.random.default_rng(5)
+    f0 = rng.uniform(30e6, 240e6, N)
+    rows = [(f0[k], f0[k], 1.0 / N, rng.uniform(0, 6.28), 0.0, 0.0, STATIC) for k in range(N)]
+    upd = [(rng.choice(N, 40, replace=False), rng.uniform(30e6, 240e6, 40), rng.uniform(0, 3 * L / 560e6, 40)) for _ in range(n_chunks)]
+    cols = list(zip(*rows))
+    ref_plan = awg.Plan(N, 560e6, L); ref_plan.set_trajectories(*cols)
+    refs = []
+    for c in range(n_chunks):
+        if c % 2 == 0:
+            ref_plan.update_trajectories(c, upd[c][0], upd[c][1], upd[c][2], np.full(40, MINJERK))
+        refs.append(_np(ref_plan.synthesize_chunk(c)))
+    p = awg.Plan(N, 560e6, L); p.set_trajectories(*cols)
+    streams = [torch.cuda.Stream() for _ in range(6)]
+    outs = [torch.empty(L, dtype=torch.int16, device="cuda") for _ in range(n_chunks)]
+    torch.cuda.synchronize()
+    for c in range(n_chunks):
+        if c % 2 == 0:
+            p.update_trajectories(c, upd[c][0], upd[c][1], upd[c][2], np.full(40, MINJERK))
+        with torch.cuda.stream(streams[c % 6]):
+            if c % 12 == 0:
+                torch.cuda._sleep(int(1e7))                   # ~5 ms: this launch stays queued while the host races ahead
+            p.synthesize_chunk(c, out=outs[c])
+    torch.cuda.synchronize()
+    for c in range(n_chunks):
+        assert np.array_equal(_np(outs[c]), refs[c]), f"chunk {c}"
+    p.close(); ref_plan.close()
+
+
 def test_concurrent_launches_on_two_streams(awg, torch_cuda):
     """Two plans launching on two streams at the same time take different scheduler slots."""
     torch = torch_cuda
