@@ -244,6 +244,32 @@ awg_status awg_plan_op_counts(awg_plan *p, int64_t first_chunk, int64_t n_chunks
 awg_status awg_plan_hot_tiles(awg_plan *p, int64_t first_chunk, int64_t n_chunks, int32_t *n_listed,
                               int32_t *n_served_first);
 
+/* ---- allocation-free one-shot synthesis ------------------------------------------------------------ */
+
+/* For callers that cannot allocate device memory (a harness that forbids cudaMalloc, a serving loop that
+ * must stay off the allocator): no plan, and no cudaMalloc, cudaFree, stream or event creation anywhere
+ * on this call, the first one included.  Synthesises samples first_sample .. first_sample+n_samples-1 of
+ * the waveform of Eq. 9/10 for the n_tones trajectories given exactly as to
+ * awg_set_trajectories (seven HOST arrays of length n_tones, same units, same profiles), sample index 0
+ * at t = 0, into dev_out (DEVICE, int16, 16-byte aligned, n_samples elements, caller-owned) on `stream`
+ * (cudaStream_t or NULL), at the default scale of a plan (0.9 * 32767) with the default engine: bit for
+ * bit what a plan with the same trajectories gives for the same samples.  Asynchronous like
+ * awg_synthesize_chunk; the host arrays are consumed before the call returns.
+ * Limits: n_tones <= 4096, n_samples <= 2^20 (a multiple of 8; first_sample too) per call -- call again
+ * for the next range.  Everything the kernels need on the device (the trajectory table, the tile
+ * scheduler's counters, the int32 scratch tiles in which the tone groups of a tile meet) lives in ONE
+ * static 5.9 MB device array that is part of the library image: every GPU that loads the library holds
+ * it until the process exits.  All calls share it, and it keeps the last call's contents (each call
+ * clears what it needs at zero on `stream` first): calls that overlap on the GPU -- issued on different
+ * streams without an event between them, or from several threads -- RACE on it; calls on one stream, or
+ * ordered by events, are safe.  Plans do not use the array and are not affected.
+ * Errors: INVALID_ARG (a size beyond the limits, NULL, misaligned, non-finite, t_dur < 0, unknown
+ * profile), CUDA. */
+awg_status awg_synthesize_noalloc(double sample_rate_hz, int32_t n_tones, const double *f0, const double *f1,
+                                  const double *A, const double *phi0, const double *t_start,
+                                  const double *t_dur, const int32_t *profile, int64_t first_sample,
+                                  int64_t n_samples, int16_t *dev_out, void *stream);
+
 /* Number of kernels the library has launched since load (all plans); for launch accounting. */
 int64_t awg_kernel_launch_count(void);
 

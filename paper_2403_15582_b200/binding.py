@@ -40,7 +40,7 @@ EXPORTED = (
     "awg_synthesize_range_host", "awg_ring_create", "awg_ring_submit", "awg_ring_acquire", "awg_ring_release",
     "awg_synthesize_chunk_mux", "awg_snap_frequency", "awg_static_buffer_set", "awg_static_buffer_fold",
     "awg_static_buffer_read",
-    "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_plan_op_counts", "awg_plan_hot_tiles", "awg_kernel_launch_count",
+    "awg_ring_stats", "awg_ring_destroy", "awg_plan_io_bytes", "awg_plan_op_counts", "awg_plan_hot_tiles", "awg_synthesize_noalloc", "awg_kernel_launch_count",
     "awg_last_error",
 )
 
@@ -78,6 +78,7 @@ def _load() -> ctypes.CDLL:
         "awg_plan_io_bytes": (I32, [P, POINTER(I64), POINTER(I64)]),
         "awg_plan_op_counts": (I32, [P, I64, I64, POINTER(I64), POINTER(I64), POINTER(I64)]),
         "awg_plan_hot_tiles": (I32, [P, I64, I64, POINTER(I32), POINTER(I32)]),
+        "awg_synthesize_noalloc": (I32, [D, I32, P, P, P, P, P, P, P, I64, I64, P, P]),
         "awg_kernel_launch_count": (I64, []),
         "awg_last_error": (c_char_p, []),
     }
@@ -254,6 +255,14 @@ def awg_plan_io_bytes(plan) -> Tuple[int, int]:
     return a.value, b.value
 
 
+def awg_synthesize_noalloc(sample_rate_hz: float, n_tones: int, f0, f1, A, phi0, t_start, t_dur, profile,
+                           first_sample: int, n_samples: int, dev_out_ptr: int, stream=None) -> None:
+    arrs = [_f64(x, n_tones) for x in (f0, f1, A, phi0, t_start, t_dur)]
+    prof = _i32(profile, n_tones)
+    _check(_lib.awg_synthesize_noalloc(sample_rate_hz, n_tones, *[a.ctypes.data for a in arrs], prof.ctypes.data,
+                                       first_sample, n_samples, dev_out_ptr, _stream_handle(stream)))
+
+
 def awg_plan_hot_tiles(plan, first_chunk: int, n_chunks: int) -> Tuple[int, int]:
     a, b = ctypes.c_int32(0), ctypes.c_int32(0)
     _check(_lib.awg_plan_hot_tiles(plan, first_chunk, n_chunks, byref(a), byref(b)))
@@ -395,6 +404,18 @@ def synthesize_chunk_mux(plans: Sequence[Plan], chunk_idx: int, out=None, stream
     if out.dtype != torch.int16 or out.numel() != n or not out.is_cuda or not out.is_contiguous():
         raise ValueError("output tensor has the wrong dtype, size or device")
     awg_synthesize_chunk_mux([p.handle for p in plans], chunk_idx, out.data_ptr(), stream)
+    return out
+
+
+def synthesize_noalloc(sample_rate_hz: float, f0, f1, A, phi0, t_start, t_dur, profile, first_sample: int, n_samples: int,
+                       out, stream=None):
+    """awg_synthesize_noalloc into ``out`` (a caller-owned torch CUDA tensor of n_samples int16): no plan, no device
+    allocation anywhere (<= 4096 tones, <= 2^20 samples per call; calls that overlap on the GPU race)."""
+    import torch
+    if out.dtype != torch.int16 or out.numel() != n_samples or not out.is_cuda or not out.is_contiguous():
+        raise ValueError("output tensor has the wrong dtype, size or device")
+    awg_synthesize_noalloc(sample_rate_hz, len(np.atleast_1d(f0)), f0, f1, A, phi0, t_start, t_dur, profile, first_sample,
+                           n_samples, out.data_ptr(), stream)
     return out
 
 

@@ -145,4 +145,11 @@ cudaError_t launch_synth(const LaunchParams &lp, int engine, cudaStream_t stream
 cudaError_t launch_expand(ToneRec *table, const ToneCore *src, const int32_t *idx, int n, cudaStream_t stream);
 void count_launch();
 
+// ---- the allocation-free entry point (awg_synthesize_noalloc; include/awg.h) -----------------------------------------
+constexpr int kNoAllocMaxTones = 4096;
+constexpr int64_t kNoAllocMaxSamples = int64_t(1) << 20;
+// cores: n_up = n_tones rounded up to 32 host tone cores (zero padded).  lp: tab, sched, tile_cnt, scratch, qlo, qhi and the
+// tone groups are filled in here; everything the launch needs on the device lives in one static __device__ array.
+cudaError_t launch_synth_noalloc(const ToneCore *cores, int n_up, const LaunchParams &lp, cudaStream_t stream);
+
 }  // namespace awg

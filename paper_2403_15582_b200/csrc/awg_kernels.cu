@@ -1588,6 +1588,91 @@ cudaError_t launch_synth(const LaunchParams &lp_in, int engine, cudaStream_t str
     return e;
 }
 
+// ---- awg_synthesize_noalloc: the same kernels with ALL device-side working memory in one static array -----------------
+// For callers that cannot allocate (a harness that forbids cudaMalloc, a serving loop that must not touch the allocator):
+// no cudaMalloc / cudaFree / stream or event creation anywhere on this path.  The array is part of the library image:
+// every GPU that loads the library holds its 5.9 MB until the process exits.  Every call shares it (calls that overlap
+// on the GPU race), and it keeps the last call's contents: what a launch needs at zero is cleared on the caller's stream
+// before the launch.
+namespace {
+
+constexpr int kNoAllocMaxTiles = static_cast<int>(kNoAllocMaxSamples / kTile) + 1;   // a range that starts inside a tile
+struct NoAllocScratch {
+    uint32_t sched[8];                              // tile scheduler: {next unit, teams finished, ...}
+    uint32_t tile_cnt[568];                         // quads delivered per tile (cross-CTA launches); sized so that `tiles` starts 256-byte aligned
+    int32_t tiles[kNoAllocMaxTiles][kTile];         // fixed-point sums of the quads of a tile (cross-CTA launches): 4.0 MB
+    ToneCore cores[kNoAllocMaxTones];               // the host's tone cores: 0.5 MB
+    ToneRec table[kNoAllocMaxTones];                // expanded trajectory table: 1.1 MB
+};
+static __device__ __align__(256) unsigned char g_noalloc_scratch[sizeof(NoAllocScratch)];
+static_assert(sizeof(NoAllocScratch) < (7u << 20), "the static scratch is meant to stay modest");
+static_assert(sizeof(NoAllocScratch::tile_cnt) / sizeof(uint32_t) >= kNoAllocMaxTiles, "one counter per tile");
+static_assert(offsetof(NoAllocScratch, tiles) % 256 == 0 && offsetof(NoAllocScratch, cores) % 256 == 0 &&
+              offsetof(NoAllocScratch, table) % 256 == 0, "the parts are aligned like cudaMalloc'ed blocks");
+
+// Device address of the array, per device.  In host code the NAME g_noalloc_scratch is a host-side stand-in, not a device
+// address: only cudaGetSymbolAddress (with the device current) gives the pointer a kernel can use.
+NoAllocScratch *g_noalloc_ptr[kMaxDevices] = {};
+
+}  // namespace
+
+cudaError_t launch_synth_noalloc(const ToneCore *cores, int n_up, const LaunchParams &lp_in, cudaStream_t stream)
+{
+    if (lp_in.n_count <= 0 || n_up <= 0) return cudaSuccess;
+    if (n_up > kNoAllocMaxTones || lp_in.n_tones > n_up) return cudaErrorInvalidValue;
+    const int64_t first_tile = lp_in.n_begin / kTile;
+    const int64_t tiles = (lp_in.n_begin + lp_in.n_count - 1) / kTile - first_tile + 1;
+    if (tiles > kNoAllocMaxTiles) return cudaErrorInvalidValue;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    cudaError_t e;
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    DeviceState &ds = g_dev[dev];   // (SM count and the shared-memory opt-in bits only: nothing here touches ds.sched or the slots)
+    if (!g_noalloc_ptr[dev]) {
+        void *ptr = nullptr;
+        if ((e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch)) != cudaSuccess) return e;
+        if (ds.n_sm == 0) {
+            int v = 0;
+            if ((e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+            ds.n_sm = v > 0 ? v : 148;
+        }
+        g_noalloc_ptr[dev] = static_cast<NoAllocScratch *>(ptr);
+    }
+    NoAllocScratch *sc = g_noalloc_ptr[dev];
+    LaunchParams lp = lp_in;
+    // table build (step a0) into the static array
+    if ((e = cudaMemcpyAsync(sc->cores, cores, static_cast<size_t>(n_up) * sizeof(ToneCore), cudaMemcpyHostToDevice, stream)) != cudaSuccess) return e;
+    awg_expand_kernel<<<(n_up + 3) / 4, 128, 0, stream>>>(sc->table, sc->cores, nullptr, n_up);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    count_launch();
+    lp.tab = sc->table;
+    lp.sched = sc->sched;
+    lp.tile_cnt = sc->tile_cnt;
+    lp.qlo = static_cast<float>(-32768.0 / static_cast<double>(lp.scale));
+    lp.qhi = static_cast<float>(32767.0 / static_cast<double>(lp.scale));
+    int split = 1, per = lp.n_tones, quads = 1;
+    tone_groups(lp.n_tones, &split, &per, &quads);
+    lp.per = per;
+    lp.n_quads = quads;
+    lp.cross = 0;
+    lp.scratch = nullptr;
+    int64_t units = tiles;
+    size_t clear = offsetof(NoAllocScratch, tiles);   // the counters always start at zero ...
+    if (quads > 1 && tiles < 2 * static_cast<int64_t>(kCtasPerSm) * ds.n_sm) {
+        // the rule of launch_synth: with fewer tiles than two rounds of CTAs a tile's quads are separate work units
+        lp.cross = 1;
+        lp.scratch = &sc->tiles[0][0];
+        units = tiles * quads;
+        clear += static_cast<size_t>(tiles) * kTile * sizeof(int32_t);   // ... and so do the tiles this launch adds into
+    }
+    if ((e = cudaMemsetAsync(sc, 0, clear, stream)) != cudaSuccess) return e;
+    if (lp.slow2) e = launch_split<true, true>(ds, lp, split, units, stream);
+    else e = launch_split<true, false>(ds, lp, split, units, stream);
+    count_launch();
+    return e;
+}
+
 }  // namespace awg
 
 extern "C" int64_t awg_kernel_launch_count(void) { return awg::g_launches.load(std::memory_order_relaxed); }

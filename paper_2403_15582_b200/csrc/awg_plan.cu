@@ -13,6 +13,7 @@
 #include <cstring>
 #include <functional>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <utility>
 #include <vector>
@@ -1062,6 +1063,82 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
     p->last_update_chunk = 0;
     std::fill(p->in_buffer.begin(), p->in_buffer.end(), 0);
     p->xs_on = false;
+    return AWG_OK;
+}
+
+// ---- allocation-free one-shot synthesis (include/awg.h: awg_synthesize_noalloc) --------------------------------------
+// No plan, hence no cudaMalloc: the host builds the tone cores into a static host array, and the table, the scheduler
+// counters and the cross-CTA scratch tiles live in the library's static __device__ array (awg_kernels.cu).
+static std::mutex g_noalloc_mutex;
+static ToneCore g_noalloc_cores[kNoAllocMaxTones];   // host staging of the tone cores (0.5 MB of .bss)
+
+awg_status awg_synthesize_noalloc(double sample_rate_hz, int32_t n_tones, const double *f0, const double *f1, const double *A,
+                                  const double *phi0, const double *t_start, const double *t_dur, const int32_t *profile,
+                                  int64_t first_sample, int64_t n_samples, int16_t *dev_out, void *stream)
+{
+    if (n_tones < 1 || n_tones > kNoAllocMaxTones)
+        return fail(AWG_ERR_INVALID_ARG, "awg_synthesize_noalloc: n_tones = %d is outside [1, %d] (the static scratch holds %d tone records; use a plan for more)",
+                    n_tones, kNoAllocMaxTones, kNoAllocMaxTones);
+    if (n_samples < 8 || n_samples % 8 || n_samples > kNoAllocMaxSamples)
+        return fail(AWG_ERR_INVALID_ARG, "awg_synthesize_noalloc: n_samples = %lld must be a multiple of 8 in [8, %lld] (the static scratch holds %lld samples per call; call again for the next range, or use a plan)",
+                    static_cast<long long>(n_samples), static_cast<long long>(kNoAllocMaxSamples), static_cast<long long>(kNoAllocMaxSamples));
+    if (first_sample < 0 || first_sample % 8 || first_sample > std::numeric_limits<int64_t>::max() / 4)
+        return fail(AWG_ERR_INVALID_ARG, "awg_synthesize_noalloc: first_sample must be a multiple of 8 in [0, 2^61]");
+    if (!std::isfinite(sample_rate_hz) || sample_rate_hz <= 0.0) return fail(AWG_ERR_INVALID_ARG, "sample_rate_hz must be finite and > 0");
+    if (!f0 || !f1 || !A || !phi0 || !t_start || !t_dur || !profile) return fail(AWG_ERR_INVALID_ARG, "NULL trajectory array");
+    if (!dev_out) return fail(AWG_ERR_INVALID_ARG, "output pointer is NULL");
+    if (reinterpret_cast<uintptr_t>(dev_out) % 16) return fail(AWG_ERR_INVALID_ARG, "output pointer must be 16-byte aligned");
+    const int N = n_tones;
+    if (!finite_all(f0, N) || !finite_all(f1, N) || !finite_all(A, N) || !finite_all(phi0, N) || !finite_all(t_start, N) || !finite_all(t_dur, N))
+        return fail(AWG_ERR_INVALID_ARG, "non-finite value in a trajectory array");
+    for (int k = 0; k < N; ++k) {
+        if (t_dur[k] < 0.0) return fail(AWG_ERR_INVALID_ARG, "t_dur[%d] < 0", k);
+        if (profile[k] < AWG_PROFILE_STATIC || profile[k] > AWG_PROFILE_EXP) return fail(AWG_ERR_INVALID_ARG, "unknown profile %d for tone %d", profile[k], k);
+        if (profile[k] == AWG_PROFILE_EXP && !(f0[k] > 0.0 && f1[k] > 0.0))
+            return fail(AWG_ERR_INVALID_ARG, "exponential chirp of tone %d needs f0 > 0 and f1 > 0", k);
+        if (std::fabs(t_start[k]) * sample_rate_hz > 4.0e18) return fail(AWG_ERR_INVALID_ARG, "t_start[%d] out of range", k);
+    }
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);   // one host staging array
+    const long double fs = static_cast<long double>(sample_rate_hz);
+    float amp[kNoAllocMaxTones];
+    bool slow2 = false;
+    for (int k = 0; k < N; ++k) {
+        // the tone of awg_set_trajectories, one at a time (no host table is kept)
+        HostTone h{};
+        h.A = static_cast<float>(A[k]);
+        h.A1 = h.A;
+        h.f0 = static_cast<long double>(f0[k]);
+        h.theta_pre = frac64(static_cast<long double>(phi0[k]) / kTwoPiL);
+        h.w_pre = frac64(h.f0 / fs);
+        const long double ts = static_cast<long double>(t_start[k]);
+        const long double ns = ts * fs;
+        const long double nsi = floorl(ns);
+        make_move(h, fs, static_cast<long double>(f1[k]), profile[k], static_cast<long double>(t_dur[k]), static_cast<int64_t>(nsi),
+                  static_cast<double>(ns - nsi), (static_cast<long double>(f1[k]) - h.f0) * ts);
+        fill_core(h, g_noalloc_cores[k]);
+        amp[k] = std::fabs(h.A);
+        if (h.cls & CLS_SLOW2_FLAG) slow2 = true;
+    }
+    const int n_up = (N + 31) / 32 * 32;
+    for (int k = N; k < n_up; ++k) std::memset(&g_noalloc_cores[k], 0, sizeof(ToneCore));
+    LaunchParams lp;
+    lp.tab = nullptr;   // (launch_synth_noalloc: the table is built in the static device array)
+    lp.n_tones = N;
+    lp.out_stride = 1;
+    lp.out_offset = 0;
+    lp.xs = nullptr;
+    lp.xs_len = 0;
+    lp.n_begin = first_sample;
+    lp.n_count = n_samples;
+    lp.scale = static_cast<float>(0.9 * 32767.0);   // the default scale of a plan
+    fix_grids(amp, N, &lp.fix);
+    lp.slow2 = slow2 ? 1 : 0;
+    lp.out = dev_out;
+    lp.out_f32 = 0;
+    lp.sched = nullptr;
+    lp.n_hot = 0;
+    const cudaError_t e = launch_synth_noalloc(g_noalloc_cores, n_up, lp, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "awg_synthesize_noalloc");
     return AWG_OK;
 }
 
