@@ -820,7 +820,7 @@ def test_concurrent_launches_on_two_streams(awg, torch_cuda):
 def test_random_soak_against_the_oracle(awg, torch_cuda, seed):
     """Forty random plans per seed: tone counts around every grouping boundary (team split at 10 / 20 tones, leaves above 256,
     quad boundaries, 128-tone leaves above 2048), ragged and tiny chunk lengths, signed amplitudes, a random mix of static
-    tones, slow movers (both slow classes), fast movers, instant retunes; both engines.  A random window of every case is
+    tones, slow movers (both slow classes), fast movers, instant retunes, short and long exponential chirps; both engines.  A random window of every case is
     compared with the oracle at the usual bars (fp32 bar scaled by max(1, sum |A|)), and the range launch over all chunks must
     equal the chunk launches bit for bit (they can take the one-CTA and the cross-CTA path)."""
     fs = 560e6
@@ -832,9 +832,13 @@ def test_random_soak_against_the_oracle(awg, torch_cuda, seed):
         rows = []
         for k in range(n):
             f0, A, ph = rng.uniform(5e6, 270e6), rng.uniform(-1, 1) / n, rng.uniform(0, 6.28)
-            kind = rng.integers(0, 5)
+            kind = rng.integers(0, 7)
             if kind == 0:
                 rows.append((f0, f0, A, ph, 0.0, 0.0, STATIC))
+            elif kind == 5:
+                rows.append((f0, f0 * rng.uniform(0.5, 2.0), A, ph, rng.uniform(-0.2 * span, span), rng.uniform(1e-7, span), W.PROFILE_EXP))
+            elif kind == 6:
+                rows.append((f0, f0 * rng.uniform(0.97, 1.03), A, ph, rng.uniform(-span, 0), rng.uniform(1e-3, 20e-3), W.PROFILE_EXP))
             elif kind == 1:
                 rows.append((f0, f0 + rng.uniform(-3e6, 3e6), A, ph, rng.uniform(-span, 0), rng.uniform(5e-3, 40e-3), MINJERK if k % 2 else LINEAR))
             elif kind == 2:
