@@ -59,7 +59,8 @@ enum {
     AWG_PROFILE_LINEAR = 1,  /* f0 -> f1 linearly over [t_start, t_start + t_dur]            */
     AWG_PROFILE_MINJERK = 2, /* f0 -> f1 along the minimum-jerk quintic 10s^3 - 15s^4 + 6s^5 */
     AWG_PROFILE_EXP = 3      /* exponential chirp f(tau) = f0 (f1/f0)^(tau/t_dur) (named at PAPER.md:137; G20):
-                                f0 and f1 must be > 0.  Evaluated in fp64 per sample inside the move (exact path)   */
+                                f0 and f1 must be > 0.  Costs what a minimum-jerk move costs (one sine per sample
+                                inside the move); chirps too fast for fp32 coefficients take the fp64 path         */
 };
 
 /* sine engine of the synthesis kernel (step a3 of the hot path) */

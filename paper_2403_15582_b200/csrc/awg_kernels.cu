@@ -200,19 +200,104 @@ enum : int {
     K_SBEG = 4,    // the move starts inside this block: pre-move carrier + P(max(k - kb, 0))
     K_SEND = 5,    // the move ends inside this block:  post-move carrier + P(max(kb - k, 0))
     K_EXACT = 6,   // anything else (both ends in one block, T = 0, CLS_EXACT tones): fp64 per sample
-    K_COUNT = 7
+    K_XEDGE = 7,   // an exponential chirp starts or ends inside this block: carrier valid outside + P(max(+-(k - kb), 0))
+    K_COUNT = 8
 };
 
 // One re-centred (tone, block) record:
 //   phase(k) = c0 + c1*k [u32 turns, wrapping] + poly(k) [radians, fp32],  k = n - block centre
 //   K_QUAD..K_DEG6: poly = k^2 (c2 + k (c3 + k (c4 + k (c5 + k c6))))     (Taylor series about the block centre)
 //   K_SBEG/K_SEND:  poly = w^2 (c2 + w^2 (c3 + w (c4 + w c5))), w = max(+-(k - kb), 0), c6 = +-kb
+//   K_XEDGE:        poly = w^2 (c2 + w (c3 + w c4)), w = max(c5 k - c6, 0), c5 = +-1, c6 = +-kb
 struct BlockRec {
     uint32_t c0, c1;
     float A;
     float c2, c3, c4, c5, c6;
     int kind;
 };
+
+// Exponential chirp f0 e^(L s), s = u/Tn (G20): the (tone, block) record of a tone of that profile (class below
+// CLS_EXACT).  Kept out of line and self-contained (it loads the core itself): the fp64 exponentials are needed for these
+// tones only and must weigh neither on the registers nor on the schedule of block_prologue().
+// q[0..3] of the core hold F = f0 T (cycles) and L = ln(f1/f0) as doubles; nc = the block's centre, bb_d = its first sample.
+struct ExpRec {
+    uint32_t c0, c1;
+    float c2, c3, c4, c5, c6;
+    int kind;
+};
+__device__ __noinline__ ExpRec exp_block(const ToneRec *rec, int c, uint64_t nc, double bb_d)
+{
+    const ToneCore &t = rec->core;
+    ExpRec r;
+    r.c2 = r.c3 = r.c4 = r.c5 = r.c6 = 0.f;
+    r.kind = K_STATIC;
+    const double ua = (bb_d - t.ns_int) - t.ns_frac;   // u of the block's first sample
+    const double ub = ua + static_cast<double>(kBlock - 1);
+    const double Tn = t.Tn, rT = t.inv_Tn;
+    uint64_t ph, w;
+    if (ub <= 0.0) {
+        w = t.w_pre;
+        ph = t.theta_pre + w * nc;
+    } else if (ua >= Tn) {
+        w = t.w_post;
+        ph = t.theta_post + w * nc;
+    } else if (ua < 0.0 && ub > Tn) {
+        r.kind = K_EXACT;   // (the caller stores the tone index)
+        r.c0 = r.c1 = 0;
+        return r;
+    } else {
+        const double F = *reinterpret_cast<const double *>(&t.q[0]), L = *reinterpret_cast<const double *>(&t.q[2]);
+        const double f0s = F * rT;   // f0/fs, cycles per sample
+        if (ua < 0.0 || ub > Tn) {
+            // One end of the move inside the block.  With w the (clamped) distance into the move from that end the phase
+            // over the carrier valid outside is a power series that starts at w^2:
+            //   start: f0/fs sum_k a^(k-1) w^k / k!     end: -f1/fs sum_k (-a)^(k-1) w^k / k!     (k >= 2; cycles; a = L/Tn)
+            // kept up to w^4 (classify_exp bounds the rest over a whole block).
+            const bool at_end = !(ua < 0.0);
+            const float a = static_cast<float>(at_end ? -(L * rT) : L * rT);
+            float ck = static_cast<float>(6.283185307179586 * (at_end ? -(f0s * exp(L)) : f0s)) * a * 0.5f;
+            r.c2 = ck;
+            ck *= a * (1.f / 3.f); r.c3 = ck;
+            ck *= a * 0.25f; r.c4 = ck;
+            r.kind = K_XEDGE;
+            if (!at_end) {
+                r.c5 = 1.f;
+                r.c6 = static_cast<float>(-(ua + static_cast<double>(kHalf)));
+                w = t.w_pre;
+                ph = t.theta_pre + w * nc;
+            } else {
+                r.c5 = -1.f;
+                r.c6 = static_cast<float>(-(Tn - ua - static_cast<double>(kHalf)));
+                w = t.w_post;
+                ph = t.theta_post + w * nc;
+            }
+        } else {
+            // Whole block inside the move: phase and frequency at the block centre in fp64 (one expm1); the Taylor coefficients
+            // of the phase are a geometric sequence, c_k = 2 pi (f/fs) a^(k-1) / k!.
+            const double s = (ua + static_cast<double>(kHalf)) * rT;
+            const double em = expm1(L * s);
+            w = t.w_pre + frac_to_fix64(f0s * em);
+            ph = t.theta_pre + t.w_pre * nc + frac_to_fix64(F * (em / L - s));
+            const float a = static_cast<float>(L * rT);
+            float ck = static_cast<float>(6.283185307179586 * f0s * (em + 1.0)) * a * 0.5f;
+            r.c2 = ck;
+            r.kind = K_QUAD;
+            if (c >= CLS_DEG4) {
+                ck *= a * (1.f / 3.f); r.c3 = ck;
+                ck *= a * 0.25f; r.c4 = ck;
+                r.kind = K_DEG4;
+                if (c >= CLS_DEG6) {
+                    ck *= a * 0.2f; r.c5 = ck;
+                    ck *= a * (1.f / 6.f); r.c6 = ck;
+                    r.kind = K_DEG6;
+                }
+            }
+        }
+    }
+    r.c0 = round32(ph);
+    r.c1 = round32(w);
+    return r;
+}
 
 // Step a1.  Lane-private: tone record `rec` (index t) at the block whose first sample is blk_base (absolute);
 // bb_d = (double)blk_base, nc = blk_base + kHalf.
@@ -246,6 +331,14 @@ __device__ __forceinline__ BlockRec block_prologue(const ToneRec *rec, int t, ui
             r.c1 = 0;
             return r;
         }
+    }
+    if (c != CLS_STATIC && c != CLS_EXACT && ((cls >> 8) & 0xff) == AWG_PROFILE_EXP) {
+        const ExpRec er = exp_block(rec, c, nc, bb_d);
+        r.c0 = er.kind == K_EXACT ? static_cast<uint32_t>(t) : er.c0;
+        r.c1 = er.c1;
+        r.c2 = er.c2; r.c3 = er.c3; r.c4 = er.c4; r.c5 = er.c5; r.c6 = er.c6;
+        r.kind = er.kind;
+        return r;
     }
     uint64_t ph, w;
     if (c == CLS_STATIC) {
@@ -492,6 +585,14 @@ __device__ __forceinline__ void mufu_rec(const float4 a, const float4 b, int kof
             float2 poly = __ffma2_rn(dup2(b.z), w, dup2(b.y));
             poly = __ffma2_rn(poly, w, dup2(b.x));
             poly = __ffma2_rn(poly, w2, dup2(a.w));
+            x = __ffma2_rn(f, K2, __fmul2_rn(poly, w2));
+        } else if (KIND == K_XEDGE) {
+            float2 w;
+            w.x = fmaxf(fmaf(b.z, kf.x, -b.w), 0.f);
+            w.y = fmaxf(fmaf(b.z, kf.y, -b.w), 0.f);
+            const float2 w2 = __fmul2_rn(w, w);
+            float2 poly = __ffma2_rn(dup2(b.y), w, dup2(b.x));
+            poly = __ffma2_rn(poly, w, dup2(a.w));
             x = __ffma2_rn(f, K2, __fmul2_rn(poly, w2));
         } else {
             const float2 kk = kks[j];
@@ -740,6 +841,7 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
             mk[K_SBEG] = kv & ~k0 & ~k1 & k2;
             mk[K_SEND] = kv & k0 & ~k1 & k2;
             mk[K_EXACT] = kv & ~k0 & k1 & k2;
+            mk[K_XEDGE] = kv & k0 & k1 & k2;
             int kbase[K_COUNT], kcnt[K_COUNT];
             int slot = 0;
             {
@@ -764,6 +866,7 @@ __device__ __forceinline__ void mover_block(const LaunchParams &lp, WarpSmem &ws
             AWG_RUN_KIND(K_DEG6)
             AWG_RUN_KIND(K_SBEG)
             AWG_RUN_KIND(K_SEND)
+            AWG_RUN_KIND(K_XEDGE)
 #pragma unroll 1
             for (int i_ = kbase[K_EXACT]; i_ < kbase[K_EXACT] + kcnt[K_EXACT]; ++i_)
                 acc = exact_rec(lp.tab, ws.mrec[i_].q[0], blk_base + lane * kSPT, acc);

@@ -95,6 +95,34 @@ int classify(int profile, long double DT, long double Tn)
     return CLS_DEG6;
 }
 
+// Polynomial class of an exponential chirp f = f0 e^(L s), s = u/Tn (G20).  The k-th derivative of the phase with
+// respect to the sample index is (f/fs) a^(k-1) cycles per sample^k with a = L/Tn, so the Taylor terms about a block centre
+// are t_k = f_max/fs a^(k-1) R^k / k! at the block's edge; the kernel carries terms up to k = 6 (block_prologue()).
+int classify_exp(long double f0, long double f1, long double fs, long double L, long double Tn)
+{
+    if (!(Tn >= 2.0L * kRadius)) return CLS_EXACT;
+    const double R = kRadius;
+    const double x = static_cast<double>(fabsl(L) / Tn) * R;                       // a R
+    const double fm = static_cast<double>(std::max(fabsl(f0), fabsl(f1)) / fs);    // cycles per sample
+    if (!(x < 0.5)) return CLS_EXACT;
+    double t[9];
+    t[1] = fm * R;
+    for (int k = 2; k <= 8; ++k) t[k] = t[k - 1] * x / k;
+    const double rest = t[7] + t[8] / (1.0 - x / 9.0);   // everything beyond the sixth term (the series falls faster than x/9 per term)
+    const double tol_drop = 2e-8, max_mag = 0.25;         // as in classify()
+    if (rest > tol_drop || t[2] + t[3] + t[4] + t[5] + t[6] > max_mag) return CLS_EXACT;
+    // the block that holds one end of the move: the same series counted from that end, up to 2R samples into the move, kept
+    // up to the fourth power (K_XEDGE)
+    const double x2 = 2.0 * x;
+    double e[6];
+    e[1] = fm * 2.0 * R;
+    for (int k = 2; k <= 5; ++k) e[k] = e[k - 1] * x2 / k;
+    if (e[5] / (1.0 - x2 / 6.0) > tol_drop || e[2] + e[3] + e[4] > 4.0 * max_mag) return CLS_EXACT;
+    if (t[3] + t[4] + t[5] + t[6] + rest <= tol_drop) return CLS_QUAD;
+    if (t[5] + t[6] + rest <= tol_drop) return CLS_DEG4;
+    return CLS_DEG6;
+}
+
 // Slow movers (flag CLS_SLOW_FLAG): inside its move the tone changes frequency so slowly that, over a whole tile, the
 // angle-addition engine can carry it: a cubic phase polynomial about the tile centre gives the phase at the pair centres
 // of a thread's four groups of 16 samples, and the pair tables (built at the tile-centre frequency) are moved to the
@@ -174,10 +202,12 @@ void make_move(HostTone &h, long double fs, long double f1, int profile, long do
     h.expL = 0.0L;
     if (profile == AWG_PROFILE_EXP) {
         // Exponential chirp (G20): f = f0 r^s, r = f1/f0; cycles over the whole move = DT / ln r, so after it
-        //   Phi = [theta - (f1-f0) t_s - (f1 T - DT/ln r)] + (f1/fs) n.   Inside the move every sample takes the fp64 path.
+        //   Phi = [theta - (f1-f0) t_s - (f1 T - DT/ln r)] + (f1/fs) n.
         h.expL = log1pl(D / h.f0);
         h.theta_post = h.theta_pre - frac64(delta_times_tstart) - frac64(f1 * T - h.DT / h.expL);
-        h.cls = CLS_EXACT;
+        // blocks wholly inside the move take the MUFU pass with a Taylor polynomial about the block centre, the blocks that hold
+        // the start or the end of the move a power series from that end (classify_exp)
+        h.cls = classify_exp(h.f0, f1, fs, h.expL, h.Tn);
         return;
     }
     h.cls = classify(profile, h.DT, h.Tn);
@@ -238,8 +268,8 @@ static void fill_core(const HostTone &h, ToneCore &r)
             r.q[k - 2] = static_cast<float>(q * inv_fact[k - 2]);
         }
         if (h.profile == AWG_PROFILE_EXP) {
-            // exponential chirp: no Taylor scales (every sample of the move takes the fp64 path); q[0..3] carry f0 T (cycles)
-            // and ln(f1/f0) as two doubles instead
+            // exponential chirp: its Taylor coefficients are a geometric sequence built in block_prologue(); q[0..3] carry
+            // f0 T (cycles) and ln(f1/f0) as two doubles instead of the five scales
             const double F = static_cast<double>(h.f0 * h.T), Lr = static_cast<double>(h.expL);
             std::memcpy(&r.q[0], &F, sizeof F);
             std::memcpy(&r.q[2], &Lr, sizeof Lr);

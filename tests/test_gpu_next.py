@@ -500,3 +500,28 @@ def test_exponential_chirp_updates_and_errors(awg, torch_cuda, eng):
         q.set_trajectories([1e6, 2e6], [1e6, 2e6], [0.1, 0.1], [0, 0], [0, 0], [1e-6, 0], [4, STATIC])
     assert ei.value.status == awg.AWG_ERR_INVALID_ARG
     p.close(); q.close()
+
+
+def test_exponential_chirps_in_step_across_the_polynomial_classes(awg, torch_cuda, eng):
+    """96 exponential chirps that start in step off the sample grid (all their start blocks fall into one tile) and end at 24
+    different times, durations 1.5 us .. 400 us and frequency ratios 0.5 .. 2: every class of classify_exp (degree 2, 4, 6 and
+    the fp64 fallback) and the edge series at both ends, equal phases so that the errors of the tones can add up."""
+    fs, L = 560e6, 1 << 15
+    t0 = 7.123456e-6
+    durs = np.geomspace(1.5e-6, 400e-6, 24)
+    ratios = (0.5, 0.93, 1.07, 2.0)
+    rows = []
+    for i, T in enumerate(durs):
+        for j, r in enumerate(ratios):
+            f0 = 40e6 + 2.1e6 * (4 * i + j)
+            rows.append((f0, f0 * r, 1.0 / 96, 0.3, t0, float(T), EXP))
+    p, op = _pair(awg, fs, L, rows, eng)
+    n_chunks = 8                                            # 468 us: every chirp ends inside
+    V = oracle.c_waveform(op, 0, n_chunks * L)
+    gotf = np.concatenate([_np(p.synthesize_chunk_f32(c)) for c in range(n_chunks)])
+    emax = assert_f32_close(gotf, V, "exponential chirps in step")
+    got = np.concatenate([_np(p.synthesize_chunk(c)) for c in range(n_chunks)])
+    assert_codes_close(got, op.quantise(V), "exponential chirps in step")
+    assert np.array_equal(_np(p.synthesize_range(0, n_chunks)), got)
+    print(f"exponential chirps in step: f32 max err {emax:.2e} of full scale")
+    p.close()
