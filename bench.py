@@ -426,6 +426,19 @@ def run_extras(torch, awg, sm_max_mhz):
     msf, worstf, countsf = device_time_chunks(torch, awg, wf)
     cfgs["FAST_4096"] = {"tones": wf.n_tones, "chunks": wf.n_chunks, "ms_total": msf, "max_chunk_ms": worstf,
                          "gts_per_s": wf.tone_samples / msf / 1e6, **frac_of(countsf, msf, sm_max_mhz)}
+    # ---- exponential chirps (PAPER.md:137 names them; G20): 1024 tones, each 3 % up in frequency over 300 us
+    # inside one 2^18-sample chunk (they start and end in step: both edge blocks of every tone fall into one tile each)
+    rngx = np.random.default_rng(11)
+    fx = rngx.uniform(30e6, 240e6, 1024)
+    p = awg.Plan(1024, 560e6, 1 << 18)
+    p.set_trajectories(fx, fx * 1.03, np.full(1024, 1.0 / 1024), rngx.uniform(0, 6.28, 1024), np.full(1024, 20e-6), np.full(1024, 300e-6),
+                       np.full(1024, W.PROFILE_EXP, np.int32))
+    bufs = make_bufs(torch, 1 << 18)
+    ms = device_time_range(torch, p, 1, bufs, 20, 3, prequeue_ms=1.0)
+    cfgs["EXP_1024"] = {"tones": 1024, "samples": 1 << 18, "ms": ms, "gts_per_s": 1024 * (1 << 18) / ms / 1e6,
+                        **frac_of(p.op_counts(0, 1), ms, sm_max_mhz)}
+    del bufs
+    p.close()
     # ---- static set (the paper's comb), per-sample and through the looped static buffer
     ws = W.capacity_toneset(4096, 560e6, 1 << 20, "static", n_chunks=4)
     p = awg.Plan.from_workload(ws)
