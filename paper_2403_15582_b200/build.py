@@ -22,7 +22,7 @@ INCLUDE = os.path.join(ROOT, "include")
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-    "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC,-O2,-Wall,-pthread", "-shared", "-cudart", "static",
 ]
 
 

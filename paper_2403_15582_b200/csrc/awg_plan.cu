@@ -15,6 +15,7 @@
 #include <limits>
 #include <mutex>
 #include <new>
+#include <thread>
 #include <utility>
 #include <vector>
 
@@ -24,6 +25,40 @@
 namespace awg {
 
 thread_local char g_err[512] = "";
+
+// Host loops over tones (x87 long double planning and table cores, 0.1 - 0.5 us per tone) run on a few threads once they are
+// long: body(begin, end) touches only the tones of its own range, and every tone goes through the same arithmetic whichever
+// thread takes it.  The threads live for one call (creating one costs about 15 us: `grain` = the shortest range worth one,
+// 512 tones of trajectory planning, 2048 tone cores; at most 8 threads).
+constexpr int kThreadedFrom = 2048;   // tones per call from which the planning loops are threaded (below: the plain loop)
+
+template <class Body>
+static void parallel_tones(int n, int grain, Body body)
+{
+    constexpr int kMaxThreads = 8;
+    static const int hw = static_cast<int>(std::thread::hardware_concurrency());   // (reads /sys: 20 us per call)
+    const int nt = std::min(std::min(kMaxThreads, hw > 0 ? hw : 1), n / grain);
+    if (nt <= 1) {
+        body(0, n);
+        return;
+    }
+    const int per = (n + nt - 1) / nt;
+    std::vector<std::thread> helpers;
+    helpers.reserve(static_cast<size_t>(nt - 1));
+    int done = per;   // [0, per) is the caller's own range; ranges from `done` on still have no thread
+    try {
+        for (int t = 1; t < nt && t * per < n; ++t) {
+            const int b = t * per, e = std::min(n, b + per);
+            helpers.emplace_back([body, b, e] { body(b, e); });
+            done = e;
+        }
+    } catch (...) {
+        // no more threads to be had: the caller takes the rest itself
+    }
+    body(0, std::min(n, per));
+    if (done < n) body(done, n);
+    for (std::thread &h : helpers) h.join();
+}
 
 awg_status fail(awg_status code, const char *fmt, ...)
 {
@@ -348,13 +383,15 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
         // the device table holds the tones that are evaluated per sample (all of them unless some are served by the
         // looped static buffer), in tone order
         int n_act = 0;
-        for (int k = 0; k < p->n_tones; ++k) {
-            if (p->in_buffer[k]) {
-                p->slot_of[k] = -1;
-            } else {
-                p->slot_of[k] = n_act;
-                fill_core(p->tones[k], host[n_act++]);
-            }
+        for (int k = 0; k < p->n_tones; ++k) p->slot_of[k] = p->in_buffer[k] ? -1 : n_act++;
+        if (p->n_tones < 4 * kThreadedFrom) {
+            for (int k = 0; k < p->n_tones; ++k)
+                if (p->slot_of[k] >= 0) fill_core(p->tones[k], host[p->slot_of[k]]);
+        } else {
+            parallel_tones(p->n_tones, 2048, [=](int k_begin, int k_end) {
+                for (int k = k_begin; k < k_end; ++k)
+                    if (p->slot_of[k] >= 0) fill_core(p->tones[k], host[p->slot_of[k]]);
+            });
         }
         p->n_active = n_act;
         const int n_up = (n_act + 31) / 32 * 32;
@@ -529,35 +566,13 @@ awg_status check_chunk_call(awg_plan *p, int64_t first_chunk, int64_t n_chunks, 
     return AWG_OK;
 }
 
-awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx, const double *f1,
-                        const double *t_dur, const int32_t *profile)
+// awg_update_trajectories at sample n_u for the updates [i_begin, i_end) of one call (validated by the caller; the tones of one
+// update are distinct, so every iteration has its own tone)
+static inline __attribute__((always_inline)) void update_tones(awg_plan *p, int64_t n_u, const int32_t *tone_idx, const double *f1, const double *t_dur,
+                         const int32_t *profile, int i_begin, int i_end)
 {
-    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
-    if (n_upd < 0 || chunk_idx < 0) return fail(AWG_ERR_INVALID_ARG, "negative count or chunk index");
-    if (n_upd > 0 && (!tone_idx || !f1 || !t_dur || !profile)) return fail(AWG_ERR_INVALID_ARG, "NULL update array");
-    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
-    if (chunk_idx < p->last_update_chunk)
-        return fail(AWG_ERR_STATE, "updates must come in non-decreasing chunk order");
-    if (chunk_idx > (std::numeric_limits<int64_t>::max() / 4) / p->chunk_len)
-        return fail(AWG_ERR_INVALID_ARG, "chunk index too large");
-    // validate everything before touching the table
-    std::vector<char> seen(p->n_tones, 0);
-    for (int i = 0; i < n_upd; ++i) {
-        const int k = tone_idx[i];
-        if (k < 0 || k >= p->n_tones) return fail(AWG_ERR_INVALID_ARG, "tone index %d out of range", k);
-        if (seen[k]) return fail(AWG_ERR_INVALID_ARG, "tone %d listed twice in one update", k);
-        seen[k] = 1;
-        if (p->in_buffer[k]) return fail(AWG_ERR_STATE, "tone %d is served by the static buffer (clear it with awg_static_buffer_set first)", k);
-        if (!std::isfinite(f1[i]) || !std::isfinite(t_dur[i]) || t_dur[i] < 0.0)
-            return fail(AWG_ERR_INVALID_ARG, "non-finite value or negative duration in update %d", i);
-        if (profile[i] < AWG_PROFILE_STATIC || profile[i] > AWG_PROFILE_EXP)
-            return fail(AWG_ERR_INVALID_ARG, "unknown profile %d", profile[i]);
-        if (profile[i] == AWG_PROFILE_EXP && !(f1[i] > 0.0 && p->tones[k].f0 > 0.0L && p->tones[k].f1 > 0.0L))
-            return fail(AWG_ERR_INVALID_ARG, "exponential chirp of tone %d needs positive frequencies", k);
-    }
     const long double fs = p->fs;
-    const int64_t n_u = chunk_idx * p->chunk_len;
-    for (int i = 0; i < n_upd; ++i) {
+    for (int i = i_begin; i < i_end; ++i) {
         HostTone &h = p->tones[tone_idx[i]];
         // an amplitude ramp that has ended by n_u is folded into the tone's amplitude (the tables then carry it)
         if (h.amp_prof != AWG_PROFILE_STATIC && static_cast<long double>(n_u) - h.amp_ns >= h.amp_Tn) {
@@ -591,6 +606,37 @@ awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int
         make_move(h, fs, f1l, profile[i], static_cast<long double>(t_dur[i]), n_u, 0.0,
                   D * static_cast<long double>(n_u) / fs);
     }
+}
+
+awg_status apply_update(awg_plan *p, int64_t chunk_idx, int32_t n_upd, const int32_t *tone_idx, const double *f1,
+                        const double *t_dur, const int32_t *profile)
+{
+    if (!p) return fail(AWG_ERR_INVALID_ARG, "plan is NULL");
+    if (n_upd < 0 || chunk_idx < 0) return fail(AWG_ERR_INVALID_ARG, "negative count or chunk index");
+    if (n_upd > 0 && (!tone_idx || !f1 || !t_dur || !profile)) return fail(AWG_ERR_INVALID_ARG, "NULL update array");
+    if (!p->have_table) return fail(AWG_ERR_STATE, "awg_set_trajectories has not been called");
+    if (chunk_idx < p->last_update_chunk)
+        return fail(AWG_ERR_STATE, "updates must come in non-decreasing chunk order");
+    if (chunk_idx > (std::numeric_limits<int64_t>::max() / 4) / p->chunk_len)
+        return fail(AWG_ERR_INVALID_ARG, "chunk index too large");
+    // validate everything before touching the table
+    std::vector<char> seen(p->n_tones, 0);
+    for (int i = 0; i < n_upd; ++i) {
+        const int k = tone_idx[i];
+        if (k < 0 || k >= p->n_tones) return fail(AWG_ERR_INVALID_ARG, "tone index %d out of range", k);
+        if (seen[k]) return fail(AWG_ERR_INVALID_ARG, "tone %d listed twice in one update", k);
+        seen[k] = 1;
+        if (p->in_buffer[k]) return fail(AWG_ERR_STATE, "tone %d is served by the static buffer (clear it with awg_static_buffer_set first)", k);
+        if (!std::isfinite(f1[i]) || !std::isfinite(t_dur[i]) || t_dur[i] < 0.0)
+            return fail(AWG_ERR_INVALID_ARG, "non-finite value or negative duration in update %d", i);
+        if (profile[i] < AWG_PROFILE_STATIC || profile[i] > AWG_PROFILE_EXP)
+            return fail(AWG_ERR_INVALID_ARG, "unknown profile %d", profile[i]);
+        if (profile[i] == AWG_PROFILE_EXP && !(f1[i] > 0.0 && p->tones[k].f0 > 0.0L && p->tones[k].f1 > 0.0L))
+            return fail(AWG_ERR_INVALID_ARG, "exponential chirp of tone %d needs positive frequencies", k);
+    }
+    const int64_t n_u = chunk_idx * p->chunk_len;
+    if (n_upd < kThreadedFrom) update_tones(p, n_u, tone_idx, f1, t_dur, profile, 0, n_upd);
+    else parallel_tones(n_upd, 512, [=](int i_begin, int i_end) { update_tones(p, n_u, tone_idx, f1, t_dur, profile, i_begin, i_end); });
     if (n_upd > 0) {
         p->dirty_tones.insert(p->dirty_tones.end(), tone_idx, tone_idx + n_upd);
         p->last_update_chunk = chunk_idx;
@@ -1053,6 +1099,28 @@ awg_status awg_set_engine(awg_plan *p, int32_t engine)
     return AWG_OK;
 }
 
+// awg_set_trajectories for the tones [k_begin, k_end) (validated by the caller)
+static inline __attribute__((always_inline)) void plan_tones(awg_plan *p, const double *f0, const double *f1, const double *A, const double *phi0, const double *t_start,
+                       const double *t_dur, const int32_t *profile, int k_begin, int k_end)
+{
+    const long double fs = p->fs;
+    for (int k = k_begin; k < k_end; ++k) {
+        HostTone &h = p->tones[k];
+        h = HostTone{};
+        h.A = static_cast<float>(A[k]);
+        h.A1 = h.A;
+        h.f0 = static_cast<long double>(f0[k]);
+        h.theta_pre = frac64(static_cast<long double>(phi0[k]) / kTwoPiL);  // radians -> turns (theta_j of Eq. 8/9)
+        h.w_pre = frac64(h.f0 / fs);
+        const long double ts = static_cast<long double>(t_start[k]);
+        const long double ns = ts * fs;
+        const long double nsi = floorl(ns);
+        make_move(h, fs, static_cast<long double>(f1[k]), profile[k], static_cast<long double>(t_dur[k]),
+                  static_cast<int64_t>(nsi), static_cast<double>(ns - nsi),
+                  (static_cast<long double>(f1[k]) - h.f0) * ts);
+    }
+}
+
 awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1, const double *A, const double *phi0,
                                 const double *t_start, const double *t_dur, const int32_t *profile)
 {
@@ -1071,22 +1139,8 @@ awg_status awg_set_trajectories(awg_plan *p, const double *f0, const double *f1,
         if (std::fabs(t_start[k]) * static_cast<double>(p->fs) > 4.0e18)
             return fail(AWG_ERR_INVALID_ARG, "t_start[%d] out of range", k);
     }
-    const long double fs = p->fs;
-    for (int k = 0; k < N; ++k) {
-        HostTone &h = p->tones[k];
-        h = HostTone{};
-        h.A = static_cast<float>(A[k]);
-        h.A1 = h.A;
-        h.f0 = static_cast<long double>(f0[k]);
-        h.theta_pre = frac64(static_cast<long double>(phi0[k]) / kTwoPiL);  // radians -> turns (theta_j of Eq. 8/9)
-        h.w_pre = frac64(h.f0 / fs);
-        const long double ts = static_cast<long double>(t_start[k]);
-        const long double ns = ts * fs;
-        const long double nsi = floorl(ns);
-        make_move(h, fs, static_cast<long double>(f1[k]), profile[k], static_cast<long double>(t_dur[k]),
-                  static_cast<int64_t>(nsi), static_cast<double>(ns - nsi),
-                  (static_cast<long double>(f1[k]) - h.f0) * ts);
-    }
+    if (N < kThreadedFrom) plan_tones(p, f0, f1, A, phi0, t_start, t_dur, profile, 0, N);
+    else parallel_tones(N, 512, [=](int k_begin, int k_end) { plan_tones(p, f0, f1, A, phi0, t_start, t_dur, profile, k_begin, k_end); });
     p->have_table = true;
     p->dirty_all = true;
     p->dirty_tones.clear();

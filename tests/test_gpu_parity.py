@@ -860,3 +860,32 @@ def test_random_soak_against_the_oracle(awg, torch_cuda, seed):
         assert_codes_close(got[a:a + wlen], op.quantise(V), f"soak seed {seed} case {case} (N={n}, L={cl})")
         assert_f32_close(gotf[a:a + wlen], V, f"soak seed {seed} case {case} (N={n}, L={cl})", tol=1e-5 * max(1.0, sa))
         p.close()
+
+
+def test_updates_of_thousands_of_tones_in_one_call(awg, torch_cuda):
+    """Calls that plan >= 2048 tones split the host loop over threads (csrc/awg_plan.cu, parallel_tones); shorter ones run the
+    plain loop.  5000 tones set in one call and re-targeted in one call per chunk (some of them mid-move) must give the same
+    bits as the same tones re-targeted in calls of 500 (plain loop), and match the oracle."""
+    N, L, fs = 5000, 1 << 14, 560e6
+    rng = np.random.default_rng(11)
+    f0 = rng.uniform(30e6, 240e6, N)
+    rows = [(f0[k], f0[k] + (rng.uniform(-3e6, 3e6) if k % 2 else 0.0), 1.0 / N, rng.uniform(0, 2 * math.pi), 0.0,
+             rng.uniform(20e-6, 90e-6), MINJERK if k % 2 else STATIC) for k in range(N)]
+    p, op = _single(awg, fs, L, rows)
+    q, _ = _single(awg, fs, L, rows)
+    idx = np.arange(N, dtype=np.int32)
+    for c in (1, 2):
+        f1 = f0 + rng.uniform(-4e6, 4e6, N)
+        td = rng.uniform(10e-6, 60e-6, N)
+        prof = np.where(idx % 3 == 0, LINEAR, MINJERK).astype(np.int32)
+        p.update_trajectories(c, idx, f1, td, prof)                       # one call: threaded
+        op.update_trajectories(c, idx, f1, td, prof)
+        for a in range(0, N, 500):                                        # ten calls: the plain loop
+            q.update_trajectories(c, idx[a:a + 500], f1[a:a + 500], td[a:a + 500], prof[a:a + 500])
+        got, gotf = _np(p.synthesize_chunk(c)), _np(p.synthesize_chunk_f32(c))
+        assert np.array_equal(got, _np(q.synthesize_chunk(c))), f"chunk {c}: one call vs ten calls"
+        V = oracle.c_waveform(op, c * L, (c + 1) * L)
+        assert_f32_close(gotf, V, f"5000 tones, chunk {c}")
+        assert_codes_close(got, op.quantise(V), f"5000 tones, chunk {c}")
+    p.close()
+    q.close()
