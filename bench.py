@@ -365,9 +365,8 @@ def realtime_capacity(awg, make_workload, host_mirror, lo=16, hi=65536):
 
 def fast_mover_capacity(torch, awg, fs, chunk_len, lo=16, hi=65536):
     """Largest count of tones that are ALL inside short minimum-jerk moves all the time (W.fast_mover_stream) whose
-    every chunk is synthesised within chunk_len/fs of device time.  (Streaming such a set through the ring re-plans
-    every tone every chunk on the host, which the host sustains only up to ~1000 tones per 468 us: the criterion here
-    is the device time of the synthesis launches.)"""
+    every chunk is synthesised within chunk_len/fs of device time.  (The criterion here is the device time of the synthesis
+    launches alone; fast_mover_ring_capacity() streams the same set through the ring, host planning included.)"""
     deadline_ms = chunk_len / fs * 1e3
 
     def ok(n):
@@ -386,6 +385,36 @@ def fast_mover_capacity(torch, awg, fs, chunk_len, lo=16, hi=65536):
     if bad is None:
         return good
     while bad - good > max(8, good // 32):
+        mid = (good + bad) // 2
+        if ok(mid):
+            good = mid
+        else:
+            bad = mid
+    return good
+
+
+def fast_mover_ring_capacity(awg, fs, chunk_len, seconds=1.0, lo=256, hi=8192):
+    """Largest all-fast-mover count (W.fast_mover_stream) the RING sustains: its own underrun counter stays at zero over
+    `seconds` of signal while, every chunk, the host re-plans every tone (awg_ring_submit with N updates), uploads the table
+    and launches.  Beside the device-time figure: this one includes the host."""
+    n_chunks = int(math.ceil(seconds * fs / chunk_len))
+
+    def ok(n):
+        und, _, _, _ = stream_through_ring(awg, W.fast_mover_stream(n, fs, chunk_len, n_chunks), False, n_slots=4)
+        return und == 0
+
+    good, bad, n = None, None, lo
+    while n <= hi:
+        if ok(n):
+            good, n = n, n * 2
+        else:
+            bad = n
+            break
+    if good is None:
+        return 0
+    if bad is None:
+        return good
+    while bad - good > max(64, good // 16):
         mid = (good + bad) // 2
         if ok(mid):
             good = mid
@@ -520,6 +549,7 @@ def run_extras(torch, awg, sm_max_mhz):
     cap["560MS_static_L18_chunks"] = realtime_capacity(awg, (lambda n: W.capacity_toneset(n, 560e6, 1 << 18, "static", n_chunks=n18)), False)
     cap["560MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 560e6, 1 << 18)
     cap["100MS_all_fast_movers_device_time"] = fast_mover_capacity(torch, awg, 100e6, 1 << 15)
+    cap["560MS_all_fast_movers_ring"] = fast_mover_ring_capacity(awg, 560e6, 1 << 18)
     out["max_realtime_tones"] = cap
     # fraction of the binding roofline AT each capacity: roofline time of one chunk of the N_max-tone set / the chunk's deadline
     def cap_frac(n, make, fs, cl, chunk=1):
@@ -537,7 +567,8 @@ def run_extras(torch, awg, sm_max_mhz):
             capf[f"{tag}_{key}"] = cap_frac(cap[f"{tag}_{key}"], (lambda n, fs=fs, cl=cl, mix=mix, n_chunks=n_chunks:
                                                                   W.capacity_toneset(n, fs, cl, mix, n_chunks=n_chunks)), fs, cl, chunk=n_chunks // 2)
     capf["560MS_static_L18_chunks"] = cap_frac(cap["560MS_static_L18_chunks"], (lambda n: W.capacity_toneset(n, 560e6, 1 << 18, "static", n_chunks=4)), 560e6, 1 << 18)
-    for fs, cl, key in ((560e6, 1 << 18, "560MS_all_fast_movers_device_time"), (100e6, 1 << 15, "100MS_all_fast_movers_device_time")):
+    for fs, cl, key in ((560e6, 1 << 18, "560MS_all_fast_movers_device_time"), (100e6, 1 << 15, "100MS_all_fast_movers_device_time"),
+                        (560e6, 1 << 18, "560MS_all_fast_movers_ring")):
         n = cap[key]
         if n:   # every tone-sample of such a set is inside a move: one sine each
             r = pipe_roofline((0, 0, n * cl), cl / fs * 1e3, "auto", sm_max_mhz)
@@ -548,7 +579,8 @@ def run_extras(torch, awg, sm_max_mhz):
         "drawn like C5 (2^20-sample chunks at 560 MS/s, 2^18 at 100 MS/s; '_L18_chunks': 2^18-sample chunks at 560 MS/s over 0.5 s); 'all_slow_movers' = one +-5 MHz minimum-jerk move "
         "spanning the probe (the slow pass); '_d2h' = pinned-host mirror on; 'all_fast_movers_device_time' = every tone "
         "inside a one-chunk minimum-jerk move all the time (2^18-sample chunks = 468 us at 560 MS/s, 2^15 = 328 us at "
-        "100 MS/s), criterion: every chunk's synthesis within chunk_len/fs of device time")
+        "100 MS/s), criterion: every chunk's synthesis within chunk_len/fs of device time; 'all_fast_movers_ring' = the same "
+        "set through the ring (4 slots, >= 1 s, underruns == 0): the host re-plans every tone every chunk (threaded from 2048 tones)")
     # ---- the paper's two scaling laws, re-fitted on this GPU (context, not a target)
     laws = {}
     # Eq. 12: N_streaming = (P / fs)^(1 / (1 - k)), N_streaming = tones that can be chirped indefinitely
