@@ -29,7 +29,7 @@ thread_local char g_err[512] = "";
 // Host loops over tones (x87 long double planning and table cores, 0.1 - 0.5 us per tone) run on a few threads once they are
 // long: body(begin, end) touches only the tones of its own range, and every tone goes through the same arithmetic whichever
 // thread takes it.  The threads live for one call (creating one costs about 15 us: `grain` = the shortest range worth one,
-// 512 tones of trajectory planning, 2048 tone cores; at most 8 threads).
+// 512 tones of trajectory planning, 1024 tone cores; at most 8 threads).
 constexpr int kThreadedFrom = 2048;   // tones per call from which the planning loops are threaded (below: the plain loop)
 
 template <class Body>
@@ -384,11 +384,11 @@ awg_status ensure_table(awg_plan *p, cudaStream_t stream)
         // looped static buffer), in tone order
         int n_act = 0;
         for (int k = 0; k < p->n_tones; ++k) p->slot_of[k] = p->in_buffer[k] ? -1 : n_act++;
-        if (p->n_tones < 4 * kThreadedFrom) {
+        if (p->n_tones < kThreadedFrom) {
             for (int k = 0; k < p->n_tones; ++k)
                 if (p->slot_of[k] >= 0) fill_core(p->tones[k], host[p->slot_of[k]]);
         } else {
-            parallel_tones(p->n_tones, 2048, [=](int k_begin, int k_end) {
+            parallel_tones(p->n_tones, 1024, [=](int k_begin, int k_end) {
                 for (int k = k_begin; k < k_end; ++k)
                     if (p->slot_of[k] >= 0) fill_core(p->tones[k], host[p->slot_of[k]]);
             });
